@@ -1,0 +1,124 @@
+/*
+ * fsei.h -- C ABI of libfsei: the fp64 pressure projection of the fractional-step
+ * Navier-Stokes scheme on a staggered grid, hand-written for NVIDIA B200 (sm_100a).
+ *
+ * What the calls compute (P:Lnnn = line nnn of the paper text, arXiv 2103.15187):
+ *   - "central second-order finite-differences discretized on a staggered mesh"   P:L87  (sec. 2.1)
+ *   - "a fractional-step method is used"; the pressure "acts only as a Lagrangian
+ *     multiplier assuring the solenoidal condition"                               P:L91  (sec. 2.1, Eq. 3)
+ *   - periodic x,y, wall-normal z                                                 P:L240 (Fig. 4), P:L260-262 (sec. 5)
+ *   - FFT as the routine of the elliptic solve, Thomas' algorithm for tridiagonals P:L30, P:L208 (sec. 3.1)
+ *   - "the elliptic equation to impose mass conservation"                         P:L248 (sec. 4)
+ * The paper prints no formula for the projection; the exact discrete operators are the
+ * readings R1..R20 of DESIGN.md sec. 3 (standard second-order staggered projection).
+ *
+ * Data layout.  A field is nx*ny*nz contiguous doubles in C order [nz][ny][nx], x fastest:
+ * element (i,j,k) at linear index (k*ny + j)*nx + i.  phi and p live at cell centres;
+ * u[k][j][i], v[k][j][i], w[k][j][i] live on the LOW x-, y-, z-face of cell (i,j,k).
+ * Periodic direction: face n is face 0.  Wall direction (z always; x or y when the bc is
+ * FSEI_BC_NEUMANN): stored face 0 IS the low wall and the caller keeps it 0 (no
+ * penetration); the high wall face is not stored and is 0.
+ *
+ * Pointers.  `zc` is a HOST pointer (copied at plan creation).  Every field pointer
+ * (u, v, w, p, rhs, phi) is a DEVICE pointer to nx*ny*nz doubles, 16-byte aligned, owned
+ * by the caller.  `cuda_stream` is a cudaStream_t cast to void* (NULL = default stream).
+ *
+ * Execution.  Calls enqueue kernels on `cuda_stream` and return; they never synchronise
+ * the device and never allocate after plan creation.  Calls on different plans may run
+ * concurrently; calls on ONE plan must be issued from one thread at a time and on one
+ * stream at a time (the plan owns factorisation tables only -- the transforms run in
+ * place in the caller's phi buffer -- but the gauge scratch is per plan).
+ *
+ * Errors.  Functions returning int return FSEI_OK or an FSEI_ERR_* code; nothing throws
+ * across this boundary; fsei_last_error() gives a thread-local message for the last
+ * failing call.  There is no CPU fallback: without a CUDA device fsei_plan_create fails
+ * with FSEI_ERR_CUDA.
+ */
+#ifndef FSEI_H
+#define FSEI_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fsei_plan fsei_plan;          /* opaque; owns device tables (wavenumbers, twiddles, z-factorisation) */
+
+enum { FSEI_BC_PERIODIC = 0, FSEI_BC_NEUMANN = 1 };      /* bc_x, bc_y; z is always Neumann-phi / no-penetration */
+enum { FSEI_OK = 0, FSEI_ERR_ARG = 1, FSEI_ERR_SIZE = 2, FSEI_ERR_GRID = 3, FSEI_ERR_ALLOC = 4, FSEI_ERR_CUDA = 5 };
+
+/*
+ * Plan for an nx x ny x nz grid (cells), uniform in x,y with extents Lx, Ly, wall-normal
+ * z with face coordinates zc[0..nz] (strictly increasing; zc[0], zc[nz] are the walls;
+ * cell centres are the midpoints).  DESIGN.md R2, R3, R5, R6.
+ *   nx, ny : of the form 2^a 3^b, even, >= 4 and <= 8192;  nz >= 2.           else FSEI_ERR_SIZE
+ *   Lx, Ly > 0, zc finite and strictly increasing                              else FSEI_ERR_GRID
+ *   bc_x, bc_y in {PERIODIC, NEUMANN}, zc != NULL                              else FSEI_ERR_ARG
+ * Returns NULL on error (see fsei_last_error / fsei_last_error_code).
+ */
+fsei_plan*  fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly,
+                             const double* zc /* HOST, nz+1 */, int bc_x, int bc_y);
+void        fsei_plan_destroy(fsei_plan* plan);
+const char* fsei_last_error(void);
+int         fsei_last_error_code(void);
+/* Device bytes the plan owns (tables + z-factorisation + scratch). */
+size_t      fsei_plan_workspace_bytes(const fsei_plan* plan);
+
+/*
+ * Step a1 (R4, R20):
+ *   rhs = [ (u[i+1]-u[i])/dx + (v[j+1]-v[j])/dy + (w[k+1]-w[k])/dzc[k] ] / alpha_dt
+ * with wrap-around in periodic directions and the missing high-wall face = 0, evaluated in
+ * IEEE double in the fixed order ((du*rdx + dv*rdy) + dw*rdzc[k]) * (1/alpha_dt), no FMA.
+ * rhs must not alias u, v, w.   alpha_dt == 0 or NULL pointer -> FSEI_ERR_ARG.
+ */
+int fsei_divergence(fsei_plan* plan, const double* u, const double* v, const double* w,
+                    double alpha_dt, double* rhs, void* cuda_stream);
+
+/*
+ * Steps a2..a6 (R5-R8, R15): phi = solution of L phi = rhs,
+ * L = D G the 7-point operator (periodic or homogeneous Neumann in x,y; homogeneous Neumann
+ * in z), made unique by the volume-weighted zero mean  sum phi*dzc = 0.  Direct method:
+ * transforms along x and y (real-to-complex FFT, or DCT-II for Neumann), one tridiagonal
+ * solve per wavenumber pair along z, the (0,0) column by two prefix sums, inverse transforms.
+ * phi may alias rhs (the solve runs in place in phi).
+ */
+int fsei_poisson_solve(fsei_plan* plan, const double* rhs, double* phi, void* cuda_stream);
+
+/*
+ * Step a7 (R4, R9), in place:
+ *   u -= alpha_dt*(phi[i]-phi[i-1])/dx,  v -= alpha_dt*(phi[j]-phi[j-1])/dy,
+ *   w[k] -= alpha_dt*(phi[k]-phi[k-1])/dzm[k] (k >= 1);  wall faces untouched;
+ *   p += phi - beta*(L phi)   (beta = alpha_dt/(2 Re); beta == 0 -> p += phi).
+ * phi must not alias u, v, w, p.
+ */
+int fsei_project(fsei_plan* plan, double* u, double* v, double* w, double* p, const double* phi,
+                 double alpha_dt, double beta, void* cuda_stream);
+
+/*
+ * One whole projection a1..a7 enqueued back to back (the divergence is fused into the
+ * x-forward transform and never written out).  phi is caller scratch of one field that
+ * holds the pressure increment on return.  Same results as the three calls above.
+ */
+int fsei_pressure_projection(fsei_plan* plan, double* u, double* v, double* w, double* p, double* phi,
+                             double alpha_dt, double beta, void* cuda_stream);
+
+/*
+ * Host-buffer convenience used for end-to-end timing: u,v,w,p are HOST pointers (pinned for
+ * full speed); copies them to plan-owned device fields, runs fsei_pressure_projection, copies
+ * u,v,w,p back and synchronises the stream.  Allocates the device fields on first use
+ * (5 fields; freed with the plan).
+ */
+int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double* w, double* p,
+                                  double alpha_dt, double beta, void* cuda_stream);
+
+/*
+ * Kernel-level timing aid for bench.py: number of kernels enqueued by the last
+ * fsei_pressure_projection / fsei_poisson_solve call on this plan.
+ */
+int fsei_plan_last_launch_count(const fsei_plan* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FSEI_H */
