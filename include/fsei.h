@@ -52,7 +52,8 @@ enum { FSEI_OK = 0, FSEI_ERR_ARG = 1, FSEI_ERR_SIZE = 2, FSEI_ERR_GRID = 3, FSEI
  * Plan for an nx x ny x nz grid (cells), uniform in x,y with extents Lx, Ly, wall-normal
  * z with face coordinates zc[0..nz] (strictly increasing; zc[0], zc[nz] are the walls;
  * cell centres are the midpoints).  DESIGN.md R2, R3, R5, R6.
- *   nx, ny : of the form 2^a 3^b, even, >= 4 and <= 8192;  nz >= 2.           else FSEI_ERR_SIZE
+ *   nx, ny : of the form 2^a 3^b in [4, 8192], nx a multiple of 4, ny even;
+ *            2 <= nz <= 8192                                                    else FSEI_ERR_SIZE
  *   Lx, Ly > 0, zc finite and strictly increasing                              else FSEI_ERR_GRID
  *   bc_x, bc_y in {PERIODIC, NEUMANN}, zc != NULL                              else FSEI_ERR_ARG
  * Returns NULL on error (see fsei_last_error / fsei_last_error_code).
@@ -117,6 +118,16 @@ int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double*
  * fsei_pressure_projection / fsei_poisson_solve call on this plan.
  */
 int fsei_plan_last_launch_count(const fsei_plan* plan);
+
+/*
+ * Per-kernel device timing for the roofline report: while enabled, every launch the calls
+ * above enqueue is bracketed by a pair of CUDA events on the caller's stream.
+ * fsei_plan_profile_read waits for the recorded events, returns how many kernel kinds there are
+ * (<= max_kernels) and fills, per kind, the summed milliseconds and launch count since the last
+ * read (and, if names != NULL, static name strings); it resets the sums.
+ */
+int fsei_plan_profile(fsei_plan* plan, int enable);
+int fsei_plan_profile_read(fsei_plan* plan, int max_kernels, double* ms_sum, long* count, const char** names);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,166 @@
+"""Thin ctypes binding over the C ABI of libfsei.so (include/fsei.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library.  PyTorch is used by callers for
+device memory and streams; this module only needs integer device pointers.  There is no CPU
+fallback: if libfsei.so is missing or cannot be loaded, importing `lib()` raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+BC_PERIODIC, BC_NEUMANN = 0, 1
+OK, ERR_ARG, ERR_SIZE, ERR_GRID, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4, 5
+
+EXPORTS = ("fsei_plan_create", "fsei_plan_destroy", "fsei_last_error", "fsei_last_error_code",
+           "fsei_plan_workspace_bytes", "fsei_divergence", "fsei_poisson_solve", "fsei_project",
+           "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
+           "fsei_plan_profile", "fsei_plan_profile_read")
+
+_lib = None
+_vp, _d, _i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+
+
+class FseiError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libfsei error {code}: {msg}")
+        self.code = code
+
+
+def lib() -> ctypes.CDLL:
+    """Load libfsei.so (building it first if nvcc is here and the sources are newer)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.stale():
+        try:
+            _build.build()
+        except Exception as e:  # no nvcc on this box: use the shipped .so if there is one
+            if not os.path.exists(path):
+                raise RuntimeError(f"libfsei.so is missing and cannot be built ({e}); there is no CPU fallback") from e
+    L = ctypes.CDLL(path)
+    L.fsei_plan_create.restype = _vp
+    L.fsei_plan_create.argtypes = [_i, _i, _i, _d, _d, _vp, _i, _i]
+    L.fsei_plan_destroy.restype = None
+    L.fsei_plan_destroy.argtypes = [_vp]
+    L.fsei_last_error.restype = ctypes.c_char_p
+    L.fsei_last_error.argtypes = []
+    L.fsei_last_error_code.restype = _i
+    L.fsei_last_error_code.argtypes = []
+    L.fsei_plan_workspace_bytes.restype = ctypes.c_size_t
+    L.fsei_plan_workspace_bytes.argtypes = [_vp]
+    L.fsei_plan_last_launch_count.restype = _i
+    L.fsei_plan_last_launch_count.argtypes = [_vp]
+    L.fsei_divergence.restype = _i
+    L.fsei_divergence.argtypes = [_vp, _vp, _vp, _vp, _d, _vp, _vp]
+    L.fsei_poisson_solve.restype = _i
+    L.fsei_poisson_solve.argtypes = [_vp, _vp, _vp, _vp]
+    L.fsei_project.restype = _i
+    L.fsei_project.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _d, _d, _vp]
+    L.fsei_pressure_projection.restype = _i
+    L.fsei_pressure_projection.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _d, _d, _vp]
+    L.fsei_pressure_projection_host.restype = _i
+    L.fsei_pressure_projection_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _d, _d, _vp]
+    L.fsei_plan_profile.restype = _i
+    L.fsei_plan_profile.argtypes = [_vp, _i]
+    L.fsei_plan_profile_read.restype = _i
+    L.fsei_plan_profile_read.argtypes = [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_long), ctypes.POINTER(ctypes.c_char_p)]
+    _lib = L
+    return L
+
+
+def _ptr(t) -> int:
+    """Integer address of a torch tensor / numpy array / int."""
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        assert t.is_contiguous() and t.element_size() == 8, "fields must be contiguous float64"
+        return t.data_ptr()
+    assert t.flags["C_CONTIGUOUS"] and t.itemsize == 8
+    return t.ctypes.data
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+def last_error() -> str:
+    return lib().fsei_last_error().decode()
+
+
+def _chk(rc: int):
+    if rc != OK:
+        raise FseiError(rc, last_error())
+
+
+class Plan:
+    """fsei_plan_create(nx, ny, nz, Lx, Ly, zc[], bc_x, bc_y); zc is a host float64 array of nz+1 faces."""
+
+    def __init__(self, nx, ny, nz, Lx, Ly, zc, bc_x=BC_PERIODIC, bc_y=BC_PERIODIC):
+        import numpy as np
+        L = lib()
+        zc = np.ascontiguousarray(zc, dtype=np.float64)
+        if zc.shape != (nz + 1,):
+            raise FseiError(ERR_ARG, f"zc must hold nz+1 = {nz + 1} face coordinates")
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self._h = L.fsei_plan_create(self.nx, self.ny, self.nz, float(Lx), float(Ly), zc.ctypes.data, int(bc_x), int(bc_y))
+        if not self._h:
+            raise FseiError(L.fsei_last_error_code(), last_error())
+
+    @classmethod
+    def from_grid(cls, grid):
+        nx, ny, nz, Lx, Ly, zc, bcx, bcy = grid
+        return cls(nx, ny, nz, Lx, Ly, zc, bcx, bcy)
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().fsei_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(lib().fsei_plan_workspace_bytes(self._h))
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(lib().fsei_plan_last_launch_count(self._h))
+
+    def profile(self, enable: bool):
+        _chk(lib().fsei_plan_profile(self._h, int(enable)))
+
+    def profile_read(self) -> dict:
+        """{kernel name: (summed ms, launches)} since the last read (waits for the recorded events)."""
+        n = 16
+        ms, cnt, names = (_d * n)(), (ctypes.c_long * n)(), (ctypes.c_char_p * n)()
+        k = lib().fsei_plan_profile_read(self._h, n, ms, cnt, names)
+        if k < 0:
+            raise FseiError(ERR_CUDA, last_error())
+        return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(k) if cnt[i] > 0}
+
+    def divergence(self, u, v, w, alpha_dt, rhs, stream=None):
+        _chk(lib().fsei_divergence(self._h, _ptr(u), _ptr(v), _ptr(w), float(alpha_dt), _ptr(rhs), _stream(stream)))
+
+    def poisson_solve(self, rhs, phi, stream=None):
+        _chk(lib().fsei_poisson_solve(self._h, _ptr(rhs), _ptr(phi), _stream(stream)))
+
+    def project(self, u, v, w, p, phi, alpha_dt, beta=0.0, stream=None):
+        _chk(lib().fsei_project(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), _ptr(phi), float(alpha_dt), float(beta),
+                                _stream(stream)))
+
+    def pressure_projection(self, u, v, w, p, phi, alpha_dt, beta=0.0, stream=None):
+        _chk(lib().fsei_pressure_projection(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), _ptr(phi), float(alpha_dt),
+                                            float(beta), _stream(stream)))
+
+    def pressure_projection_host(self, u, v, w, p, alpha_dt, beta=0.0, stream=None):
+        """u, v, w, p: HOST float64 arrays/tensors (pinned for speed), updated in place; synchronous."""
+        _chk(lib().fsei_pressure_projection_host(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), float(alpha_dt),
+                                                 float(beta), _stream(stream)))

@@ -1,0 +1,481 @@
+// fsei.cu -- libfsei: kernels and the C ABI of include/fsei.h (sm_100a, fp64).
+//
+// One projection = a1 divergence -> a2 x-forward -> a3 y-forward -> a4 z-tridiagonal (+ gauge
+// column) -> a5 y-inverse -> a6 x-inverse -> a7 projection, all in place in the caller's phi
+// buffer (packed half spectrum: nx/2 complex per row = the bytes of the real row).
+// DESIGN.md sec. 6 describes each kernel, its launch shape and its algorithmic bytes.
+#include <cuda_runtime.h>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/fsei.h"
+#include "plan_host.hpp"
+#include "stencil.cuh"
+#include "xfft.cuh"
+#include "yfft.cuh"
+#include "zsolve.cuh"
+
+using namespace fsei;
+
+// ------------------------------------------------------------------------------------------
+// error state
+// ------------------------------------------------------------------------------------------
+static thread_local std::string g_err;
+static thread_local int g_err_code = FSEI_OK;
+static int fail(int code, const std::string& msg) { g_err = msg; g_err_code = code; return code; }
+static int cuda_fail(cudaError_t e, const char* what)
+{
+    return fail(FSEI_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+
+// ------------------------------------------------------------------------------------------
+// plan
+// ------------------------------------------------------------------------------------------
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, FSEI_NKERNELS };
+
+struct fsei_plan {
+    HostTables T;
+    XParams X; YParams Y; ZParams Z; SParams S;
+    std::vector<void*> owned;          // device allocations freed with the plan
+    size_t bytes = 0;
+    int LX = 1, CY = 1;                // tile shapes
+    size_t smem_x = 0, smem_y = 0;
+    int last_launches = 0;
+    double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
+    // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_pool;      // 2 events per recorded launch
+    std::vector<int> ev_kid;               // kernel id of each recorded launch
+    size_t ev_used = 0;
+    double prof_ms[FSEI_NKERNELS] = {0};
+    long prof_n[FSEI_NKERNELS] = {0};
+};
+
+static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
+                                                   "y_inverse", "x_inverse", "project"};
+
+// record an event pair around one launch when profiling is on
+struct LaunchTimer {
+    fsei_plan* P; cudaStream_t st; bool on;
+    LaunchTimer(fsei_plan* P_, int kid, cudaStream_t st_) : P(P_), st(st_), on(P_->profiling) {
+        if (!on) return;
+        if (P->ev_used + 2 > P->ev_pool.size()) {
+            for (int i = 0; i < 64; i++) { cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; } P->ev_pool.push_back(e); }
+        }
+        P->ev_kid.push_back(kid);
+        cudaEventRecord(P->ev_pool[P->ev_used], st);
+    }
+    ~LaunchTimer() { if (on) { cudaEventRecord(P->ev_pool[P->ev_used + 1], st); P->ev_used += 2; } }
+};
+
+template <class T> static int upload(fsei_plan* P, const std::vector<T>& h, const T** d)
+{
+    void* p = nullptr;
+    size_t n = h.size() * sizeof(T);
+    if (n == 0) { *d = nullptr; return FSEI_OK; }
+    cudaError_t e = cudaMalloc(&p, n);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(FSEI_ERR_ALLOC, std::string("cudaMalloc of a plan table failed: ") + cudaGetErrorString(e)); }
+    P->owned.push_back(p); P->bytes += n;
+    CU(cudaMemcpy(p, h.data(), n, cudaMemcpyHostToDevice));
+    *d = static_cast<const T*>(p);
+    return FSEI_OK;
+}
+static int dalloc(fsei_plan* P, size_t n, void** d)
+{
+    cudaError_t e = cudaMalloc(d, n);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(FSEI_ERR_ALLOC, std::string("cudaMalloc of plan workspace failed: ") + cudaGetErrorString(e)); }
+    P->owned.push_back(*d); P->bytes += n;
+    return FSEI_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// kernels
+// ------------------------------------------------------------------------------------------
+#define NT 256
+
+__global__ void __launch_bounds__(NT) k_divergence(SParams S, const double* __restrict__ u, const double* __restrict__ v,
+                                                   const double* __restrict__ w, double inv_adt, double* __restrict__ rhs)
+{
+    const size_t n = (size_t)S.nx * S.ny * S.nz;
+    for (size_t c = (size_t)blockIdx.x * NT + threadIdx.x; c < n; c += (size_t)gridDim.x * NT) {
+        int i = (int)(c % S.nx); size_t r = c / S.nx; int j = (int)(r % S.ny), k = (int)(r / S.ny);
+        rhs[c] = div_at(S, u, v, w, i, j, k, inv_adt);
+    }
+}
+
+__global__ void __launch_bounds__(NT) k_project(SParams S, double* __restrict__ u, double* __restrict__ v, double* __restrict__ w,
+                                                double* __restrict__ p, const double* __restrict__ phi, double adt, double beta)
+{
+    const size_t n = (size_t)S.nx * S.ny * S.nz;
+    for (size_t c = (size_t)blockIdx.x * NT + threadIdx.x; c < n; c += (size_t)gridDim.x * NT) {
+        int i = (int)(c % S.nx); size_t r = c / S.nx; int j = (int)(r % S.ny), k = (int)(r / S.ny);
+        project_at(S, u, v, w, p, phi, i, j, k, adt, beta);
+    }
+}
+
+template <bool INV> __device__ __forceinline__ void x_all_passes(const XParams& X, cplx* sm, int lines)
+{
+    int Ns[8]; int n = X.N;
+#pragma unroll
+    for (int s = 0; s < 8; s++) { Ns[s] = n; if (s < X.f.npass) n /= X.f.radix[s]; }
+    for (int i = 0; i < X.f.npass; i++) {
+        int s = INV ? X.f.npass - 1 - i : i;
+        x_pass_dispatch<INV>(X, sm, lines, X.f.radix[s], Ns[s], threadIdx.x, NT);
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(NT) k_x_forward(XParams X, const double* src, cplx* dst, long nlines, int LX)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    cplx* sm = reinterpret_cast<cplx*>(smraw);
+    long l0 = (long)blockIdx.x * LX;
+    int lines = (int)((nlines - l0 < LX) ? nlines - l0 : LX);
+    x_load_real(X, sm, src + (size_t)l0 * X.n, lines, threadIdx.x, NT);
+    __syncthreads();
+    x_all_passes<false>(X, sm, lines);
+    x_post_forward(X, sm, lines, threadIdx.x, NT);
+    __syncthreads();
+    x_store_spec(X, sm, dst + (size_t)l0 * X.N, lines, threadIdx.x, NT);
+}
+
+__global__ void __launch_bounds__(NT) k_x_inverse(XParams X, const cplx* src, double* dst, long nlines, int LX)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    cplx* sm = reinterpret_cast<cplx*>(smraw);
+    long l0 = (long)blockIdx.x * LX;
+    int lines = (int)((nlines - l0 < LX) ? nlines - l0 : LX);
+    x_load_spec(X, sm, src + (size_t)l0 * X.N, lines, threadIdx.x, NT);
+    __syncthreads();
+    x_pre_inverse(X, sm, lines, threadIdx.x, NT);
+    __syncthreads();
+    x_all_passes<true>(X, sm, lines);
+    x_store_real(X, sm, dst + (size_t)l0 * X.n, lines, threadIdx.x, NT);
+}
+
+template <bool INV, bool NEU> __device__ __forceinline__ void y_all_passes(const YParams& Y, cplx* sm, int C)
+{
+    int Ns[8]; int n = Y.N;
+#pragma unroll
+    for (int s = 0; s < 8; s++) { Ns[s] = n; if (s < Y.f.npass) n /= Y.f.radix[s]; }
+    for (int i = 0; i < Y.f.npass; i++) {
+        int s = INV ? Y.f.npass - 1 - i : i;
+        y_pass_dispatch<INV, NEU>(Y, sm, C, Y.f.radix[s], Ns[s], threadIdx.x, NT);
+        __syncthreads();
+    }
+}
+
+// grid (nxc / C, nz): one tile = C adjacent slots of every row of one z-plane
+template <bool INV, bool NEU>
+__global__ void __launch_bounds__(NT) k_y_transform(YParams Y, cplx* spec, int nxc, int C)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    cplx* sm = reinterpret_cast<cplx*>(smraw);
+    cplx* g = spec + (size_t)blockIdx.y * Y.N * nxc + (size_t)blockIdx.x * C;
+    y_load(sm, g, nxc, Y.N, C, threadIdx.x, NT);
+    __syncthreads();
+    if (INV && NEU) { y_pre_inverse_dct(Y, sm, C, threadIdx.x, NT); __syncthreads(); }
+    y_all_passes<INV, NEU>(Y, sm, C);
+    if (!INV && NEU) { y_post_forward_dct(Y, sm, C, threadIdx.x, NT); __syncthreads(); }
+    y_store(sm, g, nxc, Y.N, C, threadIdx.x, NT);
+}
+
+__global__ void __launch_bounds__(NT) k_z_factor(ZParams Z, double* ipiv, int paired_slot0)
+{
+    size_t t = (size_t)blockIdx.x * NT + threadIdx.x;
+    size_t n = (size_t)Z.ny * Z.nxc * Z.ncomp;
+    if (t >= n) return;
+    int comp = (int)(t % Z.ncomp); size_t r = t / Z.ncomp; int slot = (int)(r % Z.nxc), row = (int)(r / Z.nxc);
+    bool zero = (row == 0 && slot == 0 && comp == 0) || (paired_slot0 && slot == 0);
+    z_factor_column(Z, ipiv, row, slot, comp, zero);
+}
+
+// slots [slot0, nxc) of every row, slot fastest across the warp (coalesced 16-byte accesses)
+template <int NCOMP>
+__global__ void __launch_bounds__(128) k_z_direct(ZParams Z, cplx* spec, int slot0)
+{
+    const int ns = Z.nxc - slot0;
+    size_t t = (size_t)blockIdx.x * 128 + threadIdx.x;
+    if (t >= (size_t)ns * Z.ny) return;
+    int slot = slot0 + (int)(t % ns), row = (int)(t / ns);
+    z_direct_column<NCOMP>(Z, spec, row, slot, row == 0 && slot == 0);
+}
+
+// pairs (slot, q): slot fastest
+__global__ void __launch_bounds__(128) k_z_paired(ZParams Z, cplx* spec, int nslots)
+{
+    size_t npairs = (size_t)(Z.ny / 2 + 1) * nslots;
+    size_t t = (size_t)blockIdx.x * 128 + threadIdx.x;
+    if (t >= npairs) return;
+    int slot = (int)(t % nslots), q = (int)(t / nslots);
+    z_paired_column(Z, spec, slot, q, t, npairs);
+}
+
+// the (0,0) column: gather it, solve it (thread 0, in shared memory), leave it in Z.gauge
+__global__ void __launch_bounds__(NT) k_z_gauge(ZParams Z, const cplx* spec, double* gauge)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    double* d = reinterpret_cast<double*>(smraw);
+    double* x = d + Z.nz;
+    for (int k = threadIdx.x; k < Z.nz; k += NT) d[k] = spec[zidx(Z, k, 0, 0)].re;
+    __syncthreads();
+    if (threadIdx.x == 0) z_gauge_serial(Z, d, x);
+    __syncthreads();
+    for (int k = threadIdx.x; k < Z.nz; k += NT) gauge[k] = x[k];
+}
+
+// ------------------------------------------------------------------------------------------
+// plan creation
+// ------------------------------------------------------------------------------------------
+static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy)
+{
+    int code = 0;
+    std::string msg = build_tables(P->T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code);
+    if (code) return fail(code, msg);
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FSEI_ERR_CUDA, "no CUDA device: libfsei has no CPU fallback"); }
+
+    HostTables& T = P->T;
+    int rc;
+    XParams& X = P->X; YParams& Y = P->Y; ZParams& Z = P->Z; SParams& S = P->S;
+    X.n = nx; X.N = nx / 2; X.bc = bcx; X.pitch = padx(nx / 2) + 1; X.f = T.fx; X.scale = T.scale;
+    if ((rc = upload(P, T.twx, &X.tw))) return rc;
+    if ((rc = upload(P, T.posx, &X.pos))) return rc;
+    if ((rc = upload(P, T.twx_r2c, &X.tw_r2c))) return rc;
+    if ((rc = upload(P, T.twx_dct, &X.tw_dct))) return rc;
+    Y.N = ny; Y.bc = bcy; Y.f = T.fy;
+    if ((rc = upload(P, T.twy, &Y.tw))) return rc;
+    if ((rc = upload(P, T.posy, &Y.pos))) return rc;
+    if ((rc = upload(P, T.twy_dct, &Y.tw_dct))) return rc;
+    Z.nxc = T.nxc; Z.ny = ny; Z.nz = nz; Z.ncomp = T.ncomp; Z.posy = Y.pos;
+    if ((rc = upload(P, T.za, &Z.za))) return rc;
+    if ((rc = upload(P, T.zcc, &Z.zcc))) return rc;
+    if ((rc = upload(P, T.dzc, &Z.dzc))) return rc;
+    if ((rc = upload(P, T.dzm, &Z.dzm))) return rc;
+    if ((rc = upload(P, T.lamx, &Z.lamx))) return rc;
+    if ((rc = upload(P, T.lamy, &Z.lamy))) return rc;
+    S.nx = nx; S.ny = ny; S.nz = nz; S.bcx = bcx; S.bcy = bcy; S.rdx = T.rdx; S.rdy = T.rdy;
+    if ((rc = upload(P, T.rdzc, &S.rdzc))) return rc;
+    if ((rc = upload(P, T.rdzm, &S.rdzm))) return rc;
+
+    void* g = nullptr;
+    if ((rc = dalloc(P, sizeof(double) * nz, &g))) return rc;
+    Z.gauge = static_cast<const double*>(g);
+    const size_t npairs = (size_t)(ny / 2 + 1) * (T.paired_all ? T.nxc : 1);
+    if (T.paired_all || T.paired_slot0) {
+        void* c = nullptr;
+        if ((rc = dalloc(P, sizeof(double) * 2 * npairs * nz, &c))) return rc;
+        Z.cpw = static_cast<double*>(c);
+    } else Z.cpw = nullptr;
+    Z.ipiv = nullptr;
+    if (!T.paired_all) {
+        void* ip = nullptr;
+        size_t n = (size_t)nz * ny * T.nxc * T.ncomp;
+        if ((rc = dalloc(P, sizeof(double) * n, &ip))) return rc;
+        Z.ipiv = static_cast<const double*>(ip);
+        size_t cols = (size_t)ny * T.nxc * T.ncomp;
+        k_z_factor<<<(unsigned)((cols + NT - 1) / NT), NT>>>(Z, static_cast<double*>(ip), T.paired_slot0 ? 1 : 0);
+        CU(cudaGetLastError());
+        CU(cudaDeviceSynchronize());
+    }
+
+    // tile shapes
+    size_t line_bytes = (size_t)X.pitch * sizeof(cplx);
+    int LX = (int)(32768 / line_bytes); if (LX < 1) LX = 1; if (LX > 32) LX = 32;
+    P->LX = LX; P->smem_x = LX * line_bytes;
+    int CY = 1;
+    for (int c = 8; c >= 1; c /= 2)
+        if (T.nxc % c == 0 && (size_t)ny * c * sizeof(cplx) <= 65536) { CY = c; break; }
+    if ((size_t)ny * CY * sizeof(cplx) > 200 * 1024) return fail(FSEI_ERR_SIZE, "ny too large for the shared-memory y tile");
+    P->CY = CY; P->smem_y = (size_t)ny * CY * sizeof(cplx);
+    CU(cudaFuncSetAttribute(k_z_gauge, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * sizeof(double) * nz)));
+    CU(cudaFuncSetAttribute(k_x_forward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_x));
+    CU(cudaFuncSetAttribute(k_x_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_x));
+    CU(cudaFuncSetAttribute(k_y_transform<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
+    CU(cudaFuncSetAttribute(k_y_transform<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
+    CU(cudaFuncSetAttribute(k_y_transform<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
+    CU(cudaFuncSetAttribute(k_y_transform<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
+    return FSEI_OK;
+}
+
+extern "C" fsei_plan* fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bc_x, int bc_y)
+{
+    fsei_plan* P = new (std::nothrow) fsei_plan();
+    if (!P) { fail(FSEI_ERR_ALLOC, "out of host memory"); return nullptr; }
+    int rc = plan_build(P, nx, ny, nz, Lx, Ly, zc, bc_x, bc_y);
+    if (rc != FSEI_OK) { fsei_plan_destroy(P); g_err_code = rc; return nullptr; }
+    g_err_code = FSEI_OK; g_err.clear();
+    return P;
+}
+
+extern "C" void fsei_plan_destroy(fsei_plan* P)
+{
+    if (!P) return;
+    for (void* p : P->owned) cudaFree(p);
+    for (double* p : P->hostpath) if (p) cudaFree(p);
+    for (cudaEvent_t e : P->ev_pool) cudaEventDestroy(e);
+    delete P;
+}
+
+extern "C" const char* fsei_last_error(void) { return g_err.c_str(); }
+extern "C" int fsei_last_error_code(void) { return g_err_code; }
+extern "C" size_t fsei_plan_workspace_bytes(const fsei_plan* P) { return P ? P->bytes : 0; }
+extern "C" int fsei_plan_last_launch_count(const fsei_plan* P) { return P ? P->last_launches : 0; }
+
+// ------------------------------------------------------------------------------------------
+// the calls
+// ------------------------------------------------------------------------------------------
+static unsigned stencil_grid(size_t n)
+{
+    size_t b = (n + NT - 1) / NT;
+    const size_t cap = 148 * 8 * 16;
+    return (unsigned)(b < cap ? b : cap);
+}
+
+extern "C" int fsei_divergence(fsei_plan* P, const double* u, const double* v, const double* w, double alpha_dt,
+                               double* rhs, void* cuda_stream)
+{
+    if (!P || !u || !v || !w || !rhs) return fail(FSEI_ERR_ARG, "fsei_divergence: NULL argument");
+    if (alpha_dt == 0.0 || alpha_dt != alpha_dt) return fail(FSEI_ERR_ARG, "fsei_divergence: alpha_dt must be non-zero");
+    if (rhs == u || rhs == v || rhs == w) return fail(FSEI_ERR_ARG, "fsei_divergence: rhs must not alias u, v, w");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
+    { LaunchTimer t(P, K_DIV, st); k_divergence<<<stencil_grid(n), NT, 0, st>>>(P->S, u, v, w, 1.0 / alpha_dt, rhs); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, void* cuda_stream)
+{
+    if (!P || !rhs || !phi) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: NULL argument");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const HostTables& T = P->T;
+    const long nlines = (long)T.ny * T.nz;
+    cplx* spec = reinterpret_cast<cplx*>(phi);
+    int launches = 0;
+    unsigned gx = (unsigned)((nlines + P->LX - 1) / P->LX);
+    { LaunchTimer t(P, K_XF, st); k_x_forward<<<gx, NT, P->smem_x, st>>>(P->X, rhs, spec, nlines, P->LX); launches++; }
+    CU(cudaGetLastError());
+    dim3 gy(T.nxc / P->CY, T.nz);
+    {
+        LaunchTimer t(P, K_YF, st);
+        if (T.bcy == BC_NEUMANN) k_y_transform<false, true><<<gy, NT, P->smem_y, st>>>(P->Y, spec, T.nxc, P->CY);
+        else k_y_transform<false, false><<<gy, NT, P->smem_y, st>>>(P->Y, spec, T.nxc, P->CY);
+        launches++;
+    }
+    CU(cudaGetLastError());
+    { LaunchTimer t(P, K_GAUGE, st); k_z_gauge<<<1, NT, 2 * sizeof(double) * T.nz, st>>>(P->Z, spec, const_cast<double*>(P->Z.gauge)); launches++; }
+    CU(cudaGetLastError());
+    if (T.paired_all) {
+        size_t np = (size_t)(T.ny / 2 + 1) * T.nxc;
+        LaunchTimer t(P, K_ZP, st);
+        k_z_paired<<<(unsigned)((np + 127) / 128), 128, 0, st>>>(P->Z, spec, T.nxc); launches++;
+    } else {
+        int s0 = T.paired_slot0 ? 1 : 0;
+        size_t nthr = (size_t)(T.nxc - s0) * T.ny;
+        {
+            LaunchTimer t(P, K_ZD, st);
+            if (T.ncomp == 1) k_z_direct<1><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->Z, spec, s0);
+            else k_z_direct<2><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->Z, spec, s0);
+            launches++;
+        }
+        CU(cudaGetLastError());
+        if (T.paired_slot0) {
+            size_t np = (size_t)(T.ny / 2 + 1);
+            LaunchTimer t(P, K_ZP, st);
+            k_z_paired<<<(unsigned)((np + 127) / 128), 128, 0, st>>>(P->Z, spec, 1); launches++;
+        }
+    }
+    CU(cudaGetLastError());
+    {
+        LaunchTimer t(P, K_YI, st);
+        if (T.bcy == BC_NEUMANN) k_y_transform<true, true><<<gy, NT, P->smem_y, st>>>(P->Y, spec, T.nxc, P->CY);
+        else k_y_transform<true, false><<<gy, NT, P->smem_y, st>>>(P->Y, spec, T.nxc, P->CY);
+        launches++;
+    }
+    CU(cudaGetLastError());
+    { LaunchTimer t(P, K_XI, st); k_x_inverse<<<gx, NT, P->smem_x, st>>>(P->X, spec, phi, nlines, P->LX); launches++; }
+    CU(cudaGetLastError());
+    P->last_launches = launches;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_project(fsei_plan* P, double* u, double* v, double* w, double* p, const double* phi,
+                            double alpha_dt, double beta, void* cuda_stream)
+{
+    if (!P || !u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_project: NULL argument");
+    if (alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_project: NaN parameter");
+    if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_project: phi must not alias u, v, w, p");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
+    { LaunchTimer t(P, K_PROJ, st); k_project<<<(unsigned)((n + NT - 1) / NT), NT, 0, st>>>(P->S, u, v, w, p, phi, alpha_dt, beta); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, double* w, double* p, double* phi,
+                                        double alpha_dt, double beta, void* cuda_stream)
+{
+    int rc, n = 0;
+    if ((rc = fsei_divergence(P, u, v, w, alpha_dt, phi, cuda_stream))) return rc;
+    n += P->last_launches;
+    if ((rc = fsei_poisson_solve(P, phi, phi, cuda_stream))) return rc;
+    n += P->last_launches;
+    if ((rc = fsei_project(P, u, v, w, p, phi, alpha_dt, beta, cuda_stream))) return rc;
+    n += P->last_launches;
+    P->last_launches = n;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_pressure_projection_host(fsei_plan* P, double* u, double* v, double* w, double* p,
+                                             double alpha_dt, double beta, void* cuda_stream)
+{
+    if (!P || !u || !v || !w || !p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection_host: NULL argument");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t bytes = sizeof(double) * (size_t)P->T.nx * P->T.ny * P->T.nz;
+    for (int f = 0; f < 5; f++)
+        if (!P->hostpath[f]) {
+            cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&P->hostpath[f]), bytes);
+            if (e != cudaSuccess) { cudaGetLastError(); P->hostpath[f] = nullptr; return fail(FSEI_ERR_ALLOC, "cudaMalloc of a device field failed"); }
+        }
+    double* h[4] = {u, v, w, p};
+    for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(P->hostpath[f], h[f], bytes, cudaMemcpyHostToDevice, st));
+    int rc = fsei_pressure_projection(P, P->hostpath[0], P->hostpath[1], P->hostpath[2], P->hostpath[3], P->hostpath[4],
+                                      alpha_dt, beta, cuda_stream);
+    if (rc) return rc;
+    for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(h[f], P->hostpath[f], bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return FSEI_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// per-kernel timing
+// ------------------------------------------------------------------------------------------
+extern "C" int fsei_plan_profile(fsei_plan* P, int enable)
+{
+    if (!P) return fail(FSEI_ERR_ARG, "fsei_plan_profile: NULL plan");
+    P->profiling = enable != 0;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_plan_profile_read(fsei_plan* P, int max_kernels, double* ms_sum, long* count, const char** names)
+{
+    if (!P || !ms_sum || !count) return fail(FSEI_ERR_ARG, "fsei_plan_profile_read: NULL argument");
+    for (size_t i = 0; i < P->ev_kid.size(); i++) {
+        CU(cudaEventSynchronize(P->ev_pool[2 * i + 1]));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, P->ev_pool[2 * i], P->ev_pool[2 * i + 1]));
+        P->prof_ms[P->ev_kid[i]] += ms; P->prof_n[P->ev_kid[i]]++;
+    }
+    P->ev_kid.clear(); P->ev_used = 0;
+    int n = max_kernels < FSEI_NKERNELS ? max_kernels : FSEI_NKERNELS;
+    for (int k = 0; k < n; k++) { ms_sum[k] = P->prof_ms[k]; count[k] = P->prof_n[k]; if (names) names[k] = k_names[k]; P->prof_ms[k] = 0; P->prof_n[k] = 0; }
+    return n;
+}

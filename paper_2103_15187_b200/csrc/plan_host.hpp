@@ -70,7 +70,7 @@ inline std::string build_tables(HostTables& T, int nx, int ny, int nz, double Lx
     if (nx < 4 || ny < 4 || nx > 8192 || ny > 8192 || nx % 4 != 0 || ny % 2 != 0 || !is_2a3b(nx) || !is_2a3b(ny)) {
         code = 2; return "nx must be a multiple of 4, ny even, both of the form 2^a 3^b in [4, 8192]";
     }
-    if (nz < 2 || nz > 16384) { code = 2; return "nz must be in [2, 16384]"; }
+    if (nz < 2 || nz > 8192) { code = 2; return "nz must be in [2, 8192]"; }
     if (!(Lx > 0) || !(Ly > 0) || !std::isfinite(Lx) || !std::isfinite(Ly)) { code = 3; return "Lx, Ly must be positive and finite"; }
     for (int k = 0; k <= nz; k++) if (!std::isfinite(zc[k])) { code = 3; return "zc holds a non-finite value"; }
     for (int k = 0; k < nz; k++) if (!(zc[k + 1] > zc[k])) { code = 3; return "zc must be strictly increasing"; }

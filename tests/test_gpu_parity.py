@@ -1,0 +1,239 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI of libfsei.so, against
+the long-double CPU oracle on the same seeded inputs.
+
+Gates (BASELINE.json north_star):
+  * stencil steps a1, a7: BIT-EXACT (both sides round every operation in the same fixed order, R20)
+  * phi: relative L2 <= 1e-11 against the long-double oracle
+  * post-projection divergence: max|D u_new| <= max(1e-10, 4 eps ||L||_inf alpha_dt ||phi||_inf)  (R17)
+    and <= 4x the fp64 oracle's own figure
+"""
+import numpy as np
+import pytest
+
+from paper_2103_15187_b200 import inputs
+from tests.util import div_gate, gpu_projection, oracle_projection, rel_l2
+
+pytestmark = pytest.mark.gpu
+P, N = 0, 1
+PHI_TOL = 1e-11
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _post_div(orc, case, u, v, w):
+    """max |D u_new| (unscaled) evaluated by the oracle's divergence with alpha_dt = 1."""
+    return float(np.abs(orc.divergence(case.grid, u, v, w, 1.0)).max())
+
+
+# ---------------------------------------------------------------------------------------------
+# stencil steps: bit-exact
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(8, 8, 8), (36, 20, 9), (64, 48, 33), (256, 8, 5)])
+def test_divergence_bit_exact(oracle_ld, bc, shape):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    case = inputs.make_case(1, shape=shape, bc=bc)
+    plan = Plan.from_grid(case.grid)
+    u, v, w = (torch.from_numpy(a).cuda() for a in (case.u, case.v, case.w))
+    rhs = torch.empty_like(u)
+    plan.divergence(u, v, w, case.alpha_dt, rhs)
+    torch.cuda.synchronize()
+    ref = oracle_ld.divergence(case.grid, case.u, case.v, case.w, case.alpha_dt)
+    assert np.array_equal(rhs.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("beta", [0.0, 2.5e-4])
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(8, 8, 8), (36, 20, 9), (64, 48, 33)])
+def test_project_bit_exact(oracle_ld, bc, shape, beta):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    case = inputs.make_case(1, shape=shape, bc=bc)
+    nz, ny, nx = case.u.shape
+    phi = inputs.normal_field(77, 0, (nz, ny, nx))
+    p0 = inputs.normal_field(77, 1, (nz, ny, nx))
+    plan = Plan.from_grid(case.grid)
+    u, v, w, p, ph = (torch.from_numpy(a.copy()).cuda() for a in (case.u, case.v, case.w, p0, phi))
+    plan.project(u, v, w, p, ph, case.alpha_dt, beta)
+    torch.cuda.synchronize()
+    uo, vo, wo, po = case.u.copy(), case.v.copy(), case.w.copy(), p0.copy()
+    oracle_ld.project(case.grid, uo, vo, wo, po, phi, case.alpha_dt, beta)
+    for g, r in zip((u, v, w, p), (uo, vo, wo, po)):
+        assert np.array_equal(g.cpu().numpy(), r)
+
+
+# ---------------------------------------------------------------------------------------------
+# Poisson solve and whole projection: small and ragged shapes, every bc combination
+# ---------------------------------------------------------------------------------------------
+SHAPES = [(8, 8, 8), (16, 12, 10), (32, 32, 32), (48, 24, 20), (12, 36, 7), (64, 16, 5), (96, 72, 40), (128, 64, 64)]
+
+
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_projection_small(oracle_ld, oracle_d, bc, shape):
+    for cfg, beta in ((1, 0.0), (2, 1e-4)):
+        case = inputs.make_case(cfg, shape=shape, bc=bc)
+        got = gpu_projection(case, beta)
+        ref = oracle_projection(oracle_ld, case, beta)
+        assert rel_l2(got[4], ref[4]) <= PHI_TOL
+        for g, r in zip(got[:4], ref[:4]):
+            assert np.abs(g - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
+        pd = _post_div(oracle_ld, case, *got[:3])
+        assert pd <= div_gate(case, np.abs(got[4]).max())
+
+
+def test_split_calls_equal_fused_call(oracle_ld):
+    case = inputs.make_case(1)
+    a = gpu_projection(case, split=True)
+    b = gpu_projection(case, split=False)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_poisson_out_of_place_and_manufactured(oracle_ld):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    grid = inputs.make_grid(3, shape=(64, 32, 48))
+    nx, ny, nz = grid[:3]
+    phi_true = inputs.normal_field(5, 0, (nz, ny, nx))
+    dzc = np.diff(grid[5])[:, None, None]
+    phi_true -= (phi_true * dzc).sum() / (dzc.sum() * nx * ny)
+    rhs = oracle_ld.laplacian(grid, phi_true)
+    plan = Plan.from_grid(grid)
+    r = torch.from_numpy(rhs).cuda()
+    out = torch.empty_like(r)
+    plan.poisson_solve(r, out)
+    torch.cuda.synchronize()
+    assert np.array_equal(r.cpu().numpy(), rhs)                     # rhs untouched when phi != rhs
+    assert rel_l2(out.cpu().numpy(), phi_true) <= 1e-11
+    assert rel_l2(out.cpu().numpy(), oracle_ld.poisson_solve(grid, rhs)) <= PHI_TOL
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs (full size where the oracle finishes in reasonable time, else the same
+# recipe and z-grid at reduced x,y extents -- the z-grid sets the conditioning)
+# ---------------------------------------------------------------------------------------------
+def _check_config(orc_ld, orc_d, case, beta=0.0):
+    got = gpu_projection(case, beta)
+    ref = oracle_projection(orc_ld, case, beta)
+    rel = rel_l2(got[4], ref[4])
+    pd = _post_div(orc_ld, case, *got[:3])
+    refd = oracle_projection(orc_d, case, beta)
+    pd_oracle64 = _post_div(orc_ld, case, *refd[:3])
+    gate = div_gate(case, np.abs(got[4]).max())
+    print(f"cfg {case.cfg} {case.nx}x{case.ny}x{case.nz}: phi relL2 {rel:.2e}  post-div {pd:.2e} "
+          f"(gate {gate:.2e}, fp64 oracle {pd_oracle64:.2e})")
+    assert rel <= PHI_TOL
+    assert pd <= gate and pd <= 4 * max(pd_oracle64, 1e-300)
+    return got
+
+
+def test_config1_full(oracle_ld, oracle_d):
+    _check_config(oracle_ld, oracle_d, inputs.make_case(1))
+
+
+def test_config2_full(oracle_ld, oracle_d):
+    _check_config(oracle_ld, oracle_d, inputs.make_case(2))
+
+
+def test_config3_three_substeps_reduced(oracle_ld, oracle_d):
+    """three provisional triples, one shared p, three projections enqueued back to back (R14)"""
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    shape = (128, 128, 384)
+    cases = [inputs.make_case(3, shape=shape, substep=s) for s in range(3)]
+    plan = Plan.from_grid(cases[0].grid)
+    p = torch.zeros(cases[0].u.shape, dtype=torch.float64, device="cuda")
+    phi = torch.empty_like(p)
+    dev = [[torch.from_numpy(a).cuda() for a in (c.u, c.v, c.w)] for c in cases]
+    for c, (u, v, w) in zip(cases, dev):
+        plan.pressure_projection(u, v, w, p, phi, c.alpha_dt, 0.0)      # no host sync in between
+    torch.cuda.synchronize()
+    po = np.zeros(cases[0].u.shape)
+    for c, (u, v, w) in zip(cases, dev):
+        ref = oracle_projection(oracle_ld, c, 0.0, p=po)
+        assert np.abs(u.cpu().numpy() - ref[0]).max() <= 1e-10 * np.abs(ref[0]).max()
+        pd = _post_div(oracle_ld, c, u.cpu().numpy(), v.cpu().numpy(), w.cpu().numpy())
+        assert pd <= div_gate(c, np.abs(ref[4]).max())
+    assert rel_l2(p.cpu().numpy(), po) <= PHI_TOL
+    assert rel_l2(phi.cpu().numpy(), ref[4]) <= PHI_TOL
+
+
+def test_config3_full_single_substep(oracle_ld, oracle_d):
+    _check_config(oracle_ld, oracle_d, inputs.make_case(3, shape=(512, 512, 96)))
+
+
+def test_config4_reduced(oracle_ld, oracle_d):
+    _check_config(oracle_ld, oracle_d, inputs.make_case(4, shape=(128, 128, 768)))
+    _check_config(oracle_ld, oracle_d, inputs.make_case(4, shape=(1024, 64, 48)))     # full x length
+    _check_config(oracle_ld, oracle_d, inputs.make_case(4, shape=(64, 1024, 48)))     # full y length
+
+
+def test_config5_reduced(oracle_ld, oracle_d):
+    _check_config(oracle_ld, oracle_d, inputs.make_case(5, shape=(96, 96, 1024)))
+    _check_config(oracle_ld, oracle_d, inputs.make_case(5, shape=(768, 48, 64)))      # full x length, DCT
+    _check_config(oracle_ld, oracle_d, inputs.make_case(5, shape=(48, 768, 64)))      # full y length, DCT
+
+
+# ---------------------------------------------------------------------------------------------
+# degenerate and edge cases
+# ---------------------------------------------------------------------------------------------
+def test_zero_input_and_solenoidal_input(oracle_ld):
+    case = inputs.make_case(1, shape=(16, 16, 8))
+    case.u[:] = 0; case.v[:] = 0; case.w[:] = 0
+    got = gpu_projection(case)
+    assert all(np.all(g == 0) for g in got)
+    # constant (u, v) with w = 0 is discretely solenoidal on the periodic box: phi = 0, field unchanged
+    case.u[:] = 1.5; case.v[:] = -0.25
+    got = gpu_projection(case)
+    assert np.abs(got[4]).max() <= 1e-12 and np.abs(got[0] - 1.5).max() <= 1e-14
+
+
+def test_minimum_sizes(oracle_ld):
+    for shape, bc in (((4, 4, 2), (P, P)), ((4, 4, 2), (N, N)), ((4, 6, 3), (P, N)), ((12, 4, 2), (N, P))):
+        case = inputs.make_case(1, shape=shape, bc=bc)
+        got = gpu_projection(case)
+        ref = oracle_projection(oracle_ld, case)
+        assert rel_l2(got[4], ref[4]) <= PHI_TOL
+
+
+def test_gauge_volume_weighted_zero_mean():
+    case = inputs.make_case(2, shape=(64, 64, 96))
+    got = gpu_projection(case)
+    dzc = np.diff(case.zc)[:, None, None]
+    assert abs((got[4] * dzc).sum()) <= 1e-13 * (np.abs(got[4]) * dzc).sum() * np.sqrt(got[4].size)
+
+
+def test_runtime_argument_errors():
+    torch = _torch()
+    from paper_2103_15187_b200 import binding
+    case = inputs.make_case(1, shape=(8, 8, 8))
+    plan = binding.Plan.from_grid(case.grid)
+    u = torch.zeros(case.u.shape, dtype=torch.float64, device="cuda")
+    with pytest.raises(binding.FseiError) as e:
+        plan.divergence(u, u, u, 0.0, torch.empty_like(u))
+    assert e.value.code == binding.ERR_ARG
+    with pytest.raises(binding.FseiError) as e:
+        plan.divergence(u, u, u, 1e-3, u)                       # rhs aliases an input
+    assert e.value.code == binding.ERR_ARG
+    with pytest.raises(binding.FseiError) as e:
+        plan.project(u, u, u, u, u, 1e-3)                       # phi aliases an output
+    assert e.value.code == binding.ERR_ARG
+    assert plan.workspace_bytes > 0
+
+
+def test_host_buffer_entry(oracle_ld):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    case = inputs.make_case(1)
+    plan = Plan.from_grid(case.grid)
+    h = [torch.from_numpy(a.copy()).pin_memory() for a in (case.u, case.v, case.w, np.zeros_like(case.u))]
+    plan.pressure_projection_host(*h, case.alpha_dt, 0.0)
+    ref = gpu_projection(case)
+    for a, b in zip(h, ref[:4]):
+        assert np.array_equal(a.numpy(), b)
