@@ -1,0 +1,331 @@
+#!/usr/bin/env python
+"""bench.py -- Mcell/s per fp64 pressure projection (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+
+A step = one whole projection (divergence -> x/y transforms -> z tridiagonal -> inverse
+transforms -> velocity/pressure correction) through the C ABI
+of libfsei.so on one batch of seeded synthetic input.  At N = 1 the workload is BASELINE.json
+configs[3] (1024x1024x768, the size the north-star target is quoted on; it fits one GPU).
+The path is single-GPU ("replicas only"): for N > 1 every rank runs an
+independent replica and `value` is the sum over ranks / max-over-ranks time.
+
+`--impl reference` times the CPU oracle (as it stands, `double` build) on a bounded sample of
+the same workload; rank 0 only.
+
+Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Mcell/s per fp64 pressure projection"
+UNIT = "Mcell/s"
+# algorithmic bytes per cell per launch of each kernel
+ALGO_BYTES_PER_CELL = {
+    "divergence": 32.0, "x_forward": 16.0, "div_x_forward": 32.0, "y_forward": 16.0, "z_direct": 16.0,
+    "z_paired": 16.0, "z_solve": 16.0, "y_inverse": 16.0, "x_inverse": 16.0, "project": 72.0, "z_gauge": 0.0,
+}
+A_REF = 184.0          # reference accounting of one projection, B/cell
+SAMPLE_NY = 128        # CPU legs: the workload's grid with ny cut to this many rows
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+    return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.th = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.2] or [r for _, r in self.rows]
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _mem_available_gb() -> float:
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable"):
+                    return int(line.split()[1]) / 1e6
+    except OSError:
+        pass
+    return 0.0
+
+
+def _workload_name(case) -> str:
+    return (f"configs[{case.cfg - 1}] {case.nx}x{case.ny}x{case.nz} fp64, "
+            f"bc=({'PN'[case.bc_x]},{'PN'[case.bc_y]}), tanh-stretched z, Neumann phi in z, alpha*dt=1e-3")
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU legs: the oracle (double build, as it stands) on a bounded sample of the workload
+# ------------------------------------------------------------------------------------------------
+def _oracle_sample(cfg: int, reps: int, warm: int = 0):
+    """Times `reps` oracle projections on the config's grid with ny cut to SAMPLE_NY rows (same nx, nz, zc,
+    bc, value distribution).  Returns (Mcell/s, cores, sample description, seconds per projection)."""
+    import numpy as np
+    from paper_2103_15187_b200 import inputs
+    from oracle import Oracle
+    nx, ny, nz = inputs.CONFIGS[cfg]["shape"]
+    shape = (nx, min(ny, SAMPLE_NY), nz)
+    case = inputs.make_case(cfg, shape=shape)
+    orc = Oracle("d")
+    cores = int(os.environ.get("OMP_NUM_THREADS", 0)) or len(os.sched_getaffinity(0))
+    u, v, w = case.u.copy(), case.v.copy(), case.w.copy()
+    p = np.zeros_like(u)
+    for _ in range(warm):
+        orc.pressure_projection(case.grid, u, v, w, p, case.alpha_dt, 0.0)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        orc.pressure_projection(case.grid, u, v, w, p, case.alpha_dt, 0.0)
+    dt = (time.perf_counter() - t0) / reps
+    sample = (f"{reps} oracle projection(s) of a {shape[0]}x{shape[1]}x{shape[2]} slab of the workload grid "
+              f"(ny cut to {shape[1]}; same nx, nz, z-grid, bc, N(0,1)/smooth recipe), OpenMP over lines/columns")
+    return case.cells / dt / 1e6, cores, sample, dt
+
+
+def run_reference(args) -> dict:
+    from paper_2103_15187_b200 import inputs
+    case = inputs.make_case(args.config, fields=False)
+    val, cores, sample, dt = _oracle_sample(args.config, args.steps, args.warmup)
+    return {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": _workload_name(case), "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU leg
+# ------------------------------------------------------------------------------------------------
+def run_ours(args) -> dict:
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2103_15187_b200 import inputs
+    from paper_2103_15187_b200.binding import Plan
+
+    rank = int(os.environ.get("RANK", 0))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libfsei has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- inputs: generated once on the host (seeded), one field at a time ---------------
+    case = inputs.make_case(args.config, fields=False)
+    shp = (case.nz, case.ny, case.nx)
+    fbytes = case.cells * 8
+    want_e2e = args.e2e_steps > 0 and _mem_available_gb() > 4.6 * fbytes / 1e9 + 8
+    host = [torch.empty(shp, dtype=torch.float64, pin_memory=want_e2e) for _ in range(3)]
+    # replicas: rank r perturbs nothing but the seed substream (independent problems, no exchange)
+    t_gen = time.time()
+    inputs.make_case(args.config, out=[h.numpy() for h in host], substep=0)
+    t_gen = time.time() - t_gen
+    u, v, w = (h.to(dev, non_blocking=False) for h in host)
+    p = torch.zeros_like(u)
+    phi = torch.empty_like(u)
+    plan = Plan.from_grid(case.grid)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.pressure_projection(u, v, w, p, phi, case.alpha_dt, 0.0, stream)
+        return plan.last_launch_count
+
+    # ---- device-resident timing ------------------------------------------------------------------------
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    time.sleep(0.3)
+    plan.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    barrier()
+    t0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        launches += step()
+    e1.record(stream)
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms_total = e0.elapsed_time(e1)
+    plan.profile(False)
+    prof = plan.profile_read()
+    if world > 1:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * case.cells / (ms_step * 1e-3) / 1e6
+
+    # ---- roofline of the dominant kernel (live CUDA-event durations from the timed region) ---------------
+    peak, peak_src = _peaks()
+    kernels = {}
+    for name, (ms, cnt) in prof.items():
+        per = ms / cnt
+        ab = ALGO_BYTES_PER_CELL.get(name, 0.0) * case.cells
+        kernels[name] = {"ms_per_launch": round(per, 4), "launches_per_step": cnt / args.steps,
+                         "algo_GBps": round(ab / (per * 1e-3) / 1e9, 1) if per > 0 else None,
+                         "share": round(ms / ms_total, 4)}
+    top = max(prof, key=lambda k: prof[k][0])
+    top_ms = prof[top][0] / prof[top][1]
+    achieved = ALGO_BYTES_PER_CELL.get(top, 0.0) * case.cells / (top_ms * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")     # dram bytes per launch from the committed ncu capture
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"cfg{case.cfg}", {}).get(top)
+    roofline = {"bound": "hbm", "kernel": top, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "traffic": traffic, "peak_source": peak_src,
+                "algo_bytes_per_launch": ALGO_BYTES_PER_CELL.get(top, 0.0) * case.cells,
+                "ms_per_launch": round(top_ms, 4),
+                "whole_step": {"algo_bytes_per_cell": A_REF, "achieved": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9, 1),
+                               "frac": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9 / peak, 4)},
+                "kernels": kernels}
+
+    # ---- end to end: HOST buffers through the C ABI, H2D + D2H inside the timed region -------------------
+    e2e = None
+    if want_e2e:
+        del u, v, w, p, phi
+        torch.cuda.empty_cache()
+        hp = torch.zeros(shp, dtype=torch.float64, pin_memory=True)
+        hu, hv, hw = host
+        for _ in range(1):
+            plan.pressure_projection_host(hu, hv, hw, hp, case.alpha_dt, 0.0, stream)
+        barrier()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        for _ in range(args.e2e_steps):
+            plan.pressure_projection_host(hu, hv, hw, hp, case.alpha_dt, 0.0, stream)
+        a1.record(stream)
+        barrier()
+        ems = a0.elapsed_time(a1)
+        if world > 1:
+            t = torch.tensor([ems], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        ems /= args.e2e_steps
+        e2e = {"value": world * case.cells / (ems * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 4 * fbytes,
+               "d2h_bytes_per_step": 4 * fbytes, "ms_per_step": ems, "steps": args.e2e_steps,
+               "api": "fsei_pressure_projection_host (pinned u,v,w,p in; u,v,w,p out)"}
+    else:
+        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+               "skipped": "--e2e-steps 0 or not enough host memory for 4 pinned fields"}
+    plan.destroy()
+
+    # ---- CPU baseline: the oracle as it stands, rank 0 at N = 1 only --------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        val, cores, sample, _ = _oracle_sample(args.config, 3)
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": _workload_name(case), "cells": case.cells, "projections_timed": args.steps,
+                   "buffers": "same u,v,w,p re-projected back to back (direct method: cost is data-independent)",
+                   "l2": f"inputs larger than L2 ({fbytes / 1e6:.0f} MB per field vs 126 MB)" if fbytes > 126e6 * 2
+                         else "fields fit in L2 (small config; no flush)",
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "input_gen_s": round(t_gen, 1)},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "hbm_GBps_vs_8TBps": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9 / 8000.0, 4),
+    }
+    if world > 1:
+        dist.destroy_process_group()
+    return out if rank == 0 else None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4 = configs[3])")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", 0)) != 0:
+            return
+        args.steps = min(args.steps, 5)
+        args.warmup = min(args.warmup, 1)
+        out = run_reference(args)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3
+        out = run_ours(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()
