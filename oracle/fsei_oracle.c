@@ -192,20 +192,37 @@ static void thomas(int n, const real_t *a, const real_t *b, const real_t *c,
     for (int k = n - 2; k >= 0; k--) x[k] -= cp[k] * x[k + 1];
 }
 
-/* Wall-normal metric coefficients of L = D G (readings R2, R5):              */
-/*   dzc[k] = zc[k+1]-zc[k]            cell heights, k = 0..nz-1              */
-/*   dzm[k] = zm[k]-zm[k-1]            centre spacings, k = 1..nz-1           */
-/*   a_k = 1/(dzm[k] dzc[k]) (a_0=0),  c_k = 1/(dzm[k+1] dzc[k]) (c_{nz-1}=0) */
+/* Wall-normal metric coefficients of L = D G (readings R2, R5, R20).          */
+/* The metrics are fp64 DATA of the grid, evaluated once in double exactly as  */
+/* the stencils a1 / a7 evaluate them (zmetric_double below):                  */
+/*   dzc[k] = zc[k+1]-zc[k]                     cell heights,   k = 0..nz-1    */
+/*   dzm[k] = (zc[k]+zc[k+1])/2 - (zc[k-1]+zc[k])/2  centre spacings, k >= 1   */
+/*   rdzc = 1/dzc, rdzm = 1/dzm                 (each rounded to double)       */
+/* and L = D G is the product of those very stencils (R5), so                  */
+/*   a_k = rdzm[k] rdzc[k] (a_0 = 0),  c_k = rdzm[k+1] rdzc[k] (c_{nz-1} = 0)  */
+/* with the products (and everything after) in real_t.  Evaluating the metrics */
+/* in real_t instead would solve an operator that differs from the stencils'   */
+/* by up to ulp(zc)/dz ~ 1e-12 near the upper wall and leave a post-projection */
+/* divergence ~30x above the fp64 floor (R5).                        */
 static void zcoef(int nz, const double *zc, real_t *dzc, real_t *dzm, real_t *a, real_t *c)
 {
-    for (int k = 0; k < nz; k++) dzc[k] = (real_t)zc[k + 1] - (real_t)zc[k];
-    dzm[0] = 0;
-    for (int k = 1; k < nz; k++)
-        dzm[k] = ((real_t)zc[k] + (real_t)zc[k + 1]) / 2 - ((real_t)zc[k - 1] + (real_t)zc[k]) / 2;
+    double *rc = malloc(sizeof(double) * nz), *rm = malloc(sizeof(double) * nz);
     for (int k = 0; k < nz; k++) {
-        a[k] = (k > 0) ? 1 / (dzm[k] * dzc[k]) : 0;
-        c[k] = (k < nz - 1) ? 1 / (dzm[k + 1] * dzc[k]) : 0;
+        double hc = zc[k + 1] - zc[k];
+        dzc[k] = (real_t)hc;
+        rc[k] = 1.0 / hc;
     }
+    dzm[0] = 0; rm[0] = 0.0;
+    for (int k = 1; k < nz; k++) {
+        double hm = 0.5 * (zc[k] + zc[k + 1]) - 0.5 * (zc[k - 1] + zc[k]);
+        dzm[k] = (real_t)hm;
+        rm[k] = 1.0 / hm;
+    }
+    for (int k = 0; k < nz; k++) {
+        a[k] = (k > 0) ? (real_t)rm[k] * (real_t)rc[k] : 0;
+        c[k] = (k < nz - 1) ? (real_t)rm[k + 1] * (real_t)rc[k] : 0;
+    }
+    free(rc); free(rm);
 }
 
 /* Modified wavenumbers (reading R6; the periodic form is B:north_star's):    */

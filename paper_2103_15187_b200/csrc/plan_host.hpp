@@ -86,21 +86,19 @@ inline std::string build_tables(HostTables& T, int nx, int ny, int nz, double Lx
     T.twy_dct.resize(ny); for (int k = 0; k < ny; k++) T.twy_dct[k] = unit(-FSEI_PI_L * k / (2.0L * ny));
     T.scale = (double)(1.0L / ((long double)N * (long double)ny));
 
-    // wall-normal metrics of L = D G
+    // Wall-normal metrics.  They are fp64 data of the grid, evaluated in double exactly as the stencils a1/a7
+    // use them (R5, R20); the tridiagonal coefficients are the products of those very reciprocals so
+    // that the operator solved IS the D G the divergence and projection kernels apply (a mismatch of
+    // ulp(zc)/dz ~ 1e-12 near the upper wall would cost ~30x in post-projection divergence).
     T.za.assign(nz, 0.0); T.zcc.assign(nz, 0.0); T.dzc.assign(nz, 0.0); T.dzm.assign(nz, 0.0);
-    std::vector<long double> dzc(nz), dzm(nz, 0.0L);
-    for (int k = 0; k < nz; k++) dzc[k] = (long double)zc[k + 1] - (long double)zc[k];
-    for (int k = 1; k < nz; k++) dzm[k] = ((long double)zc[k] + (long double)zc[k + 1]) / 2 - ((long double)zc[k - 1] + (long double)zc[k]) / 2;
-    for (int k = 0; k < nz; k++) {
-        T.dzc[k] = (double)dzc[k]; T.dzm[k] = (double)dzm[k];
-        T.za[k] = (k > 0) ? (double)(1.0L / (dzm[k] * dzc[k])) : 0.0;
-        T.zcc[k] = (k < nz - 1) ? (double)(1.0L / (dzm[k + 1] * dzc[k])) : 0.0;
-    }
-    // stencil metrics: plain double, exactly as the definition states them
     T.rdx = 1.0 / (Lx / (double)nx); T.rdy = 1.0 / (Ly / (double)ny);
     T.rdzc.assign(nz, 0.0); T.rdzm.assign(nz, 0.0);
-    for (int k = 0; k < nz; k++) T.rdzc[k] = 1.0 / (zc[k + 1] - zc[k]);
-    for (int k = 1; k < nz; k++) T.rdzm[k] = 1.0 / (0.5 * (zc[k] + zc[k + 1]) - 0.5 * (zc[k - 1] + zc[k]));
+    for (int k = 0; k < nz; k++) { T.dzc[k] = zc[k + 1] - zc[k]; T.rdzc[k] = 1.0 / T.dzc[k]; }
+    for (int k = 1; k < nz; k++) { T.dzm[k] = 0.5 * (zc[k] + zc[k + 1]) - 0.5 * (zc[k - 1] + zc[k]); T.rdzm[k] = 1.0 / T.dzm[k]; }
+    for (int k = 0; k < nz; k++) {
+        T.za[k] = (k > 0) ? T.rdzm[k] * T.rdzc[k] : 0.0;
+        T.zcc[k] = (k < nz - 1) ? T.rdzm[k + 1] * T.rdzc[k] : 0.0;
+    }
 
     // modified wavenumbers per x-slot (Re part, Im part) and per physical y-row
     const long double hx = (long double)Lx / nx, hy = (long double)Ly / ny;
