@@ -1,0 +1,18 @@
+// fast_configs.hpp -- the line lengths that have a register-resident Stockham instantiation, with their
+// radices (first radix a power of two that divides the largest one; a radix 6 goes last) and tile shapes.
+#pragma once
+
+// x direction: complex line length N = nx / 2 -> (N, R0, R1, R2)
+#define FSEI_X_CONFIGS(X) \
+    X(16, 4, 4, 1) X(32, 8, 4, 1) X(64, 8, 8, 1) X(128, 8, 16, 1) X(256, 16, 16, 1) X(512, 8, 8, 8) X(1024, 16, 8, 8) \
+    X(48, 8, 6, 1) X(96, 16, 6, 1) X(192, 8, 4, 6) X(384, 8, 8, 6)
+
+// y direction: column length N = ny -> (N, R0, R1, R2, CY); CY adjacent slots (CY * 16 contiguous bytes) per tile row
+#define FSEI_Y_CONFIGS(X) \
+    X(16, 4, 4, 1, 8) X(32, 8, 4, 1, 8) X(64, 8, 8, 1, 8) X(128, 8, 16, 1, 8) X(256, 16, 16, 1, 8) X(512, 8, 8, 8, 4) \
+    X(1024, 16, 8, 8, 4) X(48, 8, 6, 1, 8) X(96, 16, 6, 1, 8) X(192, 8, 4, 6, 8) X(384, 8, 8, 6, 4) X(768, 16, 8, 6, 4)
+
+namespace fsei {
+// lines per CTA of the x kernels: about 256 threads
+template <class C> struct XShape { static constexpr int LPB = (256 / C::T) > 0 ? (256 / C::T) : 1; };
+}

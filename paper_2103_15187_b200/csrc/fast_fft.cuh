@@ -1,18 +1,34 @@
 // fast_fft.cuh -- register-resident Stockham passes shared by the fast x and y transforms.
 //
-// Fast path (x and y periodic, power-of-two lengths): a line of N complex values is transformed
-// by NP <= 3 radix passes (radices R0 R1 R2 from {2,4,8,16}).  Pass s with Ns = R0..R_{s-1}:
-// butterfly b in [0, N/R) reads elements b + q N/R (q < R), multiplies element q by
-// w_{Ns R}^{q (b mod Ns)}, takes the R-point DFT in registers and writes output q to
-// (b / Ns) Ns R + (b mod Ns) + q Ns  (Stockham autosort: natural order in, natural order out,
-// every pass reads with unit stride across threads).  The first pass reads global memory, the last
-// writes it; in between the data sits in shared memory, alternating between two buffers so that one
-// barrier per pass is enough.  Twiddles come from per-pass shared-memory tables laid out [q-1][m]
-// (conflict-free for consecutive m).  Conventions as in fft_core.cuh (R15).
+// Fast path (lengths 2^a and 3*2^a, a line of N complex values): N = R0 R1 R2 with radices from
+// {2,4,6,8,16}.  Pass s with Ns = R0..R_{s-1}: butterfly b in [0, N/R) reads elements b + q N/R
+// (q < R), multiplies element q by w_{Ns R}^{q (b mod Ns)}, takes the R-point DFT in registers and
+// writes output q to (b / Ns) Ns R + (b mod Ns) + q Ns  (Stockham autosort: natural order in, natural
+// order out, every pass reads with unit stride across threads).  The first pass reads global memory
+// (or a staging tile), the last writes global memory (or a tile for the pair post-processing); in
+// between the data sits in ONE shared buffer (read -> barrier -> write -> barrier).  Twiddles come
+// from per-pass shared-memory tables laid out [q-1][m] (unit stride across threads).
+// Conventions as in fft_core.cuh (R15): forward e^{-i..} unnormalised, the inverse is the
+// conjugate pass sequence without 1/N.
 #pragma once
 #include "fft_core.cuh"
+#include "kernel_env.cuh"
 
 namespace fsei {
+
+// 6 = 3 x 2:  n = 2 n1 + n2,  k = k1 + 3 k2
+template <bool INV> struct SmallDft<6, INV> {
+    static FSEI_HD void run(cplx* v) {
+        cplx e[3] = {v[0], v[2], v[4]}, o[3] = {v[1], v[3], v[5]};
+        SmallDft<3, INV>::run(e); SmallDft<3, INV>::run(o);
+        o[1] = ctw<INV>(o[1], 0.5, -FSEI_SQRT3_2);
+        o[2] = ctw<INV>(o[2], -0.5, -FSEI_SQRT3_2);
+#pragma unroll
+        for (int k = 0; k < 3; k++) { v[k] = cadd(e[k], o[k]); v[k + 3] = csub(e[k], o[k]); }
+    }
+};
+
+constexpr int ilog2c(int n) { return n <= 1 ? 0 : 1 + ilog2c(n >> 1); }
 
 template <int N_, int R0_, int R1_, int R2_> struct FftCfg {
     static constexpr int N = N_, R0 = R0_, R1 = R1_, R2 = R2_;
@@ -20,36 +36,63 @@ template <int N_, int R0_, int R1_, int R2_> struct FftCfg {
     static constexpr int NP = 1 + (R1_ > 1) + (R2_ > 1);
     static constexpr int RMAX = (R0_ > R1_ ? (R0_ > R2_ ? R0_ : R2_) : (R1_ > R2_ ? R1_ : R2_));
     static constexpr int T = N_ / RMAX;                 // threads per line
-    static constexpr int E = RMAX;                      // elements per thread
-    static constexpr int TW1 = (R1_ > 1) ? (R1_ - 1) * R0_ : 0;          // table sizes (complex)
+    static constexpr int TW1 = (R1_ > 1) ? (R1_ - 1) * R0_ : 0;          // twiddle table sizes (complex)
     static constexpr int TW2 = (R2_ > 1) ? (R2_ - 1) * R0_ * R1_ : 0;
     static constexpr int TW = TW1 + TW2;
+    // shared-memory index padding: one extra element every R0 (R0 a power of two): makes the stride-R0
+    // writes of the first pass conflict-free for 16-byte elements and keeps aligned groups of 8 whole
+    static constexpr int PSH = ilog2c(R0_);
+    static_assert((1 << PSH) == R0_ || NP == 1, "first radix must be a power of two");
+    static FSEI_HD int pad(int n) { return n + (n >> PSH); }
+    static constexpr int PITCH = N_ + (N_ >> PSH) + 1;  // complex elements per padded line
 };
 
-// shared-memory index padding for 16-byte elements: one extra slot every 8
-__host__ __device__ __forceinline__ constexpr int padi(int n) { return n + (n >> 3); }
-
-// One pass for one thread.  in(n) -> cplx, out(n, cplx).  tl = thread index within the line.
-template <int N, int R, int NS, int T, bool INV, class In, class Out>
-__device__ __forceinline__ void fft_pass(int tl, const cplx* __restrict__ tw, In in, Out out)
+// per-pass twiddle tables in shared memory: tws[(q-1) NS + m] = e^{-2 pi i q m / (NS R)}, from the plan's
+// table tw[j] = e^{-2 pi i j / N}.  Called by all threads of the CTA (no barrier inside).
+template <class C> FSEI_DEV void fft_fill_twiddles(cplx* tws, const cplx* tw, int tid, int nt)
 {
-    constexpr int NB = N / R;                 // butterflies per line
-    constexpr int PER = (NB + T - 1) / T;     // butterflies per thread
-    cplx v[PER][R];
+    if (C::NP >= 2) {
+        constexpr int NS = C::R0, R = C::R1;
+        for (int i = tid; i < (R - 1) * NS; i += nt) { int q = i / NS + 1, m = i % NS; tws[i] = tw[q * m * (C::N / (NS * R))]; }
+    }
+    if (C::NP >= 3) {
+        constexpr int NS = C::R0 * C::R1, R = C::R2;
+        for (int i = tid; i < (R - 1) * NS; i += nt) { int q = i / NS + 1, m = i % NS; tws[C::TW1 + i] = tw[q * m * (C::N / (NS * R))]; }
+    }
+}
+
+// Pass s of one line for one thread: tl = thread index within the line (T threads per line).
+// in(n) -> cplx, out(n, cplx); `active` false = the thread's line does not exist (ragged tile).
+template <int N, int R, int NS, int T> struct PassShape {
+    static constexpr int NB = N / R;                  // butterflies per line
+    static constexpr int PER = (NB + T - 1) / T;      // butterflies per thread
+    static constexpr bool FULL = (NB % T == 0);
+};
+
+template <int N, int R, int NS, int T, class In>
+FSEI_DEV void fft_pass_load(int tl, In in, cplx (*v)[R])
+{
+    using S = PassShape<N, R, NS, T>;
 #pragma unroll
-    for (int i = 0; i < PER; i++) {
+    for (int i = 0; i < S::PER; i++) {
         const int b = tl + i * T;
-        if (NB % T == 0 || b < NB) {
+        if (S::FULL || b < S::NB) {
 #pragma unroll
-            for (int q = 0; q < R; q++) v[i][q] = in(b + q * NB);
+            for (int q = 0; q < R; q++) v[i][q] = in(b + q * S::NB);
         }
     }
+}
+
+template <int N, int R, int NS, int T, bool INV, class Out>
+FSEI_DEV void fft_pass_compute(int tl, const cplx* tw, cplx (*v)[R], Out out)
+{
+    using S = PassShape<N, R, NS, T>;
 #pragma unroll
-    for (int i = 0; i < PER; i++) {
+    for (int i = 0; i < S::PER; i++) {
         const int b = tl + i * T;
-        if (NB % T == 0 || b < NB) {
+        if (S::FULL || b < S::NB) {
+            const int m = b % NS;
             if (NS > 1) {
-                const int m = b % NS;
 #pragma unroll
                 for (int q = 1; q < R; q++) {
                     const cplx w = tw[(q - 1) * NS + m];
@@ -57,40 +100,10 @@ __device__ __forceinline__ void fft_pass(int tl, const cplx* __restrict__ tw, In
                 }
             }
             SmallDft<R, INV>::run(v[i]);
-            const int j0 = (b / NS) * NS * R + (b % NS);
+            const int j0 = (b / NS) * NS * R + m;
 #pragma unroll
             for (int q = 0; q < R; q++) out(j0 + q * NS, v[i][q]);
         }
-    }
-}
-
-struct SmIn {
-    const cplx* s;
-    __device__ __forceinline__ cplx operator()(int n) const { return s[padi(n)]; }
-};
-struct SmOut {
-    cplx* s;
-    __device__ __forceinline__ void operator()(int n, cplx v) const { s[padi(n)] = v; }
-};
-
-// Whole line: first pass from `in`, last pass to `out`, shared buffers bufA/bufB (each padi(N)+1 complex
-// for this line).  tws: shared twiddle tables [TW1 | TW2].  Must be called by all threads of the CTA
-// (contains __syncthreads()).
-template <class C, bool INV, class In, class Out>
-__device__ __forceinline__ void fft_line(int tl, cplx* bufA, cplx* bufB, const cplx* tws, In in, Out out)
-{
-    if (C::NP == 1) {
-        fft_pass<C::N, C::R0, 1, C::T, INV>(tl, nullptr, in, out);
-    } else if (C::NP == 2) {
-        fft_pass<C::N, C::R0, 1, C::T, INV>(tl, nullptr, in, SmOut{bufA});
-        __syncthreads();
-        fft_pass<C::N, C::R1, C::R0, C::T, INV>(tl, tws, SmIn{bufA}, out);
-    } else {
-        fft_pass<C::N, C::R0, 1, C::T, INV>(tl, nullptr, in, SmOut{bufA});
-        __syncthreads();
-        fft_pass<C::N, C::R1, C::R0, C::T, INV>(tl, tws, SmIn{bufA}, SmOut{bufB});
-        __syncthreads();
-        fft_pass<C::N, C::R2, C::R0 * C::R1, C::T, INV>(tl, tws + C::TW1, SmIn{bufB}, out);
     }
 }
 

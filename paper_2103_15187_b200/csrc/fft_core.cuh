@@ -26,7 +26,7 @@
 
 namespace fsei {
 
-struct cplx { double re, im; };
+struct alignas(16) cplx { double re, im; };      // 16-byte aligned: one 128-bit load/store per element
 
 FSEI_HD cplx cmake(double a, double b) { cplx c; c.re = a; c.im = b; return c; }
 FSEI_HD cplx cadd(cplx a, cplx b) { return cmake(a.re + b.re, a.im + b.im); }

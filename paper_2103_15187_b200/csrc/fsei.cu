@@ -17,6 +17,10 @@
 #include "xfft.cuh"
 #include "yfft.cuh"
 #include "zsolve.cuh"
+#include "fast_launch.hpp"
+#include "zfast.cuh"
+#include "stencil_fast.cuh"
+#include <cstdlib>
 
 using namespace fsei;
 
@@ -35,11 +39,13 @@ static int cuda_fail(cudaError_t e, const char* what)
 // ------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------
-enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, FSEI_NKERNELS };
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, FSEI_NKERNELS };
 
 struct fsei_plan {
     HostTables T;
     XParams X; YParams Y; ZParams Z; SParams S;
+    bool fast = false;                 // register-resident Stockham path (xfast / yfast / zfast), natural-order spectrum
+    XFast XF; YFast YF; ZFast ZF;
     std::vector<void*> owned;          // device allocations freed with the plan
     size_t bytes = 0;
     int LX = 1, CY = 1;                // tile shapes
@@ -56,7 +62,7 @@ struct fsei_plan {
 };
 
 static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
-                                                   "y_inverse", "x_inverse", "project"};
+                                                   "y_inverse", "x_inverse", "project", "div_x_forward"};
 
 // record an event pair around one launch when profiling is on
 struct LaunchTimer {
@@ -234,8 +240,13 @@ __global__ void __launch_bounds__(NT) k_z_gauge(ZParams Z, const cplx* spec, dou
 static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy)
 {
     int code = 0;
-    std::string msg = build_tables(P->T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code);
+    // fast path: line lengths with a register-resident Stockham instantiation, special columns fit in shared memory
+    const char* force = std::getenv("FSEI_FORCE_GENERIC");
+    const bool fast = !(force && force[0] == '1') && nx >= 4 && ny >= 2 && xfast_supported(nx / 2) && yfast_supported(ny) &&
+                      (size_t)nz * 4 * sizeof(cplx) <= 200 * 1024;
+    std::string msg = build_tables(P->T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code, fast);
     if (code) return fail(code, msg);
+    P->fast = fast;
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FSEI_ERR_CUDA, "no CUDA device: libfsei has no CPU fallback"); }
@@ -262,6 +273,33 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     S.nx = nx; S.ny = ny; S.nz = nz; S.bcx = bcx; S.bcy = bcy; S.rdx = T.rdx; S.rdy = T.rdy;
     if ((rc = upload(P, T.rdzc, &S.rdzc))) return rc;
     if ((rc = upload(P, T.rdzm, &S.rdzm))) return rc;
+
+    if (fast) {
+        XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
+        XF.nx = nx; XF.ny = ny; XF.nz = nz; XF.N = nx / 2; XF.tw = X.tw; XF.tw_r2c = X.tw_r2c; XF.tw_dct = X.tw_dct; XF.scale = T.scale;
+        XF.kchunk = nz < 16 ? nz : 16;
+        YF.nxc = T.nxc; YF.ny = ny; YF.nz = nz; YF.tw = Y.tw; YF.tw_dct = Y.tw_dct;
+        YF.untangle = (bcy == BC_PERIODIC) ? (bcx == BC_PERIODIC ? 1 : T.nxc) : 0;
+        ZF.nxc = T.nxc; ZF.ny = ny; ZF.nz = nz; ZF.bcx = bcx; ZF.bcy = bcy;
+        ZF.ncomp = (bcx == BC_PERIODIC && bcy == BC_PERIODIC) ? 1 : 2;
+        ZF.za = Z.za; ZF.zcc = Z.zcc; ZF.lamx = Z.lamx; ZF.lamy = Z.lamy; ZF.dzc = Z.dzc; ZF.dzm = Z.dzm;
+        void* q = nullptr;
+        if ((rc = dalloc(P, sizeof(cplx) * 2 * nz, &q))) return rc;
+        ZF.special = static_cast<cplx*>(q);
+        if ((rc = dalloc(P, sizeof(double) * 4 * nz, &q))) return rc;
+        ZF.cpw = static_cast<double*>(q);
+        size_t nip = (size_t)nz * ny * T.nxc * ZF.ncomp;
+        if ((rc = dalloc(P, sizeof(double) * nip, &q))) return rc;
+        ZF.ipiv = static_cast<const double*>(q);
+        size_t cols = (size_t)ny * T.nxc * ZF.ncomp;
+        k_zf_factor<<<(unsigned)((cols + 255) / 256), 256>>>(ZF, static_cast<double*>(q));
+        CU(cudaGetLastError());
+        CU(cudaDeviceSynchronize());
+        CU(xfast_init());
+        CU(yfast_init());
+        CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz)));
+        return FSEI_OK;
+    }
 
     void* g = nullptr;
     if ((rc = dalloc(P, sizeof(double) * nz, &g))) return rc;
@@ -345,9 +383,29 @@ extern "C" int fsei_divergence(fsei_plan* P, const double* u, const double* v, c
     if (rhs == u || rhs == v || rhs == w) return fail(FSEI_ERR_ARG, "fsei_divergence: rhs must not alias u, v, w");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
-    { LaunchTimer t(P, K_DIV, st); k_divergence<<<stencil_grid(n), NT, 0, st>>>(P->S, u, v, w, 1.0 / alpha_dt, rhs); }
+    { LaunchTimer t(P, K_DIV, st); k_divergence_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, 1.0 / alpha_dt, rhs); }
     CU(cudaGetLastError());
     P->last_launches = 1;
+    return FSEI_OK;
+}
+
+// a3 .. a6 of the fast path on a spectrum already in x-forward form: y forward, z solve, y inverse, x inverse
+static int fast_spectral_solve(fsei_plan* P, cplx* spec, cudaStream_t st)
+{
+    const HostTables& T = P->T;
+    const bool ny_neu = T.bcy == BC_NEUMANN;
+    { LaunchTimer t(P, K_YF, st); CU(launch_y_fast(P->YF, false, ny_neu, spec, st)); }
+    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz, st>>>(P->ZF, spec); }
+    CU(cudaGetLastError());
+    {
+        LaunchTimer t(P, K_ZD, st);
+        size_t nthr = (size_t)T.nxc * T.ny;
+        if (P->ZF.ncomp == 1) k_zf_sweep<1><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->ZF, spec);
+        else k_zf_sweep<2><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->ZF, spec);
+    }
+    CU(cudaGetLastError());
+    { LaunchTimer t(P, K_YI, st); CU(launch_y_fast(P->YF, true, ny_neu, spec, st)); }
+    { LaunchTimer t(P, K_XI, st); CU(launch_xi_fast(P->XF, T.bcx == BC_NEUMANN, spec, reinterpret_cast<double*>(spec), st)); }
     return FSEI_OK;
 }
 
@@ -359,6 +417,13 @@ extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, 
     const long nlines = (long)T.ny * T.nz;
     cplx* spec = reinterpret_cast<cplx*>(phi);
     int launches = 0;
+    if (P->fast) {
+        { LaunchTimer t(P, K_XF, st); CU(launch_xf_fast(P->XF, P->S, T.bcx == BC_NEUMANN, false, rhs, nullptr, nullptr, 0.0, spec, st)); }
+        int rc = fast_spectral_solve(P, spec, st);
+        if (rc) return rc;
+        P->last_launches = 6;
+        return FSEI_OK;
+    }
     unsigned gx = (unsigned)((nlines + P->LX - 1) / P->LX);
     { LaunchTimer t(P, K_XF, st); k_x_forward<<<gx, NT, P->smem_x, st>>>(P->X, rhs, spec, nlines, P->LX); launches++; }
     CU(cudaGetLastError());
@@ -414,7 +479,7 @@ extern "C" int fsei_project(fsei_plan* P, double* u, double* v, double* w, doubl
     if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_project: phi must not alias u, v, w, p");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
-    { LaunchTimer t(P, K_PROJ, st); k_project<<<(unsigned)((n + NT - 1) / NT), NT, 0, st>>>(P->S, u, v, w, p, phi, alpha_dt, beta); }
+    { LaunchTimer t(P, K_PROJ, st); k_project_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, p, phi, alpha_dt, beta); }
     CU(cudaGetLastError());
     P->last_launches = 1;
     return FSEI_OK;
@@ -424,6 +489,18 @@ extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, doub
                                         double alpha_dt, double beta, void* cuda_stream)
 {
     int rc, n = 0;
+    if (P && P->fast) {
+        if (!u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: NULL argument");
+        if (alpha_dt == 0.0 || alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: alpha_dt must be non-zero, beta not NaN");
+        if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: phi must not alias u, v, w, p");
+        cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+        cplx* spec = reinterpret_cast<cplx*>(phi);
+        { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, P->T.bcx == BC_NEUMANN, true, u, v, w, 1.0 / alpha_dt, spec, st)); }
+        if ((rc = fast_spectral_solve(P, spec, st))) return rc;
+        if ((rc = fsei_project(P, u, v, w, p, phi, alpha_dt, beta, cuda_stream))) return rc;
+        P->last_launches = 7;
+        return FSEI_OK;
+    }
     if ((rc = fsei_divergence(P, u, v, w, alpha_dt, phi, cuda_stream))) return rc;
     n += P->last_launches;
     if ((rc = fsei_poisson_solve(P, phi, phi, cuda_stream))) return rc;

@@ -22,6 +22,7 @@ struct HostTables {
     int ncomp;          // 1 or 2 reciprocal-pivot components per slot (see ZParams)
     bool paired_all;    // x Neumann + y periodic: every slot goes through the paired kernel
     bool paired_slot0;  // x periodic + y periodic: slot 0 only
+    bool fast;          // natural-order spectrum layout of the fast path (xfast.cuh / yfast.cuh): pos tables are the identity
 };
 
 static const long double FSEI_PI_L = 3.14159265358979323846264338327950288L;
@@ -62,7 +63,7 @@ inline long double lam_neumann(int m, int n, long double h) { long double s = si
 
 // returns "" on success, else a message; code = FSEI_ERR_* value (2 size, 3 grid, 1 arg)
 inline std::string build_tables(HostTables& T, int nx, int ny, int nz, double Lx, double Ly, const double* zc,
-                                int bcx, int bcy, int& code)
+                                int bcx, int bcy, int& code, bool fast_layout = false)
 {
     code = 0;
     if (zc == nullptr) { code = 1; return "zc is NULL"; }
@@ -79,6 +80,11 @@ inline std::string build_tables(HostTables& T, int nx, int ny, int nz, double Lx
     const int N = nx / 2;
     T.fx = make_fft_plan(N); T.fy = make_fft_plan(ny);
     T.posx = make_pos(T.fx); T.posy = make_pos(T.fy);
+    T.fast = fast_layout;
+    if (fast_layout) {                      // Stockham passes leave natural order
+        for (int k = 0; k < N; k++) T.posx[k] = k;
+        for (int k = 0; k < ny; k++) T.posy[k] = k;
+    }
     T.twx.resize(N); for (int m = 0; m < N; m++) T.twx[m] = unit(-2.0L * FSEI_PI_L * m / N);
     T.twx_r2c.resize(N / 2 + 1); for (int k = 0; k <= N / 2; k++) T.twx_r2c[k] = unit(-2.0L * FSEI_PI_L * k / nx);
     T.twx_dct.resize(N + 1); for (int k = 0; k <= N; k++) T.twx_dct[k] = unit(-FSEI_PI_L * k / (2.0L * nx));
@@ -113,7 +119,7 @@ inline std::string build_tables(HostTables& T, int nx, int ny, int nz, double Lx
     T.lamy.assign(ny, 0.0);
     for (int k = 0; k < ny; k++) {
         if (bcy == BC_PERIODIC) T.lamy[T.posy[k]] = (double)lam_periodic(k, ny, hy);
-        else T.lamy[dct_perm(T.posy[k], ny)] = (double)lam_neumann(k, ny, hy);
+        else T.lamy[fast_layout ? k : dct_perm(T.posy[k], ny)] = (double)lam_neumann(k, ny, hy);
     }
     T.paired_all = (bcx == BC_NEUMANN && bcy == BC_PERIODIC);
     T.paired_slot0 = (bcx == BC_PERIODIC && bcy == BC_PERIODIC);

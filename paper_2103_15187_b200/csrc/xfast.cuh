@@ -1,0 +1,288 @@
+// xfast.cuh -- fast-path kernels of steps a1+a2 (divergence fused into the x-forward transform) and a6
+// (x-inverse transform), for line lengths nx = 2 N with N = 2^a or 3 2^a (include/fsei.h; P:L30, P:L87,
+// P:L91; R15, sec. 6).
+//
+// A CTA of T*LPB threads owns LPB adjacent x-lines (rows j) and marches along z over `kchunk` planes:
+// T threads per line, each holding the line's butterflies of one Stockham pass in registers
+// (fast_fft.cuh).  Real lines are transformed as N complex values z_t = x[2t] + i x[2t+1] followed
+// (forward) or preceded (inverse) by the Hermitian pair step; Neumann lines go through Makhoul's
+// even/odd reorder (staged in shared memory) and the quarter-wave twiddle (DCT-II / DCT-III).
+//
+// Spectrum layout (natural order, in place in the phi buffer): line (j,k) holds N complex slots;
+//   periodic: slot 0 = (X_0, X_N) (both real), slot s = X_s for s = 1..N-1
+//   Neumann : slot 0 = (X_0, X_N),             slot s = (X_s, X_{nx-s})
+// Marching along z gives the fused divergence its reuse: the w(k+1) lines a CTA reads for plane k are the
+// w(k) lines it reads one iteration later, so u, v, w each come from DRAM once.
+#pragma once
+#include "kernel_env.cuh"
+#include "fast_fft.cuh"
+#include "plan_types.cuh"
+#include "stencil.cuh"
+#include "xfft.cuh"
+
+namespace fsei {
+
+struct XFast {
+    int nx, ny, nz, N;          // N = nx / 2
+    int kchunk;                 // planes per CTA
+    const cplx* tw;             // e^{-2 pi i j / N},  j in [0, N)
+    const cplx* tw_r2c;         // e^{-2 pi i k / nx}, k in [0, N/2]
+    const cplx* tw_dct;         // e^{-i pi k / (2 nx)}, k in [0, N]   (Neumann only)
+    double scale;               // 1 / (N ny), applied by the inverse store
+};
+
+template <class C> struct SmIn {
+    const cplx* s;
+    FSEI_HD cplx operator()(int n) const { return s[C::pad(n)]; }
+};
+template <class C> struct SmOut {
+    cplx* s;
+    FSEI_HD void operator()(int n, cplx v) const { s[C::pad(n)] = v; }
+};
+
+// staging tile of a real line (Neumann): one pad double every 4 keeps the stride-4 reads of the reorder
+// conflict-free
+FSEI_HD int xs_pad(int s) { return s + (s >> 2); }
+FSEI_HD int xs_pitch(int n) { return n + (n >> 2) + 2; }
+// Makhoul: index of the natural line element that sits at position s of the reordered sequence v
+FSEI_HD int makhoul(int s, int n) { return (s < (n >> 1)) ? 2 * s : 2 * (n - 1 - s) + 1; }
+
+template <class C, int LPB, bool NEU> struct XSmemLayout {
+    static constexpr int N = C::N;
+    static constexpr int BUF = LPB * C::PITCH;                  // complex
+    static constexpr int TWS = C::TW;
+    static constexpr int R2C = N / 2 + 1;
+    static constexpr int DCT = NEU ? N + 1 : 0;
+    static constexpr int XS = NEU ? LPB * (2 * N + (2 * N >> 2) + 2) : 0;     // doubles
+    static constexpr size_t BYTES = sizeof(cplx) * (BUF + TWS + R2C + DCT) + sizeof(double) * XS;
+};
+
+// Whole line transform for the threads of one line.  load0(v) fills the first pass' registers (from global
+// memory / staging; IN_BUF: from the line buffer itself, then a barrier separates its reads from the writes);
+// `out` receives the natural-order result (OUT_BUF: it writes the line buffer, so a barrier precedes it).
+// Must be reached by every thread of the CTA; `act` false = this thread's line does not exist.
+template <class C, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out>
+FSEI_DEV void fft_line(int tl, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out)
+{
+    constexpr int N = C::N, T = C::T;
+    SmIn<C> bin{buf}; SmOut<C> bout{buf};
+    {
+        cplx v[PassShape<N, C::R0, 1, T>::PER][C::R0];
+        if (act) load0(v);
+        if constexpr (C::NP == 1) {
+            if (IN_BUF && OUT_BUF) FSEI_SYNC();
+            if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, out);
+            return;
+        } else {
+            if (IN_BUF) FSEI_SYNC();
+            if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, bout);
+        }
+    }
+    FSEI_SYNC();
+    if constexpr (C::NP >= 2) {
+        cplx v[PassShape<N, C::R1, C::R0, T>::PER][C::R1];
+        if (act) fft_pass_load<N, C::R1, C::R0, T>(tl, bin, v);
+        if constexpr (C::NP == 2) {
+            if (OUT_BUF) FSEI_SYNC();
+            if (act) fft_pass_compute<N, C::R1, C::R0, T, INV>(tl, tws, v, out);
+            return;
+        } else {
+            FSEI_SYNC();
+            if (act) fft_pass_compute<N, C::R1, C::R0, T, INV>(tl, tws, v, bout);
+        }
+    }
+    FSEI_SYNC();
+    if constexpr (C::NP >= 3) {
+        cplx v[PassShape<N, C::R2, C::R0 * C::R1, T>::PER][C::R2];
+        if (act) fft_pass_load<N, C::R2, C::R0 * C::R1, T>(tl, bin, v);
+        if (OUT_BUF) FSEI_SYNC();
+        if (act) fft_pass_compute<N, C::R2, C::R0 * C::R1, T, INV>(tl, tws + C::TW1, v, out);
+    }
+}
+
+FSEI_HD cplx ld2(const double* p) { return *reinterpret_cast<const cplx*>(p); }
+FSEI_HD void st2(double* p, cplx v) { *reinterpret_cast<cplx*>(p) = v; }
+
+// ---------------------------------------------------------------------------------------------------
+// a1 + a2: spec(line) = R2C / DCT-II of  rhs(line),  rhs = D(u,v,w)/(alpha dt) (FUSED) or read from `u`
+// grid (ceil(ny / LPB), ceil(nz / kchunk)), block T*LPB, dynamic shared memory XSmemLayout::BYTES
+// ---------------------------------------------------------------------------------------------------
+template <class C, int LPB, bool NEU, bool FUSED>
+FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xf_fast(XFast P, SParams S, const double* u, const double* v, const double* w,
+                                     double inv_adt, cplx* spec)
+{
+    using L = XSmemLayout<C, LPB, NEU>;
+    constexpr int N = C::N, T = C::T, R0 = C::R0;
+    constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
+    static_assert(NB0 % T == 0, "first pass must tile the line exactly");
+    constexpr int NPAIR = N / T;                                  // real pairs per thread
+    FSEI_DYN_SMEM(smraw);
+    cplx* buf = reinterpret_cast<cplx*>(smraw);
+    cplx* tws = buf + L::BUF;
+    cplx* tr2c = tws + L::TWS;
+    cplx* tdct = tr2c + L::R2C;
+    double* xs = reinterpret_cast<double*>(tdct + L::DCT);
+    const int tid = threadIdx.x, nt = T * LPB;
+    const int li = tid / T, tl = tid - li * T;
+    fft_fill_twiddles<C>(tws, P.tw, tid, nt);
+    for (int i = tid; i < L::R2C; i += nt) tr2c[i] = P.tw_r2c[i];
+    if (NEU) for (int i = tid; i < L::DCT; i += nt) tdct[i] = P.tw_dct[i];
+    FSEI_SYNC();
+
+    const int n = 2 * N, ny = P.ny, nz = P.nz;
+    const int j = blockIdx.x * LPB + li;
+    const bool act = j < ny;
+    const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
+    cplx* lbuf = buf + li * C::PITCH;
+    double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
+    const size_t plane = (size_t)ny * n;
+    const bool has_jp = (j + 1 < ny) || S.bcy == BC_PERIODIC;
+    const bool xper = S.bcx == BC_PERIODIC;
+
+    // (rhs[2t], rhs[2t+1]) of line (j,k).  The CTA marches along z, so the w(k+1) pairs read here are read
+    // again as w(k) by the same threads one iteration later (from L1/L2, not from DRAM).
+    auto rhs_pair = [&](int k, int t) -> cplx {
+        const size_t line = ((size_t)k * ny + j) * n;
+        if (!FUSED) return ld2(u + line + 2 * t);
+        const size_t linejp = (j + 1 < ny) ? line + n : line - (size_t)(ny - 1) * n;
+        cplx uu = ld2(u + line + 2 * t);
+        double un = (2 * t + 2 < n) ? u[line + 2 * t + 2] : (xper ? u[line] : 0.0);
+        cplx vv = ld2(v + line + 2 * t);
+        cplx vp = has_jp ? ld2(v + linejp + 2 * t) : cmake(0.0, 0.0);
+        cplx wk = ld2(w + line + 2 * t);
+        cplx wp = (k + 1 < nz) ? ld2(w + line + plane + 2 * t) : cmake(0.0, 0.0);
+        const double rdz = S.rdzc[k];
+        return cmake(div_cell(uu.re, uu.im, vv.re, vp.re, wk.re, wp.re, S.rdx, S.rdy, rdz, inv_adt),
+                     div_cell(uu.im, un, vv.im, vp.im, wk.im, wp.im, S.rdx, S.rdy, rdz, inv_adt));
+    };
+
+    for (int k = k0; k < k1; k++) {
+        if (NEU) {
+            // stage the real line (coalesced), then the first pass reads it through Makhoul's reorder
+            if (act) {
+#pragma unroll
+                for (int e = 0; e < NPAIR; e++) {
+                    int t = tl + e * T;
+                    cplx r = rhs_pair(k, t);
+                    lxs[xs_pad(2 * t)] = r.re; lxs[xs_pad(2 * t + 1)] = r.im;
+                }
+            }
+            FSEI_SYNC();
+        }
+        auto load0 = [&](cplx (*v0)[R0]) {
+#pragma unroll
+            for (int i = 0; i < PER0; i++) {
+#pragma unroll
+                for (int q = 0; q < R0; q++) {
+                    const int t = tl + i * T + q * NB0;
+                    if (NEU) v0[i][q] = cmake(lxs[xs_pad(makhoul(2 * t, n))], lxs[xs_pad(makhoul(2 * t + 1, n))]);
+                    else v0[i][q] = rhs_pair(k, t);
+                }
+            }
+        };
+        fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf});
+        FSEI_SYNC();
+        // Hermitian pair step (+ quarter-wave twiddle): Z -> packed half spectrum, written to global memory
+        if (act) {
+            cplx* g = spec + ((size_t)k * ny + j) * N;
+            for (int p = tl; p <= N / 2; p += T) {
+                if (p == 0) {
+                    cplx z = lbuf[0];
+                    double x0 = z.re + z.im, xn = z.re - z.im;
+                    if (NEU) xn *= FSEI_SQRT1_2;                               // X_{n/2} = V_{n/2} cos(pi/4)
+                    g[0] = cmake(x0, xn);
+                } else {
+                    cplx zk = lbuf[C::pad(p)], zm = lbuf[C::pad(N - p)];
+                    cplx E = cmake(0.5 * (zk.re + zm.re), 0.5 * (zk.im - zm.im));   // (Zk + conj Zm)/2
+                    cplx D = cmake(zk.re - zm.re, zk.im + zm.im);                   // Zk - conj Zm
+                    cplx O = cmake(0.5 * D.im, -0.5 * D.re);                        // D / (2i)
+                    cplx Tt = cmul(O, tr2c[p]);
+                    cplx xk = cadd(E, Tt), xm = cconj(csub(E, Tt));
+                    if (NEU) { xk = dct_tw_fwd(xk, tdct[p]); xm = dct_tw_fwd(xm, tdct[N - p]); }
+                    g[p] = xk;
+                    if (p != N - p) g[N - p] = xm;
+                }
+            }
+        }
+        FSEI_SYNC();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a6: phi(line) = scale * C2R / DCT-III of spec(line), in place
+// ---------------------------------------------------------------------------------------------------
+template <class C, int LPB, bool NEU>
+FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xi_fast(XFast P, const cplx* spec, double* phi)
+{
+    using L = XSmemLayout<C, LPB, NEU>;
+    constexpr int N = C::N, T = C::T, R0 = C::R0;
+    constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
+    constexpr int NPAIR = N / T;
+    FSEI_DYN_SMEM(smraw);
+    cplx* buf = reinterpret_cast<cplx*>(smraw);
+    cplx* tws = buf + L::BUF;
+    cplx* tr2c = tws + L::TWS;
+    cplx* tdct = tr2c + L::R2C;
+    double* xs = reinterpret_cast<double*>(tdct + L::DCT);
+    const int tid = threadIdx.x, nt = T * LPB;
+    const int li = tid / T, tl = tid - li * T;
+    fft_fill_twiddles<C>(tws, P.tw, tid, nt);
+    for (int i = tid; i < L::R2C; i += nt) tr2c[i] = P.tw_r2c[i];
+    if (NEU) for (int i = tid; i < L::DCT; i += nt) tdct[i] = P.tw_dct[i];
+    FSEI_SYNC();
+
+    const int n = 2 * N, ny = P.ny, nz = P.nz;
+    const int j = blockIdx.x * LPB + li;
+    const bool act = j < ny;
+    const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
+    cplx* lbuf = buf + li * C::PITCH;
+    double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
+    const double scale = P.scale;
+
+    for (int k = k0; k < k1; k++) {
+        // packed half spectrum -> Z (Hermitian pair step, preceded by the inverse quarter-wave twiddle)
+        if (act) {
+            const cplx* g = spec + ((size_t)k * ny + j) * N;
+            for (int p = tl; p <= N / 2; p += T) {
+                if (p == 0) {
+                    cplx s = g[0];
+                    double x0 = s.re, xn = s.im;
+                    if (NEU) xn *= 1.41421356237309504880168872420969808;
+                    lbuf[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
+                } else {
+                    cplx xk = g[p], xm = g[N - p];
+                    if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
+                    cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
+                    cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2
+                    cplx O = cmulc(Tt, tr2c[p]);
+                    lbuf[C::pad(p)] = cmake(E.re - O.im, E.im + O.re);               // E + i O
+                    if (p != N - p) lbuf[C::pad(N - p)] = cmake(E.re + O.im, -(E.im - O.re));   // conj(E - i O)
+                }
+            }
+        }
+        FSEI_SYNC();
+        double* gl = phi + ((size_t)k * ny + j) * n;
+        auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, SmIn<C>{lbuf}, v0); };
+        if (!NEU) {
+            auto out = [&](int t, cplx z) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
+            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out);
+        } else {
+            auto out = [&](int t, cplx z) {
+                lxs[xs_pad(makhoul(2 * t, n))] = z.re * scale; lxs[xs_pad(makhoul(2 * t + 1, n))] = z.im * scale;
+            };
+            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out);
+            FSEI_SYNC();
+            if (act) {
+#pragma unroll
+                for (int e = 0; e < NPAIR; e++) {
+                    int t = tl + e * T;
+                    st2(gl + 2 * t, cmake(lxs[xs_pad(2 * t)], lxs[xs_pad(2 * t + 1)]));
+                }
+            }
+        }
+        FSEI_SYNC();
+    }
+    (void)NB0; (void)PER0;
+}
+
+}  // namespace fsei

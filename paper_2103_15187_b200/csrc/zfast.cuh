@@ -1,0 +1,182 @@
+// zfast.cuh -- step a4 on the fast path: one real tridiagonal system per wavenumber pair and component,
+//   a_k x_{k-1} + (-(a_k + c_k) + lambda) x_k + c_k x_{k+1} = d_k
+// solved by Thomas' algorithm along z, in place in the spectrum (natural-order layout of
+// xfast.cuh / yfast.cuh), and the singular (0,0) column by two prefix sums + volume-weighted zero mean
+// (R7, R8).
+#pragma once
+#include "kernel_env.cuh"
+#include "plan_types.cuh"
+
+namespace fsei {
+
+struct ZFast {
+    int nxc, ny, nz;
+    int ncomp;            // reciprocal-pivot components per column in `ipiv` (1: Re and Im share lambda)
+    int bcx, bcy;
+    const double* za;     // a_k  (a_0 = 0)
+    const double* zcc;    // c_k  (c_{nz-1} = 0)
+    const double* lamx;   // [nxc][2]  lambda_x of the Re part, of the Im part, per slot
+    const double* lamy;   // [ny]      lambda_y per row (natural order)
+    const double* dzc;    // [nz]
+    const double* dzm;    // [nz] (dzm[0] unused)
+    const double* ipiv;   // [nz][ny][nxc][ncomp] reciprocal pivots (plan time)
+    cplx* special;        // [2][nz] solved special columns: (row 0, slot 0) and, on (P,P), (row ny/2, slot 0)
+    double* cpw;          // [4][nz] scratch of the special kernel (c' of its on-the-fly factorisations)
+};
+
+FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot) { return ((size_t)k * Z.ny + row) * Z.nxc + slot; }
+
+// lambda of component comp (0 = Re, 1 = Im) of column (row, slot).  Periodic y: columns that the y-forward
+// kernel split (yfast.cuh) hold A^(ky) in rows 1..ny/2-1 and B^(ky) in rows ny-ky, both parts of a row
+// belonging to the same x-sequence.
+FSEI_HD double z_lambda(const ZFast& Z, int row, int slot, int comp)
+{
+    int cx = comp;
+    if (Z.bcy == BC_PERIODIC && (slot == 0 || Z.bcx == BC_NEUMANN)) {
+        const int h = Z.ny >> 1;
+        if (row != 0 && row != h) cx = (row < h) ? 0 : 1;
+    }
+    return Z.lamx[2 * slot + cx] + Z.lamy[row];
+}
+
+// special columns: index into Z.special (or -1) and the mask of components taken from there.
+// (P,P): the table has one component per column, so the two columns whose parts differ in lambda --
+// (row 0, slot 0) = (gauge, (N_x, 0)) and (row ny/2, slot 0) -- are solved by k_z_special entirely;
+// otherwise only the gauge component (row 0, slot 0, Re) is.
+FSEI_HD int z_special(const ZFast& Z, int row, int slot, int& mask)
+{
+    mask = 0;
+    if (slot != 0) return -1;
+    const bool pp = (Z.bcx == BC_PERIODIC && Z.bcy == BC_PERIODIC);
+    if (row == 0) { mask = pp ? 3 : 1; return 0; }
+    if (pp && row == (Z.ny >> 1)) { mask = 3; return 1; }
+    return -1;
+}
+
+// plan time: reciprocal pivots of one component of one column
+FSEI_HD void zf_factor_column(const ZFast& Z, double* ipiv, int row, int slot, int comp)
+{
+    int mask; z_special(Z, row, slot, mask);
+    const bool zero_it = (Z.ncomp == 1) ? (mask != 0) : ((mask >> comp) & 1);
+    const double lam = z_lambda(Z, row, slot, comp);
+    double cp = 0.0;
+    for (int k = 0; k < Z.nz; k++) {
+        double a = Z.za[k], c = Z.zcc[k];
+        double piv = (-(a + c) + lam) - a * cp;
+        double ip = zero_it ? 0.0 : 1.0 / piv;
+        ipiv[zf_idx(Z, k, row, slot) * Z.ncomp + comp] = ip;
+        cp = c * ip;
+    }
+}
+
+// one thread per column: forward elimination then back substitution, in place (two passes over the column)
+template <int NCOMP>
+FSEI_HD void zf_sweep_column(const ZFast& Z, cplx* S, int row, int slot)
+{
+    const int nz = Z.nz;
+    int mask; const int sp = z_special(Z, row, slot, mask);
+    cplx prev = cmake(0.0, 0.0);
+    for (int k = 0; k < nz; k++) {
+        size_t i = zf_idx(Z, k, row, slot);
+        cplx d = S[i];
+        double ipr = Z.ipiv[i * NCOMP], ipi = Z.ipiv[i * NCOMP + (NCOMP - 1)];
+        double a = Z.za[k];
+        prev = cmake((d.re - a * prev.re) * ipr, (d.im - a * prev.im) * ipi);
+        S[i] = prev;
+    }
+    cplx next = cmake(0.0, 0.0);
+    for (int k = nz - 1; k >= 0; k--) {
+        size_t i = zf_idx(Z, k, row, slot);
+        cplx dp = S[i];
+        double ipr = Z.ipiv[i * NCOMP], ipi = Z.ipiv[i * NCOMP + (NCOMP - 1)];
+        double c = Z.zcc[k];
+        next = cmake(dp.re - (c * ipr) * next.re, dp.im - (c * ipi) * next.im);
+        cplx o = next;
+        if (sp >= 0) {
+            cplx s = Z.special[(size_t)sp * nz + k];
+            if (mask & 1) o.re = s.re;
+            if (mask & 2) o.im = s.im;
+        }
+        S[i] = o;
+    }
+}
+
+// the (0,0) component: serial definition (R7):
+//   F_k = F_{k-1} + d_{k-1} dzc[k-1],  x_0 = 0,  x_k = x_{k-1} + F_k dzm[k],  x -= sum x dzc / sum dzc
+// d, x: arrays of cplx; comp selects the part (stride 2 doubles)
+FSEI_HD void zf_gauge_serial(const ZFast& Z, const double* d, double* x)
+{
+    double F = 0.0, acc = 0.0, vol = 0.0;
+    x[0] = 0.0;
+    for (int k = 1; k < Z.nz; k++) {
+        F += d[2 * (k - 1)] * Z.dzc[k - 1];
+        x[2 * k] = x[2 * (k - 1)] + F * Z.dzm[k];
+    }
+    for (int k = 0; k < Z.nz; k++) { acc += x[2 * k] * Z.dzc[k]; vol += Z.dzc[k]; }
+    double mean = acc / vol;
+    for (int k = 0; k < Z.nz; k++) x[2 * k] -= mean;
+}
+
+// Thomas with on-the-fly factorisation on one component of a column held in shared memory
+FSEI_HD void zf_thomas_serial(const ZFast& Z, double lam, const double* d, double* x, double* cp)
+{
+    double cprev = 0.0, prev = 0.0;
+    for (int k = 0; k < Z.nz; k++) {
+        double a = Z.za[k], c = Z.zcc[k];
+        double ip = 1.0 / ((-(a + c) + lam) - a * cprev);
+        cprev = c * ip; cp[k] = cprev;
+        prev = (d[2 * k] - a * prev) * ip;
+        x[2 * k] = prev;
+    }
+    double next = 0.0;
+    for (int k = Z.nz - 1; k >= 0; k--) { next = x[2 * k] - cp[k] * next; x[2 * k] = next; }
+}
+
+// grid 1, block 128, dynamic shared memory 2 * 2 * nz * sizeof(cplx): gathers the special columns, solves
+// them (one thread per component), leaves them in Z.special
+FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec)
+{
+    FSEI_DYN_SMEM(smraw);
+    cplx* d = reinterpret_cast<cplx*>(smraw);            // [2][nz]
+    cplx* x = d + 2 * Z.nz;                              // [2][nz]
+    const int nz = Z.nz, tid = threadIdx.x;
+    const bool pp = (Z.bcx == BC_PERIODIC && Z.bcy == BC_PERIODIC);
+    const int ncol = pp ? 2 : 1;
+    for (int i = tid; i < ncol * nz; i += 128) {
+        int col = i / nz, k = i - col * nz;
+        d[i] = spec[zf_idx(Z, k, col == 0 ? 0 : (Z.ny >> 1), 0)];
+        x[i] = cmake(0.0, 0.0);
+    }
+    FSEI_SYNC();
+    if (tid < 2 * ncol) {
+        const int col = tid >> 1, comp = tid & 1;
+        const double* dd = reinterpret_cast<const double*>(d + col * nz) + comp;
+        double* xx = reinterpret_cast<double*>(x + col * nz) + comp;
+        if (tid == 0) zf_gauge_serial(Z, dd, xx);
+        else if (pp) zf_thomas_serial(Z, z_lambda(Z, col == 0 ? 0 : (Z.ny >> 1), 0, comp), dd, xx, Z.cpw + (size_t)tid * nz);
+    }
+    FSEI_SYNC();
+    for (int i = tid; i < ncol * nz; i += 128) Z.special[i] = x[i];
+}
+
+// plan time.  grid ceil(ny nxc ncomp / 256), block 256
+FSEI_GLOBAL(256, 1) k_zf_factor(ZFast Z, double* ipiv)
+{
+    size_t t = (size_t)blockIdx.x * 256 + threadIdx.x;
+    size_t n = (size_t)Z.ny * Z.nxc * Z.ncomp;
+    if (t >= n) return;
+    int comp = (int)(t % Z.ncomp); size_t r = t / Z.ncomp; int slot = (int)(r % Z.nxc), row = (int)(r / Z.nxc);
+    zf_factor_column(Z, ipiv, row, slot, comp);
+}
+
+// grid ceil(ny nxc / 128), block 128: slot fastest across the warp (coalesced 16-byte accesses)
+template <int NCOMP>
+FSEI_GLOBAL(128, 1) k_zf_sweep(ZFast Z, cplx* spec)
+{
+    size_t t = (size_t)blockIdx.x * 128 + threadIdx.x;
+    if (t >= (size_t)Z.nxc * Z.ny) return;
+    int slot = (int)(t % Z.nxc), row = (int)(t / Z.nxc);
+    zf_sweep_column<NCOMP>(Z, spec, row, slot);
+}
+
+}  // namespace fsei

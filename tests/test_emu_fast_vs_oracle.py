@@ -1,0 +1,53 @@
+"""Host logic of the fast path (-m "not gpu"): the fast-path kernels of csrc/{xfast,yfast,zfast,stencil_fast}.cuh
+compiled for the host (tests/emu/emu_fast.cpp, a CTA = a team of host threads with a barrier) against the long-double
+oracle.  Checks the Stockham passes, padded tiles, Hermitian pair steps, split y-spectra and special z columns of every
+line-length instantiation without a GPU; the GPU parity tests proper are in test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_2103_15187_b200 import inputs
+from tests.util import emu_fast_lib, emu_fast_projection, oracle_projection, rel_l2
+
+P, N = 0, 1
+
+
+def _check(oracle_ld, shape, bc, split=False, cfg=2, beta=1e-4):
+    case = inputs.make_case(cfg, shape=shape, bc=bc)
+    got = emu_fast_projection(case, beta, split)
+    ref = oracle_projection(oracle_ld, case, beta)
+    assert rel_l2(got[4], ref[4]) < 1e-13
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-11 * max(1.0, np.abs(r).max())
+    return got
+
+
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(32, 32, 8), (64, 16, 5), (96, 48, 7), (128, 64, 3)])
+def test_fast_kernels_match_oracle(oracle_ld, bc, shape):
+    a = _check(oracle_ld, shape, bc, split=False)
+    b = _check(oracle_ld, shape, bc, split=True)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)                    # fused divergence == divergence kernel + x-forward
+
+
+# every x line length (nx = 2 N) and every y column length with an instantiation, both transforms types
+@pytest.mark.parametrize("nx", [32, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 2048])
+def test_every_x_length(oracle_ld, nx):
+    for bc in ((P, P), (N, N)):
+        _check(oracle_ld, (nx, 16, 2), bc)
+
+
+@pytest.mark.parametrize("ny", [16, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024])
+def test_every_y_length(oracle_ld, ny):
+    for bc in ((P, P), (N, N), (N, P)):
+        _check(oracle_ld, (32, ny, 2), bc)
+
+
+def test_fast_config1_full(oracle_ld):
+    _check(oracle_ld, (32, 32, 32), (P, P), cfg=1, beta=0.0)
+
+
+def test_fast_support_matrix():
+    L = emu_fast_lib()
+    assert L.emu_fast_supported(1024, 1024) and L.emu_fast_supported(768, 768) and L.emu_fast_supported(32, 32)
+    assert not L.emu_fast_supported(12, 36) and not L.emu_fast_supported(8, 8)

@@ -29,6 +29,36 @@ def emu_lib():
     return L
 
 
+_EMUF_SRC = os.path.join(ROOT, "tests", "emu", "emu_fast.cpp")
+_EMUF_LIB = os.path.join(ROOT, "tests", "emu", "libfsei_emu_fast.so")
+
+
+def emu_fast_lib():
+    """tests/emu/emu_fast.cpp: the fast-path kernels of libfsei run on the host (a CTA = a team of host threads)."""
+    csrc = os.path.join(ROOT, "paper_2103_15187_b200", "csrc")
+    deps = [_EMUF_SRC, os.path.join(ROOT, "tests", "emu", "cuda_shim.hpp")] + \
+        [os.path.join(csrc, f) for f in os.listdir(csrc) if f.endswith((".cuh", ".hpp"))]
+    if not os.path.exists(_EMUF_LIB) or any(os.path.getmtime(d) > os.path.getmtime(_EMUF_LIB) for d in deps):
+        subprocess.run(["g++", "-std=c++20", "-O1", "-ffp-contract=off", "-fPIC", "-shared", "-pthread", "-Wno-unknown-pragmas",
+                        "-I" + os.path.join(ROOT, "tests", "emu"), _EMUF_SRC, "-o", _EMUF_LIB], check=True)
+    L = ctypes.CDLL(_EMUF_LIB)
+    i, d = ctypes.c_int, ctypes.c_double
+    L.emu_fast_pressure_projection.argtypes = [i, i, i, d, d, _dp, i, i, _dp, _dp, _dp, _dp, _dp, d, d, i]
+    L.emu_fast_supported.argtypes = [i, i]
+    return L
+
+
+def emu_fast_projection(case, beta=0.0, split=False):
+    L = emu_fast_lib()
+    u, v, w = case.u.copy(), case.v.copy(), case.w.copy()
+    p, phi = np.zeros_like(u), np.empty_like(u)
+    zc = np.ascontiguousarray(case.zc)
+    rc = L.emu_fast_pressure_projection(case.nx, case.ny, case.nz, case.Lx, case.Ly, _p(zc), case.bc_x, case.bc_y,
+                                        _p(u), _p(v), _p(w), _p(p), _p(phi), case.alpha_dt, beta, int(split))
+    assert rc == 0, rc
+    return u, v, w, p, phi
+
+
 def _p(a):
     assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
     return a.ctypes.data_as(_dp)
