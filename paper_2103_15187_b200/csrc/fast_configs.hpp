@@ -11,8 +11,3 @@
 #define FSEI_Y_CONFIGS(X) \
     X(16, 4, 4, 1, 8) X(32, 8, 4, 1, 8) X(64, 8, 8, 1, 8) X(128, 8, 16, 1, 8) X(256, 16, 16, 1, 8) X(512, 8, 8, 8, 4) \
     X(1024, 16, 8, 8, 4) X(48, 8, 6, 1, 8) X(96, 16, 6, 1, 8) X(192, 8, 4, 6, 8) X(384, 8, 8, 6, 4) X(768, 16, 8, 6, 4)
-
-namespace fsei {
-// lines per CTA of the x kernels: about 256 threads
-template <class C> struct XShape { static constexpr int LPB = (256 / C::T) > 0 ? (256 / C::T) : 1; };
-}

@@ -18,12 +18,12 @@ bool xfast_supported(int N)
 
 template <class C, bool NEU> static cudaError_t init_one()
 {
-    constexpr int LPB = XShape<C>::LPB;
-    const int bytes = (int)XSmemLayout<C, LPB, NEU>::BYTES;
+    constexpr int LPB = XShape<C, NEU>::LPB;
+    const int bf = (int)XSmemLayout<C, LPB, NEU, 4 * LPB + 1>::BYTES, b1 = (int)XSmemLayout<C, LPB, NEU, LPB>::BYTES;
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e;
-    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e;
-    return cudaFuncSetAttribute(k_xi_fast<C, LPB, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bf))) return e;
+    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1))) return e;
+    return cudaFuncSetAttribute(k_xi_fast<C, LPB, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1);
 }
 
 cudaError_t xfast_init()
@@ -40,11 +40,10 @@ cudaError_t xfast_init()
 template <class C, bool NEU> static cudaError_t xf_one(const XFast& P, const SParams& S, bool fused, const double* u, const double* v,
                                                        const double* w, double inv_adt, cplx* spec, cudaStream_t st)
 {
-    constexpr int LPB = XShape<C>::LPB;
+    constexpr int LPB = XShape<C, NEU>::LPB;
     dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
-    const size_t bytes = XSmemLayout<C, LPB, NEU>::BYTES;
-    if (fused) k_xf_fast<C, LPB, NEU, true><<<grid, C::T * LPB, bytes, st>>>(P, S, u, v, w, inv_adt, spec);
-    else k_xf_fast<C, LPB, NEU, false><<<grid, C::T * LPB, bytes, st>>>(P, S, u, v, w, inv_adt, spec);
+    if (fused) k_xf_fast<C, LPB, NEU, true><<<grid, C::T * LPB, XSmemLayout<C, LPB, NEU, 4 * LPB + 1>::BYTES, st>>>(P, S, u, v, w, inv_adt, spec);
+    else k_xf_fast<C, LPB, NEU, false><<<grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, st>>>(P, S, u, v, w, inv_adt, spec);
     return cudaGetLastError();
 }
 
@@ -63,9 +62,9 @@ cudaError_t launch_xf_fast(const XFast& P, const SParams& S, bool neu, bool fuse
 
 template <class C, bool NEU> static cudaError_t xi_one(const XFast& P, const cplx* spec, double* phi, cudaStream_t st)
 {
-    constexpr int LPB = XShape<C>::LPB;
+    constexpr int LPB = XShape<C, NEU>::LPB;
     dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
-    k_xi_fast<C, LPB, NEU><<<grid, C::T * LPB, XSmemLayout<C, LPB, NEU>::BYTES, st>>>(P, spec, phi);
+    k_xi_fast<C, LPB, NEU><<<grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, st>>>(P, spec, phi);
     return cudaGetLastError();
 }
 

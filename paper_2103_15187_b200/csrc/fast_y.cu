@@ -4,6 +4,37 @@
 
 namespace fsei {
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libfsei does not link libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// 2-D fp64 view of the spectrum: inner dimension 2 nxc doubles (one row of one plane), outer ny nz rows;
+// box = 2 CY doubles x box_rows rows
+static cudaError_t make_map(const YFast& P, int CY, int box_rows, cplx* spec, TmaMap2D* out)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return cudaErrorNotSupported;
+    cuuint64_t dims[2] = {(cuuint64_t)2 * P.nxc, (cuuint64_t)P.ny * P.nz};
+    cuuint64_t strides[1] = {(cuuint64_t)P.nxc * sizeof(cplx)};
+    cuuint32_t box[2] = {(cuuint32_t)(2 * CY), (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(&out->m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, spec, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 bool yfast_supported(int N)
 {
     switch (N) {
@@ -41,10 +72,13 @@ template <class C, int CY> static cudaError_t y_one(const YFast& P, bool inv, bo
     dim3 grid(gx, gy);
     const int nt = C::T * CY;
     const size_t b0 = YSmemLayout<C, CY, false>::BYTES, b1 = YSmemLayout<C, CY, true>::BYTES;
-    if (!inv && !neu) k_y_fast<C, CY, false, false><<<grid, nt, b0, st>>>(P, spec);
-    else if (inv && !neu) k_y_fast<C, CY, true, false><<<grid, nt, b0, st>>>(P, spec);
-    else if (!inv && neu) k_y_fast<C, CY, false, true><<<grid, nt, b1, st>>>(P, spec);
-    else k_y_fast<C, CY, true, true><<<grid, nt, b1, st>>>(P, spec);
+    TmaMap2D map;
+    cudaError_t e = make_map(P, CY, y_box_rows(C::N), spec, &map);
+    if (e != cudaSuccess) return e;
+    if (!inv && !neu) k_y_fast<C, CY, false, false><<<grid, nt, b0, st>>>(P, map, spec);
+    else if (inv && !neu) k_y_fast<C, CY, true, false><<<grid, nt, b0, st>>>(P, map, spec);
+    else if (!inv && neu) k_y_fast<C, CY, false, true><<<grid, nt, b1, st>>>(P, map, spec);
+    else k_y_fast<C, CY, true, true><<<grid, nt, b1, st>>>(P, map, spec);
     return cudaGetLastError();
 }
 

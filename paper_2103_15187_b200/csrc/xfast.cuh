@@ -4,7 +4,9 @@
 //
 // A CTA of T*LPB threads owns LPB adjacent x-lines (rows j) and marches along z over `kchunk` planes:
 // T threads per line, each holding the line's butterflies of one Stockham pass in registers
-// (fast_fft.cuh).  Real lines are transformed as N complex values z_t = x[2t] + i x[2t+1] followed
+// (fast_fft.cuh).  The lines of plane k+1 are fetched by the TMA engine (cp.async.bulk into a shared-memory
+// landing tile, completion on an mbarrier) while the CTA transforms plane k, so no thread ever waits on a
+// global load.  Real lines are transformed as N complex values z_t = x[2t] + i x[2t+1] followed
 // (forward) or preceded (inverse) by the Hermitian pair step; Neumann lines go through Makhoul's
 // even/odd reorder (staged in shared memory) and the quarter-wave twiddle (DCT-II / DCT-III).
 //
@@ -47,39 +49,56 @@ FSEI_HD int xs_pitch(int n) { return n + (n >> 2) + 2; }
 // Makhoul: index of the natural line element that sits at position s of the reordered sequence v
 FSEI_HD int makhoul(int s, int n) { return (s < (n >> 1)) ? 2 * s : 2 * (n - 1 - s) + 1; }
 
-template <class C, int LPB, bool NEU> struct XSmemLayout {
+// lines per CTA and shared-memory carve-up of the x kernels.
+//   [mbarrier | landing tile (TMA destination) | line buffers | twiddles | r2c twiddles | dct twiddles | staging]
+// landing tile: forward: u lines [LPB], v lines [LPB+1] (row j+1 of the last line), w lines of planes k and k+1
+// [2][LPB] (doubles, n per line); inverse / non-fused forward: LPB lines of n doubles.
+template <class C, bool NEU> struct XShape {
     static constexpr int N = C::N;
+    static constexpr size_t tables = sizeof(cplx) * (C::TW + N / 2 + 1 + (NEU ? N + 1 : 0));
+    static constexpr size_t bytes(int L) {
+        return 128 + sizeof(double) * (size_t)(4 * L + 1) * 2 * N + sizeof(cplx) * (size_t)L * C::PITCH + tables +
+               (NEU ? sizeof(double) * (size_t)L * (2 * N + (2 * N >> 2) + 2) : 0);
+    }
+    static constexpr int fit(int L) { return (L <= 1 || bytes(L) <= 200 * 1024) ? L : fit(L - 1); }
+    static constexpr int LPB = fit((256 / C::T) > 0 ? (256 / C::T) : 1);      // about 256 threads, <= 200 KB
+};
+
+// LL = lines of n doubles in the landing tile: 4 LPB + 1 (fused forward) or LPB
+template <class C, int LPB, bool NEU, int LL> struct XSmemLayout {
+    static constexpr int N = C::N;
+    static constexpr int LAND = LL * 2 * N;                     // doubles
     static constexpr int BUF = LPB * C::PITCH;                  // complex
     static constexpr int TWS = C::TW;
     static constexpr int R2C = N / 2 + 1;
     static constexpr int DCT = NEU ? N + 1 : 0;
     static constexpr int XS = NEU ? LPB * (2 * N + (2 * N >> 2) + 2) : 0;     // doubles
-    static constexpr size_t BYTES = sizeof(cplx) * (BUF + TWS + R2C + DCT) + sizeof(double) * XS;
+    static constexpr size_t BYTES = 128 + sizeof(double) * LAND + sizeof(cplx) * (BUF + TWS + R2C + DCT) + sizeof(double) * XS;
 };
 
-// Whole line transform for the threads of one line.  load0(v) fills the first pass' registers (from global
-// memory / staging; IN_BUF: from the line buffer itself, then a barrier separates its reads from the writes);
+struct NoHook { FSEI_HD void operator()() const {} };
+
+// Whole line transform for the threads of one line.  load0(v) fills the first pass' registers (from the landing
+// tile / staging; IN_BUF: from the line buffer itself, then a barrier separates its reads from the writes);
 // `out` receives the natural-order result (OUT_BUF: it writes the line buffer, so a barrier precedes it).
-// Must be reached by every thread of the CTA; `act` false = this thread's line does not exist.
-template <class C, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out>
-FSEI_DEV void fft_line(int tl, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out)
+// hook() runs on every thread right after the first barrier, i.e. once every thread has consumed its first-pass
+// input (that is where the next tile's asynchronous load is issued).  Must be reached by every thread of the CTA;
+// `act` false = this thread's line does not exist.
+template <class C, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out, class Hook>
+FSEI_DEV void fft_line(int tl, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook)
 {
     constexpr int N = C::N, T = C::T;
+    static_assert(C::NP >= 2, "pipelined kernels need at least two passes");
     SmIn<C> bin{buf}; SmOut<C> bout{buf};
     {
         cplx v[PassShape<N, C::R0, 1, T>::PER][C::R0];
         if (act) load0(v);
-        if constexpr (C::NP == 1) {
-            if (IN_BUF && OUT_BUF) FSEI_SYNC();
-            if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, out);
-            return;
-        } else {
-            if (IN_BUF) FSEI_SYNC();
-            if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, bout);
-        }
+        if (IN_BUF) { FSEI_SYNC(); hook(); }
+        if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, bout);
     }
     FSEI_SYNC();
-    if constexpr (C::NP >= 2) {
+    if (!IN_BUF) hook();
+    {
         cplx v[PassShape<N, C::R1, C::R0, T>::PER][C::R1];
         if (act) fft_pass_load<N, C::R1, C::R0, T>(tl, bin, v);
         if constexpr (C::NP == 2) {
@@ -108,66 +127,101 @@ FSEI_HD void st2(double* p, cplx v) { *reinterpret_cast<cplx*>(p) = v; }
 // grid (ceil(ny / LPB), ceil(nz / kchunk)), block T*LPB, dynamic shared memory XSmemLayout::BYTES
 // ---------------------------------------------------------------------------------------------------
 template <class C, int LPB, bool NEU, bool FUSED>
-FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xf_fast(XFast P, SParams S, const double* u, const double* v, const double* w,
+FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const double* v, const double* w,
                                      double inv_adt, cplx* spec)
 {
-    using L = XSmemLayout<C, LPB, NEU>;
+    using L = XSmemLayout<C, LPB, NEU, (FUSED ? 4 * LPB + 1 : LPB)>;
     constexpr int N = C::N, T = C::T, R0 = C::R0;
     constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
     static_assert(NB0 % T == 0, "first pass must tile the line exactly");
     constexpr int NPAIR = N / T;                                  // real pairs per thread
+    constexpr int n = 2 * N;
     FSEI_DYN_SMEM(smraw);
-    cplx* buf = reinterpret_cast<cplx*>(smraw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
+    double* land = reinterpret_cast<double*>(smraw + 128);
+    cplx* buf = reinterpret_cast<cplx*>(land + L::LAND);
     cplx* tws = buf + L::BUF;
     cplx* tr2c = tws + L::TWS;
     cplx* tdct = tr2c + L::R2C;
     double* xs = reinterpret_cast<double*>(tdct + L::DCT);
+    double* LU = land;                                            // [LPB][n]
+    double* LV = LU + LPB * n;                                    // [LPB + 1][n]
+    double* LW = LV + (LPB + 1) * n;                              // [2][LPB][n], plane k in slot k & 1
     const int tid = threadIdx.x, nt = T * LPB;
     const int li = tid / T, tl = tid - li * T;
+    const int ny = P.ny, nz = P.nz;
+    const int j0 = blockIdx.x * LPB, j = j0 + li;
+    const int nl = (ny - j0 < LPB) ? ny - j0 : LPB;               // lines of this CTA that exist
+    const bool act = j < ny;
+    const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
+    const size_t plane = (size_t)ny * n;
+    const bool yper = S.bcy == BC_PERIODIC, xper = S.bcx == BC_PERIODIC;
+    const bool wrap = (j0 + nl == ny);                            // row j+1 of the last line wraps (or is a wall)
+    const bool has_jp = (j + 1 < ny) || yper;
+
+    // asynchronous load of the tile of plane k (one thread)
+    auto issue = [&](int k) {
+        const unsigned lb = n * sizeof(double);
+        const size_t g0 = ((size_t)k * ny + j0) * n;
+        if (!FUSED) {
+            abar_expect(bar, nl * lb);
+            bulk_g2s(LU, u + g0, nl * lb, bar);
+            return;
+        }
+        const int nv = wrap ? nl : nl + 1;
+        const bool first = (k == k0), up = (k + 1 < nz);
+        unsigned total = nl * lb + nv * lb + ((wrap && yper) ? lb : 0) + (first ? nl * lb : 0) + (up ? nl * lb : 0);
+        abar_expect(bar, total);
+        bulk_g2s(LU, u + g0, nl * lb, bar);
+        bulk_g2s(LV, v + g0, nv * lb, bar);
+        if (wrap && yper) bulk_g2s(LV + nl * n, v + (size_t)k * plane, lb, bar);
+        if (first) bulk_g2s(LW + (size_t)(k & 1) * LPB * n, w + g0, nl * lb, bar);
+        if (up) bulk_g2s(LW + (size_t)((k + 1) & 1) * LPB * n, w + g0 + plane, nl * lb, bar);
+    };
+
+    if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, nt);
     for (int i = tid; i < L::R2C; i += nt) tr2c[i] = P.tw_r2c[i];
     if (NEU) for (int i = tid; i < L::DCT; i += nt) tdct[i] = P.tw_dct[i];
     FSEI_SYNC();
+    if (tid == 0 && k0 < k1) issue(k0);
+    unsigned parity = 0;
 
-    const int n = 2 * N, ny = P.ny, nz = P.nz;
-    const int j = blockIdx.x * LPB + li;
-    const bool act = j < ny;
-    const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
     cplx* lbuf = buf + li * C::PITCH;
     double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
-    const size_t plane = (size_t)ny * n;
-    const bool has_jp = (j + 1 < ny) || S.bcy == BC_PERIODIC;
-    const bool xper = S.bcx == BC_PERIODIC;
-
-    // (rhs[2t], rhs[2t+1]) of line (j,k).  The CTA marches along z, so the w(k+1) pairs read here are read
-    // again as w(k) by the same threads one iteration later (from L1/L2, not from DRAM).
-    auto rhs_pair = [&](int k, int t) -> cplx {
-        const size_t line = ((size_t)k * ny + j) * n;
-        if (!FUSED) return ld2(u + line + 2 * t);
-        const size_t linejp = (j + 1 < ny) ? line + n : line - (size_t)(ny - 1) * n;
-        cplx uu = ld2(u + line + 2 * t);
-        double un = (2 * t + 2 < n) ? u[line + 2 * t + 2] : (xper ? u[line] : 0.0);
-        cplx vv = ld2(v + line + 2 * t);
-        cplx vp = has_jp ? ld2(v + linejp + 2 * t) : cmake(0.0, 0.0);
-        cplx wk = ld2(w + line + 2 * t);
-        cplx wp = (k + 1 < nz) ? ld2(w + line + plane + 2 * t) : cmake(0.0, 0.0);
-        const double rdz = S.rdzc[k];
-        return cmake(div_cell(uu.re, uu.im, vv.re, vp.re, wk.re, wp.re, S.rdx, S.rdy, rdz, inv_adt),
-                     div_cell(uu.im, un, vv.im, vp.im, wk.im, wp.im, S.rdx, S.rdy, rdz, inv_adt));
-    };
+    const double* lu = LU + li * n;
+    const double* lv = LV + li * n;
 
     for (int k = k0; k < k1; k++) {
+        abar_wait(bar, parity); parity ^= 1;
+        // (rhs[2t], rhs[2t+1]) of line (j,k) from the landing tile
+        auto rhs_pair = [&](int t) -> cplx {
+            if (!FUSED) return ld2(lu + 2 * t);
+            const double* lwk = LW + ((size_t)(k & 1) * LPB + li) * n;
+            const double* lwp = LW + ((size_t)((k + 1) & 1) * LPB + li) * n;
+            cplx uu = ld2(lu + 2 * t);
+            double un = (2 * t + 2 < n) ? lu[2 * t + 2] : (xper ? lu[0] : 0.0);
+            cplx vv = ld2(lv + 2 * t);
+            cplx vp = has_jp ? ld2(lv + n + 2 * t) : cmake(0.0, 0.0);
+            cplx wk = ld2(lwk + 2 * t);
+            cplx wp = (k + 1 < nz) ? ld2(lwp + 2 * t) : cmake(0.0, 0.0);
+            const double rdz = S.rdzc[k];
+            return cmake(div_cell(uu.re, uu.im, vv.re, vp.re, wk.re, wp.re, S.rdx, S.rdy, rdz, inv_adt),
+                         div_cell(uu.im, un, vv.im, vp.im, wk.im, wp.im, S.rdx, S.rdy, rdz, inv_adt));
+        };
+        auto next = [&]() { if (tid == 0 && k + 1 < k1) issue(k + 1); };
         if (NEU) {
-            // stage the real line (coalesced), then the first pass reads it through Makhoul's reorder
+            // stage the real line, then the first pass reads it through Makhoul's reorder
             if (act) {
 #pragma unroll
                 for (int e = 0; e < NPAIR; e++) {
                     int t = tl + e * T;
-                    cplx r = rhs_pair(k, t);
+                    cplx r = rhs_pair(t);
                     lxs[xs_pad(2 * t)] = r.re; lxs[xs_pad(2 * t + 1)] = r.im;
                 }
             }
             FSEI_SYNC();
+            next();
         }
         auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll
@@ -176,11 +230,12 @@ FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xf_fast(XFast P, SParams S, c
                 for (int q = 0; q < R0; q++) {
                     const int t = tl + i * T + q * NB0;
                     if (NEU) v0[i][q] = cmake(lxs[xs_pad(makhoul(2 * t, n))], lxs[xs_pad(makhoul(2 * t + 1, n))]);
-                    else v0[i][q] = rhs_pair(k, t);
+                    else v0[i][q] = rhs_pair(t);
                 }
             }
         };
-        fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf});
+        if (NEU) fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, NoHook{});
+        else fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, next);
         FSEI_SYNC();
         // Hermitian pair step (+ quarter-wave twiddle): Z -> packed half spectrum, written to global memory
         if (act) {
@@ -212,37 +267,49 @@ FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xf_fast(XFast P, SParams S, c
 // a6: phi(line) = scale * C2R / DCT-III of spec(line), in place
 // ---------------------------------------------------------------------------------------------------
 template <class C, int LPB, bool NEU>
-FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xi_fast(XFast P, const cplx* spec, double* phi)
+FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const cplx* spec, double* phi)
 {
-    using L = XSmemLayout<C, LPB, NEU>;
+    using L = XSmemLayout<C, LPB, NEU, LPB>;
     constexpr int N = C::N, T = C::T, R0 = C::R0;
-    constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
     constexpr int NPAIR = N / T;
+    constexpr int n = 2 * N;
     FSEI_DYN_SMEM(smraw);
-    cplx* buf = reinterpret_cast<cplx*>(smraw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
+    cplx* land = reinterpret_cast<cplx*>(smraw + 128);             // [LPB][N] packed spectrum lines
+    cplx* buf = reinterpret_cast<cplx*>(reinterpret_cast<double*>(smraw + 128) + L::LAND);
     cplx* tws = buf + L::BUF;
     cplx* tr2c = tws + L::TWS;
     cplx* tdct = tr2c + L::R2C;
     double* xs = reinterpret_cast<double*>(tdct + L::DCT);
     const int tid = threadIdx.x, nt = T * LPB;
     const int li = tid / T, tl = tid - li * T;
+    const int ny = P.ny, nz = P.nz;
+    const int j0 = blockIdx.x * LPB, j = j0 + li;
+    const int nl = (ny - j0 < LPB) ? ny - j0 : LPB;
+    const bool act = j < ny;
+    const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
+    auto issue = [&](int k) {
+        const unsigned bytes = (unsigned)(nl * N * sizeof(cplx));
+        abar_expect(bar, bytes);
+        bulk_g2s(land, spec + ((size_t)k * ny + j0) * N, bytes, bar);
+    };
+    if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, nt);
     for (int i = tid; i < L::R2C; i += nt) tr2c[i] = P.tw_r2c[i];
     if (NEU) for (int i = tid; i < L::DCT; i += nt) tdct[i] = P.tw_dct[i];
     FSEI_SYNC();
+    if (tid == 0 && k0 < k1) issue(k0);
+    unsigned parity = 0;
 
-    const int n = 2 * N, ny = P.ny, nz = P.nz;
-    const int j = blockIdx.x * LPB + li;
-    const bool act = j < ny;
-    const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
     cplx* lbuf = buf + li * C::PITCH;
     double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
+    const cplx* g = land + li * N;
     const double scale = P.scale;
 
     for (int k = k0; k < k1; k++) {
+        abar_wait(bar, parity); parity ^= 1;
         // packed half spectrum -> Z (Hermitian pair step, preceded by the inverse quarter-wave twiddle)
         if (act) {
-            const cplx* g = spec + ((size_t)k * ny + j) * N;
             for (int p = tl; p <= N / 2; p += T) {
                 if (p == 0) {
                     cplx s = g[0];
@@ -261,16 +328,17 @@ FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xi_fast(XFast P, const cplx* 
             }
         }
         FSEI_SYNC();
+        if (tid == 0 && k + 1 < k1) issue(k + 1);                   // landing tile consumed: prefetch the next plane
         double* gl = phi + ((size_t)k * ny + j) * n;
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, SmIn<C>{lbuf}, v0); };
         if (!NEU) {
             auto out = [&](int t, cplx z) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
-            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out);
+            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{});
         } else {
             auto out = [&](int t, cplx z) {
                 lxs[xs_pad(makhoul(2 * t, n))] = z.re * scale; lxs[xs_pad(makhoul(2 * t + 1, n))] = z.im * scale;
             };
-            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out);
+            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{});
             FSEI_SYNC();
             if (act) {
 #pragma unroll
@@ -282,7 +350,6 @@ FSEI_GLOBAL(C::T * LPB, (C::RMAX >= 16 ? 1 : 2)) k_xi_fast(XFast P, const cplx* 
         }
         FSEI_SYNC();
     }
-    (void)NB0; (void)PER0;
 }
 
 }  // namespace fsei

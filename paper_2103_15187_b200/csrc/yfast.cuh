@@ -2,9 +2,12 @@
 // place, for ny = 2^a or 3 2^a (include/fsei.h; R15, sec. 6).
 //
 // A CTA of T*CY threads owns a tile of CY adjacent x-slots (CY*16 contiguous bytes per row) times all ny
-// rows of one z-plane and loops over planes.  Thread (c, tl) holds butterflies of column c in registers;
-// the first pass reads global memory directly (row stride nxc), the last writes it; in between the
-// column tile sits in one shared buffer [pad(n)][CY].
+// rows of one z-plane and loops over planes.  The tile of the next plane is fetched by the TMA engine
+// (cp.async.bulk.tensor.2d boxes of <= 256 rows x CY*16 bytes through a CUtensorMap of the spectrum, into a
+// dense shared-memory landing tile [n][CY], completion on an mbarrier) while the CTA transforms the current
+// one.  Thread (c, tl) holds butterflies of column c in registers: the first pass reads the landing tile,
+// the last writes global memory (row stride nxc); in between the column tile sits in a padded shared
+// buffer [pad(n)][CY].
 //
 //   periodic y: complex FFT.  Columns whose Re and Im are two different real x-sequences A, B (slot 0 of
 //               a periodic x-transform: (X_0, X_N); every slot of a Neumann x-transform) carry two
@@ -26,11 +29,14 @@ struct YFast {
 };
 
 template <class C, int CY, bool NEU> struct YSmemLayout {
+    static constexpr int LAND = C::N * CY;                      // complex, dense TMA destination
     static constexpr int BUF = C::PITCH * CY;
     static constexpr int TWS = C::TW;
     static constexpr int DCT = NEU ? C::N / 2 + 1 : 0;
-    static constexpr size_t BYTES = sizeof(cplx) * (BUF + TWS + DCT);
+    static constexpr size_t BYTES = 128 + sizeof(cplx) * (LAND + BUF + TWS + DCT);
 };
+// rows per TMA box: the largest divisor of N that is <= 256
+FSEI_HD constexpr int y_box_rows(int N) { int b = N < 256 ? N : 256; while (N % b) b--; return b; }
 
 template <class C, int CY> struct YIn {
     const cplx* s; int c;
@@ -42,25 +48,21 @@ template <class C, int CY> struct YOut {
 };
 
 // same pass sequence as fft_line (xfast.cuh) on a column of the [n][CY] tile
-template <class C, int CY, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out>
-FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out)
+template <class C, int CY, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out, class Hook>
+FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook)
 {
     constexpr int N = C::N, T = C::T;
+    static_assert(C::NP >= 2, "pipelined kernels need at least two passes");
     YIn<C, CY> bin{buf, c}; YOut<C, CY> bout{buf, c};
     {
         cplx v[PassShape<N, C::R0, 1, T>::PER][C::R0];
         if (act) load0(v);
-        if constexpr (C::NP == 1) {
-            if (IN_BUF && OUT_BUF) FSEI_SYNC();
-            if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, out);
-            return;
-        } else {
-            if (IN_BUF) FSEI_SYNC();
-            if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, bout);
-        }
+        if (IN_BUF) { FSEI_SYNC(); hook(); }
+        if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, bout);
     }
     FSEI_SYNC();
-    if constexpr (C::NP >= 2) {
+    if (!IN_BUF) hook();
+    {
         cplx v[PassShape<N, C::R1, C::R0, T>::PER][C::R1];
         if (act) fft_pass_load<N, C::R1, C::R0, T>(tl, bin, v);
         if constexpr (C::NP == 2) {
@@ -81,47 +83,64 @@ FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Lo
     }
 }
 
-// grid (ceil(nxc / CY), gy <= nz), block T*CY, dynamic shared memory YSmemLayout::BYTES
+// grid (ceil(nxc / CY), gy <= nz), block T*CY, dynamic shared memory YSmemLayout::BYTES.
+// map: 2-D tensor map of the spectrum, inner dimension 2 nxc doubles, outer ny nz rows, box 2 CY x y_box_rows(ny)
 template <class C, int CY, bool INV, bool NEU>
-FSEI_GLOBAL(C::T * CY, (C::RMAX >= 16 || C::T * CY > 256 ? 1 : 2)) k_y_fast(YFast P, cplx* spec)
+FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D map, cplx* spec)
 {
     using L = YSmemLayout<C, CY, NEU>;
     constexpr int N = C::N, T = C::T, R0 = C::R0;
     constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
+    constexpr int BOX = y_box_rows(N);
     static_assert(NB0 % T == 0, "first pass must tile the column exactly");
     FSEI_DYN_SMEM(smraw);
-    cplx* buf = reinterpret_cast<cplx*>(smraw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
+    cplx* land = reinterpret_cast<cplx*>(smraw + 128);           // [N][CY]
+    cplx* buf = land + L::LAND;
     cplx* tws = buf + L::BUF;
     cplx* tdct = tws + L::TWS;
     const int tid = threadIdx.x, nt = T * CY;
     const int tl = tid / CY, c = tid - tl * CY;
-    fft_fill_twiddles<C>(tws, P.tw, tid, nt);
-    if (NEU) for (int i = tid; i < L::DCT; i += nt) tdct[i] = P.tw_dct[i];
-    FSEI_SYNC();
-
     const int nxc = P.nxc;
     const int c0 = blockIdx.x * CY, col = c0 + c;
     const bool act = col < nxc;
     const bool pairing = NEU || (c0 < P.untangle);            // CTA-uniform
     const bool mine = NEU || (col < P.untangle);              // this column is split / merged
     const double SQ2 = 1.41421356237309504880168872420969808;
+    const int kstep = gridDim.y;
 
-    for (int k = blockIdx.y; k < P.nz; k += gridDim.y) {
+    auto issue = [&](int k) {
+        abar_expect(bar, (unsigned)(N * CY * sizeof(cplx)));
+#pragma unroll
+        for (int b = 0; b < N / BOX; b++) tma_load_2d(land + b * BOX * CY, &map, 2 * c0, k * N + b * BOX, bar);
+    };
+    if (tid == 0) abar_init(bar);
+    fft_fill_twiddles<C>(tws, P.tw, tid, nt);
+    if (NEU) for (int i = tid; i < L::DCT; i += nt) tdct[i] = P.tw_dct[i];
+    FSEI_SYNC();
+    if (tid == 0 && (int)blockIdx.y < P.nz) issue(blockIdx.y);
+    unsigned parity = 0;
+
+    for (int k = blockIdx.y; k < P.nz; k += kstep) {
+        abar_wait(bar, parity); parity ^= 1;
         cplx* g = spec + (size_t)k * N * nxc + col;            // row r of this column at g[r * nxc]
-        auto row_of = [&](int n) -> size_t { return (size_t)(NEU ? dct_perm(n, N) : n) * nxc; };
+        auto next = [&]() { if (tid == 0 && k + kstep < P.nz) issue(k + kstep); };
         if (!INV) {
             auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll
                 for (int i = 0; i < PER0; i++) {
 #pragma unroll
-                    for (int q = 0; q < R0; q++) v0[i][q] = g[row_of(tl + i * T + q * NB0)];
+                    for (int q = 0; q < R0; q++) {
+                        const int n = tl + i * T + q * NB0;
+                        v0[i][q] = land[(NEU ? dct_perm(n, N) : n) * CY + c];
+                    }
                 }
             };
             if (!pairing) {
                 auto out = [&](int n, cplx z) { g[(size_t)n * nxc] = z; };
-                fft_column<C, CY, false, false, false>(tl, c, act, buf, tws, load0, out);
+                fft_column<C, CY, false, false, false>(tl, c, act, buf, tws, load0, out, next);
             } else {
-                fft_column<C, CY, false, false, true>(tl, c, act, buf, tws, load0, YOut<C, CY>{buf, c});
+                fft_column<C, CY, false, false, true>(tl, c, act, buf, tws, load0, YOut<C, CY>{buf, c}, next);
                 FSEI_SYNC();
                 if (act) {
                     for (int kk = tl; kk <= N / 2; kk += T) {
@@ -148,27 +167,27 @@ FSEI_GLOBAL(C::T * CY, (C::RMAX >= 16 || C::T * CY > 256 ? 1 : 2)) k_y_fast(YFas
                 }
             }
         } else {
-            auto out = [&](int n, cplx z) { g[row_of(n)] = z; };
+            auto out = [&](int n, cplx z) { g[(size_t)(NEU ? dct_perm(n, N) : n) * nxc] = z; };
             if (!pairing) {
                 auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll
                     for (int i = 0; i < PER0; i++) {
 #pragma unroll
-                        for (int q = 0; q < R0; q++) v0[i][q] = g[(size_t)(tl + i * T + q * NB0) * nxc];
+                        for (int q = 0; q < R0; q++) v0[i][q] = land[(tl + i * T + q * NB0) * CY + c];
                     }
                 };
-                fft_column<C, CY, true, false, false>(tl, c, act, buf, tws, load0, out);
+                fft_column<C, CY, true, false, false>(tl, c, act, buf, tws, load0, out, next);
             } else {
                 if (act) {
                     for (int kk = tl; kk <= N / 2; kk += T) {
-                        cplx a = g[(size_t)kk * nxc];
+                        cplx a = land[kk * CY + c];
                         if (kk == 0 || (!NEU && (2 * kk == N || !mine))) {
                             buf[C::pad(kk) * CY + c] = a;
-                            if (kk != 0 && 2 * kk != N) buf[C::pad(N - kk) * CY + c] = g[(size_t)(N - kk) * nxc];
+                            if (kk != 0 && 2 * kk != N) buf[C::pad(N - kk) * CY + c] = land[(N - kk) * CY + c];
                             continue;
                         }
                         if (NEU && 2 * kk == N) { buf[C::pad(kk) * CY + c] = cmake(a.re * SQ2, a.im * SQ2); continue; }
-                        cplx b = g[(size_t)(N - kk) * nxc];
+                        cplx b = land[(N - kk) * CY + c];
                         if (NEU) {
                             cplx wk = tdct[kk];
                             cplx ta = cmulc(cmake(a.re, -b.re), wk);     // V^a_k
@@ -180,8 +199,9 @@ FSEI_GLOBAL(C::T * CY, (C::RMAX >= 16 || C::T * CY > 256 ? 1 : 2)) k_y_fast(YFas
                     }
                 }
                 FSEI_SYNC();
+                next();                                         // landing tile consumed
                 auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, YIn<C, CY>{buf, c}, v0); };
-                fft_column<C, CY, true, true, false>(tl, c, act, buf, tws, load0, out);
+                fft_column<C, CY, true, true, false>(tl, c, act, buf, tws, load0, out, NoHook{});
             }
         }
         FSEI_SYNC();

@@ -34,11 +34,10 @@ bool y_ok(int N) { switch (N) {
 template <class C, bool NEU> void xf_one(const XFast& P, const SParams& S, bool fused, const double* u, const double* v, const double* w,
                                          double inv_adt, cplx* spec)
 {
-    constexpr int LPB = XShape<C>::LPB;
+    constexpr int LPB = XShape<C, NEU>::LPB;
     dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
-    const size_t bytes = XSmemLayout<C, LPB, NEU>::BYTES;
-    if (fused) cuda_shim::launch(grid, C::T * LPB, bytes, [&] { k_xf_fast<C, LPB, NEU, true>(P, S, u, v, w, inv_adt, spec); });
-    else cuda_shim::launch(grid, C::T * LPB, bytes, [&] { k_xf_fast<C, LPB, NEU, false>(P, S, u, v, w, inv_adt, spec); });
+    if (fused) cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, 4 * LPB + 1>::BYTES, [&] { k_xf_fast<C, LPB, NEU, true>(P, S, u, v, w, inv_adt, spec); });
+    else cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xf_fast<C, LPB, NEU, false>(P, S, u, v, w, inv_adt, spec); });
 }
 void xf(const XFast& P, const SParams& S, bool neu, bool fused, const double* u, const double* v, const double* w, double inv_adt, cplx* spec)
 {
@@ -51,9 +50,9 @@ void xf(const XFast& P, const SParams& S, bool neu, bool fused, const double* u,
 }
 template <class C, bool NEU> void xi_one(const XFast& P, const cplx* spec, double* phi)
 {
-    constexpr int LPB = XShape<C>::LPB;
+    constexpr int LPB = XShape<C, NEU>::LPB;
     dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
-    cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU>::BYTES, [&] { k_xi_fast<C, LPB, NEU>(P, spec, phi); });
+    cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xi_fast<C, LPB, NEU>(P, spec, phi); });
 }
 void xi(const XFast& P, bool neu, const cplx* spec, double* phi)
 {
@@ -70,10 +69,12 @@ template <class C, int CY> void y_one(const YFast& P, bool inv, bool neu, cplx* 
     dim3 grid(gx, gy);
     const int nt = C::T * CY;
     const size_t b0 = YSmemLayout<C, CY, false>::BYTES, b1 = YSmemLayout<C, CY, true>::BYTES;
-    if (!inv && !neu) cuda_shim::launch(grid, nt, b0, [&] { k_y_fast<C, CY, false, false>(P, spec); });
-    else if (inv && !neu) cuda_shim::launch(grid, nt, b0, [&] { k_y_fast<C, CY, true, false>(P, spec); });
-    else if (!inv && neu) cuda_shim::launch(grid, nt, b1, [&] { k_y_fast<C, CY, false, true>(P, spec); });
-    else cuda_shim::launch(grid, nt, b1, [&] { k_y_fast<C, CY, true, true>(P, spec); });
+    TmaMap2D map{reinterpret_cast<const unsigned char*>(spec), (size_t)P.nxc * sizeof(cplx), (unsigned)sizeof(double), 2u * CY,
+                 (unsigned)y_box_rows(C::N)};
+    if (!inv && !neu) cuda_shim::launch(grid, nt, b0, [&] { k_y_fast<C, CY, false, false>(P, map, spec); });
+    else if (inv && !neu) cuda_shim::launch(grid, nt, b0, [&] { k_y_fast<C, CY, true, false>(P, map, spec); });
+    else if (!inv && neu) cuda_shim::launch(grid, nt, b1, [&] { k_y_fast<C, CY, false, true>(P, map, spec); });
+    else cuda_shim::launch(grid, nt, b1, [&] { k_y_fast<C, CY, true, true>(P, map, spec); });
 }
 void yf(const YFast& P, bool inv, bool neu, cplx* spec)
 {
