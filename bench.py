@@ -37,7 +37,7 @@ ALGO_BYTES_PER_CELL = {
     "z_paired": 16.0, "z_solve": 16.0, "y_inverse": 16.0, "x_inverse": 16.0, "project": 72.0, "z_gauge": 0.0,
 }
 A_REF = 184.0          # reference accounting of one projection, B/cell
-SAMPLE_NY = 128        # CPU legs: the workload's grid with ny cut to this many rows
+SAMPLE_NY = 256        # CPU legs: the workload's grid with ny cut to this many rows
 
 
 def _peaks():
@@ -46,6 +46,20 @@ def _peaks():
         with open(path) as f:
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
     return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def _ncu_traffic(cfg: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the newest committed
+    `ncu --set full` capture (profiles/*_traffic.csv; the .md beside it names the command)."""
+    import glob
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
+        with open(path) as f:
+            for line in f.read().splitlines()[1:]:
+                c = line.split(",")
+                if len(c) >= 4 and c[0] == f"cfg{cfg}" and c[1] == kernel:
+                    best = float(c[2]) + float(c[3])
+    return best
 
 
 class ClockSampler:
@@ -237,11 +251,7 @@ def run_ours(args) -> dict:
     top = max(prof, key=lambda k: prof[k][0])
     top_ms = prof[top][0] / prof[top][1]
     achieved = ALGO_BYTES_PER_CELL.get(top, 0.0) * case.cells / (top_ms * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")     # dram bytes per launch from the committed ncu capture
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get(f"cfg{case.cfg}", {}).get(top)
+    traffic = _ncu_traffic(case.cfg, top)
     roofline = {"bound": "hbm", "kernel": top, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
                 "frac": round(achieved / peak, 4), "traffic": traffic, "peak_source": peak_src,
                 "algo_bytes_per_launch": ALGO_BYTES_PER_CELL.get(top, 0.0) * case.cells,
@@ -283,7 +293,7 @@ def run_ours(args) -> dict:
     # ---- CPU baseline: the oracle as it stands, rank 0 at N = 1 only --------------------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        val, cores, sample, _ = _oracle_sample(args.config, 3)
+        val, cores, sample, _ = _oracle_sample(args.config, 5)
         cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
     out = {
