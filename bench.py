@@ -35,6 +35,8 @@ UNIT = "Mcell/s"
 ALGO_BYTES_PER_CELL = {
     "divergence": 32.0, "x_forward": 16.0, "div_x_forward": 32.0, "y_forward": 16.0, "z_direct": 16.0,
     "z_paired": 16.0, "z_solve": 16.0, "y_inverse": 16.0, "x_inverse": 16.0, "project": 72.0, "z_gauge": 0.0,
+    # fused path: a3 + first Thomas sweep, second sweep + a5 (y 16 + half of the z step's 16 each)
+    "yz_forward": 24.0, "yz_backward": 24.0,
 }
 A_REF = 184.0          # reference accounting of one projection, B/cell
 SAMPLE_NY = 256        # CPU legs: the workload's grid with ny cut to this many rows

@@ -11,3 +11,11 @@
 #define FSEI_Y_CONFIGS(X) \
     X(16, 4, 4, 1, 8) X(32, 8, 4, 1, 8) X(64, 8, 8, 1, 8) X(128, 8, 16, 1, 8) X(256, 16, 16, 1, 8) X(512, 8, 8, 8, 4) \
     X(1024, 16, 8, 8, 4) X(48, 8, 6, 1, 8) X(96, 16, 6, 1, 8) X(192, 8, 4, 6, 8) X(384, 8, 8, 6, 4) X(768, 16, 8, 6, 4)
+
+// Fused path (blocked spectrum, z-marching y kernels of yzfused.cuh): slots per tile, and the lengths it is
+// instantiated for -- the large grids, where one CTA per x-slot tile fills the GPU.
+#define FSEI_CB 2
+// x direction, blocked stores / loads: (N, R0, R1, R2) -- same radices as FSEI_X_CONFIGS
+#define FSEI_XB_CONFIGS(X) X(256, 16, 16, 1) X(512, 8, 8, 8) X(1024, 16, 8, 8) X(384, 8, 8, 6)
+// y direction: (N, R0, R1, R2) -- same radices as FSEI_Y_CONFIGS
+#define FSEI_YZ_CONFIGS(X) X(384, 8, 8, 6) X(512, 8, 8, 8) X(768, 16, 8, 6) X(1024, 16, 8, 8)

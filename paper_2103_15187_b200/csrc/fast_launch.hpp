@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include "xfast.cuh"
 #include "yfast.cuh"
+#include "yzfused.cuh"
 
 namespace fsei {
 
@@ -13,10 +14,22 @@ bool yfast_supported(int N);     // N = ny
 cudaError_t xfast_init();
 cudaError_t yfast_init();
 
+// fused path (blocked spectrum layout, FSEI_CB slots per tile)
+bool xblocked_supported(int N);  // N = nx / 2
+bool yzfused_supported(int N);   // N = ny
+cudaError_t xblocked_init();
+cudaError_t yzfused_init();
+// tensor map of the blocked spectrum for the x-inverse loads (plan time; spec = the plan's workspace)
+cudaError_t make_xi_blocked_map(const XFast& P, bool neu, const cplx* spec, TmaMap3D* out);
+cudaError_t launch_yz_forward(const YZFused& P, bool neu, int ncomp, cplx* spec, cudaStream_t st);
+cudaError_t launch_yz_backward(const YZFused& P, bool neu, int ncomp, cplx* spec, cudaStream_t st);
+
 // a1+a2 (fused: rhs = D(u,v,w) * inv_adt) or a2 alone (u = rhs, v = w = nullptr)
+// blocked: spec is in the blocked layout (xi: read through `map`)
 cudaError_t launch_xf_fast(const XFast& P, const SParams& S, bool neu, bool fused, const double* u, const double* v,
-                           const double* w, double inv_adt, cplx* spec, cudaStream_t st);
-cudaError_t launch_xi_fast(const XFast& P, bool neu, const cplx* spec, double* phi, cudaStream_t st);
+                           const double* w, double inv_adt, cplx* spec, cudaStream_t st, bool blocked = false);
+cudaError_t launch_xi_fast(const XFast& P, bool neu, const cplx* spec, double* phi, cudaStream_t st,
+                           const TmaMap3D* map = nullptr);
 // a3 / a5, in place
 cudaError_t launch_y_fast(const YFast& P, bool inv, bool neu, cplx* spec, cudaStream_t st);
 

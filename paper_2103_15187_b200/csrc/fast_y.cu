@@ -1,30 +1,15 @@
 // fast_y.cu -- instantiations and launchers of the fast y-direction kernel (yfast.cuh).
 #include "fast_launch.hpp"
 #include "fast_configs.hpp"
+#include "tma_host.hpp"
 
 namespace fsei {
-
-// cuTensorMapEncodeTiled through the runtime's driver entry point (libfsei does not link libcuda)
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static EncodeTiledFn encode_fn()
-{
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(p);
-    }
-    return fn;
-}
 
 // 2-D fp64 view of the spectrum: inner dimension 2 nxc doubles (one row of one plane), outer ny nz rows;
 // box = 2 CY doubles x box_rows rows
 static cudaError_t make_map(const YFast& P, int CY, int box_rows, cplx* spec, TmaMap2D* out)
 {
-    EncodeTiledFn fn = encode_fn();
+    EncodeTiledFn fn = tma_encode_fn();
     if (!fn) return cudaErrorNotSupported;
     cuuint64_t dims[2] = {(cuuint64_t)2 * P.nxc, (cuuint64_t)P.ny * P.nz};
     cuuint64_t strides[1] = {(cuuint64_t)P.nxc * sizeof(cplx)};

@@ -18,6 +18,7 @@
 #include "yfft.cuh"
 #include "zsolve.cuh"
 #include "fast_launch.hpp"
+#include "fast_configs.hpp"
 #include "zfast.cuh"
 #include "stencil_fast.cuh"
 #include <cstdlib>
@@ -39,13 +40,15 @@ static int cuda_fail(cudaError_t e, const char* what)
 // ------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------
-enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, FSEI_NKERNELS };
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, FSEI_NKERNELS };
 
 struct fsei_plan {
     HostTables T;
     XParams X; YParams Y; ZParams Z; SParams S;
     bool fast = false;                 // register-resident Stockham path (xfast / yfast / zfast), natural-order spectrum
     XFast XF; YFast YF; ZFast ZF;
+    bool fused = false;                // fast path on the blocked spectrum layout with the z sweeps fused into the y kernels
+    YZFused YZ; TmaMap3D xi_map; cplx* work = nullptr;   // work: plan-owned spectrum field (blocked layout)
     std::vector<void*> owned;          // device allocations freed with the plan
     size_t bytes = 0;
     int LX = 1, CY = 1;                // tile shapes
@@ -62,7 +65,7 @@ struct fsei_plan {
 };
 
 static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
-                                                   "y_inverse", "x_inverse", "project", "div_x_forward"};
+                                                   "y_inverse", "x_inverse", "project", "div_x_forward", "yz_forward", "yz_backward"};
 
 // record an event pair around one launch when profiling is on
 struct LaunchTimer {
@@ -241,12 +244,18 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
 {
     int code = 0;
     // fast path: line lengths with a register-resident Stockham instantiation, special columns fit in shared memory
+    // fused path: the fast path on the blocked layout, where one CTA per x-slot tile marches along z -- for grids
+    // with enough tiles to fill the GPU.  FSEI_PATH = generic | fast | fused overrides the choice (tests).
     const char* force = std::getenv("FSEI_FORCE_GENERIC");
-    const bool fast = !(force && force[0] == '1') && nx >= 4 && ny >= 2 && xfast_supported(nx / 2) && yfast_supported(ny) &&
+    const char* path = std::getenv("FSEI_PATH");
+    const std::string want = path ? path : ((force && force[0] == '1') ? "generic" : "");
+    const bool fast = want != "generic" && nx >= 4 && ny >= 2 && xfast_supported(nx / 2) && yfast_supported(ny) &&
                       (size_t)nz * 4 * sizeof(cplx) <= 200 * 1024;
+    const bool fused_ok = fast && xblocked_supported(nx / 2) && yzfused_supported(ny) && (nx / 2) % FSEI_CB == 0;
+    const bool fused = fused_ok && want != "fast" && (want == "fused" || (nx / 2) / FSEI_CB >= 128);
     std::string msg = build_tables(P->T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code, fast);
     if (code) return fail(code, msg);
-    P->fast = fast;
+    P->fast = fast; P->fused = fused;
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FSEI_ERR_CUDA, "no CUDA device: libfsei has no CPU fallback"); }
@@ -288,6 +297,12 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         ZF.special = static_cast<cplx*>(q);
         if ((rc = dalloc(P, sizeof(double) * 4 * nz, &q))) return rc;
         ZF.cpw = static_cast<double*>(q);
+        ZF.cb = fused ? FSEI_CB : 0; ZF.special_in = nullptr;
+        if (fused) {
+            if ((rc = dalloc(P, sizeof(cplx) * 2 * nz, &q))) return rc;
+            CU(cudaMemset(q, 0, sizeof(cplx) * 2 * nz));
+            ZF.special_in = static_cast<const cplx*>(q);
+        }
         size_t nip = (size_t)nz * ny * T.nxc * ZF.ncomp;
         if ((rc = dalloc(P, sizeof(double) * nip, &q))) return rc;
         ZF.ipiv = static_cast<const double*>(q);
@@ -297,6 +312,18 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         CU(cudaDeviceSynchronize());
         CU(xfast_init());
         CU(yfast_init());
+        if (fused) {
+            YZFused& YZ = P->YZ;
+            YZ.nxc = T.nxc; YZ.ny = ny; YZ.nz = nz; YZ.untangle = YF.untangle;
+            YZ.pp = (bcx == BC_PERIODIC && bcy == BC_PERIODIC) ? 1 : 0;
+            YZ.tw = Y.tw; YZ.tw_dct = Y.tw_dct; YZ.za = Z.za; YZ.zcc = Z.zcc; YZ.ip = ZF.ipiv;
+            YZ.special_in = const_cast<cplx*>(ZF.special_in); YZ.special = ZF.special;
+            if ((rc = dalloc(P, sizeof(double) * (size_t)nx * ny * nz, &q))) return rc;
+            P->work = static_cast<cplx*>(q);
+            CU(xblocked_init());
+            CU(yzfused_init());
+            CU(make_xi_blocked_map(XF, bcx == BC_NEUMANN, P->work, &P->xi_map));
+        }
         CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz)));
         return FSEI_OK;
     }
@@ -409,6 +436,19 @@ static int fast_spectral_solve(fsei_plan* P, cplx* spec, cudaStream_t st)
     return FSEI_OK;
 }
 
+// a3 .. a6 of the fused path on the blocked spectrum in the plan's workspace; phi receives the result
+static int fused_spectral_solve(fsei_plan* P, double* phi, cudaStream_t st)
+{
+    const HostTables& T = P->T;
+    const bool ny_neu = T.bcy == BC_NEUMANN;
+    { LaunchTimer t(P, K_YZF, st); CU(launch_yz_forward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
+    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz, st>>>(P->ZF, P->work); }
+    CU(cudaGetLastError());
+    { LaunchTimer t(P, K_YZB, st); CU(launch_yz_backward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
+    { LaunchTimer t(P, K_XI, st); CU(launch_xi_fast(P->XF, T.bcx == BC_NEUMANN, P->work, phi, st, &P->xi_map)); }
+    return FSEI_OK;
+}
+
 extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, void* cuda_stream)
 {
     if (!P || !rhs || !phi) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: NULL argument");
@@ -417,6 +457,13 @@ extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, 
     const long nlines = (long)T.ny * T.nz;
     cplx* spec = reinterpret_cast<cplx*>(phi);
     int launches = 0;
+    if (P->fused) {
+        { LaunchTimer t(P, K_XF, st); CU(launch_xf_fast(P->XF, P->S, T.bcx == BC_NEUMANN, false, rhs, nullptr, nullptr, 0.0, P->work, st, true)); }
+        int rc = fused_spectral_solve(P, phi, st);
+        if (rc) return rc;
+        P->last_launches = 5;
+        return FSEI_OK;
+    }
     if (P->fast) {
         { LaunchTimer t(P, K_XF, st); CU(launch_xf_fast(P->XF, P->S, T.bcx == BC_NEUMANN, false, rhs, nullptr, nullptr, 0.0, spec, st)); }
         int rc = fast_spectral_solve(P, spec, st);
@@ -494,11 +541,11 @@ extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, doub
         if (alpha_dt == 0.0 || alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: alpha_dt must be non-zero, beta not NaN");
         if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: phi must not alias u, v, w, p");
         cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-        cplx* spec = reinterpret_cast<cplx*>(phi);
-        { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, P->T.bcx == BC_NEUMANN, true, u, v, w, 1.0 / alpha_dt, spec, st)); }
-        if ((rc = fast_spectral_solve(P, spec, st))) return rc;
+        cplx* spec = P->fused ? P->work : reinterpret_cast<cplx*>(phi);
+        { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, P->T.bcx == BC_NEUMANN, true, u, v, w, 1.0 / alpha_dt, spec, st, P->fused)); }
+        if ((rc = P->fused ? fused_spectral_solve(P, phi, st) : fast_spectral_solve(P, spec, st))) return rc;
         if ((rc = fsei_project(P, u, v, w, p, phi, alpha_dt, beta, cuda_stream))) return rc;
-        P->last_launches = 7;
+        P->last_launches = P->fused ? 6 : 7;
         return FSEI_OK;
     }
     if ((rc = fsei_divergence(P, u, v, w, alpha_dt, phi, cuda_stream))) return rc;

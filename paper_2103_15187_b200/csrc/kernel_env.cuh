@@ -23,6 +23,7 @@
 namespace fsei {
 
 struct alignas(64) TmaMap2D { CUtensorMap m; };
+struct alignas(64) TmaMap3D { CUtensorMap m; };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -48,6 +49,12 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const TmaMap2D* map, int 
 {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(x0), "r"(y0), "r"(smem_u32(bar)) : "memory");
+}
+// box (x0 .., y0 .., z0 ..) of a 3-D tensor, x = fastest coordinate
+__device__ __forceinline__ void tma_load_3d(void* dst, const TmaMap3D* map, int x0, int y0, int z0, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(x0), "r"(y0), "r"(z0), "r"(smem_u32(bar)) : "memory");
 }
 // every thread that reads the landing tile
 __device__ __forceinline__ void abar_wait(uint64_t* bar, unsigned parity)
@@ -76,6 +83,9 @@ namespace fsei {
 // host stand-in of a tiled tensor map: boxes of box_rows rows x box_bytes bytes out of a row-strided array
 struct TmaMap2D { const unsigned char* base; size_t pitch_bytes; unsigned elem_bytes, box_elems, box_rows; };
 
+// 3-D: dims (nx elements, ny, nz) with byte pitches of y and z; boxes of (bx, by, bz); out-of-range elements read 0
+struct TmaMap3D { const unsigned char* base; size_t pitch_y, pitch_z; unsigned elem_bytes, nx, ny, nz, bx, by, bz; };
+
 inline void abar_init(uint64_t*) {}
 inline void abar_expect(uint64_t*, unsigned) {}
 inline void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t*) { std::memcpy(dst, src, bytes); }
@@ -84,6 +94,18 @@ inline void tma_load_2d(void* dst, const TmaMap2D* m, int x0, int y0, uint64_t*)
     const size_t bb = (size_t)m->box_elems * m->elem_bytes;
     for (unsigned r = 0; r < m->box_rows; r++)
         std::memcpy(static_cast<unsigned char*>(dst) + r * bb, m->base + (size_t)(y0 + (int)r) * m->pitch_bytes + (size_t)x0 * m->elem_bytes, bb);
+}
+inline void tma_load_3d(void* dst, const TmaMap3D* m, int x0, int y0, int z0, uint64_t*)
+{
+    unsigned char* d = static_cast<unsigned char*>(dst);
+    for (unsigned z = 0; z < m->bz; z++)
+        for (unsigned y = 0; y < m->by; y++)
+            for (unsigned x = 0; x < m->bx; x++, d += m->elem_bytes) {
+                const unsigned X = x0 + x, Y = y0 + y, Z = z0 + z;
+                if (X < m->nx && Y < m->ny && Z < m->nz)
+                    std::memcpy(d, m->base + (size_t)Z * m->pitch_z + (size_t)Y * m->pitch_y + (size_t)X * m->elem_bytes, m->elem_bytes);
+                else std::memset(d, 0, m->elem_bytes);
+            }
 }
 inline void abar_wait(uint64_t*, unsigned) { ::cuda_shim::sync_block(); }      // the issuing thread copied before it got here
 

@@ -122,11 +122,29 @@ FSEI_DEV void fft_line(int tl, bool act, cplx* buf, const cplx* tws, Load0 load0
 FSEI_HD cplx ld2(const double* p) { return *reinterpret_cast<const cplx*>(p); }
 FSEI_HD void st2(double* p, cplx v) { *reinterpret_cast<cplx*>(p) = v; }
 
+// Spectrum layouts.  CB = 0: natural, line (j,k) holds its N slots contiguously at (k ny + j) N.
+// CB > 0: blocked by x-slot tiles of CB slots, [N / CB][nz][ny][CB] -- the (ny x CB) tile of one plane is contiguous,
+// which is what the z-marching y kernels (yzfused.cuh) stream; slot p of line (j,k) sits at
+// ((p / CB) nz + k) ny + j) CB + p % CB.
+template <int CB> FSEI_HD size_t spec_index(int N, int ny, int nz, int k, int j, int p)
+{
+    if (CB == 0) return ((size_t)k * ny + j) * N + p;
+    return (((size_t)(p / (CB ? CB : 1)) * nz + k) * ny + j) * CB + p % (CB ? CB : 1);
+}
+template <int CB> struct SpecLine {
+    cplx* base; size_t tstride;
+    FSEI_HD SpecLine(cplx* spec, int N, int ny, int nz, int k, int j)
+        : base(spec + ((size_t)k * ny + j) * (CB ? CB : N)), tstride((size_t)nz * ny * CB) {}
+    FSEI_HD cplx& operator[](int p) const { return CB ? base[(size_t)(p / (CB ? CB : 1)) * tstride + p % (CB ? CB : 1)] : base[p]; }
+};
+// rows (x-slot tiles) per TMA box of the blocked x-inverse load: the largest divisor of nxt that is <= 256
+FSEI_HD constexpr int xi_box_tiles(int nxt) { int b = nxt < 256 ? nxt : 256; while (nxt % b) b--; return b; }
+
 // ---------------------------------------------------------------------------------------------------
 // a1 + a2: spec(line) = R2C / DCT-II of  rhs(line),  rhs = D(u,v,w)/(alpha dt) (FUSED) or read from `u`
 // grid (ceil(ny / LPB), ceil(nz / kchunk)), block T*LPB, dynamic shared memory XSmemLayout::BYTES
 // ---------------------------------------------------------------------------------------------------
-template <class C, int LPB, bool NEU, bool FUSED>
+template <class C, int LPB, bool NEU, bool FUSED, int CB = 0>
 FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const double* v, const double* w,
                                      double inv_adt, cplx* spec)
 {
@@ -239,7 +257,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
         FSEI_SYNC();
         // Hermitian pair step (+ quarter-wave twiddle): Z -> packed half spectrum, written to global memory
         if (act) {
-            cplx* g = spec + ((size_t)k * ny + j) * N;
+            const SpecLine<CB> g(spec, N, ny, nz, k, j);
             for (int p = tl; p <= N / 2; p += T) {
                 if (p == 0) {
                     cplx z = lbuf[0];
@@ -266,8 +284,10 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
 // ---------------------------------------------------------------------------------------------------
 // a6: phi(line) = scale * C2R / DCT-III of spec(line), in place
 // ---------------------------------------------------------------------------------------------------
-template <class C, int LPB, bool NEU>
-FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const cplx* spec, double* phi)
+// CB > 0: the spectrum is in the blocked layout and the landing tile is fetched through `map`, a 3-D view
+// (2 ny CB doubles, nz, N / CB) of it with boxes (2 LPB CB, 1, xi_box_tiles(N / CB)): landing tile [N / CB][LPB][CB].
+template <class C, int LPB, bool NEU, int CB = 0>
+FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D map, const cplx* spec, double* phi)
 {
     using L = XSmemLayout<C, LPB, NEU, LPB>;
     constexpr int N = C::N, T = C::T, R0 = C::R0;
@@ -289,9 +309,16 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const cplx* spec, double* phi)
     const bool act = j < ny;
     const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
     auto issue = [&](int k) {
-        const unsigned bytes = (unsigned)(nl * N * sizeof(cplx));
-        abar_expect(bar, bytes);
-        bulk_g2s(land, spec + ((size_t)k * ny + j0) * N, bytes, bar);
+        if (CB == 0) {
+            const unsigned bytes = (unsigned)(nl * N * sizeof(cplx));
+            abar_expect(bar, bytes);
+            bulk_g2s(land, spec + ((size_t)k * ny + j0) * N, bytes, bar);
+        } else {                                                   // whole boxes: rows past ny arrive as zeros
+            constexpr int NXT = N / (CB ? CB : 1), BT = xi_box_tiles(NXT);
+            abar_expect(bar, (unsigned)(LPB * N * sizeof(cplx)));
+#pragma unroll
+            for (int b = 0; b < NXT / BT; b++) tma_load_3d(land + (size_t)b * BT * LPB * CB, &map, 2 * j0 * CB, k, b * BT, bar);
+        }
     };
     if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, nt);
@@ -303,7 +330,8 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const cplx* spec, double* phi)
 
     cplx* lbuf = buf + li * C::PITCH;
     double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
-    const cplx* g = land + li * N;
+    // slot p of this thread's line in the landing tile
+    auto g = [&](int p) -> cplx { return CB ? land[((p / (CB ? CB : 1)) * LPB + li) * CB + p % (CB ? CB : 1)] : land[li * N + p]; };
     const double scale = P.scale;
 
     for (int k = k0; k < k1; k++) {
@@ -312,12 +340,12 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const cplx* spec, double* phi)
         if (act) {
             for (int p = tl; p <= N / 2; p += T) {
                 if (p == 0) {
-                    cplx s = g[0];
+                    cplx s = g(0);
                     double x0 = s.re, xn = s.im;
                     if (NEU) xn *= 1.41421356237309504880168872420969808;
                     lbuf[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
                 } else {
-                    cplx xk = g[p], xm = g[N - p];
+                    cplx xk = g(p), xm = g(N - p);
                     if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
                     cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
                     cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2

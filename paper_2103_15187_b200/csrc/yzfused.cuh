@@ -1,0 +1,233 @@
+// yzfused.cuh -- steps a3+a4 (first half) and a4 (second half)+a5 as TWO z-marching kernels on the blocked
+// spectrum layout (xfast.cuh: [nxc / CB][nz][ny][CB]); include/fsei.h, P:L208 (Thomas); DESIGN.md sec. 6.
+//
+// Thomas' algorithm along z is a forward elimination that needs plane k-1 only and a back substitution that
+// needs plane k+1 only.  So the elimination rides on the y-forward transform and the substitution on the
+// y-inverse transform, if those kernels march along z:
+//
+//   k_yz_forward : a CTA owns one x-slot tile (CB slots x all ny rows) and visits k = 0 .. nz-1.  Per plane: the
+//                  tile (contiguous in the blocked layout) and its reciprocal pivots arrive by cp.async.bulk
+//                  while the previous plane is transformed; register-resident Stockham FFT (or DCT-II) along y;
+//                  split of the two Hermitian y-spectra where a column carries two real x-sequences; then
+//                  d'_k = (d_k - a_k d'_{k-1}) / piv_k with d'_{k-1} carried in registers; d'_k is stored.
+//   k_yz_backward: same tiles, k = nz-1 .. 0: x_k = d'_k - (c_k / piv_k) x_{k+1} (x_{k+1} in registers), the
+//                  special columns are replaced by their separately solved values, merge + inverse transform,
+//                  store.
+// The spectrum therefore makes two round trips through HBM for a3+a4+a5 instead of four (y, two Thomas sweeps, y).
+// The arithmetic per element is exactly that of yfast.cuh / zfast.cuh (same operations in the same order).
+#pragma once
+#include "yfast.cuh"
+
+namespace fsei {
+
+struct YZFused {
+    int nxc, ny, nz;
+    int untangle;               // periodic y: columns [0, untangle) are split / merged (0, 1 or nxc)
+    int pp;                     // bc = (P,P): special columns (row 0, slot 0) AND (row ny/2, slot 0), both parts;
+                                // otherwise only the Re part of (row 0, slot 0)
+    const cplx* tw;             // e^{-2 pi i j / ny}
+    const cplx* tw_dct;         // e^{-i pi k / (2 ny)}   (Neumann y only)
+    const double* za;           // a_k
+    const double* zcc;          // c_k
+    const double* ip;           // reciprocal pivots, blocked [nxc / CB][nz][ny][CB][NCOMP]
+    cplx* special_in;           // [2][nz] right-hand sides of the special columns (written by k_yz_forward)
+    const cplx* special;        // [2][nz] their solutions (k_z_special)
+};
+
+template <class C, int CB, bool NEU, int NCOMP> struct YZSmem {
+    static constexpr int TILE = C::N * CB;                      // complex per plane tile
+    static constexpr int IPT = C::N * CB * NCOMP;               // doubles per pivot tile
+    static constexpr int BUF = C::PITCH * CB;
+    static constexpr int DCT = NEU ? C::N / 2 + 1 : 0;
+    static constexpr size_t COMMON = 128 + sizeof(cplx) * (TILE + BUF + C::TW + DCT);
+    static constexpr size_t FWD = COMMON + sizeof(double) * 2 * IPT;      // pivots double-buffered (consumed late)
+    static constexpr size_t BWD = COMMON + sizeof(double) * IPT;
+};
+
+// grid nxc / CB, block T*CB, dynamic shared memory YZSmem::FWD.  spec: blocked spectrum after the x-forward step.
+template <class C, int CB, bool NEU, int NCOMP>
+FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
+{
+    using L = YZSmem<C, CB, NEU, NCOMP>;
+    constexpr int N = C::N, T = C::T, R0 = C::R0, NT = T * CB;
+    constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
+    constexpr int EPT = (N * CB) / NT;                           // elements per thread in the elimination
+    static_assert(NB0 % T == 0, "first pass must tile the column exactly");
+    static_assert((N * CB) % NT == 0, "tile must split evenly over the threads");
+    FSEI_DYN_SMEM(smraw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
+    cplx* land = reinterpret_cast<cplx*>(smraw + 128);           // [N][CB] dense
+    cplx* buf = land + L::TILE;
+    cplx* tws = buf + L::BUF;
+    cplx* tdct = tws + C::TW;
+    double* ipb = reinterpret_cast<double*>(tdct + L::DCT);      // [2][IPT]
+    const int tid = threadIdx.x;
+    const int tl = tid / CB, c = tid - tl * CB;
+    const int tile = blockIdx.x, c0 = tile * CB, col = c0 + c;
+    const int nz = P.nz;
+    const bool pairing = NEU || (c0 < P.untangle);             // CTA-uniform
+    const bool mine = NEU || (col < P.untangle);
+    cplx* tile0 = spec + (size_t)tile * nz * L::TILE;            // plane k of this tile at tile0 + k TILE
+    const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
+
+    auto issue = [&](int k) {
+        abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx) + L::IPT * sizeof(double)));
+        bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
+        bulk_g2s(ipb + (k & 1) * L::IPT, ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)), bar);
+    };
+    if (tid == 0) abar_init(bar);
+    fft_fill_twiddles<C>(tws, P.tw, tid, NT);
+    if (NEU) for (int i = tid; i < L::DCT; i += NT) tdct[i] = P.tw_dct[i];
+    FSEI_SYNC();
+    if (tid == 0) issue(0);
+    unsigned parity = 0;
+
+    cplx carry[EPT];                                             // d'_{k-1} of this thread's elements
+#pragma unroll
+    for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
+
+    for (int k = 0; k < nz; k++) {
+        abar_wait(bar, parity); parity ^= 1;
+        auto next = [&]() { if (tid == 0 && k + 1 < nz) issue(k + 1); };
+        auto load0 = [&](cplx (*v0)[R0]) {
+#pragma unroll
+            for (int i = 0; i < PER0; i++) {
+#pragma unroll
+                for (int q = 0; q < R0; q++) {
+                    const int n = tl + i * T + q * NB0;
+                    v0[i][q] = land[(NEU ? dct_perm(n, N) : n) * CB + c];
+                }
+            }
+        };
+        fft_column<C, CB, false, false, true>(tl, c, true, buf, tws, load0, YOut<C, CB>{buf, c}, next);
+        FSEI_SYNC();
+        if (pairing) {
+            // split in place: rows kk and N-kk of a column are handled by one thread
+            for (int kk = tl; kk <= N / 2; kk += T) {
+                if (kk == 0 || (!NEU && (2 * kk == N || !mine))) continue;
+                const cplx p1 = buf[C::pad(kk) * CB + c], p2 = buf[C::pad(N - kk) * CB + c];
+                cplx A = cmake(0.5 * (p1.re + p2.re), 0.5 * (p1.im - p2.im));       // (P1 + conj P2)/2
+                cplx D = cmake(p1.re - p2.re, p1.im + p2.im);
+                cplx B = cmake(0.5 * D.im, -0.5 * D.re);                            // (P1 - conj P2)/(2i)
+                if (NEU) {
+                    const cplx wk = tdct[kk];
+                    const cplx ta = cmul(A, wk), tb = cmul(B, wk);
+                    buf[C::pad(kk) * CB + c] = cmake(ta.re, tb.re);
+                    if (2 * kk != N) buf[C::pad(N - kk) * CB + c] = cmake(-ta.im, -tb.im);
+                } else {
+                    buf[C::pad(kk) * CB + c] = A;
+                    buf[C::pad(N - kk) * CB + c] = B;
+                }
+            }
+            FSEI_SYNC();
+        }
+        // forward elimination of plane k; element e of the tile = (row e / CB, slot c0 + e % CB)
+        {
+            const double a = P.za[k];
+            const double* ipk = ipb + (k & 1) * L::IPT;
+            cplx* gk = tile0 + (size_t)k * L::TILE;
+#pragma unroll
+            for (int m = 0; m < EPT; m++) {
+                const int e = tid + m * NT;
+                const int row = e / CB, cc = e - row * CB;
+                const cplx d = buf[C::pad(row) * CB + cc];
+                if (tile == 0 && cc == 0) {
+                    if (row == 0) P.special_in[k] = d;
+                    else if (P.pp && 2 * row == N) P.special_in[nz + k] = d;
+                }
+                const double ipr = ipk[e * NCOMP], ipi = ipk[e * NCOMP + (NCOMP - 1)];
+                carry[m] = cmake((d.re - a * carry[m].re) * ipr, (d.im - a * carry[m].im) * ipi);
+                gk[e] = carry[m];
+            }
+        }
+        FSEI_SYNC();
+    }
+}
+
+// grid nxc / CB, block T*CB, dynamic shared memory YZSmem::BWD.  spec: d' from k_yz_forward; P.special solved.
+template <class C, int CB, bool NEU, int NCOMP>
+FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
+{
+    using L = YZSmem<C, CB, NEU, NCOMP>;
+    constexpr int N = C::N, T = C::T, R0 = C::R0, NT = T * CB;
+    constexpr int EPT = (N * CB) / NT;
+    FSEI_DYN_SMEM(smraw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
+    cplx* land = reinterpret_cast<cplx*>(smraw + 128);
+    cplx* buf = land + L::TILE;
+    cplx* tws = buf + L::BUF;
+    cplx* tdct = tws + C::TW;
+    double* ipb = reinterpret_cast<double*>(tdct + L::DCT);      // [IPT]
+    const int tid = threadIdx.x;
+    const int tl = tid / CB, c = tid - tl * CB;
+    const int tile = blockIdx.x, c0 = tile * CB, col = c0 + c;
+    const int nz = P.nz;
+    const bool pairing = NEU || (c0 < P.untangle);
+    const bool mine = NEU || (col < P.untangle);
+    const double SQ2 = 1.41421356237309504880168872420969808;
+    cplx* tile0 = spec + (size_t)tile * nz * L::TILE;
+    const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
+
+    auto issue = [&](int k) {
+        abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx) + L::IPT * sizeof(double)));
+        bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
+        bulk_g2s(ipb, ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)), bar);
+    };
+    if (tid == 0) abar_init(bar);
+    fft_fill_twiddles<C>(tws, P.tw, tid, NT);
+    if (NEU) for (int i = tid; i < L::DCT; i += NT) tdct[i] = P.tw_dct[i];
+    FSEI_SYNC();
+    if (tid == 0) issue(nz - 1);
+    unsigned parity = 0;
+
+    cplx carry[EPT];                                             // x_{k+1} of this thread's elements
+#pragma unroll
+    for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
+
+    for (int k = nz - 1; k >= 0; k--) {
+        abar_wait(bar, parity); parity ^= 1;
+        {
+            const double cz = P.zcc[k];
+#pragma unroll
+            for (int m = 0; m < EPT; m++) {
+                const int e = tid + m * NT;
+                const int row = e / CB, cc = e - row * CB;
+                const cplx dp = land[e];
+                const double ipr = ipb[e * NCOMP], ipi = ipb[e * NCOMP + (NCOMP - 1)];
+                carry[m] = cmake(dp.re - (cz * ipr) * carry[m].re, dp.im - (cz * ipi) * carry[m].im);
+                cplx x = carry[m];
+                if (tile == 0 && cc == 0) {
+                    if (row == 0) { const cplx s = P.special[k]; x.re = s.re; if (P.pp) x.im = s.im; }
+                    else if (P.pp && 2 * row == N) x = P.special[nz + k];
+                }
+                buf[C::pad(row) * CB + cc] = x;
+            }
+        }
+        FSEI_SYNC();
+        if (tid == 0 && k > 0) issue(k - 1);                     // landing tiles consumed: prefetch the next plane
+        if (pairing) {
+            for (int kk = tl; kk <= N / 2; kk += T) {
+                if (kk == 0 || (!NEU && (2 * kk == N || !mine))) continue;
+                cplx a = buf[C::pad(kk) * CB + c];
+                if (NEU && 2 * kk == N) { buf[C::pad(kk) * CB + c] = cmake(a.re * SQ2, a.im * SQ2); continue; }
+                cplx b = buf[C::pad(N - kk) * CB + c];
+                if (NEU) {
+                    const cplx wk = tdct[kk];
+                    const cplx ta = cmulc(cmake(a.re, -b.re), wk);     // V^a_k
+                    const cplx tb = cmulc(cmake(a.im, -b.im), wk);     // V^b_k
+                    a = ta; b = tb;
+                }
+                buf[C::pad(kk) * CB + c] = cmake(a.re - b.im, a.im + b.re);          // A + i B
+                buf[C::pad(N - kk) * CB + c] = cmake(a.re + b.im, -a.im + b.re);     // conj A + i conj B
+            }
+            FSEI_SYNC();
+        }
+        cplx* gk = tile0 + (size_t)k * L::TILE;
+        auto out = [&](int n, cplx z) { gk[(NEU ? dct_perm(n, N) : n) * CB + c] = z; };
+        auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, YIn<C, CB>{buf, c}, v0); };
+        fft_column<C, CB, true, true, false>(tl, c, true, buf, tws, load0, out, NoHook{});
+        FSEI_SYNC();
+    }
+}
+
+}  // namespace fsei

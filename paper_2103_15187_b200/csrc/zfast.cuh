@@ -21,10 +21,16 @@ struct ZFast {
     const double* dzm;    // [nz] (dzm[0] unused)
     const double* ipiv;   // [nz][ny][nxc][ncomp] reciprocal pivots (plan time)
     cplx* special;        // [2][nz] solved special columns: (row 0, slot 0) and, on (P,P), (row ny/2, slot 0)
+    int cb;               // spectrum / pivot-table layout: 0 = natural, else blocked by tiles of cb slots (xfast.cuh)
+    const cplx* special_in;   // fused path: [2][nz] right-hand sides of the special columns (else read from the spectrum)
     double* cpw;          // [4][nz] scratch of the special kernel (c' of its on-the-fly factorisations)
 };
 
-FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot) { return ((size_t)k * Z.ny + row) * Z.nxc + slot; }
+FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot)
+{
+    if (Z.cb == 0) return ((size_t)k * Z.ny + row) * Z.nxc + slot;
+    return (((size_t)(slot / Z.cb) * Z.nz + k) * Z.ny + row) * Z.cb + slot % Z.cb;
+}
 
 // lambda of component comp (0 = Re, 1 = Im) of column (row, slot).  Periodic y: columns that the y-forward
 // kernel split (yfast.cuh) hold A^(ky) in rows 1..ny/2-1 and B^(ky) in rows ny-ky, both parts of a row
@@ -144,7 +150,7 @@ FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec)
     const int ncol = pp ? 2 : 1;
     for (int i = tid; i < ncol * nz; i += 128) {
         int col = i / nz, k = i - col * nz;
-        d[i] = spec[zf_idx(Z, k, col == 0 ? 0 : (Z.ny >> 1), 0)];
+        d[i] = Z.special_in ? Z.special_in[i] : spec[zf_idx(Z, k, col == 0 ? 0 : (Z.ny >> 1), 0)];
         x[i] = cmake(0.0, 0.0);
     }
     FSEI_SYNC();

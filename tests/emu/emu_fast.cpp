@@ -13,6 +13,7 @@
 #include "../../paper_2103_15187_b200/csrc/fast_configs.hpp"
 #include "../../paper_2103_15187_b200/csrc/xfast.cuh"
 #include "../../paper_2103_15187_b200/csrc/yfast.cuh"
+#include "../../paper_2103_15187_b200/csrc/yzfused.cuh"
 #include "../../paper_2103_15187_b200/csrc/zfast.cuh"
 #include "../../paper_2103_15187_b200/csrc/stencil_fast.cuh"
 
@@ -52,7 +53,8 @@ template <class C, bool NEU> void xi_one(const XFast& P, const cplx* spec, doubl
 {
     constexpr int LPB = XShape<C, NEU>::LPB;
     dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
-    cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xi_fast<C, LPB, NEU>(P, spec, phi); });
+    TmaMap3D none{};
+    cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xi_fast<C, LPB, NEU>(P, none, spec, phi); });
 }
 void xi(const XFast& P, bool neu, const cplx* spec, double* phi)
 {
@@ -85,14 +87,78 @@ void yf(const YFast& P, bool inv, bool neu, cplx* spec)
     }
 }
 
+// ---- fused path: blocked spectrum layout, z-marching y kernels ------------------------------------------
+bool xb_ok(int N) { switch (N) {
+#define X(n, a, b, c) case n:
+    FSEI_XB_CONFIGS(X)
+#undef X
+    return true; default: return false; } }
+bool yz_ok(int N) { switch (N) {
+#define X(n, a, b, c) case n:
+    FSEI_YZ_CONFIGS(X)
+#undef X
+    return true; default: return false; } }
+
+template <class C, bool NEU> void xfb_one(const XFast& P, const SParams& S, bool fused, const double* u, const double* v, const double* w,
+                                          double inv_adt, cplx* spec)
+{
+    constexpr int LPB = XShape<C, NEU>::LPB;
+    dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
+    if (fused) cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, 4 * LPB + 1>::BYTES, [&] { k_xf_fast<C, LPB, NEU, true, FSEI_CB>(P, S, u, v, w, inv_adt, spec); });
+    else cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xf_fast<C, LPB, NEU, false, FSEI_CB>(P, S, u, v, w, inv_adt, spec); });
+}
+void xfb(const XFast& P, const SParams& S, bool neu, bool fused, const double* u, const double* v, const double* w, double inv_adt, cplx* spec)
+{
+    switch (P.N) {
+#define X(n, a, b, c) case n: if (neu) xfb_one<FftCfg<n, a, b, c>, true>(P, S, fused, u, v, w, inv_adt, spec); \
+                              else xfb_one<FftCfg<n, a, b, c>, false>(P, S, fused, u, v, w, inv_adt, spec); break;
+        FSEI_XB_CONFIGS(X)
+#undef X
+    }
+}
+template <class C, bool NEU> void xib_one(const XFast& P, const cplx* spec, double* phi)
+{
+    constexpr int LPB = XShape<C, NEU>::LPB, CB = FSEI_CB, NXT = C::N / CB;
+    dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
+    // the view make_xi_blocked_map (fast_x.cu) encodes: (2 ny CB doubles, nz, N / CB), boxes (2 LPB CB, 1, xi_box_tiles)
+    TmaMap3D map{reinterpret_cast<const unsigned char*>(spec), (size_t)P.ny * CB * sizeof(cplx), (size_t)P.nz * P.ny * CB * sizeof(cplx),
+                 (unsigned)sizeof(double), 2u * P.ny * CB, (unsigned)P.nz, (unsigned)NXT, 2u * LPB * CB, 1u, (unsigned)xi_box_tiles(NXT)};
+    cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xi_fast<C, LPB, NEU, FSEI_CB>(P, map, spec, phi); });
+}
+void xib(const XFast& P, bool neu, const cplx* spec, double* phi)
+{
+    switch (P.N) {
+#define X(n, a, b, c) case n: if (neu) xib_one<FftCfg<n, a, b, c>, true>(P, spec, phi); else xib_one<FftCfg<n, a, b, c>, false>(P, spec, phi); break;
+        FSEI_XB_CONFIGS(X)
+#undef X
+    }
+}
+template <class C, bool NEU, int NCOMP> void yz_variant(const YZFused& P, bool backward, cplx* spec)
+{
+    using L = YZSmem<C, FSEI_CB, NEU, NCOMP>;
+    const unsigned grid = P.nxc / FSEI_CB, nt = C::T * FSEI_CB;
+    if (!backward) cuda_shim::launch(grid, nt, L::FWD, [&] { k_yz_forward<C, FSEI_CB, NEU, NCOMP>(P, spec); });
+    else cuda_shim::launch(grid, nt, L::BWD, [&] { k_yz_backward<C, FSEI_CB, NEU, NCOMP>(P, spec); });
+}
+void yz(const YZFused& P, bool backward, bool neu, int ncomp, cplx* spec)
+{
+    switch (P.ny) {
+#define X(n, a, b, c) case n: if (neu) yz_variant<FftCfg<n, a, b, c>, true, 2>(P, backward, spec); \
+                              else if (ncomp == 1) yz_variant<FftCfg<n, a, b, c>, false, 1>(P, backward, spec); \
+                              else yz_variant<FftCfg<n, a, b, c>, false, 2>(P, backward, spec); break;
+        FSEI_YZ_CONFIGS(X)
+#undef X
+    }
+}
+
 struct Ctx {
     HostTables T;
     SParams S; XFast XF; YFast YF; ZFast ZF;
     std::vector<double> ipiv, cpw;
-    std::vector<cplx> special;
+    std::vector<cplx> special, special_in;
 };
 
-void setup(Ctx& c)
+void setup(Ctx& c, bool blocked = false)
 {
     HostTables& T = c.T;
     c.S.nx = T.nx; c.S.ny = T.ny; c.S.nz = T.nz; c.S.bcx = T.bcx; c.S.bcy = T.bcy; c.S.rdx = T.rdx; c.S.rdy = T.rdy;
@@ -107,6 +173,8 @@ void setup(Ctx& c)
     ZF.za = T.za.data(); ZF.zcc = T.zcc.data(); ZF.lamx = T.lamx.data(); ZF.lamy = T.lamy.data(); ZF.dzc = T.dzc.data(); ZF.dzm = T.dzm.data();
     c.special.assign(2 * (size_t)T.nz, cmake(0, 0)); ZF.special = c.special.data();
     c.cpw.assign(4 * (size_t)T.nz, 0.0); ZF.cpw = c.cpw.data();
+    ZF.cb = blocked ? FSEI_CB : 0; ZF.special_in = nullptr;
+    if (blocked) { c.special_in.assign(2 * (size_t)T.nz, cmake(0, 0)); ZF.special_in = c.special_in.data(); }
     c.ipiv.assign((size_t)T.nz * T.ny * T.nxc * ZF.ncomp, 0.0); ZF.ipiv = c.ipiv.data();
     size_t cols = (size_t)T.ny * T.nxc * ZF.ncomp;
     cuda_shim::launch((unsigned)((cols + 255) / 256), 256, 0, [&] { k_zf_factor(ZF, c.ipiv.data()); });
@@ -124,9 +192,51 @@ void spectral_solve(Ctx& c, cplx* spec)
     yf(c.YF, true, yneu, spec);
     xi(c.XF, T.bcx == BC_NEUMANN, spec, reinterpret_cast<double*>(spec));
 }
+
+// a3 .. a6 of the fused path: work = blocked spectrum, phi receives the result
+void fused_spectral_solve(Ctx& c, cplx* work, double* phi)
+{
+    const HostTables& T = c.T;
+    YZFused YZ;
+    YZ.nxc = T.nxc; YZ.ny = T.ny; YZ.nz = T.nz; YZ.untangle = c.YF.untangle;
+    YZ.pp = (T.bcx == BC_PERIODIC && T.bcy == BC_PERIODIC) ? 1 : 0;
+    YZ.tw = T.twy.data(); YZ.tw_dct = T.twy_dct.data(); YZ.za = T.za.data(); YZ.zcc = T.zcc.data(); YZ.ip = c.ipiv.data();
+    YZ.special_in = c.special_in.data(); YZ.special = c.special.data();
+    const bool yneu = T.bcy == BC_NEUMANN;
+    yz(YZ, false, yneu, c.ZF.ncomp, work);
+    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz, [&] { k_z_special(c.ZF, work); });
+    yz(YZ, true, yneu, c.ZF.ncomp, work);
+    xib(c.XF, T.bcx == BC_NEUMANN, work, phi);
+}
 }  // namespace
 
 extern "C" {
+
+int emu_fused_supported(int nx, int ny) { return nx >= 4 && nx % 2 == 0 && xb_ok(nx / 2) && yz_ok(ny) && (nx / 2) % FSEI_CB == 0; }
+
+// whole projection through the fused-path kernels (blocked spectrum in a workspace field)
+int emu_fused_pressure_projection(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy,
+                                  double* u, double* v, double* w, double* p, double* phi, double alpha_dt, double beta, int split)
+{
+    if (!emu_fused_supported(nx, ny)) return -1;
+    Ctx c; int code = 0;
+    std::string msg = build_tables(c.T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code, true);
+    if (code) { std::fprintf(stderr, "emu: %s\n", msg.c_str()); return code; }
+    setup(c, true);
+    const size_t n = (size_t)nx * ny * nz;
+    const unsigned gpairs = (unsigned)((n / 2 + 255) / 256);
+    std::vector<cplx> work(n / 2);
+    const bool xneu = bcx == BC_NEUMANN;
+    if (split) {
+        cuda_shim::launch(gpairs, 256, 0, [&] { k_divergence_fast(c.S, u, v, w, 1.0 / alpha_dt, phi); });
+        xfb(c.XF, c.S, xneu, false, phi, nullptr, nullptr, 0.0, work.data());
+    } else {
+        xfb(c.XF, c.S, xneu, true, u, v, w, 1.0 / alpha_dt, work.data());
+    }
+    fused_spectral_solve(c, work.data(), phi);
+    cuda_shim::launch(gpairs, 256, 0, [&] { k_project_fast(c.S, u, v, w, p, phi, alpha_dt, beta); });
+    return 0;
+}
 
 int emu_fast_supported(int nx, int ny) { return nx >= 4 && nx % 2 == 0 && x_ok(nx / 2) && y_ok(ny); }
 

@@ -51,3 +51,36 @@ def test_fast_support_matrix():
     L = emu_fast_lib()
     assert L.emu_fast_supported(1024, 1024) and L.emu_fast_supported(768, 768) and L.emu_fast_supported(32, 32)
     assert not L.emu_fast_supported(12, 36) and not L.emu_fast_supported(8, 8)
+
+
+# ---- fused path: blocked spectrum layout, Thomas sweeps riding on the z-marching y kernels (yzfused.cuh) ----------
+def _check_fused(oracle_ld, shape, bc, cfg=2, beta=1e-4):
+    case = inputs.make_case(cfg, shape=shape, bc=bc)
+    got = emu_fast_projection(case, beta, False, fused=True)
+    ref = oracle_projection(oracle_ld, case, beta)
+    assert rel_l2(got[4], ref[4]) < 1e-13
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-11 * max(1.0, np.abs(r).max())
+    return got
+
+
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+def test_fused_kernels_match_oracle(oracle_ld, bc):
+    a = _check_fused(oracle_ld, (512, 384, 5), bc)
+    case = inputs.make_case(2, shape=(512, 384, 5), bc=bc)
+    b = emu_fast_projection(case, 1e-4, True, fused=True)        # divergence kernel + non-fused blocked x-forward
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+# every blocked x length and every z-marching y length that has an instantiation
+@pytest.mark.parametrize("shape", [(768, 512, 2), (1024, 384, 2), (2048, 384, 2), (512, 768, 2), (512, 1024, 3)])
+def test_fused_every_length(oracle_ld, shape):
+    for bc in ((P, P), (N, N)):
+        _check_fused(oracle_ld, shape, bc)
+
+
+def test_fused_support_matrix():
+    L = emu_fast_lib()
+    assert L.emu_fused_supported(1024, 1024) and L.emu_fused_supported(768, 768) and L.emu_fused_supported(512, 384)
+    assert not L.emu_fused_supported(256, 256) and not L.emu_fused_supported(32, 32)

@@ -237,3 +237,64 @@ def test_host_buffer_entry(oracle_ld):
     ref = gpu_projection(case)
     for a, b in zip(h, ref[:4]):
         assert np.array_equal(a.numpy(), b)
+
+
+# ---------------------------------------------------------------------------------------------
+# fused path (blocked spectrum, Thomas sweeps inside the z-marching y kernels): chosen automatically for
+# grids with >= 128 x-slot tiles (configs[2..4] at full size); forced here on shapes the oracle finishes
+# in seconds through FSEI_PATH, which fsei_plan_create reads
+# ---------------------------------------------------------------------------------------------
+@pytest.fixture
+def fused_path(monkeypatch):
+    monkeypatch.setenv("FSEI_PATH", "fused")
+    yield
+    monkeypatch.delenv("FSEI_PATH", raising=False)
+
+
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 6), (512, 768, 5), (2048, 1024, 3)])
+def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
+    from paper_2103_15187_b200.binding import Plan
+    for cfg, beta in ((1, 0.0), (2, 1e-4)):
+        case = inputs.make_case(cfg, shape=shape, bc=bc)
+        plan = Plan.from_grid(case.grid)
+        got = gpu_projection(case, beta, plan=plan)
+        assert plan.last_launch_count == 6                      # div+x, y+z fwd, special, z+y bwd, x inverse, project
+        plan.destroy()
+        ref = oracle_projection(oracle_ld, case, beta)
+        assert rel_l2(got[4], ref[4]) <= PHI_TOL
+        for g, r in zip(got[:4], ref[:4]):
+            assert np.abs(g - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
+        pd = _post_div(oracle_ld, case, *got[:3])
+        assert pd <= div_gate(case, np.abs(got[4]).max())
+    # same arithmetic per element as the unfused fast path
+    monkeypatch.setenv("FSEI_PATH", "fast")
+    fast = gpu_projection(case, beta)
+    assert rel_l2(got[4], fast[4]) <= 1e-14
+
+
+def test_fused_split_calls_and_aliasing(oracle_ld, fused_path):
+    case = inputs.make_case(2, shape=(512, 384, 12))
+    a = gpu_projection(case, split=True)                          # poisson_solve with phi aliasing rhs
+    b = gpu_projection(case, split=False)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_fused_config4_grid_reduced(oracle_ld, oracle_d, fused_path):
+    """configs[3] z-grid (768 planes, clustering 3.5) and full x length through the fused kernels"""
+    _check_config(oracle_ld, oracle_d, inputs.make_case(4, shape=(1024, 384, 768)))
+
+
+def test_fused_config5_grid_reduced(oracle_ld, oracle_d, fused_path):
+    _check_config(oracle_ld, oracle_d, inputs.make_case(5, shape=(768, 384, 256)))
+
+
+def test_fused_is_the_default_on_large_grids():
+    from paper_2103_15187_b200.binding import Plan
+    case = inputs.make_case(3, shape=(512, 512, 8))
+    plan = Plan.from_grid(case.grid)
+    got = gpu_projection(case, plan=plan)
+    assert plan.last_launch_count == 6
+    plan.destroy()
+    assert np.isfinite(got[4]).all()

@@ -45,15 +45,18 @@ def emu_fast_lib():
     i, d = ctypes.c_int, ctypes.c_double
     L.emu_fast_pressure_projection.argtypes = [i, i, i, d, d, _dp, i, i, _dp, _dp, _dp, _dp, _dp, d, d, i]
     L.emu_fast_supported.argtypes = [i, i]
+    L.emu_fused_pressure_projection.argtypes = [i, i, i, d, d, _dp, i, i, _dp, _dp, _dp, _dp, _dp, d, d, i]
+    L.emu_fused_supported.argtypes = [i, i]
     return L
 
 
-def emu_fast_projection(case, beta=0.0, split=False):
+def emu_fast_projection(case, beta=0.0, split=False, fused=False):
     L = emu_fast_lib()
     u, v, w = case.u.copy(), case.v.copy(), case.w.copy()
     p, phi = np.zeros_like(u), np.empty_like(u)
     zc = np.ascontiguousarray(case.zc)
-    rc = L.emu_fast_pressure_projection(case.nx, case.ny, case.nz, case.Lx, case.Ly, _p(zc), case.bc_x, case.bc_y,
+    fn = L.emu_fused_pressure_projection if fused else L.emu_fast_pressure_projection
+    rc = fn(case.nx, case.ny, case.nz, case.Lx, case.Ly, _p(zc), case.bc_x, case.bc_y,
                                         _p(u), _p(v), _p(w), _p(p), _p(phi), case.alpha_dt, beta, int(split))
     assert rc == 0, rc
     return u, v, w, p, phi
