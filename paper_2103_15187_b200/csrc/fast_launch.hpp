@@ -8,6 +8,15 @@
 
 namespace fsei {
 
+// raise a kernel's dynamic shared-memory limit and ask for the largest shared-memory carve-out, so that as many
+// CTAs as fit in 227 KB are resident (the default carve-out heuristic stops at one CTA for these kernels)
+template <class K> inline cudaError_t kernel_smem(K kernel, int bytes)
+{
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+
 bool xfast_supported(int N);     // N = nx / 2
 bool yfast_supported(int N);     // N = ny
 // raise the dynamic shared-memory limit of every instantiation (once per process)

@@ -22,9 +22,9 @@ template <class C, bool NEU> static cudaError_t init_one()
     constexpr int LPB = XShape<C, NEU>::LPB;
     const int bf = (int)XSmemLayout<C, LPB, NEU, 4 * LPB + 1>::BYTES, b1 = (int)XSmemLayout<C, LPB, NEU, LPB>::BYTES;
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bf))) return e;
-    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1))) return e;
-    return cudaFuncSetAttribute(k_xi_fast<C, LPB, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1);
+    if ((e = kernel_smem(k_xf_fast<C, LPB, NEU, true>, bf))) return e;
+    if ((e = kernel_smem(k_xf_fast<C, LPB, NEU, false>, b1))) return e;
+    return kernel_smem(k_xi_fast<C, LPB, NEU>, b1);
 }
 
 template <class C, bool NEU> static cudaError_t init_one_blocked()
@@ -32,9 +32,9 @@ template <class C, bool NEU> static cudaError_t init_one_blocked()
     constexpr int LPB = XShape<C, NEU>::LPB;
     const int bf = (int)XSmemLayout<C, LPB, NEU, 4 * LPB + 1>::BYTES, b1 = (int)XSmemLayout<C, LPB, NEU, LPB>::BYTES;
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, true, FSEI_CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, bf))) return e;
-    if ((e = cudaFuncSetAttribute(k_xf_fast<C, LPB, NEU, false, FSEI_CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1))) return e;
-    return cudaFuncSetAttribute(k_xi_fast<C, LPB, NEU, FSEI_CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1);
+    if ((e = kernel_smem(k_xf_fast<C, LPB, NEU, true, FSEI_CB>, bf))) return e;
+    if ((e = kernel_smem(k_xf_fast<C, LPB, NEU, false, FSEI_CB>, b1))) return e;
+    return kernel_smem(k_xi_fast<C, LPB, NEU, FSEI_CB>, b1);
 }
 
 bool xblocked_supported(int N)

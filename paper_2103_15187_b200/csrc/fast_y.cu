@@ -35,10 +35,10 @@ template <class C, int CY> static cudaError_t init_one()
 {
     cudaError_t e;
     const int b0 = (int)YSmemLayout<C, CY, false>::BYTES, b1 = (int)YSmemLayout<C, CY, true>::BYTES;
-    if ((e = cudaFuncSetAttribute(k_y_fast<C, CY, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b0))) return e;
-    if ((e = cudaFuncSetAttribute(k_y_fast<C, CY, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b0))) return e;
-    if ((e = cudaFuncSetAttribute(k_y_fast<C, CY, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1))) return e;
-    return cudaFuncSetAttribute(k_y_fast<C, CY, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1);
+    if ((e = kernel_smem(k_y_fast<C, CY, false, false>, b0))) return e;
+    if ((e = kernel_smem(k_y_fast<C, CY, true, false>, b0))) return e;
+    if ((e = kernel_smem(k_y_fast<C, CY, false, true>, b1))) return e;
+    return kernel_smem(k_y_fast<C, CY, true, true>, b1);
 }
 
 cudaError_t yfast_init()

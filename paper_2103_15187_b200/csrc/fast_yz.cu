@@ -20,8 +20,8 @@ template <class C, bool NEU, int NCOMP> static cudaError_t init_variant()
 {
     using L = YZSmem<C, FSEI_CB, NEU, NCOMP>;
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_yz_forward<C, FSEI_CB, NEU, NCOMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::FWD))) return e;
-    return cudaFuncSetAttribute(k_yz_backward<C, FSEI_CB, NEU, NCOMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::BWD);
+    if ((e = kernel_smem(k_yz_forward<C, FSEI_CB, NEU, NCOMP>, (int)L::FWD))) return e;
+    return kernel_smem(k_yz_backward<C, FSEI_CB, NEU, NCOMP>, (int)L::BWD);
 }
 
 cudaError_t yzfused_init()

@@ -318,6 +318,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             YZ.pp = (bcx == BC_PERIODIC && bcy == BC_PERIODIC) ? 1 : 0;
             YZ.tw = Y.tw; YZ.tw_dct = Y.tw_dct; YZ.za = Z.za; YZ.zcc = Z.zcc; YZ.ip = ZF.ipiv;
             YZ.special_in = const_cast<cplx*>(ZF.special_in); YZ.special = ZF.special;
+            { const char* d = std::getenv("FSEI_DBG"); YZ.dbg = d ? std::atoi(d) : 0; }
             if ((rc = dalloc(P, sizeof(double) * (size_t)nx * ny * nz, &q))) return rc;
             P->work = static_cast<cplx*>(q);
             CU(xblocked_init());

@@ -56,6 +56,23 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const TmaMap3D* map, int 
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(x0), "r"(y0), "r"(z0), "r"(smem_u32(bar)) : "memory");
 }
+// L2 prefetch of contiguous bytes / of a box: deepens the load pipeline at the DRAM level without shared memory
+// (the later bulk load of the same bytes then completes at L2 latency)
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_3d(const TmaMap3D* map, int x0, int y0, int z0)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map), "r"(x0), "r"(y0), "r"(z0) : "memory");
+}
+// read-only 8-byte load that does not allocate in L1
+__device__ __forceinline__ double ld_stream(const double* p)
+{
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
 // every thread that reads the landing tile
 __device__ __forceinline__ void abar_wait(uint64_t* bar, unsigned parity)
 {
@@ -107,6 +124,9 @@ inline void tma_load_3d(void* dst, const TmaMap3D* m, int x0, int y0, int z0, ui
                 else std::memset(d, 0, m->elem_bytes);
             }
 }
+inline void bulk_prefetch_l2(const void*, unsigned) {}
+inline void tma_prefetch_3d(const TmaMap3D*, int, int, int) {}
+inline double ld_stream(const double* p) { return *p; }
 inline void abar_wait(uint64_t*, unsigned) { ::cuda_shim::sync_block(); }      // the issuing thread copied before it got here
 
 }  // namespace fsei

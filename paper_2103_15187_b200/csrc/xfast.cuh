@@ -256,25 +256,37 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
         else fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, next);
         FSEI_SYNC();
         // Hermitian pair step (+ quarter-wave twiddle): Z -> packed half spectrum, written to global memory
-        if (act) {
-            const SpecLine<CB> g(spec, N, ny, nz, k, j);
-            for (int p = tl; p <= N / 2; p += T) {
-                if (p == 0) {
-                    cplx z = lbuf[0];
-                    double x0 = z.re + z.im, xn = z.re - z.im;
-                    if (NEU) xn *= FSEI_SQRT1_2;                               // X_{n/2} = V_{n/2} cos(pi/4)
-                    g[0] = cmake(x0, xn);
-                } else {
-                    cplx zk = lbuf[C::pad(p)], zm = lbuf[C::pad(N - p)];
-                    cplx E = cmake(0.5 * (zk.re + zm.re), 0.5 * (zk.im - zm.im));   // (Zk + conj Zm)/2
-                    cplx D = cmake(zk.re - zm.re, zk.im + zm.im);                   // Zk - conj Zm
-                    cplx O = cmake(0.5 * D.im, -0.5 * D.re);                        // D / (2i)
-                    cplx Tt = cmul(O, tr2c[p]);
-                    cplx xk = cadd(E, Tt), xm = cconj(csub(E, Tt));
-                    if (NEU) { xk = dct_tw_fwd(xk, tdct[p]); xm = dct_tw_fwd(xm, tdct[N - p]); }
-                    g[p] = xk;
-                    if (p != N - p) g[N - p] = xm;
-                }
+        auto pair_store = [&](const cplx* lb, const SpecLine<CB>& g, int p) {
+            if (p == 0) {
+                cplx z = lb[0];
+                double x0 = z.re + z.im, xn = z.re - z.im;
+                if (NEU) xn *= FSEI_SQRT1_2;                               // X_{n/2} = V_{n/2} cos(pi/4)
+                g[0] = cmake(x0, xn);
+            } else {
+                cplx zk = lb[C::pad(p)], zm = lb[C::pad(N - p)];
+                cplx E = cmake(0.5 * (zk.re + zm.re), 0.5 * (zk.im - zm.im));   // (Zk + conj Zm)/2
+                cplx D = cmake(zk.re - zm.re, zk.im + zm.im);                   // Zk - conj Zm
+                cplx O = cmake(0.5 * D.im, -0.5 * D.re);                        // D / (2i)
+                cplx Tt = cmul(O, tr2c[p]);
+                cplx xk = cadd(E, Tt), xm = cconj(csub(E, Tt));
+                if (NEU) { xk = dct_tw_fwd(xk, tdct[p]); xm = dct_tw_fwd(xm, tdct[N - p]); }
+                g[p] = xk;
+                if (p != N - p) g[N - p] = xm;
+            }
+        };
+        if (CB == 0) {
+            if (act) {
+                const SpecLine<CB> g(spec, N, ny, nz, k, j);
+                for (int p = tl; p <= N / 2; p += T) pair_store(lbuf, g, p);
+            }
+        } else {
+            // blocked layout: adjacent threads take (slot within tile, line, tile) in that order, so that a warp
+            // writes whole 16 LPB CB-byte segments of the [tile][k][j][CB] array
+            constexpr int CBq = CB ? CB : 1, HP = N / 2 / CBq + 1;
+            for (int wi = tid; wi < HP * LPB * CBq; wi += nt) {
+                const int cc = wi % CBq, l2 = (wi / CBq) % LPB, p = (wi / (CBq * LPB)) * CBq + cc;
+                if (p > N / 2 || l2 >= nl) continue;
+                pair_store(buf + l2 * C::PITCH, SpecLine<CB>(spec, N, ny, nz, k, j0 + l2), p);
             }
         }
         FSEI_SYNC();
@@ -287,7 +299,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
 // CB > 0: the spectrum is in the blocked layout and the landing tile is fetched through `map`, a 3-D view
 // (2 ny CB doubles, nz, N / CB) of it with boxes (2 LPB CB, 1, xi_box_tiles(N / CB)): landing tile [N / CB][LPB][CB].
 template <class C, int LPB, bool NEU, int CB = 0>
-FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D map, const cplx* spec, double* phi)
+FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 : 1)) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D map, const cplx* spec, double* phi)
 {
     using L = XSmemLayout<C, LPB, NEU, LPB>;
     constexpr int N = C::N, T = C::T, R0 = C::R0;
@@ -318,6 +330,10 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D 
             abar_expect(bar, (unsigned)(LPB * N * sizeof(cplx)));
 #pragma unroll
             for (int b = 0; b < NXT / BT; b++) tma_load_3d(land + (size_t)b * BT * LPB * CB, &map, 2 * j0 * CB, k, b * BT, bar);
+            if (k + 1 < k1) {                                      // the plane after: DRAM -> L2 now
+#pragma unroll
+                for (int b = 0; b < NXT / BT; b++) tma_prefetch_3d(&map, 2 * j0 * CB, k + 1, b * BT);
+            }
         }
     };
     if (tid == 0) abar_init(bar);
@@ -330,29 +346,38 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D 
 
     cplx* lbuf = buf + li * C::PITCH;
     double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
-    // slot p of this thread's line in the landing tile
-    auto g = [&](int p) -> cplx { return CB ? land[((p / (CB ? CB : 1)) * LPB + li) * CB + p % (CB ? CB : 1)] : land[li * N + p]; };
     const double scale = P.scale;
 
     for (int k = k0; k < k1; k++) {
         abar_wait(bar, parity); parity ^= 1;
         // packed half spectrum -> Z (Hermitian pair step, preceded by the inverse quarter-wave twiddle)
-        if (act) {
-            for (int p = tl; p <= N / 2; p += T) {
-                if (p == 0) {
-                    cplx s = g(0);
-                    double x0 = s.re, xn = s.im;
-                    if (NEU) xn *= 1.41421356237309504880168872420969808;
-                    lbuf[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
-                } else {
-                    cplx xk = g(p), xm = g(N - p);
-                    if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
-                    cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
-                    cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2
-                    cplx O = cmulc(Tt, tr2c[p]);
-                    lbuf[C::pad(p)] = cmake(E.re - O.im, E.im + O.re);               // E + i O
-                    if (p != N - p) lbuf[C::pad(N - p)] = cmake(E.re + O.im, -(E.im - O.re));   // conj(E - i O)
-                }
+        // gl(p): slot p of line l2 in the landing tile; lb: that line's buffer
+        auto pair_load = [&](int l2, cplx* lb, int p) {
+            auto g = [&](int q) -> cplx { return CB ? land[((q / (CB ? CB : 1)) * LPB + l2) * CB + q % (CB ? CB : 1)] : land[l2 * N + q]; };
+            if (p == 0) {
+                cplx s = g(0);
+                double x0 = s.re, xn = s.im;
+                if (NEU) xn *= 1.41421356237309504880168872420969808;
+                lb[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
+            } else {
+                cplx xk = g(p), xm = g(N - p);
+                if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
+                cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
+                cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2
+                cplx O = cmulc(Tt, tr2c[p]);
+                lb[C::pad(p)] = cmake(E.re - O.im, E.im + O.re);               // E + i O
+                if (p != N - p) lb[C::pad(N - p)] = cmake(E.re + O.im, -(E.im - O.re));   // conj(E - i O)
+            }
+        };
+        if (CB == 0) {
+            if (act) for (int p = tl; p <= N / 2; p += T) pair_load(li, lbuf, p);
+        } else {
+            // landing tile is [tile][line][CB]: adjacent threads read adjacent elements of it
+            constexpr int CBq = CB ? CB : 1, HP = N / 2 / CBq + 1;
+            for (int wi = tid; wi < HP * LPB * CBq; wi += nt) {
+                const int cc = wi % CBq, l2 = (wi / CBq) % LPB, p = (wi / (CBq * LPB)) * CBq + cc;
+                if (p > N / 2 || l2 >= nl) continue;
+                pair_load(l2, buf + l2 * C::PITCH, p);
             }
         }
         FSEI_SYNC();

@@ -32,6 +32,7 @@ struct YZFused {
     const double* ip;           // reciprocal pivots, blocked [nxc / CB][nz][ny][CB][NCOMP]
     cplx* special_in;           // [2][nz] right-hand sides of the special columns (written by k_yz_forward)
     const cplx* special;        // [2][nz] their solutions (k_z_special)
+    int dbg;                    // timing experiments only (FSEI_DBG): 1 = skip the transform, 2 = skip the pivot loads
 };
 
 template <class C, int CB, bool NEU, int NCOMP> struct YZSmem {
@@ -40,8 +41,8 @@ template <class C, int CB, bool NEU, int NCOMP> struct YZSmem {
     static constexpr int BUF = C::PITCH * CB;
     static constexpr int DCT = NEU ? C::N / 2 + 1 : 0;
     static constexpr size_t COMMON = 128 + sizeof(cplx) * (TILE + BUF + C::TW + DCT);
-    static constexpr size_t FWD = COMMON + sizeof(double) * 2 * IPT;      // pivots double-buffered (consumed late)
-    static constexpr size_t BWD = COMMON + sizeof(double) * IPT;
+    static constexpr size_t FWD = COMMON;                                  // pivots read from global memory (L2-prefetched)
+    static constexpr size_t BWD = COMMON + sizeof(double) * IPT;          // pivots land beside the tile
 };
 
 // grid nxc / CB, block T*CB, dynamic shared memory YZSmem::FWD.  spec: blocked spectrum after the x-forward step.
@@ -60,7 +61,6 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     cplx* buf = land + L::TILE;
     cplx* tws = buf + L::BUF;
     cplx* tdct = tws + C::TW;
-    double* ipb = reinterpret_cast<double*>(tdct + L::DCT);      // [2][IPT]
     const int tid = threadIdx.x;
     const int tl = tid / CB, c = tid - tl * CB;
     const int tile = blockIdx.x, c0 = tile * CB, col = c0 + c;
@@ -70,10 +70,13 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;            // plane k of this tile at tile0 + k TILE
     const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
 
+    // plane k: the tile lands in shared memory; the tile of plane k+1 and the pivots of plane k are pulled into L2
+    // (the bulk load one plane later and the pivot loads at the end of this plane then complete at L2 latency)
     auto issue = [&](int k) {
-        abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx) + L::IPT * sizeof(double)));
+        abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx)));
         bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
-        bulk_g2s(ipb + (k & 1) * L::IPT, ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)), bar);
+        if (k + 1 < nz) bulk_prefetch_l2(tile0 + (size_t)(k + 1) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
+        if (!(P.dbg & 2)) bulk_prefetch_l2(ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)));
     };
     if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, NT);
@@ -99,7 +102,22 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
                 }
             }
         };
+        if (P.dbg & 1) {
+            for (int m = 0; m < EPT; m++) { const int e = tid + m * NT; buf[C::pad(e / CB) * CB + e % CB] = land[e]; }
+            FSEI_SYNC();
+            next();
+        } else
         fft_column<C, CB, false, false, true>(tl, c, true, buf, tws, load0, YOut<C, CB>{buf, c}, next);
+        // reciprocal pivots of this thread's elements (L2 hits), in flight across the barrier(s) below
+        double ipv[EPT][NCOMP];
+        {
+            const double* ipk = ip0 + (size_t)k * L::IPT;
+#pragma unroll
+            for (int m = 0; m < EPT; m++) {
+#pragma unroll
+                for (int q = 0; q < NCOMP; q++) ipv[m][q] = (P.dbg & 2) ? 1.0 : ld_stream(ipk + (size_t)(tid + m * NT) * NCOMP + q);
+            }
+        }
         FSEI_SYNC();
         if (pairing) {
             // split in place: rows kk and N-kk of a column are handled by one thread
@@ -124,7 +142,6 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
         // forward elimination of plane k; element e of the tile = (row e / CB, slot c0 + e % CB)
         {
             const double a = P.za[k];
-            const double* ipk = ipb + (k & 1) * L::IPT;
             cplx* gk = tile0 + (size_t)k * L::TILE;
 #pragma unroll
             for (int m = 0; m < EPT; m++) {
@@ -135,7 +152,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
                     if (row == 0) P.special_in[k] = d;
                     else if (P.pp && 2 * row == N) P.special_in[nz + k] = d;
                 }
-                const double ipr = ipk[e * NCOMP], ipi = ipk[e * NCOMP + (NCOMP - 1)];
+                const double ipr = ipv[m][0], ipi = ipv[m][NCOMP - 1];
                 carry[m] = cmake((d.re - a * carry[m].re) * ipr, (d.im - a * carry[m].im) * ipi);
                 gk[e] = carry[m];
             }
@@ -169,9 +186,18 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
     const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
 
     auto issue = [&](int k) {
+        if (P.dbg & 2) {
+            abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx)));
+            bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
+            return;
+        }
         abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx) + L::IPT * sizeof(double)));
         bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
         bulk_g2s(ipb, ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)), bar);
+        if (k > 0) {                                             // next plane's bytes: DRAM -> L2 now
+            bulk_prefetch_l2(tile0 + (size_t)(k - 1) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
+            bulk_prefetch_l2(ip0 + (size_t)(k - 1) * L::IPT, (unsigned)(L::IPT * sizeof(double)));
+        }
     };
     if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, NT);
@@ -225,6 +251,9 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
         cplx* gk = tile0 + (size_t)k * L::TILE;
         auto out = [&](int n, cplx z) { gk[(NEU ? dct_perm(n, N) : n) * CB + c] = z; };
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, YIn<C, CB>{buf, c}, v0); };
+        if (P.dbg & 1) {
+            for (int m = 0; m < EPT; m++) { const int e = tid + m * NT; gk[e] = buf[C::pad(e / CB) * CB + e % CB]; }
+        } else
         fft_column<C, CB, true, true, false>(tl, c, true, buf, tws, load0, out, NoHook{});
         FSEI_SYNC();
     }
