@@ -87,18 +87,26 @@ template <int N, int R, int NS, int T, bool INV, class Out>
 FSEI_DEV void fft_pass_compute(int tl, const cplx* tw, cplx (*v)[R], Out out)
 {
     using S = PassShape<N, R, NS, T>;
+    // twiddle loads of every butterfly first (shared-memory loads cannot be hoisted over the stores below)
+    if (NS > 1) {
 #pragma unroll
-    for (int i = 0; i < S::PER; i++) {
-        const int b = tl + i * T;
-        if (S::FULL || b < S::NB) {
-            const int m = b % NS;
-            if (NS > 1) {
+        for (int i = 0; i < S::PER; i++) {
+            const int b = tl + i * T;
+            if (S::FULL || b < S::NB) {
+                const int m = b % NS;
 #pragma unroll
                 for (int q = 1; q < R; q++) {
                     const cplx w = tw[(q - 1) * NS + m];
                     v[i][q] = INV ? cmulc(v[i][q], w) : cmul(v[i][q], w);
                 }
             }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < S::PER; i++) {
+        const int b = tl + i * T;
+        if (S::FULL || b < S::NB) {
+            const int m = b % NS;
             SmallDft<R, INV>::run(v[i]);
             const int j0 = (b / NS) * NS * R + m;
 #pragma unroll

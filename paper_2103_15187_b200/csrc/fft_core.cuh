@@ -23,6 +23,7 @@
 #else
 #define FSEI_HD inline
 #endif
+#define FSEI_RESTRICT __restrict__
 
 namespace fsei {
 

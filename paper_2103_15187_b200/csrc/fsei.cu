@@ -295,7 +295,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         void* q = nullptr;
         if ((rc = dalloc(P, sizeof(cplx) * 2 * nz, &q))) return rc;
         ZF.special = static_cast<cplx*>(q);
-        if ((rc = dalloc(P, sizeof(double) * 4 * nz, &q))) return rc;
+        if ((rc = dalloc(P, sizeof(double) * 8 * nz, &q))) return rc;
         ZF.cpw = static_cast<double*>(q);
         ZF.cb = fused ? FSEI_CB : 0; ZF.special_in = nullptr;
         if (fused) {
@@ -308,6 +308,8 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         ZF.ipiv = static_cast<const double*>(q);
         size_t cols = (size_t)ny * T.nxc * ZF.ncomp;
         k_zf_factor<<<(unsigned)((cols + 255) / 256), 256>>>(ZF, static_cast<double*>(q));
+        CU(cudaGetLastError());
+        k_z_special_factor<<<1, 32>>>(ZF);
         CU(cudaGetLastError());
         CU(cudaDeviceSynchronize());
         CU(xfast_init());
@@ -325,7 +327,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             CU(yzfused_init());
             CU(make_xi_blocked_map(XF, bcx == BC_NEUMANN, P->work, &P->xi_map));
         }
-        CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz)));
+        CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz + 16)));
         return FSEI_OK;
     }
 
@@ -423,7 +425,7 @@ static int fast_spectral_solve(fsei_plan* P, cplx* spec, cudaStream_t st)
     const HostTables& T = P->T;
     const bool ny_neu = T.bcy == BC_NEUMANN;
     { LaunchTimer t(P, K_YF, st); CU(launch_y_fast(P->YF, false, ny_neu, spec, st)); }
-    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz, st>>>(P->ZF, spec); }
+    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, spec); }
     CU(cudaGetLastError());
     {
         LaunchTimer t(P, K_ZD, st);
@@ -443,7 +445,7 @@ static int fused_spectral_solve(fsei_plan* P, double* phi, cudaStream_t st)
     const HostTables& T = P->T;
     const bool ny_neu = T.bcy == BC_NEUMANN;
     { LaunchTimer t(P, K_YZF, st); CU(launch_yz_forward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
-    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz, st>>>(P->ZF, P->work); }
+    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, P->work); }
     CU(cudaGetLastError());
     { LaunchTimer t(P, K_YZB, st); CU(launch_yz_backward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
     { LaunchTimer t(P, K_XI, st); CU(launch_xi_fast(P->XF, T.bcx == BC_NEUMANN, P->work, phi, st, &P->xi_map)); }

@@ -184,6 +184,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
         if (!FUSED) {
             abar_expect(bar, nl * lb);
             bulk_g2s(LU, u + g0, nl * lb, bar);
+            if (k + 1 < k1) bulk_prefetch_l2(u + g0 + plane, nl * lb);
             return;
         }
         const int nv = wrap ? nl : nl + 1;
@@ -195,6 +196,11 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
         if (wrap && yper) bulk_g2s(LV + nl * n, v + (size_t)k * plane, lb, bar);
         if (first) bulk_g2s(LW + (size_t)(k & 1) * LPB * n, w + g0, nl * lb, bar);
         if (up) bulk_g2s(LW + (size_t)((k + 1) & 1) * LPB * n, w + g0 + plane, nl * lb, bar);
+        if (k + 1 < k1) {                                          // the plane after: DRAM -> L2 now
+            bulk_prefetch_l2(u + g0 + plane, nl * lb);
+            bulk_prefetch_l2(v + g0 + plane, nv * lb);
+            if (k + 2 < nz) bulk_prefetch_l2(w + g0 + 2 * plane, nl * lb);
+        }
     };
 
     if (tid == 0) abar_init(bar);

@@ -88,6 +88,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     cplx carry[EPT];                                             // d'_{k-1} of this thread's elements
 #pragma unroll
     for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
+    double a_k = P.za[0];
 
     for (int k = 0; k < nz; k++) {
         abar_wait(bar, parity); parity ^= 1;
@@ -139,23 +140,34 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
             }
             FSEI_SYNC();
         }
-        // forward elimination of plane k; element e of the tile = (row e / CB, slot c0 + e % CB)
+        // forward elimination of plane k; element e of the tile = (row e / CB, slot c0 + e % CB).
+        // Loads first, then arithmetic, then stores: the compiler cannot reorder shared-memory accesses itself.
         {
-            const double a = P.za[k];
+            const double a = a_k;
+            a_k = (k + 1 < nz) ? P.za[k + 1] : 0.0;             // next plane's coefficient: latency hidden by this plane
             cplx* gk = tile0 + (size_t)k * L::TILE;
+            cplx d[EPT];
 #pragma unroll
             for (int m = 0; m < EPT; m++) {
                 const int e = tid + m * NT;
                 const int row = e / CB, cc = e - row * CB;
-                const cplx d = buf[C::pad(row) * CB + cc];
-                if (tile == 0 && cc == 0) {
-                    if (row == 0) P.special_in[k] = d;
-                    else if (P.pp && 2 * row == N) P.special_in[nz + k] = d;
-                }
-                const double ipr = ipv[m][0], ipi = ipv[m][NCOMP - 1];
-                carry[m] = cmake((d.re - a * carry[m].re) * ipr, (d.im - a * carry[m].im) * ipi);
-                gk[e] = carry[m];
+                d[m] = buf[C::pad(row) * CB + cc];
             }
+            if (tile == 0) {                                    // rows 0 and N/2 of slot 0 (elements 0 and N CB / 2)
+#pragma unroll
+                for (int m = 0; m < EPT; m++) {
+                    const int e = tid + m * NT;
+                    if (e == 0) P.special_in[k] = d[m];
+                    else if (P.pp && e == (N / 2) * CB) P.special_in[nz + k] = d[m];
+                }
+            }
+#pragma unroll
+            for (int m = 0; m < EPT; m++) {
+                const double ipr = ipv[m][0], ipi = ipv[m][NCOMP - 1];
+                carry[m] = cmake((d[m].re - a * carry[m].re) * ipr, (d[m].im - a * carry[m].im) * ipi);
+            }
+#pragma unroll
+            for (int m = 0; m < EPT; m++) gk[tid + m * NT] = carry[m];
         }
         FSEI_SYNC();
     }
@@ -209,21 +221,32 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
     cplx carry[EPT];                                             // x_{k+1} of this thread's elements
 #pragma unroll
     for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
+    double c_k = P.zcc[nz - 1];
 
     for (int k = nz - 1; k >= 0; k--) {
         abar_wait(bar, parity); parity ^= 1;
         {
-            const double cz = P.zcc[k];
+            const double cz = c_k;
+            c_k = (k > 0) ? P.zcc[k - 1] : 0.0;
+            cplx dp[EPT];
+            double ipv[EPT][NCOMP];
+#pragma unroll
+            for (int m = 0; m < EPT; m++) {
+                const int e = tid + m * NT;
+                dp[m] = land[e];
+#pragma unroll
+                for (int q = 0; q < NCOMP; q++) ipv[m][q] = ipb[e * NCOMP + q];
+            }
+#pragma unroll
+            for (int m = 0; m < EPT; m++)
+                carry[m] = cmake(dp[m].re - (cz * ipv[m][0]) * carry[m].re, dp[m].im - (cz * ipv[m][NCOMP - 1]) * carry[m].im);
 #pragma unroll
             for (int m = 0; m < EPT; m++) {
                 const int e = tid + m * NT;
                 const int row = e / CB, cc = e - row * CB;
-                const cplx dp = land[e];
-                const double ipr = ipb[e * NCOMP], ipi = ipb[e * NCOMP + (NCOMP - 1)];
-                carry[m] = cmake(dp.re - (cz * ipr) * carry[m].re, dp.im - (cz * ipi) * carry[m].im);
                 cplx x = carry[m];
                 if (tile == 0 && cc == 0) {
-                    if (row == 0) { const cplx s = P.special[k]; x.re = s.re; if (P.pp) x.im = s.im; }
+                    if (row == 0) { const cplx sv = P.special[k]; x.re = sv.re; if (P.pp) x.im = sv.im; }
                     else if (P.pp && 2 * row == N) x = P.special[nz + k];
                 }
                 buf[C::pad(row) * CB + cc] = x;

@@ -23,7 +23,8 @@ struct ZFast {
     cplx* special;        // [2][nz] solved special columns: (row 0, slot 0) and, on (P,P), (row ny/2, slot 0)
     int cb;               // spectrum / pivot-table layout: 0 = natural, else blocked by tiles of cb slots (xfast.cuh)
     const cplx* special_in;   // fused path: [2][nz] right-hand sides of the special columns (else read from the spectrum)
-    double* cpw;          // [4][nz] scratch of the special kernel (c' of its on-the-fly factorisations)
+    double* cpw;          // [8][nz] plan-time factorisation of the special columns: c'_k of component t at [t][k],
+                          // reciprocal pivots at [4 + t][k]   (t = 2 col + comp; k_z_special_factor)
 };
 
 FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot)
@@ -109,42 +110,94 @@ FSEI_HD void zf_sweep_column(const ZFast& Z, cplx* S, int row, int slot)
 
 // the (0,0) component: serial definition (R7):
 //   F_k = F_{k-1} + d_{k-1} dzc[k-1],  x_0 = 0,  x_k = x_{k-1} + F_k dzm[k],  x -= sum x dzc / sum dzc
-// d, x: arrays of cplx; comp selects the part (stride 2 doubles)
-FSEI_HD void zf_gauge_serial(const ZFast& Z, const double* d, double* x)
+// d, x: arrays of cplx; comp selects the part (stride 2 doubles).  Chunks of ZCH planes: all loads of a chunk are
+// issued before its dependent chain (the compiler cannot reorder loads over the stores of x itself).
+#define FSEI_ZCH 16
+// Returns the volume-weighted mean; the caller subtracts it from x (in parallel).
+FSEI_HD double zf_gauge_serial(const ZFast& Z, const double* FSEI_RESTRICT d, double* FSEI_RESTRICT x)
 {
-    double F = 0.0, acc = 0.0, vol = 0.0;
+    const int nz = Z.nz;
+    double F = 0.0, acc = 0.0, vol = 0.0, xp = 0.0;
     x[0] = 0.0;
-    for (int k = 1; k < Z.nz; k++) {
-        F += d[2 * (k - 1)] * Z.dzc[k - 1];
-        x[2 * k] = x[2 * (k - 1)] + F * Z.dzm[k];
+    for (int k0 = 1; k0 < nz; k0 += FSEI_ZCH) {
+        double dd[FSEI_ZCH], wc[FSEI_ZCH], wm[FSEI_ZCH];
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) {
+            const int k = (k0 + j < nz) ? k0 + j : nz - 1;
+            dd[j] = d[2 * (k - 1)]; wc[j] = Z.dzc[k - 1]; wm[j] = Z.dzm[k];
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) {
+            if (k0 + j < nz) { F += dd[j] * wc[j]; xp = xp + F * wm[j]; dd[j] = xp; }
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) if (k0 + j < nz) x[2 * (k0 + j)] = dd[j];
     }
-    for (int k = 0; k < Z.nz; k++) { acc += x[2 * k] * Z.dzc[k]; vol += Z.dzc[k]; }
-    double mean = acc / vol;
-    for (int k = 0; k < Z.nz; k++) x[2 * k] -= mean;
+    for (int k0 = 0; k0 < nz; k0 += FSEI_ZCH) {
+        double xx[FSEI_ZCH], wc[FSEI_ZCH];
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) {
+            const int k = (k0 + j < nz) ? k0 + j : nz - 1;
+            xx[j] = x[2 * k]; wc[j] = Z.dzc[k];
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) if (k0 + j < nz) { acc += xx[j] * wc[j]; vol += wc[j]; }
+    }
+    return acc / vol;
 }
 
-// Thomas with on-the-fly factorisation on one component of a column held in shared memory
-FSEI_HD void zf_thomas_serial(const ZFast& Z, double lam, const double* d, double* x, double* cp)
+// plan time: factorisation of one component of a special column (same recurrence as zf_factor_column)
+FSEI_HD void zf_special_factor(const ZFast& Z, double lam, double* cp, double* ip)
 {
-    double cprev = 0.0, prev = 0.0;
+    double cprev = 0.0;
     for (int k = 0; k < Z.nz; k++) {
         double a = Z.za[k], c = Z.zcc[k];
-        double ip = 1.0 / ((-(a + c) + lam) - a * cprev);
-        cprev = c * ip; cp[k] = cprev;
-        prev = (d[2 * k] - a * prev) * ip;
-        x[2 * k] = prev;
+        double r = 1.0 / ((-(a + c) + lam) - a * cprev);
+        ip[k] = r; cprev = c * r; cp[k] = cprev;
     }
-    double next = 0.0;
-    for (int k = Z.nz - 1; k >= 0; k--) { next = x[2 * k] - cp[k] * next; x[2 * k] = next; }
 }
 
-// grid 1, block 128, dynamic shared memory 2 * 2 * nz * sizeof(cplx): gathers the special columns, solves
+// Thomas on one component of a column held in shared memory, factorisation from the plan's tables
+FSEI_HD void zf_thomas_serial(const ZFast& Z, const double* FSEI_RESTRICT d, double* FSEI_RESTRICT x,
+                              const double* FSEI_RESTRICT cp, const double* FSEI_RESTRICT ip)
+{
+    const int nz = Z.nz;
+    double prev = 0.0;
+    for (int k0 = 0; k0 < nz; k0 += FSEI_ZCH) {
+        double dd[FSEI_ZCH], aa[FSEI_ZCH], ii[FSEI_ZCH];
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) {
+            const int k = (k0 + j < nz) ? k0 + j : nz - 1;
+            dd[j] = d[2 * k]; aa[j] = Z.za[k]; ii[j] = ip[k];
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) if (k0 + j < nz) { prev = (dd[j] - aa[j] * prev) * ii[j]; dd[j] = prev; }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) if (k0 + j < nz) x[2 * (k0 + j)] = dd[j];
+    }
+    double next = 0.0;
+    for (int k1 = nz - 1; k1 >= 0; k1 -= FSEI_ZCH) {
+        double xx[FSEI_ZCH], cc[FSEI_ZCH];
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) {
+            const int k = (k1 - j >= 0) ? k1 - j : 0;
+            xx[j] = x[2 * k]; cc[j] = cp[k];
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) if (k1 - j >= 0) { next = xx[j] - cc[j] * next; xx[j] = next; }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZCH; j++) if (k1 - j >= 0) x[2 * (k1 - j)] = xx[j];
+    }
+}
+
+// grid 1, block 128, dynamic shared memory 2 * 2 * nz * sizeof(cplx) + 16: gathers the special columns, solves
 // them (one thread per component), leaves them in Z.special
 FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec)
 {
     FSEI_DYN_SMEM(smraw);
     cplx* d = reinterpret_cast<cplx*>(smraw);            // [2][nz]
     cplx* x = d + 2 * Z.nz;                              // [2][nz]
+    double* mean = reinterpret_cast<double*>(x + 2 * Z.nz);
     const int nz = Z.nz, tid = threadIdx.x;
     const bool pp = (Z.bcx == BC_PERIODIC && Z.bcy == BC_PERIODIC);
     const int ncol = pp ? 2 : 1;
@@ -154,15 +207,30 @@ FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec)
         x[i] = cmake(0.0, 0.0);
     }
     FSEI_SYNC();
-    if (tid < 2 * ncol) {
-        const int col = tid >> 1, comp = tid & 1;
+    if ((tid & 31) == 0 && (tid >> 5) < 2 * ncol) {          // component t on lane 0 of warp t: the four chains run side by side
+        const int t = tid >> 5, col = t >> 1, comp = t & 1;
         const double* dd = reinterpret_cast<const double*>(d + col * nz) + comp;
         double* xx = reinterpret_cast<double*>(x + col * nz) + comp;
-        if (tid == 0) zf_gauge_serial(Z, dd, xx);
-        else if (pp) zf_thomas_serial(Z, z_lambda(Z, col == 0 ? 0 : (Z.ny >> 1), 0, comp), dd, xx, Z.cpw + (size_t)tid * nz);
+        if (t == 0) mean[0] = zf_gauge_serial(Z, dd, xx);
+        else if (pp) zf_thomas_serial(Z, dd, xx, Z.cpw + (size_t)t * nz, Z.cpw + (size_t)(4 + t) * nz);
     }
     FSEI_SYNC();
-    for (int i = tid; i < ncol * nz; i += 128) Z.special[i] = x[i];
+    const double gm = mean[0];
+    for (int i = tid; i < ncol * nz; i += 128) {
+        cplx v = x[i];
+        if (i < nz) v.re -= gm;                              // gauge: volume-weighted zero mean of the (0,0) component
+        Z.special[i] = v;
+    }
+}
+
+// plan time.  grid 1, block 32: tables of the special Thomas components (threads 1..3 on (P,P))
+FSEI_GLOBAL(32, 1) k_z_special_factor(ZFast Z)
+{
+    const int tid = threadIdx.x;
+    const bool pp = (Z.bcx == BC_PERIODIC && Z.bcy == BC_PERIODIC);
+    if (!pp || tid < 1 || tid > 3) return;
+    const int col = tid >> 1, comp = tid & 1;
+    zf_special_factor(Z, z_lambda(Z, col == 0 ? 0 : (Z.ny >> 1), 0, comp), Z.cpw + (size_t)tid * Z.nz, Z.cpw + (size_t)(4 + tid) * Z.nz);
 }
 
 // plan time.  grid ceil(ny nxc ncomp / 256), block 256

@@ -172,12 +172,13 @@ void setup(Ctx& c, bool blocked = false)
     ZF.ncomp = (T.bcx == BC_PERIODIC && T.bcy == BC_PERIODIC) ? 1 : 2;
     ZF.za = T.za.data(); ZF.zcc = T.zcc.data(); ZF.lamx = T.lamx.data(); ZF.lamy = T.lamy.data(); ZF.dzc = T.dzc.data(); ZF.dzm = T.dzm.data();
     c.special.assign(2 * (size_t)T.nz, cmake(0, 0)); ZF.special = c.special.data();
-    c.cpw.assign(4 * (size_t)T.nz, 0.0); ZF.cpw = c.cpw.data();
+    c.cpw.assign(8 * (size_t)T.nz, 0.0); ZF.cpw = c.cpw.data();
     ZF.cb = blocked ? FSEI_CB : 0; ZF.special_in = nullptr;
     if (blocked) { c.special_in.assign(2 * (size_t)T.nz, cmake(0, 0)); ZF.special_in = c.special_in.data(); }
     c.ipiv.assign((size_t)T.nz * T.ny * T.nxc * ZF.ncomp, 0.0); ZF.ipiv = c.ipiv.data();
     size_t cols = (size_t)T.ny * T.nxc * ZF.ncomp;
     cuda_shim::launch((unsigned)((cols + 255) / 256), 256, 0, [&] { k_zf_factor(ZF, c.ipiv.data()); });
+    cuda_shim::launch(1, 32, 0, [&] { k_z_special_factor(ZF); });
 }
 
 void spectral_solve(Ctx& c, cplx* spec)
@@ -185,7 +186,7 @@ void spectral_solve(Ctx& c, cplx* spec)
     const HostTables& T = c.T;
     const bool yneu = T.bcy == BC_NEUMANN;
     yf(c.YF, false, yneu, spec);
-    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz, [&] { k_z_special(c.ZF, spec); });
+    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz + 16, [&] { k_z_special(c.ZF, spec); });
     size_t nthr = (size_t)T.nxc * T.ny;
     if (c.ZF.ncomp == 1) cuda_shim::launch((unsigned)((nthr + 127) / 128), 128, 0, [&] { k_zf_sweep<1>(c.ZF, spec); });
     else cuda_shim::launch((unsigned)((nthr + 127) / 128), 128, 0, [&] { k_zf_sweep<2>(c.ZF, spec); });
@@ -204,7 +205,7 @@ void fused_spectral_solve(Ctx& c, cplx* work, double* phi)
     YZ.special_in = c.special_in.data(); YZ.special = c.special.data(); YZ.dbg = 0;
     const bool yneu = T.bcy == BC_NEUMANN;
     yz(YZ, false, yneu, c.ZF.ncomp, work);
-    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz, [&] { k_z_special(c.ZF, work); });
+    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz + 16, [&] { k_z_special(c.ZF, work); });
     yz(YZ, true, yneu, c.ZF.ncomp, work);
     xib(c.XF, T.bcx == BC_NEUMANN, work, phi);
 }
