@@ -110,6 +110,22 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(ms: float, device=None) -> float:
+    """Device time of the slowest rank (the contract's max over ranks); identity on one rank."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(cells: int, world: int, ms_step: float) -> float:
+    """Whole-job Mcell/s of `world` independent replicas ("replicas only")."""
+    return world * cells / (ms_step * 1e-3) / 1e6
+
+
 def _mem_available_gb() -> float:
     try:
         with open("/proc/meminfo") as f:
@@ -234,12 +250,9 @@ def run_ours(args) -> dict:
     ms_total = e0.elapsed_time(e1)
     plan.profile(False)
     prof = plan.profile_read()
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dev)
     ms_step = ms_total / args.steps
-    value = world * case.cells / (ms_step * 1e-3) / 1e6
+    value = replica_throughput(case.cells, world, ms_step)
 
     # ---- roofline of the dominant kernel (live CUDA-event durations from the timed region) ---------------
     peak, peak_src = _peaks()
@@ -278,13 +291,8 @@ def run_ours(args) -> dict:
             plan.pressure_projection_host(hu, hv, hw, hp, case.alpha_dt, 0.0, stream)
         a1.record(stream)
         barrier()
-        ems = a0.elapsed_time(a1)
-        if world > 1:
-            t = torch.tensor([ems], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
-        ems /= args.e2e_steps
-        e2e = {"value": world * case.cells / (ems * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 4 * fbytes,
+        ems = max_over_ranks(a0.elapsed_time(a1), dev) / args.e2e_steps
+        e2e = {"value": replica_throughput(case.cells, world, ems), "unit": UNIT, "h2d_bytes_per_step": 4 * fbytes,
                "d2h_bytes_per_step": 4 * fbytes, "ms_per_step": ems, "steps": args.e2e_steps,
                "api": "fsei_pressure_projection_host (pinned u,v,w,p in; u,v,w,p out)"}
     else:
