@@ -298,3 +298,66 @@ def test_fused_is_the_default_on_large_grids():
     assert plan.last_launch_count == 6
     plan.destroy()
     assert np.isfinite(got[4]).all()
+
+
+# ---------------------------------------------------------------------------------------------
+# configs[3] at FULL size (1024x1024x768), in the launch configuration bench.py times (fused path chosen by the
+# plan, one fsei_pressure_projection call on device-resident fields), against the long-double oracle run on the
+# whole grid (the GPU box has the host memory for it: about 100 GB)
+# ---------------------------------------------------------------------------------------------
+def _full_size_check(oracle_ld, cfg, launches):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    if torch.cuda.get_device_properties(0).total_memory < 60e9:
+        pytest.skip("needs a GPU with >= 60 GB")
+    avail = 0.0
+    with open("/proc/meminfo") as f:
+        for line in f:
+            if line.startswith("MemAvailable"):
+                avail = int(line.split()[1]) / 1e6
+    if avail < 120:
+        pytest.skip(f"full-size oracle needs about 100 GB of host memory, {avail:.0f} GB available")
+    case = inputs.make_case(cfg)
+    plan = Plan.from_grid(case.grid)
+    u, v, w = (torch.from_numpy(a).cuda() for a in (case.u, case.v, case.w))
+    p = torch.zeros_like(u)
+    phi = torch.empty_like(u)
+    plan.pressure_projection(u, v, w, p, phi, case.alpha_dt, 0.0)
+    torch.cuda.synchronize()
+    assert plan.last_launch_count == launches
+    assert torch.equal(p, phi)                              # p0 = 0, beta = 0: p += phi exactly
+    del p
+    # oracle, in place on the host copies
+    po = np.zeros_like(case.u)
+    phio = oracle_ld.pressure_projection(case.grid, case.u, case.v, case.w, po, case.alpha_dt, 0.0)
+    del po
+    g = phi.cpu().numpy()
+    num = float(np.sqrt(np.sum((g - phio) ** 2))); den = float(np.sqrt(np.sum(phio ** 2)))
+    phimax = float(np.abs(g).max())
+    del g, phio, phi
+    rel = num / den
+    worst = 0.0
+    outs = []
+    for t, r in zip((u, v, w), (case.u, case.v, case.w)):
+        h = t.cpu().numpy()
+        worst = max(worst, float(np.abs(h - r).max()) / max(1.0, float(np.abs(r).max())))
+        outs.append(h)
+    pd = _post_div(oracle_ld, case, *outs)
+    gate = div_gate(case, phimax)
+    print(f"cfg {cfg} FULL {case.nx}x{case.ny}x{case.nz}: phi relL2 {rel:.2e}  max|du|/max|u| {worst:.2e}  post-div {pd:.2e} (gate {gate:.2e})")
+    plan.destroy()
+    assert rel <= PHI_TOL
+    assert worst <= 1e-10
+    assert pd <= gate
+
+
+def test_config4_full_size(oracle_ld):
+    _full_size_check(oracle_ld, 4, 6)                       # 6 launches = the fused path, as bench.py times it
+
+
+def test_config5_full_size(oracle_ld):
+    _full_size_check(oracle_ld, 5, 6)                       # 768x768x1024 DCT box, fused path
+
+
+def test_config3_full_size(oracle_ld):
+    _full_size_check(oracle_ld, 3, 6)                       # 512x512x384, first substep, fused path (128 tiles)
