@@ -62,7 +62,7 @@ template <class C> FSEI_DEV void fft_fill_twiddles(cplx* tws, const cplx* tw, in
 }
 
 // Pass s of one line for one thread: tl = thread index within the line (T threads per line).
-// in(n) -> cplx, out(n, cplx); `active` false = the thread's line does not exist (ragged tile).
+// in(n) -> cplx, out(n, cplx, slot) with slot = i R + q the (compile-time) register index of the value; `active` false = the thread's line does not exist (ragged tile).
 template <int N, int R, int NS, int T> struct PassShape {
     static constexpr int NB = N / R;                  // butterflies per line
     static constexpr int PER = (NB + T - 1) / T;      // butterflies per thread
@@ -110,7 +110,7 @@ FSEI_DEV void fft_pass_compute(int tl, const cplx* tw, cplx (*v)[R], Out out)
             SmallDft<R, INV>::run(v[i]);
             const int j0 = (b / NS) * NS * R + m;
 #pragma unroll
-            for (int q = 0; q < R; q++) out(j0 + q * NS, v[i][q]);
+            for (int q = 0; q < R; q++) out(j0 + q * NS, v[i][q], i * R + q);      // slot = register index of the value
         }
     }
 }

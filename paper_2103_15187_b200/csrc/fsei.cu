@@ -321,6 +321,16 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             YZ.tw = Y.tw; YZ.tw_dct = Y.tw_dct; YZ.za = Z.za; YZ.zcc = Z.zcc; YZ.ip = ZF.ipiv;
             YZ.special_in = const_cast<cplx*>(ZF.special_in); YZ.special = ZF.special;
             { const char* d = std::getenv("FSEI_DBG"); YZ.dbg = d ? std::atoi(d) : 0; }
+            {
+                // CTAs are dealt to the SMs breadth first: with nsm < ntiles < 2 nsm the CTAs ntiles - nsm .. nsm - 1 get
+                // an SM to themselves; the straggler tile goes to the last of them
+                int dev = 0, nsm = 148;
+                CU(cudaGetDevice(&dev));
+                CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+                const int ntiles = T.nxc / FSEI_CB;
+                const int bx0 = (ntiles > nsm && ntiles < 2 * nsm) ? nsm - 1 : 0;
+                YZ.tile_shift = (ntiles - bx0) % ntiles;
+            }
             if ((rc = dalloc(P, sizeof(double) * (size_t)nx * ny * nz, &q))) return rc;
             P->work = static_cast<cplx*>(q);
             CU(xblocked_init());

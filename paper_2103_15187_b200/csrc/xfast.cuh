@@ -39,7 +39,7 @@ template <class C> struct SmIn {
 };
 template <class C> struct SmOut {
     cplx* s;
-    FSEI_HD void operator()(int n, cplx v) const { s[C::pad(n)] = v; }
+    FSEI_HD void operator()(int n, cplx v, int = 0) const { s[C::pad(n)] = v; }
 };
 
 // staging tile of a real line (Neumann): one pad double every 4 keeps the stride-4 reads of the reorder
@@ -391,10 +391,10 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
         double* gl = phi + ((size_t)k * ny + j) * n;
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, SmIn<C>{lbuf}, v0); };
         if (!NEU) {
-            auto out = [&](int t, cplx z) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
+            auto out = [&](int t, cplx z, int) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
             fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{});
         } else {
-            auto out = [&](int t, cplx z) {
+            auto out = [&](int t, cplx z, int) {
                 lxs[xs_pad(makhoul(2 * t, n))] = z.re * scale; lxs[xs_pad(makhoul(2 * t + 1, n))] = z.im * scale;
             };
             fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{});

@@ -44,12 +44,13 @@ template <class C, int CY> struct YIn {
 };
 template <class C, int CY> struct YOut {
     cplx* s; int c;
-    FSEI_HD void operator()(int n, cplx v) const { s[C::pad(n) * CY + c] = v; }
+    FSEI_HD void operator()(int n, cplx v, int = 0) const { s[C::pad(n) * CY + c] = v; }
 };
 
 // same pass sequence as fft_line (xfast.cuh) on a column of the [n][CY] tile
-template <class C, int CY, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out, class Hook>
-FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook)
+// hook_last() runs right before the arithmetic of the last pass (its inputs are already in registers).
+template <class C, int CY, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out, class Hook, class HookL>
+FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook, HookL hook_last)
 {
     constexpr int N = C::N, T = C::T;
     static_assert(C::NP >= 2, "pipelined kernels need at least two passes");
@@ -67,6 +68,7 @@ FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Lo
         if (act) fft_pass_load<N, C::R1, C::R0, T>(tl, bin, v);
         if constexpr (C::NP == 2) {
             if (OUT_BUF) FSEI_SYNC();
+            hook_last();
             if (act) fft_pass_compute<N, C::R1, C::R0, T, INV>(tl, tws, v, out);
             return;
         } else {
@@ -79,8 +81,14 @@ FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Lo
         cplx v[PassShape<N, C::R2, C::R0 * C::R1, T>::PER][C::R2];
         if (act) fft_pass_load<N, C::R2, C::R0 * C::R1, T>(tl, bin, v);
         if (OUT_BUF) FSEI_SYNC();
+        hook_last();
         if (act) fft_pass_compute<N, C::R2, C::R0 * C::R1, T, INV>(tl, tws + C::TW1, v, out);
     }
+}
+template <class C, int CY, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out, class Hook>
+FSEI_DEV void fft_column(int tl, int c, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook)
+{
+    fft_column<C, CY, INV, IN_BUF, OUT_BUF>(tl, c, act, buf, tws, load0, out, hook, NoHook{});
 }
 
 // grid (ceil(nxc / CY), gy <= nz), block T*CY, dynamic shared memory YSmemLayout::BYTES.
@@ -137,7 +145,7 @@ FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D ma
                 }
             };
             if (!pairing) {
-                auto out = [&](int n, cplx z) { g[(size_t)n * nxc] = z; };
+                auto out = [&](int n, cplx z, int) { g[(size_t)n * nxc] = z; };
                 fft_column<C, CY, false, false, false>(tl, c, act, buf, tws, load0, out, next);
             } else {
                 fft_column<C, CY, false, false, true>(tl, c, act, buf, tws, load0, YOut<C, CY>{buf, c}, next);
@@ -167,7 +175,7 @@ FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D ma
                 }
             }
         } else {
-            auto out = [&](int n, cplx z) { g[(size_t)(NEU ? dct_perm(n, N) : n) * nxc] = z; };
+            auto out = [&](int n, cplx z, int) { g[(size_t)(NEU ? dct_perm(n, N) : n) * nxc] = z; };
             if (!pairing) {
                 auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll

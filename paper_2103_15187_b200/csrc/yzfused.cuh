@@ -32,6 +32,8 @@ struct YZFused {
     const double* ip;           // reciprocal pivots, blocked [nxc / CB][nz][ny][CB][NCOMP]
     cplx* special_in;           // [2][nz] right-hand sides of the special columns (written by k_yz_forward)
     const cplx* special;        // [2][nz] their solutions (k_z_special)
+    int tile_shift;             // tile = (blockIdx.x + tile_shift) % ntiles: puts the one tile that carries the split /
+                                // merge work (tile 0 on (P,P)) on a CTA that is likely alone on its SM
     int dbg;                    // timing experiments only (FSEI_DBG): 1 = skip the transform, 2 = skip the pivot loads
 };
 
@@ -63,9 +65,9 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     cplx* tdct = tws + C::TW;
     const int tid = threadIdx.x;
     const int tl = tid / CB, c = tid - tl * CB;
-    const int tile = blockIdx.x, c0 = tile * CB, col = c0 + c;
+    const int tile = (int)((blockIdx.x + P.tile_shift) % gridDim.x), c0 = tile * CB, col = c0 + c;
     const int nz = P.nz;
-    const bool pairing = NEU || (c0 < P.untangle);             // CTA-uniform
+    const bool pairing = (NEU || (c0 < P.untangle)) && !(P.dbg & 4);             // CTA-uniform
     const bool mine = NEU || (col < P.untangle);
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;            // plane k of this tile at tile0 + k TILE
     const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
@@ -85,9 +87,12 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     if (tid == 0) issue(0);
     unsigned parity = 0;
 
-    cplx carry[EPT];                                             // d'_{k-1} of this thread's elements
+    constexpr int RL = (C::NP == 3) ? C::R2 : C::R1, NSL = N / RL;   // last pass: output slot i RL + q = row tl + i T + q NSL
+    constexpr int NSLOT = PassShape<N, RL, NSL, T>::PER * RL;
+    constexpr int NCARRY = NSLOT > EPT ? NSLOT : EPT;
+    cplx carry[NCARRY];                                          // d'_{k-1} of this thread's elements
 #pragma unroll
-    for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
+    for (int m = 0; m < NCARRY; m++) carry[m] = cmake(0.0, 0.0);
     double a_k = P.za[0];
 
     for (int k = 0; k < nz; k++) {
@@ -103,6 +108,32 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
                 }
             }
         };
+        if (!pairing && !(P.dbg & 1)) {
+            // Columns with a single spectrum: the elimination runs on the last pass' outputs while they are still in
+            // registers (output slot s of this thread is row RB(s) every plane, so d'_{k-1} is carried per slot).
+            const double a = a_k;
+            a_k = (k + 1 < nz) ? P.za[k + 1] : 0.0;
+            const double* ipk = ip0 + (size_t)k * L::IPT;
+            cplx* gk = tile0 + (size_t)k * L::TILE;
+            double ipv[NSLOT][NCOMP];
+            auto pivots = [&]() {
+#pragma unroll
+                for (int s = 0; s < NSLOT; s++) {
+                    const int b = tl + (s / RL) * T, n = b + (s % RL) * NSL;
+                    if (b < NSL) {
+#pragma unroll
+                        for (int q = 0; q < NCOMP; q++) ipv[s][q] = (P.dbg & 2) ? 1.0 : ld_stream(ipk + (size_t)(n * CB + c) * NCOMP + q);
+                    }
+                }
+            };
+            auto elim = [&](int n, cplx d, int s) {
+                carry[s] = cmake((d.re - a * carry[s].re) * ipv[s][0], (d.im - a * carry[s].im) * ipv[s][NCOMP - 1]);
+                gk[n * CB + c] = carry[s];
+            };
+            fft_column<C, CB, false, false, false>(tl, c, true, buf, tws, load0, elim, next, pivots);
+            FSEI_SYNC();
+            continue;
+        }
         if (P.dbg & 1) {
             for (int m = 0; m < EPT; m++) { const int e = tid + m * NT; buf[C::pad(e / CB) * CB + e % CB] = land[e]; }
             FSEI_SYNC();
@@ -189,9 +220,9 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
     double* ipb = reinterpret_cast<double*>(tdct + L::DCT);      // [IPT]
     const int tid = threadIdx.x;
     const int tl = tid / CB, c = tid - tl * CB;
-    const int tile = blockIdx.x, c0 = tile * CB, col = c0 + c;
+    const int tile = (int)((blockIdx.x + P.tile_shift) % gridDim.x), c0 = tile * CB, col = c0 + c;
     const int nz = P.nz;
-    const bool pairing = NEU || (c0 < P.untangle);
+    const bool pairing = (NEU || (c0 < P.untangle)) && !(P.dbg & 4);
     const bool mine = NEU || (col < P.untangle);
     const double SQ2 = 1.41421356237309504880168872420969808;
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;
@@ -225,6 +256,33 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
 
     for (int k = nz - 1; k >= 0; k--) {
         abar_wait(bar, parity); parity ^= 1;
+        if (!pairing && !(P.dbg & 1)) {
+            // Columns with a single spectrum (no special column among them): the substitution feeds the first pass
+            // of the inverse transform directly; x_{k+1} is carried per input slot of that pass.
+            constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
+            static_assert(NB0 % T == 0 && PER0 * R0 == EPT, "first pass must tile the column exactly");
+            const double cz = c_k;
+            c_k = (k > 0) ? P.zcc[k - 1] : 0.0;
+            cplx* gk = tile0 + (size_t)k * L::TILE;
+            auto load0 = [&](cplx (*v0)[R0]) {
+#pragma unroll
+                for (int i = 0; i < PER0; i++) {
+#pragma unroll
+                    for (int q = 0; q < R0; q++) {
+                        const int e = (tl + i * T + q * NB0) * CB + c, s = i * R0 + q;
+                        const cplx dp = land[e];
+                        const double ipr = ipb[e * NCOMP], ipi = ipb[e * NCOMP + (NCOMP - 1)];
+                        carry[s] = cmake(dp.re - (cz * ipr) * carry[s].re, dp.im - (cz * ipi) * carry[s].im);
+                        v0[i][q] = carry[s];
+                    }
+                }
+            };
+            auto next = [&]() { if (tid == 0 && k > 0) issue(k - 1); };
+            auto out = [&](int n, cplx z, int) { gk[n * CB + c] = z; };
+            fft_column<C, CB, true, false, false>(tl, c, true, buf, tws, load0, out, next);
+            FSEI_SYNC();
+            continue;
+        }
         {
             const double cz = c_k;
             c_k = (k > 0) ? P.zcc[k - 1] : 0.0;
@@ -272,7 +330,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
             FSEI_SYNC();
         }
         cplx* gk = tile0 + (size_t)k * L::TILE;
-        auto out = [&](int n, cplx z) { gk[(NEU ? dct_perm(n, N) : n) * CB + c] = z; };
+        auto out = [&](int n, cplx z, int) { gk[(NEU ? dct_perm(n, N) : n) * CB + c] = z; };
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, YIn<C, CB>{buf, c}, v0); };
         if (P.dbg & 1) {
             for (int m = 0; m < EPT; m++) { const int e = tid + m * NT; gk[e] = buf[C::pad(e / CB) * CB + e % CB]; }
