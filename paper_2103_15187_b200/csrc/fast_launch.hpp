@@ -19,6 +19,7 @@ template <class K> inline cudaError_t kernel_smem(K kernel, int bytes)
 
 bool xfast_supported(int N);     // N = nx / 2
 bool yfast_supported(int N);     // N = ny
+int xfast_lines_per_block(int N, bool neu);   // LPB of the x kernels for this line length
 // raise the dynamic shared-memory limit of every instantiation (once per process)
 cudaError_t xfast_init();
 cudaError_t yfast_init();

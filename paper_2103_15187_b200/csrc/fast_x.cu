@@ -17,6 +17,16 @@ bool xfast_supported(int N)
     }
 }
 
+int xfast_lines_per_block(int N, bool neu)
+{
+    switch (N) {
+#define X(n, a, b, c) case n: return neu ? XShape<FftCfg<n, a, b, c>, true>::LPB : XShape<FftCfg<n, a, b, c>, false>::LPB;
+        FSEI_X_CONFIGS(X)
+#undef X
+        default: return 1;
+    }
+}
+
 template <class C, bool NEU> static cudaError_t init_one()
 {
     constexpr int LPB = XShape<C, NEU>::LPB;

@@ -286,7 +286,16 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     if (fast) {
         XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
         XF.nx = nx; XF.ny = ny; XF.nz = nz; XF.N = nx / 2; XF.tw = X.tw; XF.tw_r2c = X.tw_r2c; XF.tw_dct = X.tw_dct; XF.scale = T.scale;
-        XF.kchunk = nz < 16 ? nz : 16;
+        {
+            // planes per CTA of the x kernels: 16 on large grids (amortises the table fill and gives the fused divergence
+            // its w(k+1) reuse), fewer on small ones so that the grid still covers the SMs a few times
+            int dev = 0, nsm = 148;
+            cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+            const int lpb = xfast_lines_per_block(nx / 2, bcx == BC_NEUMANN);
+            const long jblocks = (ny + lpb - 1) / lpb;
+            long kc = (jblocks * nz) / (4L * nsm);
+            XF.kchunk = (int)(kc < 1 ? 1 : (kc > 16 ? 16 : kc));
+        }
         YF.nxc = T.nxc; YF.ny = ny; YF.nz = nz; YF.tw = Y.tw; YF.tw_dct = Y.tw_dct;
         YF.untangle = (bcy == BC_PERIODIC) ? (bcx == BC_PERIODIC ? 1 : T.nxc) : 0;
         ZF.nxc = T.nxc; ZF.ny = ny; ZF.nz = nz; ZF.bcx = bcx; ZF.bcy = bcy;
@@ -440,7 +449,8 @@ static int fast_spectral_solve(fsei_plan* P, cplx* spec, cudaStream_t st)
     {
         LaunchTimer t(P, K_ZD, st);
         size_t nthr = (size_t)T.nxc * T.ny;
-        if (P->ZF.ncomp == 1) k_zf_sweep<1><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->ZF, spec);
+        if (T.nz <= 32) k_zf_pcr<<<(unsigned)((nthr * 32 + 127) / 128), 128, 0, st>>>(P->ZF, spec);     // one warp per column
+        else if (P->ZF.ncomp == 1) k_zf_sweep<1><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->ZF, spec);
         else k_zf_sweep<2><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->ZF, spec);
     }
     CU(cudaGetLastError());

@@ -73,6 +73,10 @@ __device__ __forceinline__ double ld_stream(const double* p)
     asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
+// value of `v` held by the lane `d` below / above (own value returned when that lane is outside the warp;
+// callers mask by lane index).  All 32 lanes of the warp must call.
+__device__ __forceinline__ double lane_up(double v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
+__device__ __forceinline__ double lane_down(double v, int d) { return __shfl_down_sync(0xffffffffu, v, d); }
 // every thread that reads the landing tile
 __device__ __forceinline__ void abar_wait(uint64_t* bar, unsigned parity)
 {
@@ -124,6 +128,8 @@ inline void tma_load_3d(void* dst, const TmaMap3D* m, int x0, int y0, int z0, ui
                 else std::memset(d, 0, m->elem_bytes);
             }
 }
+inline double lane_up(double v, int d) { return ::cuda_shim::shfl(v, -d); }      // every thread of the block must call
+inline double lane_down(double v, int d) { return ::cuda_shim::shfl(v, d); }
 inline void bulk_prefetch_l2(const void*, unsigned) {}
 inline void tma_prefetch_3d(const TmaMap3D*, int, int, int) {}
 inline double ld_stream(const double* p) { return *p; }

@@ -216,7 +216,10 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
     const double* lu = LU + li * n;
     const double* lv = LV + li * n;
 
+    double rdz_next = (FUSED && k0 < k1) ? S.rdzc[k0] : 0.0;
     for (int k = k0; k < k1; k++) {
+        const double rdz_k = rdz_next;                             // metric of this plane, loaded one plane ahead
+        if (FUSED && k + 1 < k1) rdz_next = S.rdzc[k + 1];
         abar_wait(bar, parity); parity ^= 1;
         // (rhs[2t], rhs[2t+1]) of line (j,k) from the landing tile
         auto rhs_pair = [&](int t) -> cplx {
@@ -229,7 +232,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
             cplx vp = has_jp ? ld2(lv + n + 2 * t) : cmake(0.0, 0.0);
             cplx wk = ld2(lwk + 2 * t);
             cplx wp = (k + 1 < nz) ? ld2(lwp + 2 * t) : cmake(0.0, 0.0);
-            const double rdz = S.rdzc[k];
+            const double rdz = rdz_k;
             return cmake(div_cell(uu.re, uu.im, vv.re, vp.re, wk.re, wp.re, S.rdx, S.rdy, rdz, inv_adt),
                          div_cell(uu.im, un, vv.im, vp.im, wk.im, wp.im, S.rdx, S.rdy, rdz, inv_adt));
         };

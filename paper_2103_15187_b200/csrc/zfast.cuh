@@ -243,6 +243,62 @@ FSEI_GLOBAL(256, 1) k_zf_factor(ZFast Z, double* ipiv)
     zf_factor_column(Z, ipiv, row, slot, comp);
 }
 
+// Short columns (nz <= 32): parallel cyclic reduction with the column spread over the lanes of ONE warp (lane = k).
+// Step s = 1, 2, 4, 8, 16 eliminates the couplings to k - s and k + s:
+//   al = -a_k / b_{k-s},  ga = -c_k / b_{k+s},
+//   a_k <- al a_{k-s},  c_k <- ga c_{k+s},  b_k <- b_k + al c_{k-s} + ga a_{k+s},  d_k <- d_k + al d_{k-s} + ga d_{k+s}
+// (rows outside [0, nz) are identity rows), after which x_k = d_k / b_k.  No factorisation table, log2(32) dependent
+// steps instead of 2 nz.  Re and Im are two systems (same a, c; b differs when the parts have different lambda).
+// The diagonal is carried as its excess over the off-diagonals, r_k = a_k + b_k + c_k (= lambda <= 0 at the start):
+// r obeys the same recurrence as d, r_k <- r_k + al r_{k-s} + ga r_{k+s}, in which every term has the same sign, and
+// b_k = r_k - (a_k + c_k) is again a sum of like-signed terms -- so the reduction never subtracts nearly equal numbers
+// (updating b directly loses the 1e-5-relative lambda of the low modes to cancellation: 3x the Thomas residual).
+struct PcrRow { double a, r, c, d; };
+FSEI_DEV void pcr_reduce(PcrRow& w, int lane)
+{
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+        const bool lo = lane - s >= 0, hi = lane + s < 32;
+        const double am = lane_up(w.a, s), rm = lane_up(w.r, s), cm = lane_up(w.c, s), dm = lane_up(w.d, s);
+        const double ap = lane_down(w.a, s), rp = lane_down(w.r, s), cp = lane_down(w.c, s), dp = lane_down(w.d, s);
+        const double al = lo ? -w.a / (rm - (am + cm)) : 0.0, ga = hi ? -w.c / (rp - (ap + cp)) : 0.0;
+        w.r = w.r + al * (lo ? rm : 0.0) + ga * (hi ? rp : 0.0);
+        w.d = w.d + al * (lo ? dm : 0.0) + ga * (hi ? dp : 0.0);
+        w.a = al * (lo ? am : 0.0);
+        w.c = ga * (hi ? cp : 0.0);
+    }
+}
+
+// grid ceil(32 ny nxc / 128), block 128: warp w of the grid owns column (row w / nxc, slot w % nxc).  nz <= 32.
+// Every thread runs the whole kernel (uniform control flow: the host harness emulates the shuffles with barriers).
+FSEI_GLOBAL(128, 1) k_zf_pcr(ZFast Z, cplx* spec)
+{
+    const size_t t = (size_t)blockIdx.x * 128 + threadIdx.x;
+    const int lane = (int)(t & 31);
+    const size_t w = t >> 5, ncol = (size_t)Z.nxc * Z.ny;
+    const bool col_ok = w < ncol;
+    const int slot = col_ok ? (int)(w % Z.nxc) : 0, row = col_ok ? (int)(w / Z.nxc) : 0;
+    const bool on = col_ok && lane < Z.nz;
+    int mask; const int sp = z_special(Z, row, slot, mask);
+    const size_t i = on ? zf_idx(Z, lane, row, slot) : 0;
+    const cplx d = on ? spec[i] : cmake(0.0, 0.0);
+    const double a = on ? Z.za[lane] : 0.0, c = on ? Z.zcc[lane] : 0.0;
+    PcrRow re, im;
+    re.a = a; re.c = c; re.d = d.re; re.r = on ? z_lambda(Z, row, slot, 0) : 1.0;
+    im.a = a; im.c = c; im.d = d.im; im.r = on ? z_lambda(Z, row, slot, 1) : 1.0;
+    pcr_reduce(re, lane);
+    pcr_reduce(im, lane);
+    if (on) {
+        cplx o = cmake(re.d / (re.r - (re.a + re.c)), im.d / (im.r - (im.a + im.c)));
+        if (sp >= 0) {                                      // singular / separately solved parts: selected, not mixed
+            const cplx s = Z.special[(size_t)sp * Z.nz + lane];
+            if (mask & 1) o.re = s.re;
+            if (mask & 2) o.im = s.im;
+        }
+        spec[i] = o;
+    }
+}
+
 // grid ceil(ny nxc / 128), block 128: slot fastest across the warp (coalesced 16-byte accesses)
 template <int NCOMP>
 FSEI_GLOBAL(128, 1) k_zf_sweep(ZFast Z, cplx* spec)

@@ -21,6 +21,18 @@ inline std::barrier<>* g_bar = nullptr;
 inline unsigned char* g_smem = nullptr;
 
 inline void sync_block() { g_bar->arrive_and_wait(); }
+inline double g_shfl[1024];
+// warp shuffle by lane offset for a block in uniform control flow: every thread of the block calls (two barriers)
+inline double shfl(double v, int delta)
+{
+    const unsigned tid = t_threadIdx.x;                   // 1-D blocks only
+    g_shfl[tid] = v;
+    g_bar->arrive_and_wait();
+    const int lane = (int)(tid & 31u), src = lane + delta;
+    const double r = (src >= 0 && src < 32 && (tid - lane + src) < g_blockDim.x) ? g_shfl[tid - lane + src] : v;
+    g_bar->arrive_and_wait();
+    return r;
+}
 inline unsigned char* dyn_smem() { return g_smem; }
 
 // run body() as every thread of every block of the grid (blocks sequential, threads concurrent)

@@ -181,14 +181,17 @@ void setup(Ctx& c, bool blocked = false)
     cuda_shim::launch(1, 32, 0, [&] { k_z_special_factor(ZF); });
 }
 
-void spectral_solve(Ctx& c, cplx* spec)
+// pcr: short columns through the warp-shuffle PCR kernel (as libfsei does for nz <= 32); the shuffle emulation costs
+// two host barriers per call, so the harness uses it on request only
+void spectral_solve(Ctx& c, cplx* spec, bool pcr = false)
 {
     const HostTables& T = c.T;
     const bool yneu = T.bcy == BC_NEUMANN;
     yf(c.YF, false, yneu, spec);
     cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz + 16, [&] { k_z_special(c.ZF, spec); });
     size_t nthr = (size_t)T.nxc * T.ny;
-    if (c.ZF.ncomp == 1) cuda_shim::launch((unsigned)((nthr + 127) / 128), 128, 0, [&] { k_zf_sweep<1>(c.ZF, spec); });
+    if (pcr && T.nz <= 32) cuda_shim::launch((unsigned)((nthr * 32 + 127) / 128), 128, 0, [&] { k_zf_pcr(c.ZF, spec); });
+    else if (c.ZF.ncomp == 1) cuda_shim::launch((unsigned)((nthr + 127) / 128), 128, 0, [&] { k_zf_sweep<1>(c.ZF, spec); });
     else cuda_shim::launch((unsigned)((nthr + 127) / 128), 128, 0, [&] { k_zf_sweep<2>(c.ZF, spec); });
     yf(c.YF, true, yneu, spec);
     xi(c.XF, T.bcx == BC_NEUMANN, spec, reinterpret_cast<double*>(spec));
@@ -241,7 +244,8 @@ int emu_fused_pressure_projection(int nx, int ny, int nz, double Lx, double Ly, 
 
 int emu_fast_supported(int nx, int ny) { return nx >= 4 && nx % 2 == 0 && x_ok(nx / 2) && y_ok(ny); }
 
-// whole projection through the fast-path kernels.  split != 0: divergence kernel + non-fused x-forward.
+// whole projection through the fast-path kernels.  split & 1: divergence kernel + non-fused x-forward;
+// split & 2: z-solve by the PCR kernel (nz <= 32).
 int emu_fast_pressure_projection(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy,
                                  double* u, double* v, double* w, double* p, double* phi, double alpha_dt, double beta, int split)
 {
@@ -254,13 +258,13 @@ int emu_fast_pressure_projection(int nx, int ny, int nz, double Lx, double Ly, c
     const unsigned gpairs = (unsigned)((n / 2 + 255) / 256);
     cplx* spec = reinterpret_cast<cplx*>(phi);
     const bool xneu = bcx == BC_NEUMANN;
-    if (split) {
+    if (split & 1) {
         cuda_shim::launch(gpairs, 256, 0, [&] { k_divergence_fast(c.S, u, v, w, 1.0 / alpha_dt, phi); });
         xf(c.XF, c.S, xneu, false, phi, nullptr, nullptr, 0.0, spec);
     } else {
         xf(c.XF, c.S, xneu, true, u, v, w, 1.0 / alpha_dt, spec);
     }
-    spectral_solve(c, spec);
+    spectral_solve(c, spec, (split & 2) != 0);
     cuda_shim::launch(gpairs, 256, 0, [&] { k_project_fast(c.S, u, v, w, p, phi, alpha_dt, beta); });
     return 0;
 }

@@ -43,6 +43,18 @@ def test_every_y_length(oracle_ld, ny):
         _check(oracle_ld, (32, ny, 2), bc)
 
 
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(32, 16, 32), (32, 16, 7)])
+def test_short_columns_pcr(oracle_ld, bc, shape):
+    """nz <= 32: the warp-shuffle PCR kernel (lane = k) instead of the Thomas sweeps"""
+    case = inputs.make_case(2, shape=shape, bc=bc)
+    got = emu_fast_projection(case, 1e-4, 2)                     # split & 2: PCR z kernel
+    ref = oracle_projection(oracle_ld, case, 1e-4)
+    assert rel_l2(got[4], ref[4]) < 1e-13
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-11 * max(1.0, np.abs(r).max())
+
+
 def test_fast_config1_full(oracle_ld):
     _check(oracle_ld, (32, 32, 32), (P, P), cfg=1, beta=0.0)
 

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 from paper_2103_15187_b200 import inputs
-from tests.util import div_gate, gpu_projection, oracle_projection, rel_l2
+from tests.util import div_gate, gpu_fields, gpu_projection, oracle_projection, rel_l2
 
 pytestmark = pytest.mark.gpu
 P, N = 0, 1
@@ -361,3 +361,38 @@ def test_config5_full_size(oracle_ld):
 
 def test_config3_full_size(oracle_ld):
     _full_size_check(oracle_ld, 3, 6)                       # 512x512x384, first substep, fused path (128 tiles)
+
+
+# ---------------------------------------------------------------------------------------------
+# the calls never synchronise or allocate, so a whole projection can be captured in a CUDA graph
+# (small grids are launch-latency-bound: configs[0] is 7 launches of a few microseconds each)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,shape,path", [(1, None, None), (3, (512, 384, 12), "fused")])
+def test_cuda_graph_capture_and_replay(monkeypatch, cfg, shape, path):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    if path:
+        monkeypatch.setenv("FSEI_PATH", path)
+    case = inputs.make_case(cfg, shape=shape)
+    plan = Plan.from_grid(case.grid)
+    eager = gpu_projection(case, plan=plan)
+    u0, v0, w0 = gpu_fields(case)
+    u, v, w = u0.clone(), v0.clone(), w0.clone()
+    p = torch.zeros_like(u)
+    phi = torch.empty_like(u)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):                                # warm-up on the capture stream
+        plan.pressure_projection(u, v, w, p, phi, case.alpha_dt, 0.0)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        plan.pressure_projection(u, v, w, p, phi, case.alpha_dt, 0.0)
+    for _ in range(2):                                           # replay twice from pristine inputs
+        u.copy_(u0); v.copy_(v0); w.copy_(w0); p.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for g, e in zip((u, v, w, p, phi), eager):
+            assert np.array_equal(g.cpu().numpy(), e)
+    plan.destroy()
