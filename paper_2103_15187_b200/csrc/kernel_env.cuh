@@ -17,6 +17,8 @@
 #define FSEI_GLOBAL(maxthreads, minblocks) __global__ void __launch_bounds__(maxthreads, minblocks)
 #define FSEI_DEV __device__ __forceinline__
 #define FSEI_SYNC() __syncthreads()
+// barrier among the `n` threads (a multiple of 32) that use named barrier `id` (1..15): the warps of one line only
+#define FSEI_GROUP_SYNC(id, n) asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory")
 #define FSEI_DYN_SMEM(name) extern __shared__ __align__(128) unsigned char name[]
 #define FSEI_GRID_CONSTANT __grid_constant__
 
@@ -96,6 +98,7 @@ __device__ __forceinline__ void abar_wait(uint64_t* bar, unsigned parity)
 #define FSEI_GLOBAL(maxthreads, minblocks) inline void
 #define FSEI_DEV inline
 #define FSEI_SYNC() ::cuda_shim::sync_block()
+#define FSEI_GROUP_SYNC(id, n) ::cuda_shim::sync_block()      // conservative stand-in (control flow is block-uniform)
 #define FSEI_DYN_SMEM(name) unsigned char* name = ::cuda_shim::dyn_smem()
 #define FSEI_GRID_CONSTANT
 

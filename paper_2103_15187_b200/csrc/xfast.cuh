@@ -21,6 +21,7 @@
 #include "plan_types.cuh"
 #include "stencil.cuh"
 #include "xfft.cuh"
+#include <type_traits>
 
 namespace fsei {
 
@@ -76,7 +77,6 @@ template <class C, int LPB, bool NEU, int LL> struct XSmemLayout {
     static constexpr size_t BYTES = 128 + sizeof(double) * LAND + sizeof(cplx) * (BUF + TWS + R2C + DCT) + sizeof(double) * XS;
 };
 
-struct NoHook { FSEI_HD void operator()() const {} };
 
 // Whole line transform for the threads of one line.  load0(v) fills the first pass' registers (from the landing
 // tile / staging; IN_BUF: from the line buffer itself, then a barrier separates its reads from the writes);
@@ -84,37 +84,44 @@ struct NoHook { FSEI_HD void operator()() const {} };
 // hook() runs on every thread right after the first barrier, i.e. once every thread has consumed its first-pass
 // input (that is where the next tile's asynchronous load is issued).  Must be reached by every thread of the CTA;
 // `act` false = this thread's line does not exist.
+struct NoHook { FSEI_HD void operator()() const {} };
+
+// gid >= 0: the line's T threads are whole warps (T % 32 == 0) and synchronise among themselves through named barrier
+// gid + 1, so that the lines of a CTA drift apart instead of meeting at every pass; the barrier that precedes a real
+// hook stays CTA-wide (the hook is where the landing tile, read by every line, is refilled).
 template <class C, bool INV, bool IN_BUF, bool OUT_BUF, class Load0, class Out, class Hook>
-FSEI_DEV void fft_line(int tl, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook)
+FSEI_DEV void fft_line(int tl, bool act, cplx* buf, const cplx* tws, Load0 load0, Out out, Hook hook, int gid = -1)
 {
     constexpr int N = C::N, T = C::T;
+    constexpr bool HOOKED = !std::is_same<Hook, NoHook>::value;
     static_assert(C::NP >= 2, "pipelined kernels need at least two passes");
     SmIn<C> bin{buf}; SmOut<C> bout{buf};
+    auto lsync = [&]() { if (T % 32 == 0 && gid >= 0) { FSEI_GROUP_SYNC(gid + 1, T); } else { FSEI_SYNC(); } };
     {
         cplx v[PassShape<N, C::R0, 1, T>::PER][C::R0];
         if (act) load0(v);
-        if (IN_BUF) { FSEI_SYNC(); hook(); }
+        if (IN_BUF) { if (HOOKED) { FSEI_SYNC(); } else lsync(); hook(); }
         if (act) fft_pass_compute<N, C::R0, 1, T, INV>(tl, tws, v, bout);
     }
-    FSEI_SYNC();
+    if (!IN_BUF && HOOKED) { FSEI_SYNC(); } else lsync();
     if (!IN_BUF) hook();
     {
         cplx v[PassShape<N, C::R1, C::R0, T>::PER][C::R1];
         if (act) fft_pass_load<N, C::R1, C::R0, T>(tl, bin, v);
         if constexpr (C::NP == 2) {
-            if (OUT_BUF) FSEI_SYNC();
+            if (OUT_BUF) lsync();
             if (act) fft_pass_compute<N, C::R1, C::R0, T, INV>(tl, tws, v, out);
             return;
         } else {
-            FSEI_SYNC();
+            lsync();
             if (act) fft_pass_compute<N, C::R1, C::R0, T, INV>(tl, tws, v, bout);
         }
     }
-    FSEI_SYNC();
+    lsync();
     if constexpr (C::NP >= 3) {
         cplx v[PassShape<N, C::R2, C::R0 * C::R1, T>::PER][C::R2];
         if (act) fft_pass_load<N, C::R2, C::R0 * C::R1, T>(tl, bin, v);
-        if (OUT_BUF) FSEI_SYNC();
+        if (OUT_BUF) lsync();
         if (act) fft_pass_compute<N, C::R2, C::R0 * C::R1, T, INV>(tl, tws + C::TW1, v, out);
     }
 }
@@ -261,8 +268,8 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
                 }
             }
         };
-        if (NEU) fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, NoHook{});
-        else fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, next);
+        if (NEU) fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, NoHook{}, li);
+        else fft_line<C, false, false, true>(tl, act, lbuf, tws, load0, SmOut<C>{lbuf}, next, li);
         FSEI_SYNC();
         // Hermitian pair step (+ quarter-wave twiddle): Z -> packed half spectrum, written to global memory
         auto pair_store = [&](const cplx* lb, const SpecLine<CB>& g, int p) {
@@ -395,12 +402,12 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, SmIn<C>{lbuf}, v0); };
         if (!NEU) {
             auto out = [&](int t, cplx z, int) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
-            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{});
+            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{}, li);
         } else {
             auto out = [&](int t, cplx z, int) {
                 lxs[xs_pad(makhoul(2 * t, n))] = z.re * scale; lxs[xs_pad(makhoul(2 * t + 1, n))] = z.im * scale;
             };
-            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{});
+            fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{}, li);
             FSEI_SYNC();
             if (act) {
 #pragma unroll
