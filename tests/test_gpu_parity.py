@@ -396,3 +396,34 @@ def test_cuda_graph_capture_and_replay(monkeypatch, cfg, shape, path):
         for g, e in zip((u, v, w, p, phi), eager):
             assert np.array_equal(g.cpu().numpy(), e)
     plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# maximum sizes of the plan (fsei.h: nx, ny <= 8192 of the form 2^a 3^b, nz <= 8192), one direction at a time
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,bc", [((8192, 4, 3), (P, P)), ((8192, 4, 3), (N, N)), ((4, 8192, 3), (P, P)),
+                                      ((4, 8192, 2), (N, N)), ((8, 8, 8192), (P, P)), ((16, 16, 3200), (P, N)),
+                                      ((6912, 6, 2), (P, P)), ((12, 5832, 2), (N, P))])
+def test_maximum_sizes(oracle_ld, oracle_d, shape, bc):
+    case = inputs.make_case(2, shape=shape, bc=bc)
+    got = gpu_projection(case, 1e-4)
+    ref = oracle_projection(oracle_ld, case, 1e-4)
+    # thousands of planes with clustering 3.0 put the low modes' Thomas conditioning above 1e-11 in ANY fp64 arithmetic
+    # (SURVEY sec. 0 Finding 3): there the gate is 4x the fp64 oracle's own distance from the long-double one
+    floor = 4 * rel_l2(oracle_projection(oracle_d, case, 1e-4)[4], ref[4])
+    assert rel_l2(got[4], ref[4]) <= max(PHI_TOL, floor)
+    assert shape[2] > 2048 or rel_l2(got[4], ref[4]) <= PHI_TOL
+    slack = max(1.0, floor / PHI_TOL)
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-10 * slack * max(1.0, np.abs(r).max())
+
+
+def test_size_limits_are_errors():
+    from paper_2103_15187_b200 import binding
+    for shape in ((16384, 8, 8), (8, 16384, 8), (8, 8, 8193), (8, 8, 1), (10, 8, 8), (8, 14, 8), (6, 8, 8)):
+        grid = list(inputs.make_grid(1, shape=(8, 8, 8)))
+        grid[0], grid[1], grid[2] = shape
+        grid[5] = inputs.tanh_grid(shape[2], 2.0)
+        with pytest.raises(binding.FseiError) as e:
+            binding.Plan.from_grid(tuple(grid))
+        assert e.value.code == binding.ERR_SIZE
