@@ -39,7 +39,8 @@ cudaError_t yzfused_init()
 template <class C, bool NEU, int NCOMP> static cudaError_t run_variant(const YZFused& P, bool backward, cplx* spec, cudaStream_t st)
 {
     using L = YZSmem<C, FSEI_CB, NEU, NCOMP>;
-    const int grid = P.nxc / FSEI_CB, nt = C::T * FSEI_CB;
+    const dim3 grid(P.nxc / FSEI_CB, P.ktw < P.nz ? 2 : 1);
+    const int nt = C::T * FSEI_CB;
     if (!backward) k_yz_forward<C, FSEI_CB, NEU, NCOMP><<<grid, nt, L::FWD, st>>>(P, spec);
     else k_yz_backward<C, FSEI_CB, NEU, NCOMP><<<grid, nt, L::BWD, st>>>(P, spec);
     return cudaGetLastError();

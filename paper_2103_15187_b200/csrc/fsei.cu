@@ -307,6 +307,13 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         if ((rc = dalloc(P, sizeof(double) * 8 * nz, &q))) return rc;
         ZF.cpw = static_cast<double*>(q);
         ZF.cb = fused ? FSEI_CB : 0; ZF.special_in = nullptr;
+        // Twisted factorisation (two CTAs per tile sweeping towards each other) where one CTA per tile would leave SMs
+        // idle: fewer tiles than SMs.  FSEI_TWIST = 0 | 1 overrides (tests).
+        int nsm = 148;
+        { int dev = 0; CU(cudaGetDevice(&dev)); CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev)); }
+        bool twist = fused && nz >= 4 && T.nxc / FSEI_CB <= nsm;
+        if (const char* tw = std::getenv("FSEI_TWIST")) twist = fused && nz >= 4 && tw[0] == '1';
+        ZF.ktw = twist ? nz / 2 : nz;
         if (fused) {
             if ((rc = dalloc(P, sizeof(cplx) * 2 * nz, &q))) return rc;
             CU(cudaMemset(q, 0, sizeof(cplx) * 2 * nz));
@@ -331,14 +338,25 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             YZ.special_in = const_cast<cplx*>(ZF.special_in); YZ.special = ZF.special;
             { const char* d = std::getenv("FSEI_DBG"); YZ.dbg = d ? std::atoi(d) : 0; }
             {
-                // CTAs are dealt to the SMs breadth first: with nsm < ntiles < 2 nsm the CTAs ntiles - nsm .. nsm - 1 get
-                // an SM to themselves; the straggler tile goes to the last of them
-                int dev = 0, nsm = 148;
-                CU(cudaGetDevice(&dev));
-                CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-                const int ntiles = T.nxc / FSEI_CB;
-                const int bx0 = (ntiles > nsm && ntiles < 2 * nsm) ? nsm - 1 : 0;
-                YZ.tile_shift = (ntiles - bx0) % ntiles;
+                // CTAs are dealt to the SMs breadth first: with nsm < total < 2 nsm CTAs the linear ids total - nsm .. nsm - 1
+                // get an SM to themselves; the tile that carries the split / merge work of a (P,P) grid (tile 0: the
+                // straggler) is given such an id in each half of the grid
+                const int ntiles = T.nxc / FSEI_CB, halves = twist ? 2 : 1, total = ntiles * halves;
+                for (int h = 0; h < 2; h++) {
+                    int bx0 = 0;
+                    if (total > nsm && total < 2 * nsm) {
+                        const int lo = total - nsm, hi = nsm - 1;             // lonely linear ids, inclusive
+                        int cand = hi - ntiles * h;                           // blockIdx.x of linear id hi in half h
+                        if (cand >= ntiles) cand = ntiles - 1;
+                        if (cand >= 0 && cand + ntiles * h >= lo) bx0 = cand;
+                    }
+                    YZ.tile_shift[h] = (ntiles - bx0) % ntiles;
+                }
+            }
+            YZ.ktw = ZF.ktw; YZ.mid = nullptr;
+            if (twist) {
+                if ((rc = dalloc(P, sizeof(cplx) * (size_t)T.nxc * ny * 2, &q))) return rc;
+                YZ.mid = static_cast<cplx*>(q);
             }
             if ((rc = dalloc(P, sizeof(double) * (size_t)nx * ny * nz, &q))) return rc;
             P->work = static_cast<cplx*>(q);

@@ -32,8 +32,13 @@ struct YZFused {
     const double* ip;           // reciprocal pivots, blocked [nxc / CB][nz][ny][CB][NCOMP]
     cplx* special_in;           // [2][nz] right-hand sides of the special columns (written by k_yz_forward)
     const cplx* special;        // [2][nz] their solutions (k_z_special)
-    int tile_shift;             // tile = (blockIdx.x + tile_shift) % ntiles: puts the one tile that carries the split /
-                                // merge work (tile 0 on (P,P)) on a CTA that is likely alone on its SM
+    int ktw;                    // twist plane (zfast.cuh): nz = plain Thomas, one CTA per tile (grid.y = 1); < nz = twisted
+                                // factorisation, planes [0, ktw) and [ktw, nz) swept towards each other by two CTAs
+                                // per tile (grid.y = 2) -- for grids with fewer tiles than SMs
+    cplx* mid;                  // twisted only: [ntiles][2][ny CB] copies of d'_{ktw-1} and e'_{ktw}, the two planes both
+                                // back-substitution CTAs of a tile start from (each overwrites one of them in place)
+    int tile_shift[2];          // tile = (blockIdx.x + tile_shift[blockIdx.y]) % ntiles: puts the one tile that carries
+                                // the split / merge work (tile 0 on (P,P)) on a CTA that is likely alone on its SM
     int dbg;                    // timing experiments only (FSEI_DBG): 1 = skip the transform, 2 = skip the pivot loads
 };
 
@@ -65,8 +70,13 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     cplx* tdct = tws + C::TW;
     const int tid = threadIdx.x;
     const int tl = tid / CB, c = tid - tl * CB;
-    const int tile = (int)((blockIdx.x + P.tile_shift) % gridDim.x), c0 = tile * CB, col = c0 + c;
+    const int tile = (int)((blockIdx.x + (blockIdx.y ? P.tile_shift[1] : P.tile_shift[0])) % gridDim.x), c0 = tile * CB, col = c0 + c;
     const int nz = P.nz;
+    // this CTA's sweep: planes [0, ktw) upwards with the coupling a_k to the plane below (blockIdx.y = 0), or planes
+    // [ktw, nz) downwards with the coupling c_k to the plane above (blockIdx.y = 1, twisted factorisation only)
+    const bool up = blockIdx.y == 0;
+    const int kfirst = up ? 0 : nz - 1, kstep = up ? 1 : -1, kcount = up ? P.ktw : nz - P.ktw;
+    const double* coef = up ? P.za : P.zcc;
     const bool pairing = (NEU || (c0 < P.untangle)) && !(P.dbg & 4);             // CTA-uniform
     const bool mine = NEU || (col < P.untangle);
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;            // plane k of this tile at tile0 + k TILE
@@ -74,17 +84,17 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
 
     // plane k: the tile lands in shared memory; the tile of plane k+1 and the pivots of plane k are pulled into L2
     // (the bulk load one plane later and the pivot loads at the end of this plane then complete at L2 latency)
-    auto issue = [&](int k) {
+    auto issue = [&](int k, bool more) {
         abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx)));
         bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
-        if (k + 1 < nz) bulk_prefetch_l2(tile0 + (size_t)(k + 1) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
+        if (more) bulk_prefetch_l2(tile0 + (size_t)(k + kstep) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
         if (!(P.dbg & 2)) bulk_prefetch_l2(ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)));
     };
     if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, NT);
     if (NEU) for (int i = tid; i < L::DCT; i += NT) tdct[i] = P.tw_dct[i];
     FSEI_SYNC();
-    if (tid == 0) issue(0);
+    if (tid == 0 && kcount > 0) issue(kfirst, kcount > 1);
     unsigned parity = 0;
 
     constexpr int RL = (C::NP == 3) ? C::R2 : C::R1, NSL = N / RL;   // last pass: output slot i RL + q = row tl + i T + q NSL
@@ -93,11 +103,13 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     cplx carry[NCARRY];                                          // d'_{k-1} of this thread's elements
 #pragma unroll
     for (int m = 0; m < NCARRY; m++) carry[m] = cmake(0.0, 0.0);
-    double a_k = P.za[0];
+    double a_k = kcount > 0 ? coef[kfirst] : 0.0;
 
-    for (int k = 0; k < nz; k++) {
+    for (int it = 0; it < kcount; it++) {
+        const int k = kfirst + it * kstep;
+        const bool more = it + 1 < kcount;
         abar_wait(bar, parity); parity ^= 1;
-        auto next = [&]() { if (tid == 0 && k + 1 < nz) issue(k + 1); };
+        auto next = [&]() { if (tid == 0 && more) issue(k + kstep, it + 2 < kcount); };
         auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll
             for (int i = 0; i < PER0; i++) {
@@ -108,11 +120,13 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
                 }
             }
         };
+        // last plane of a twisted sweep: also kept aside for the back substitution's start
+        cplx* gm = (P.ktw < nz && !more) ? P.mid + ((size_t)tile * 2 + (up ? 0 : 1)) * L::TILE : nullptr;
         if (!pairing && !(P.dbg & 1)) {
             // Columns with a single spectrum: the elimination runs on the last pass' outputs while they are still in
             // registers (output slot s of this thread is row RB(s) every plane, so d'_{k-1} is carried per slot).
             const double a = a_k;
-            a_k = (k + 1 < nz) ? P.za[k + 1] : 0.0;
+            a_k = more ? coef[k + kstep] : 0.0;
             const double* ipk = ip0 + (size_t)k * L::IPT;
             cplx* gk = tile0 + (size_t)k * L::TILE;
             double ipv[NSLOT][NCOMP];
@@ -129,6 +143,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
             auto elim = [&](int n, cplx d, int s) {
                 carry[s] = cmake((d.re - a * carry[s].re) * ipv[s][0], (d.im - a * carry[s].im) * ipv[s][NCOMP - 1]);
                 gk[n * CB + c] = carry[s];
+                if (gm) gm[n * CB + c] = carry[s];
             };
             fft_column<C, CB, false, false, false>(tl, c, true, buf, tws, load0, elim, next, pivots);
             FSEI_SYNC();
@@ -175,7 +190,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
         // Loads first, then arithmetic, then stores: the compiler cannot reorder shared-memory accesses itself.
         {
             const double a = a_k;
-            a_k = (k + 1 < nz) ? P.za[k + 1] : 0.0;             // next plane's coefficient: latency hidden by this plane
+            a_k = more ? coef[k + kstep] : 0.0;             // next plane's coefficient: latency hidden by this plane
             cplx* gk = tile0 + (size_t)k * L::TILE;
             cplx d[EPT];
 #pragma unroll
@@ -199,6 +214,10 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
             }
 #pragma unroll
             for (int m = 0; m < EPT; m++) gk[tid + m * NT] = carry[m];
+            if (gm) {
+#pragma unroll
+                for (int m = 0; m < EPT; m++) gm[tid + m * NT] = carry[m];
+            }
         }
         FSEI_SYNC();
     }
@@ -220,15 +239,20 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
     double* ipb = reinterpret_cast<double*>(tdct + L::DCT);      // [IPT]
     const int tid = threadIdx.x;
     const int tl = tid / CB, c = tid - tl * CB;
-    const int tile = (int)((blockIdx.x + P.tile_shift) % gridDim.x), c0 = tile * CB, col = c0 + c;
+    const int tile = (int)((blockIdx.x + (blockIdx.y ? P.tile_shift[1] : P.tile_shift[0])) % gridDim.x), c0 = tile * CB, col = c0 + c;
     const int nz = P.nz;
+    // this CTA's sweep: planes [0, ktw) downwards from ktw-1 (blockIdx.y = 0; the whole column when ktw = nz), or planes
+    // [ktw, nz) upwards from ktw (blockIdx.y = 1, twisted factorisation only)
+    const bool down = blockIdx.y == 0;
+    const int kfirst = down ? P.ktw - 1 : P.ktw, kstep = down ? -1 : 1, kcount = down ? P.ktw : nz - P.ktw;
+    const double* coef = down ? P.zcc : P.za;
     const bool pairing = (NEU || (c0 < P.untangle)) && !(P.dbg & 4);
     const bool mine = NEU || (col < P.untangle);
     const double SQ2 = 1.41421356237309504880168872420969808;
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;
     const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
 
-    auto issue = [&](int k) {
+    auto issue = [&](int k, bool more) {
         if (P.dbg & 2) {
             abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx)));
             bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
@@ -237,24 +261,53 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
         abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx) + L::IPT * sizeof(double)));
         bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
         bulk_g2s(ipb, ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)), bar);
-        if (k > 0) {                                             // next plane's bytes: DRAM -> L2 now
-            bulk_prefetch_l2(tile0 + (size_t)(k - 1) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
-            bulk_prefetch_l2(ip0 + (size_t)(k - 1) * L::IPT, (unsigned)(L::IPT * sizeof(double)));
+        if (more) {                                              // next plane's bytes: DRAM -> L2 now
+            bulk_prefetch_l2(tile0 + (size_t)(k + kstep) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
+            bulk_prefetch_l2(ip0 + (size_t)(k + kstep) * L::IPT, (unsigned)(L::IPT * sizeof(double)));
         }
     };
     if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, NT);
     if (NEU) for (int i = tid; i < L::DCT; i += NT) tdct[i] = P.tw_dct[i];
     FSEI_SYNC();
-    if (tid == 0) issue(nz - 1);
+    if (tid == 0 && kcount > 0) issue(kfirst, kcount > 1);
     unsigned parity = 0;
 
-    cplx carry[EPT];                                             // x_{k+1} of this thread's elements
+    cplx carry[EPT];                                             // x of the plane just left, per element of this thread
 #pragma unroll
     for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
-    double c_k = P.zcc[nz - 1];
+    if (P.ktw < nz) {
+        // Twisted factorisation: the two eliminations met between planes m-1 and m,
+        //   x_{m-1} + cp x_m = d'_{m-1},   ap x_{m-1} + x_m = e'_m      (cp = c_{m-1} / piv_{m-1}, ap = a_m / piv_m)
+        // so x_m = (e'_m - ap d'_{m-1}) / (1 - ap cp) and x_{m-1} = d'_{m-1} - cp x_m.  The downward sweep starts from x_m,
+        // the upward one from x_{m-1}; each CTA works them out for its own elements (slot order of its substitution).
+        const int m = P.ktw;
+        const double cm1 = P.zcc[m - 1], am = P.za[m];
+        const cplx* dm1 = P.mid + (size_t)tile * 2 * L::TILE;      // copies left by k_yz_forward
+        const cplx* em = dm1 + L::TILE;
+        const double* ipm1 = ip0 + (size_t)(m - 1) * L::IPT;
+        const double* iqm = ip0 + (size_t)m * L::IPT;
+#pragma unroll
+        for (int s = 0; s < EPT; s++) {
+            const int e = pairing ? tid + s * NT : (tl + (s / R0) * T + (s % R0) * (N / R0)) * CB + c;
+            const cplx d1 = dm1[e], e0 = em[e];
+            double x[2];
+#pragma unroll
+            for (int q = 0; q < 2; q++) {
+                const int qc = q ? NCOMP - 1 : 0;
+                const double cp = cm1 * ipm1[e * NCOMP + qc], ap = am * iqm[e * NCOMP + qc];
+                const double dv = q ? d1.im : d1.re, ev = q ? e0.im : e0.re;
+                const double xm = (ev - ap * dv) / (1.0 - ap * cp);
+                x[q] = down ? xm : dv - cp * xm;
+            }
+            carry[s] = cmake(x[0], x[1]);
+        }
+    }
+    double c_k = kcount > 0 ? coef[kfirst] : 0.0;
 
-    for (int k = nz - 1; k >= 0; k--) {
+    for (int it = 0; it < kcount; it++) {
+        const int k = kfirst + it * kstep;
+        const bool more = it + 1 < kcount;
         abar_wait(bar, parity); parity ^= 1;
         if (!pairing && !(P.dbg & 1)) {
             // Columns with a single spectrum (no special column among them): the substitution feeds the first pass
@@ -262,7 +315,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
             constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
             static_assert(NB0 % T == 0 && PER0 * R0 == EPT, "first pass must tile the column exactly");
             const double cz = c_k;
-            c_k = (k > 0) ? P.zcc[k - 1] : 0.0;
+            c_k = more ? coef[k + kstep] : 0.0;
             cplx* gk = tile0 + (size_t)k * L::TILE;
             auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll
@@ -277,7 +330,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
                     }
                 }
             };
-            auto next = [&]() { if (tid == 0 && k > 0) issue(k - 1); };
+            auto next = [&]() { if (tid == 0 && more) issue(k + kstep, it + 2 < kcount); };
             auto out = [&](int n, cplx z, int) { gk[n * CB + c] = z; };
             fft_column<C, CB, true, false, false>(tl, c, true, buf, tws, load0, out, next);
             FSEI_SYNC();
@@ -285,7 +338,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
         }
         {
             const double cz = c_k;
-            c_k = (k > 0) ? P.zcc[k - 1] : 0.0;
+            c_k = more ? coef[k + kstep] : 0.0;
             cplx dp[EPT];
             double ipv[EPT][NCOMP];
 #pragma unroll
@@ -311,7 +364,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
             }
         }
         FSEI_SYNC();
-        if (tid == 0 && k > 0) issue(k - 1);                     // landing tiles consumed: prefetch the next plane
+        if (tid == 0 && more) issue(k + kstep, it + 2 < kcount); // landing tiles consumed: prefetch the next plane
         if (pairing) {
             for (int kk = tl; kk <= N / 2; kk += T) {
                 if (kk == 0 || (!NEU && (2 * kk == N || !mine))) continue;

@@ -21,6 +21,8 @@ struct ZFast {
     const double* dzm;    // [nz] (dzm[0] unused)
     const double* ipiv;   // [nz][ny][nxc][ncomp] reciprocal pivots (plan time)
     cplx* special;        // [2][nz] solved special columns: (row 0, slot 0) and, on (P,P), (row ny/2, slot 0)
+    int ktw;              // twist plane: nz = plain Thomas (pivots eliminated from k = 0 upwards); < nz = twisted
+                          // factorisation (fused path, few tiles): planes [0, ktw) from below, planes [ktw, nz) from above
     int cb;               // spectrum / pivot-table layout: 0 = natural, else blocked by tiles of cb slots (xfast.cuh)
     const cplx* special_in;   // fused path: [2][nz] right-hand sides of the special columns (else read from the spectrum)
     double* cpw;          // [8][nz] plan-time factorisation of the special columns: c'_k of component t at [t][k],
@@ -60,19 +62,28 @@ FSEI_HD int z_special(const ZFast& Z, int row, int slot, int& mask)
     return -1;
 }
 
-// plan time: reciprocal pivots of one component of one column
+// plan time: reciprocal pivots of one component of one column.  Planes [0, ktw): piv_k = b_k - a_k (c_{k-1} / piv_{k-1});
+// planes [ktw, nz) (twisted): piv_k = b_k - c_k (a_{k+1} / piv_{k+1}), eliminated from the top wall downwards.
 FSEI_HD void zf_factor_column(const ZFast& Z, double* ipiv, int row, int slot, int comp)
 {
     int mask; z_special(Z, row, slot, mask);
     const bool zero_it = (Z.ncomp == 1) ? (mask != 0) : ((mask >> comp) & 1);
     const double lam = z_lambda(Z, row, slot, comp);
     double cp = 0.0;
-    for (int k = 0; k < Z.nz; k++) {
+    for (int k = 0; k < Z.ktw; k++) {
         double a = Z.za[k], c = Z.zcc[k];
         double piv = (-(a + c) + lam) - a * cp;
         double ip = zero_it ? 0.0 : 1.0 / piv;
         ipiv[zf_idx(Z, k, row, slot) * Z.ncomp + comp] = ip;
         cp = c * ip;
+    }
+    double ap = 0.0;
+    for (int k = Z.nz - 1; k >= Z.ktw; k--) {
+        double a = Z.za[k], c = Z.zcc[k];
+        double piv = (-(a + c) + lam) - c * ap;
+        double iq = zero_it ? 0.0 : 1.0 / piv;
+        ipiv[zf_idx(Z, k, row, slot) * Z.ncomp + comp] = iq;
+        ap = a * iq;
     }
 }
 

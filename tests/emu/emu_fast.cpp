@@ -136,7 +136,8 @@ void xib(const XFast& P, bool neu, const cplx* spec, double* phi)
 template <class C, bool NEU, int NCOMP> void yz_variant(const YZFused& P, bool backward, cplx* spec)
 {
     using L = YZSmem<C, FSEI_CB, NEU, NCOMP>;
-    const unsigned grid = P.nxc / FSEI_CB, nt = C::T * FSEI_CB;
+    const dim3 grid(P.nxc / FSEI_CB, P.ktw < P.nz ? 2 : 1);
+    const unsigned nt = C::T * FSEI_CB;
     if (!backward) cuda_shim::launch(grid, nt, L::FWD, [&] { k_yz_forward<C, FSEI_CB, NEU, NCOMP>(P, spec); });
     else cuda_shim::launch(grid, nt, L::BWD, [&] { k_yz_backward<C, FSEI_CB, NEU, NCOMP>(P, spec); });
 }
@@ -155,10 +156,10 @@ struct Ctx {
     HostTables T;
     SParams S; XFast XF; YFast YF; ZFast ZF;
     std::vector<double> ipiv, cpw;
-    std::vector<cplx> special, special_in;
+    std::vector<cplx> special, special_in, mid;
 };
 
-void setup(Ctx& c, bool blocked = false)
+void setup(Ctx& c, bool blocked = false, bool twist = false)
 {
     HostTables& T = c.T;
     c.S.nx = T.nx; c.S.ny = T.ny; c.S.nz = T.nz; c.S.bcx = T.bcx; c.S.bcy = T.bcy; c.S.rdx = T.rdx; c.S.rdy = T.rdy;
@@ -174,6 +175,7 @@ void setup(Ctx& c, bool blocked = false)
     c.special.assign(2 * (size_t)T.nz, cmake(0, 0)); ZF.special = c.special.data();
     c.cpw.assign(8 * (size_t)T.nz, 0.0); ZF.cpw = c.cpw.data();
     ZF.cb = blocked ? FSEI_CB : 0; ZF.special_in = nullptr;
+    ZF.ktw = (twist && T.nz >= 4) ? T.nz / 2 : T.nz;
     if (blocked) { c.special_in.assign(2 * (size_t)T.nz, cmake(0, 0)); ZF.special_in = c.special_in.data(); }
     c.ipiv.assign((size_t)T.nz * T.ny * T.nxc * ZF.ncomp, 0.0); ZF.ipiv = c.ipiv.data();
     size_t cols = (size_t)T.ny * T.nxc * ZF.ncomp;
@@ -205,7 +207,9 @@ void fused_spectral_solve(Ctx& c, cplx* work, double* phi)
     YZ.nxc = T.nxc; YZ.ny = T.ny; YZ.nz = T.nz; YZ.untangle = c.YF.untangle;
     YZ.pp = (T.bcx == BC_PERIODIC && T.bcy == BC_PERIODIC) ? 1 : 0;
     YZ.tw = T.twy.data(); YZ.tw_dct = T.twy_dct.data(); YZ.za = T.za.data(); YZ.zcc = T.zcc.data(); YZ.ip = c.ipiv.data();
-    YZ.special_in = c.special_in.data(); YZ.special = c.special.data(); YZ.dbg = 0; YZ.tile_shift = 3 % (T.nxc / FSEI_CB);
+    YZ.special_in = c.special_in.data(); YZ.special = c.special.data(); YZ.dbg = 0;
+    YZ.tile_shift[0] = 3 % (T.nxc / FSEI_CB); YZ.tile_shift[1] = 5 % (T.nxc / FSEI_CB);
+    YZ.ktw = c.ZF.ktw; c.mid.assign((size_t)T.nxc * T.ny * 2, cmake(0, 0)); YZ.mid = c.mid.data();
     const bool yneu = T.bcy == BC_NEUMANN;
     yz(YZ, false, yneu, c.ZF.ncomp, work);
     cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz + 16, [&] { k_z_special(c.ZF, work); });
@@ -226,12 +230,12 @@ int emu_fused_pressure_projection(int nx, int ny, int nz, double Lx, double Ly, 
     Ctx c; int code = 0;
     std::string msg = build_tables(c.T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code, true);
     if (code) { std::fprintf(stderr, "emu: %s\n", msg.c_str()); return code; }
-    setup(c, true);
+    setup(c, true, (split & 4) != 0);                      // split & 4: twisted factorisation (two CTAs per tile)
     const size_t n = (size_t)nx * ny * nz;
     const unsigned gpairs = (unsigned)((n / 2 + 255) / 256);
     std::vector<cplx> work(n / 2);
     const bool xneu = bcx == BC_NEUMANN;
-    if (split) {
+    if (split & 1) {
         cuda_shim::launch(gpairs, 256, 0, [&] { k_divergence_fast(c.S, u, v, w, 1.0 / alpha_dt, phi); });
         xfb(c.XF, c.S, xneu, false, phi, nullptr, nullptr, 0.0, work.data());
     } else {

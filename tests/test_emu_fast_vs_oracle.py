@@ -96,3 +96,14 @@ def test_fused_support_matrix():
     L = emu_fast_lib()
     assert L.emu_fused_supported(1024, 1024) and L.emu_fused_supported(768, 768) and L.emu_fused_supported(512, 384)
     assert not L.emu_fused_supported(256, 256) and not L.emu_fused_supported(32, 32)
+
+
+@pytest.mark.parametrize("bc,nz", [((P, P), 4), ((P, P), 7), ((N, N), 7), ((P, N), 12), ((N, P), 5)])
+def test_fused_twisted_factorisation(oracle_ld, bc, nz):
+    """two CTAs per tile: planes [0, nz/2) eliminated upwards, planes [nz/2, nz) downwards, met in the middle"""
+    case = inputs.make_case(2, shape=(512, 384, nz), bc=bc)
+    got = emu_fast_projection(case, 1e-4, 4, fused=True)         # split & 4: twisted
+    ref = oracle_projection(oracle_ld, case, 1e-4)
+    assert rel_l2(got[4], ref[4]) < 1e-13
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-11 * max(1.0, np.abs(r).max())

@@ -273,6 +273,25 @@ def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
     assert rel_l2(got[4], fast[4]) <= 1e-14
 
 
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 64), (512, 1024, 4)])
+def test_fused_twisted_factorisation(oracle_ld, fused_path, monkeypatch, bc, shape):
+    """two CTAs per tile sweep towards each other (the plan's choice when there are fewer tiles than SMs; forced
+    here), against the oracle and against the plain Thomas order of the same kernels"""
+    from paper_2103_15187_b200.binding import Plan
+    monkeypatch.setenv("FSEI_TWIST", "1")
+    case = inputs.make_case(2, shape=shape, bc=bc)
+    got = gpu_projection(case, 1e-4)
+    ref = oracle_projection(oracle_ld, case, 1e-4)
+    assert rel_l2(got[4], ref[4]) <= PHI_TOL
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
+    assert _post_div(oracle_ld, case, *got[:3]) <= div_gate(case, np.abs(got[4]).max())
+    monkeypatch.setenv("FSEI_TWIST", "0")
+    plain = gpu_projection(case, 1e-4)
+    assert rel_l2(got[4], plain[4]) <= 1e-12
+
+
 def test_fused_split_calls_and_aliasing(oracle_ld, fused_path):
     case = inputs.make_case(2, shape=(512, 384, 12))
     a = gpu_projection(case, split=True)                          # poisson_solve with phi aliasing rhs
