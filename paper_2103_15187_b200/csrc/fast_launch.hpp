@@ -27,6 +27,7 @@ cudaError_t yfast_init();
 // fused path (blocked spectrum layout, FSEI_CB slots per tile)
 bool xblocked_supported(int N);  // N = nx / 2
 bool yzfused_supported(int N);   // N = ny
+int yzfused_block_threads(int N);  // threads per CTA of the z-marching y kernels
 cudaError_t xblocked_init();
 cudaError_t yzfused_init();
 // tensor map of the blocked spectrum for the x-inverse loads (plan time; spec = the plan's workspace)

@@ -15,6 +15,16 @@ bool yzfused_supported(int N)
     }
 }
 
+int yzfused_block_threads(int N)
+{
+    switch (N) {
+#define X(n, a, b, c) case n: return FftCfg<n, a, b, c>::T * FSEI_CB;
+        FSEI_YZ_CONFIGS(X)
+#undef X
+        default: return 0;
+    }
+}
+
 // boundary-condition variants: (periodic y, 1 pivot component) = (P,P); (periodic y, 2) = (N,P); (Neumann y, 2)
 template <class C, bool NEU, int NCOMP> static cudaError_t init_variant()
 {

@@ -311,7 +311,8 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         // idle: fewer tiles than SMs.  FSEI_TWIST = 0 | 1 overrides (tests).
         int nsm = 148;
         { int dev = 0; CU(cudaGetDevice(&dev)); CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev)); }
-        bool twist = fused && nz >= 4 && T.nxc / FSEI_CB <= nsm;
+        // ... or three-warp CTAs (ny = 3 2^a) that cannot fill their SM even two at a time (configs[4]: 23.5 -> 22.1 ms)
+        bool twist = fused && nz >= 4 && (T.nxc / FSEI_CB <= nsm || (yzfused_block_threads(ny) < 128 && T.nxc / FSEI_CB <= 2 * nsm));
         if (const char* tw = std::getenv("FSEI_TWIST")) twist = fused && nz >= 4 && tw[0] == '1';
         ZF.ktw = twist ? nz / 2 : nz;
         if (fused) {

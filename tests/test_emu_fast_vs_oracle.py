@@ -66,9 +66,11 @@ def test_fast_support_matrix():
 
 
 # ---- fused path: blocked spectrum layout, Thomas sweeps riding on the z-marching y kernels (yzfused.cuh) ----------
-def _check_fused(oracle_ld, shape, bc, cfg=2, beta=1e-4):
+# The short line lengths (nx = 32, 64, 96; ny = 16, 32, 48) are instantiated for tests; the plan picks the fused path
+# on large grids only, and the GPU parity tests cover the production lengths.
+def _check_fused(oracle_ld, shape, bc, cfg=2, beta=1e-4, mode=0):
     case = inputs.make_case(cfg, shape=shape, bc=bc)
-    got = emu_fast_projection(case, beta, False, fused=True)
+    got = emu_fast_projection(case, beta, mode, fused=True)
     ref = oracle_projection(oracle_ld, case, beta)
     assert rel_l2(got[4], ref[4]) < 1e-13
     for g, r in zip(got[:4], ref[:4]):
@@ -77,33 +79,30 @@ def _check_fused(oracle_ld, shape, bc, cfg=2, beta=1e-4):
 
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
-def test_fused_kernels_match_oracle(oracle_ld, bc):
-    a = _check_fused(oracle_ld, (512, 384, 5), bc)
-    case = inputs.make_case(2, shape=(512, 384, 5), bc=bc)
-    b = emu_fast_projection(case, 1e-4, True, fused=True)        # divergence kernel + non-fused blocked x-forward
+@pytest.mark.parametrize("shape", [(32, 32, 5), (64, 16, 9), (96, 48, 4)])
+def test_fused_kernels_match_oracle(oracle_ld, bc, shape):
+    a = _check_fused(oracle_ld, shape, bc)
+    b = _check_fused(oracle_ld, shape, bc, mode=1)               # divergence kernel + non-fused blocked x-forward
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
 
 
-# every blocked x length and every z-marching y length that has an instantiation
-@pytest.mark.parametrize("shape", [(768, 512, 2), (1024, 384, 2), (2048, 384, 2), (512, 768, 2), (512, 1024, 3)])
-def test_fused_every_length(oracle_ld, shape):
-    for bc in ((P, P), (N, N)):
-        _check_fused(oracle_ld, shape, bc)
+@pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
+@pytest.mark.parametrize("shape", [(32, 32, 4), (64, 48, 7), (96, 16, 12), (32, 16, 5)])
+def test_fused_twisted_factorisation(oracle_ld, bc, shape):
+    """two CTAs per tile: planes [0, nz/2) eliminated upwards, planes [nz/2, nz) downwards, met in the middle"""
+    a = _check_fused(oracle_ld, shape, bc, mode=4)               # mode & 4: twisted
+    b = _check_fused(oracle_ld, shape, bc)
+    assert rel_l2(a[4], b[4]) < 1e-13
+
+
+# production lengths: one blocked x length and one z-marching y length per run (nz = 2 keeps the thread teams cheap)
+@pytest.mark.parametrize("shape,bc", [((512, 384, 2), (P, P)), ((768, 512, 2), (N, N))])
+def test_fused_production_lengths(oracle_ld, shape, bc):
+    _check_fused(oracle_ld, shape, bc)
 
 
 def test_fused_support_matrix():
     L = emu_fast_lib()
     assert L.emu_fused_supported(1024, 1024) and L.emu_fused_supported(768, 768) and L.emu_fused_supported(512, 384)
-    assert not L.emu_fused_supported(256, 256) and not L.emu_fused_supported(32, 32)
-
-
-@pytest.mark.parametrize("bc,nz", [((P, P), 4), ((P, P), 7), ((N, N), 7), ((P, N), 12), ((N, P), 5)])
-def test_fused_twisted_factorisation(oracle_ld, bc, nz):
-    """two CTAs per tile: planes [0, nz/2) eliminated upwards, planes [nz/2, nz) downwards, met in the middle"""
-    case = inputs.make_case(2, shape=(512, 384, nz), bc=bc)
-    got = emu_fast_projection(case, 1e-4, 4, fused=True)         # split & 4: twisted
-    ref = oracle_projection(oracle_ld, case, 1e-4)
-    assert rel_l2(got[4], ref[4]) < 1e-13
-    for g, r in zip(got[:4], ref[:4]):
-        assert np.abs(g - r).max() <= 1e-11 * max(1.0, np.abs(r).max())
+    assert L.emu_fused_supported(32, 32) and not L.emu_fused_supported(256, 256) and not L.emu_fused_supported(128, 64)
