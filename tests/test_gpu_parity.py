@@ -252,7 +252,8 @@ def fused_path(monkeypatch):
 
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
-@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 6), (512, 768, 5), (2048, 1024, 3)])
+@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 6), (512, 768, 5), (2048, 1024, 3), (32, 32, 33), (64, 16, 9),
+                                   (96, 48, 40)])
 def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
     from paper_2103_15187_b200.binding import Plan
     for cfg, beta in ((1, 0.0), (2, 1e-4)):
@@ -274,7 +275,7 @@ def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
 
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
-@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 64), (512, 1024, 4)])
+@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 64), (512, 1024, 4), (32, 32, 33), (96, 16, 5), (64, 48, 4)])
 def test_fused_twisted_factorisation(oracle_ld, fused_path, monkeypatch, bc, shape):
     """two CTAs per tile sweep towards each other (the plan's choice when there are fewer tiles than SMs; forced
     here), against the oracle and against the plain Thomas order of the same kernels"""
