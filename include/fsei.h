@@ -26,8 +26,9 @@
  * Execution.  Calls enqueue kernels on `cuda_stream` and return; they never synchronise
  * the device and never allocate after plan creation.  Calls on different plans may run
  * concurrently; calls on ONE plan must be issued from one thread at a time and on one
- * stream at a time (the plan owns factorisation tables only -- the transforms run in
- * place in the caller's phi buffer -- but the gauge scratch is per plan).
+ * stream at a time (the plan owns the factorisation tables, the scratch of the gauge
+ * column and, on large grids, one workspace field that holds the spectrum in a blocked
+ * layout; on small grids the transforms run in place in the caller's phi buffer).
  *
  * Errors.  Functions returning int return FSEI_OK or an FSEI_ERR_* code; nothing throws
  * across this boundary; fsei_last_error() gives a thread-local message for the last
@@ -63,7 +64,7 @@ fsei_plan*  fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly,
 void        fsei_plan_destroy(fsei_plan* plan);
 const char* fsei_last_error(void);
 int         fsei_last_error_code(void);
-/* Device bytes the plan owns (tables + z-factorisation + scratch). */
+/* Device bytes the plan owns (tables + z-factorisation + scratch +, on large grids, one spectrum field). */
 size_t      fsei_plan_workspace_bytes(const fsei_plan* plan);
 
 /*
