@@ -62,7 +62,10 @@ template <class C, bool NEU> struct XShape {
                (NEU ? sizeof(double) * (size_t)L * (2 * N + (2 * N >> 2) + 2) : 0);
     }
     static constexpr int fit(int L) { return (L <= 1 || bytes(L) <= 200 * 1024) ? L : fit(L - 1); }
-    static constexpr int LPB = fit((256 / C::T) > 0 ? (256 / C::T) : 1);      // about 256 threads, <= 200 KB
+    static constexpr int pow2_floor(int v) { return v <= 1 ? 1 : 2 * pow2_floor(v / 2); }
+    // about 256 threads, <= 200 KB, a power of two: the blocked layout's segments (16 LPB CB bytes) stay 128-byte
+    // aligned and LPB divides the usual ny
+    static constexpr int LPB = fit(pow2_floor((256 / C::T) > 0 ? (256 / C::T) : 1));
 };
 
 // LL = lines of n doubles in the landing tile: 4 LPB + 1 (fused forward) or LPB

@@ -447,3 +447,40 @@ def test_size_limits_are_errors():
         with pytest.raises(binding.FseiError) as e:
             binding.Plan.from_grid(tuple(grid))
         assert e.value.code == binding.ERR_SIZE
+
+
+# ---------------------------------------------------------------------------------------------
+# execution contract of fsei.h: deterministic, plans independent of each other, any stream
+# ---------------------------------------------------------------------------------------------
+def test_deterministic_and_concurrent_plans(monkeypatch):
+    torch = _torch()
+    from paper_2103_15187_b200.binding import Plan
+    monkeypatch.setenv("FSEI_PATH", "fused")
+    ca = inputs.make_case(2, shape=(512, 384, 16))
+    pa = Plan.from_grid(ca.grid)
+    monkeypatch.delenv("FSEI_PATH")
+    cb = inputs.make_case(1, shape=(96, 72, 40), bc=(N, P))
+    pb = Plan.from_grid(cb.grid)
+    assert pa.workspace_bytes >= 8 * ca.cells                  # fused path: the blocked spectrum field is plan-owned
+    ref_a, ref_b = gpu_projection(ca, plan=pa), gpu_projection(cb, plan=pb)
+    again = gpu_projection(ca, plan=pa)
+    for x, y in zip(ref_a, again):
+        assert np.array_equal(x, y)                            # no atomics, no races: bit-identical reruns
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    fa = [t.clone() for t in gpu_fields(ca)]; fb = [t.clone() for t in gpu_fields(cb)]
+    qa, qb = torch.zeros_like(fa[0]), torch.zeros_like(fb[0])
+    ha, hb = torch.empty_like(fa[0]), torch.empty_like(fb[0])
+    torch.cuda.synchronize()
+    for _ in range(3):                                           # interleave the two plans on two streams
+        with torch.cuda.stream(sa):
+            pa.pressure_projection(*fa, qa, ha, ca.alpha_dt, 0.0)
+        with torch.cuda.stream(sb):
+            pb.pressure_projection(*fb, qb, hb, cb.alpha_dt, 0.0)
+    torch.cuda.synchronize()
+    seq_a = [t.clone() for t in gpu_fields(ca)]; pq = torch.zeros_like(seq_a[0]); ph = torch.empty_like(pq)
+    for _ in range(3):
+        pa.pressure_projection(*seq_a, pq, ph, ca.alpha_dt, 0.0)
+    torch.cuda.synchronize()
+    for x, y in zip(fa + [qa, ha], seq_a + [pq, ph]):
+        assert torch.equal(x, y)
+    pa.destroy(); pb.destroy()
