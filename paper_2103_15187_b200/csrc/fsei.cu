@@ -337,7 +337,6 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             YZ.pp = (bcx == BC_PERIODIC && bcy == BC_PERIODIC) ? 1 : 0;
             YZ.tw = Y.tw; YZ.tw_dct = Y.tw_dct; YZ.za = Z.za; YZ.zcc = Z.zcc; YZ.ip = ZF.ipiv;
             YZ.special_in = const_cast<cplx*>(ZF.special_in); YZ.special = ZF.special;
-            { const char* d = std::getenv("FSEI_DBG"); YZ.dbg = d ? std::atoi(d) : 0; }
             {
                 // CTAs are dealt to the SMs breadth first: with nsm < total < 2 nsm CTAs the linear ids total - nsm .. nsm - 1
                 // get an SM to themselves; the tile that carries the split / merge work of a (P,P) grid (tile 0: the

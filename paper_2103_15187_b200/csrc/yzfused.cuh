@@ -39,7 +39,6 @@ struct YZFused {
                                 // back-substitution CTAs of a tile start from (each overwrites one of them in place)
     int tile_shift[2];          // tile = (blockIdx.x + tile_shift[blockIdx.y]) % ntiles: puts the one tile that carries
                                 // the split / merge work (tile 0 on (P,P)) on a CTA that is likely alone on its SM
-    int dbg;                    // timing experiments only (FSEI_DBG): 1 = skip the transform, 2 = skip the pivot loads
 };
 
 template <class C, int CB, bool NEU, int NCOMP> struct YZSmem {
@@ -77,7 +76,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     const bool up = blockIdx.y == 0;
     const int kfirst = up ? 0 : nz - 1, kstep = up ? 1 : -1, kcount = up ? P.ktw : nz - P.ktw;
     const double* coef = up ? P.za : P.zcc;
-    const bool pairing = (NEU || (c0 < P.untangle)) && !(P.dbg & 4);             // CTA-uniform
+    const bool pairing = NEU || (c0 < P.untangle);             // CTA-uniform
     const bool mine = NEU || (col < P.untangle);
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;            // plane k of this tile at tile0 + k TILE
     const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
@@ -88,7 +87,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
         abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx)));
         bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
         if (more) bulk_prefetch_l2(tile0 + (size_t)(k + kstep) * L::TILE, (unsigned)(L::TILE * sizeof(cplx)));
-        if (!(P.dbg & 2)) bulk_prefetch_l2(ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)));
+        bulk_prefetch_l2(ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)));
     };
     if (tid == 0) abar_init(bar);
     fft_fill_twiddles<C>(tws, P.tw, tid, NT);
@@ -122,7 +121,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
         };
         // last plane of a twisted sweep: also kept aside for the back substitution's start
         cplx* gm = (P.ktw < nz && !more) ? P.mid + ((size_t)tile * 2 + (up ? 0 : 1)) * L::TILE : nullptr;
-        if (!pairing && !(P.dbg & 1)) {
+        if (!pairing) {
             // Columns with a single spectrum: the elimination runs on the last pass' outputs while they are still in
             // registers (output slot s of this thread is row RB(s) every plane, so d'_{k-1} is carried per slot).
             const double a = a_k;
@@ -136,7 +135,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
                     const int b = tl + (s / RL) * T, n = b + (s % RL) * NSL;
                     if (b < NSL) {
 #pragma unroll
-                        for (int q = 0; q < NCOMP; q++) ipv[s][q] = (P.dbg & 2) ? 1.0 : ld_stream(ipk + (size_t)(n * CB + c) * NCOMP + q);
+                        for (int q = 0; q < NCOMP; q++) ipv[s][q] = ld_stream(ipk + (size_t)(n * CB + c) * NCOMP + q);
                     }
                 }
             };
@@ -149,11 +148,6 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
             FSEI_SYNC();
             continue;
         }
-        if (P.dbg & 1) {
-            for (int m = 0; m < EPT; m++) { const int e = tid + m * NT; buf[C::pad(e / CB) * CB + e % CB] = land[e]; }
-            FSEI_SYNC();
-            next();
-        } else
         fft_column<C, CB, false, false, true>(tl, c, true, buf, tws, load0, YOut<C, CB>{buf, c}, next);
         // reciprocal pivots of this thread's elements (L2 hits), in flight across the barrier(s) below
         double ipv[EPT][NCOMP];
@@ -162,7 +156,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
 #pragma unroll
             for (int m = 0; m < EPT; m++) {
 #pragma unroll
-                for (int q = 0; q < NCOMP; q++) ipv[m][q] = (P.dbg & 2) ? 1.0 : ld_stream(ipk + (size_t)(tid + m * NT) * NCOMP + q);
+                for (int q = 0; q < NCOMP; q++) ipv[m][q] = ld_stream(ipk + (size_t)(tid + m * NT) * NCOMP + q);
             }
         }
         FSEI_SYNC();
@@ -246,18 +240,13 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
     const bool down = blockIdx.y == 0;
     const int kfirst = down ? P.ktw - 1 : P.ktw, kstep = down ? -1 : 1, kcount = down ? P.ktw : nz - P.ktw;
     const double* coef = down ? P.zcc : P.za;
-    const bool pairing = (NEU || (c0 < P.untangle)) && !(P.dbg & 4);
+    const bool pairing = NEU || (c0 < P.untangle);
     const bool mine = NEU || (col < P.untangle);
     const double SQ2 = 1.41421356237309504880168872420969808;
     cplx* tile0 = spec + (size_t)tile * nz * L::TILE;
     const double* ip0 = P.ip + (size_t)tile * nz * L::IPT;
 
     auto issue = [&](int k, bool more) {
-        if (P.dbg & 2) {
-            abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx)));
-            bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
-            return;
-        }
         abar_expect(bar, (unsigned)(L::TILE * sizeof(cplx) + L::IPT * sizeof(double)));
         bulk_g2s(land, tile0 + (size_t)k * L::TILE, (unsigned)(L::TILE * sizeof(cplx)), bar);
         bulk_g2s(ipb, ip0 + (size_t)k * L::IPT, (unsigned)(L::IPT * sizeof(double)), bar);
@@ -309,7 +298,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
         const int k = kfirst + it * kstep;
         const bool more = it + 1 < kcount;
         abar_wait(bar, parity); parity ^= 1;
-        if (!pairing && !(P.dbg & 1)) {
+        if (!pairing) {
             // Columns with a single spectrum (no special column among them): the substitution feeds the first pass
             // of the inverse transform directly; x_{k+1} is carried per input slot of that pass.
             constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
@@ -385,9 +374,6 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
         cplx* gk = tile0 + (size_t)k * L::TILE;
         auto out = [&](int n, cplx z, int) { gk[(NEU ? dct_perm(n, N) : n) * CB + c] = z; };
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, YIn<C, CB>{buf, c}, v0); };
-        if (P.dbg & 1) {
-            for (int m = 0; m < EPT; m++) { const int e = tid + m * NT; gk[e] = buf[C::pad(e / CB) * CB + e % CB]; }
-        } else
         fft_column<C, CB, true, true, false>(tl, c, true, buf, tws, load0, out, NoHook{});
         FSEI_SYNC();
     }

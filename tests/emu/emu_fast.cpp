@@ -207,7 +207,7 @@ void fused_spectral_solve(Ctx& c, cplx* work, double* phi)
     YZ.nxc = T.nxc; YZ.ny = T.ny; YZ.nz = T.nz; YZ.untangle = c.YF.untangle;
     YZ.pp = (T.bcx == BC_PERIODIC && T.bcy == BC_PERIODIC) ? 1 : 0;
     YZ.tw = T.twy.data(); YZ.tw_dct = T.twy_dct.data(); YZ.za = T.za.data(); YZ.zcc = T.zcc.data(); YZ.ip = c.ipiv.data();
-    YZ.special_in = c.special_in.data(); YZ.special = c.special.data(); YZ.dbg = 0;
+    YZ.special_in = c.special_in.data(); YZ.special = c.special.data();
     YZ.tile_shift[0] = 3 % (T.nxc / FSEI_CB); YZ.tile_shift[1] = 5 % (T.nxc / FSEI_CB);
     YZ.ktw = c.ZF.ktw; c.mid.assign((size_t)T.nxc * T.ny * 2, cmake(0, 0)); YZ.mid = c.mid.data();
     const bool yneu = T.bcy == BC_NEUMANN;
