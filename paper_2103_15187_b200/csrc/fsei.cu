@@ -106,26 +106,6 @@ static int dalloc(fsei_plan* P, size_t n, void** d)
 // ------------------------------------------------------------------------------------------
 #define NT 256
 
-__global__ void __launch_bounds__(NT) k_divergence(SParams S, const double* __restrict__ u, const double* __restrict__ v,
-                                                   const double* __restrict__ w, double inv_adt, double* __restrict__ rhs)
-{
-    const size_t n = (size_t)S.nx * S.ny * S.nz;
-    for (size_t c = (size_t)blockIdx.x * NT + threadIdx.x; c < n; c += (size_t)gridDim.x * NT) {
-        int i = (int)(c % S.nx); size_t r = c / S.nx; int j = (int)(r % S.ny), k = (int)(r / S.ny);
-        rhs[c] = div_at(S, u, v, w, i, j, k, inv_adt);
-    }
-}
-
-__global__ void __launch_bounds__(NT) k_project(SParams S, double* __restrict__ u, double* __restrict__ v, double* __restrict__ w,
-                                                double* __restrict__ p, const double* __restrict__ phi, double adt, double beta)
-{
-    const size_t n = (size_t)S.nx * S.ny * S.nz;
-    for (size_t c = (size_t)blockIdx.x * NT + threadIdx.x; c < n; c += (size_t)gridDim.x * NT) {
-        int i = (int)(c % S.nx); size_t r = c / S.nx; int j = (int)(r % S.ny), k = (int)(r / S.ny);
-        project_at(S, u, v, w, p, phi, i, j, k, adt, beta);
-    }
-}
-
 template <bool INV> __device__ __forceinline__ void x_all_passes(const XParams& X, cplx* sm, int lines)
 {
     int Ns[8]; int n = X.N;
@@ -435,13 +415,6 @@ extern "C" int fsei_plan_last_launch_count(const fsei_plan* P) { return P ? P->l
 // ------------------------------------------------------------------------------------------
 // the calls
 // ------------------------------------------------------------------------------------------
-static unsigned stencil_grid(size_t n)
-{
-    size_t b = (n + NT - 1) / NT;
-    const size_t cap = 148 * 8 * 16;
-    return (unsigned)(b < cap ? b : cap);
-}
-
 extern "C" int fsei_divergence(fsei_plan* P, const double* u, const double* v, const double* w, double alpha_dt,
                                double* rhs, void* cuda_stream)
 {
