@@ -371,8 +371,13 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
         abar_wait(bar, parity); parity ^= 1;
         // packed half spectrum -> Z (Hermitian pair step, preceded by the inverse quarter-wave twiddle)
         // gl(p): slot p of line l2 in the landing tile; lb: that line's buffer
-        auto pair_load = [&](int l2, cplx* lb, int p) {
-            auto g = [&](int q) -> cplx { return CB ? land[((q / (CB ? CB : 1)) * LPB + l2) * CB + q % (CB ? CB : 1)] : land[l2 * N + q]; };
+        // (restrict: the landing tile and the tables are only read here, the line buffers only written, so the loads of
+        // the next pair may be issued before the stores of this one)
+        const cplx* FSEI_RESTRICT land_r = land;
+        const cplx* FSEI_RESTRICT tr2c_r = tr2c;
+        const cplx* FSEI_RESTRICT tdct_r = tdct;
+        auto pair_load = [&](int l2, cplx* FSEI_RESTRICT lb, int p) {
+            auto g = [&](int q) -> cplx { return CB ? land_r[((q / (CB ? CB : 1)) * LPB + l2) * CB + q % (CB ? CB : 1)] : land_r[l2 * N + q]; };
             if (p == 0) {
                 cplx s = g(0);
                 double x0 = s.re, xn = s.im;
@@ -380,10 +385,10 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
                 lb[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
             } else {
                 cplx xk = g(p), xm = g(N - p);
-                if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
+                if (NEU) { xk = dct_tw_inv(xk, tdct_r[p]); xm = dct_tw_inv(xm, tdct_r[N - p]); }
                 cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
                 cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2
-                cplx O = cmulc(Tt, tr2c[p]);
+                cplx O = cmulc(Tt, tr2c_r[p]);
                 lb[C::pad(p)] = cmake(E.re - O.im, E.im + O.re);               // E + i O
                 if (p != N - p) lb[C::pad(N - p)] = cmake(E.re + O.im, -(E.im - O.re));   // conj(E - i O)
             }
@@ -392,10 +397,12 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
             if (act) for (int p = tl; p <= N / 2; p += T) pair_load(li, lbuf, p);
         } else {
             // landing tile is [tile][line][CB]: adjacent threads read adjacent elements of it
-            constexpr int CBq = CB ? CB : 1, HP = N / 2 / CBq + 1;
-            for (int wi = tid; wi < HP * LPB * CBq; wi += nt) {
+            constexpr int CBq = CB ? CB : 1, HP = N / 2 / CBq + 1, NW = HP * LPB * CBq, IT = (NW + T * LPB - 1) / (T * LPB);
+#pragma unroll
+            for (int it = 0; it < IT; it++) {
+                const int wi = tid + it * nt;
                 const int cc = wi % CBq, l2 = (wi / CBq) % LPB, p = (wi / (CBq * LPB)) * CBq + cc;
-                if (p > N / 2 || l2 >= nl) continue;
+                if (wi >= NW || p > N / 2 || l2 >= nl) continue;
                 pair_load(l2, buf + l2 * C::PITCH, p);
             }
         }
