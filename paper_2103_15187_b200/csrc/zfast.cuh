@@ -87,35 +87,56 @@ FSEI_HD void zf_factor_column(const ZFast& Z, double* ipiv, int row, int slot, i
     }
 }
 
-// one thread per column: forward elimination then back substitution, in place (two passes over the column)
+// one thread per column: forward elimination then back substitution, in place (two passes over the column).
+// Planes are taken in chunks of ZSW: all loads of a chunk are issued before its dependent chain and its stores (the
+// compiler cannot move the loads of plane k+1 over the store of plane k, and a chain of exposed L2 latencies is what
+// this kernel would otherwise be).
+#define FSEI_ZSW 8
 template <int NCOMP>
 FSEI_HD void zf_sweep_column(const ZFast& Z, cplx* S, int row, int slot)
 {
     const int nz = Z.nz;
     int mask; const int sp = z_special(Z, row, slot, mask);
     cplx prev = cmake(0.0, 0.0);
-    for (int k = 0; k < nz; k++) {
-        size_t i = zf_idx(Z, k, row, slot);
-        cplx d = S[i];
-        double ipr = Z.ipiv[i * NCOMP], ipi = Z.ipiv[i * NCOMP + (NCOMP - 1)];
-        double a = Z.za[k];
-        prev = cmake((d.re - a * prev.re) * ipr, (d.im - a * prev.im) * ipi);
-        S[i] = prev;
+    for (int k0 = 0; k0 < nz; k0 += FSEI_ZSW) {
+        cplx d[FSEI_ZSW]; double ip[FSEI_ZSW][2], a[FSEI_ZSW];
+#pragma unroll
+        for (int j = 0; j < FSEI_ZSW; j++) {
+            const int k = (k0 + j < nz) ? k0 + j : nz - 1;
+            const size_t i = zf_idx(Z, k, row, slot);
+            d[j] = S[i]; ip[j][0] = Z.ipiv[i * NCOMP]; ip[j][1] = Z.ipiv[i * NCOMP + (NCOMP - 1)]; a[j] = Z.za[k];
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZSW; j++) {
+            if (k0 + j < nz) { prev = cmake((d[j].re - a[j] * prev.re) * ip[j][0], (d[j].im - a[j] * prev.im) * ip[j][1]); d[j] = prev; }
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZSW; j++) if (k0 + j < nz) S[zf_idx(Z, k0 + j, row, slot)] = d[j];
     }
     cplx next = cmake(0.0, 0.0);
-    for (int k = nz - 1; k >= 0; k--) {
-        size_t i = zf_idx(Z, k, row, slot);
-        cplx dp = S[i];
-        double ipr = Z.ipiv[i * NCOMP], ipi = Z.ipiv[i * NCOMP + (NCOMP - 1)];
-        double c = Z.zcc[k];
-        next = cmake(dp.re - (c * ipr) * next.re, dp.im - (c * ipi) * next.im);
-        cplx o = next;
-        if (sp >= 0) {
-            cplx s = Z.special[(size_t)sp * nz + k];
-            if (mask & 1) o.re = s.re;
-            if (mask & 2) o.im = s.im;
+    for (int k1 = nz - 1; k1 >= 0; k1 -= FSEI_ZSW) {
+        cplx d[FSEI_ZSW], sv[FSEI_ZSW]; double ip[FSEI_ZSW][2], c[FSEI_ZSW];
+#pragma unroll
+        for (int j = 0; j < FSEI_ZSW; j++) {
+            const int k = (k1 - j >= 0) ? k1 - j : 0;
+            const size_t i = zf_idx(Z, k, row, slot);
+            d[j] = S[i]; ip[j][0] = Z.ipiv[i * NCOMP]; ip[j][1] = Z.ipiv[i * NCOMP + (NCOMP - 1)]; c[j] = Z.zcc[k];
+            sv[j] = (sp >= 0) ? Z.special[(size_t)sp * nz + k] : cmake(0.0, 0.0);
         }
-        S[i] = o;
+#pragma unroll
+        for (int j = 0; j < FSEI_ZSW; j++) {
+            if (k1 - j >= 0) {
+                next = cmake(d[j].re - (c[j] * ip[j][0]) * next.re, d[j].im - (c[j] * ip[j][1]) * next.im);
+                cplx o = next;
+                if (sp >= 0) {
+                    if (mask & 1) o.re = sv[j].re;
+                    if (mask & 2) o.im = sv[j].im;
+                }
+                d[j] = o;
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < FSEI_ZSW; j++) if (k1 - j >= 0) S[zf_idx(Z, k1 - j, row, slot)] = d[j];
     }
 }
 
