@@ -6,10 +6,11 @@
 // y-inverse transform, if those kernels march along z:
 //
 //   k_yz_forward : a CTA owns one x-slot tile (CB slots x all ny rows) and visits k = 0 .. nz-1.  Per plane: the
-//                  tile (contiguous in the blocked layout) and its reciprocal pivots arrive by cp.async.bulk
-//                  while the previous plane is transformed; register-resident Stockham FFT (or DCT-II) along y;
-//                  split of the two Hermitian y-spectra where a column carries two real x-sequences; then
-//                  d'_k = (d_k - a_k d'_{k-1}) / piv_k with d'_{k-1} carried in registers; d'_k is stored.
+//                  tile (contiguous in the blocked layout) arrives by cp.async.bulk while the previous plane is
+//                  transformed; register-resident Stockham FFT (or DCT-II) along y; then
+//                  d'_k = (d_k - a_k d'_{k-1}) / piv_k with d'_{k-1} carried in registers, either on the last pass'
+//                  outputs (single-spectrum tiles) or in one pass over the row pairs (kk, ny-kk) that also splits
+//                  the two Hermitian y-spectra of a column that carries two real x-sequences; d'_k is stored.
 //   k_yz_backward: same tiles, k = nz-1 .. 0: x_k = d'_k - (c_k / piv_k) x_{k+1} (x_{k+1} in registers), the
 //                  special columns are replaced by their separately solved values, merge + inverse transform,
 //                  store.
@@ -58,9 +59,7 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
     using L = YZSmem<C, CB, NEU, NCOMP>;
     constexpr int N = C::N, T = C::T, R0 = C::R0, NT = T * CB;
     constexpr int NB0 = N / R0, PER0 = PassShape<N, R0, 1, T>::PER;
-    constexpr int EPT = (N * CB) / NT;                           // elements per thread in the elimination
     static_assert(NB0 % T == 0, "first pass must tile the column exactly");
-    static_assert((N * CB) % NT == 0, "tile must split evenly over the threads");
     FSEI_DYN_SMEM(smraw);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
     cplx* land = reinterpret_cast<cplx*>(smraw + 128);           // [N][CB] dense
@@ -98,7 +97,8 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
 
     constexpr int RL = (C::NP == 3) ? C::R2 : C::R1, NSL = N / RL;   // last pass: output slot i RL + q = row tl + i T + q NSL
     constexpr int NSLOT = PassShape<N, RL, NSL, T>::PER * RL;
-    constexpr int NCARRY = NSLOT > EPT ? NSLOT : EPT;
+    constexpr int ITP = N / (2 * T) + 1;                             // two-spectra tiles: row pairs (kk, N-kk), kk = tl + i T
+    constexpr int NCARRY = (NSLOT > 2 * ITP) ? NSLOT : 2 * ITP;
     cplx carry[NCARRY];                                          // d'_{k-1} of this thread's elements
 #pragma unroll
     for (int m = 0; m < NCARRY; m++) carry[m] = cmake(0.0, 0.0);
@@ -148,69 +148,64 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_forward(YZFused P, cplx* spec)
             FSEI_SYNC();
             continue;
         }
+        // Tiles whose columns carry two spectra: transform into the staging buffer, then ONE pass per thread over its row
+        // pairs (kk, N-kk): split (+ quarter-wave twiddle), elimination with d'_{k-1} carried per pair slot, stores.
         fft_column<C, CB, false, false, true>(tl, c, true, buf, tws, load0, YOut<C, CB>{buf, c}, next);
-        // reciprocal pivots of this thread's elements (L2 hits), in flight across the barrier(s) below
-        double ipv[EPT][NCOMP];
+        double ipv[2 * ITP][NCOMP];                              // reciprocal pivots (L2 hits), in flight across the barrier
         {
             const double* ipk = ip0 + (size_t)k * L::IPT;
 #pragma unroll
-            for (int m = 0; m < EPT; m++) {
+            for (int i2 = 0; i2 < ITP; i2++) {
+                const int kk = tl + i2 * T;
+                if (kk <= N / 2) {
 #pragma unroll
-                for (int q = 0; q < NCOMP; q++) ipv[m][q] = ld_stream(ipk + (size_t)(tid + m * NT) * NCOMP + q);
+                    for (int q = 0; q < NCOMP; q++) {
+                        ipv[2 * i2][q] = ld_stream(ipk + (size_t)(kk * CB + c) * NCOMP + q);
+                        ipv[2 * i2 + 1][q] = ld_stream(ipk + (size_t)((kk ? N - kk : 0) * CB + c) * NCOMP + q);
+                    }
+                }
             }
         }
         FSEI_SYNC();
-        if (pairing) {
-            // split in place: rows kk and N-kk of a column are handled by one thread
-            for (int kk = tl; kk <= N / 2; kk += T) {
-                if (kk == 0 || (!NEU && (2 * kk == N || !mine))) continue;
-                const cplx p1 = buf[C::pad(kk) * CB + c], p2 = buf[C::pad(N - kk) * CB + c];
+        {
+            const double a = a_k;
+            a_k = more ? coef[k + kstep] : 0.0;             // next plane's coefficient: latency hidden by this plane
+            cplx* gk = tile0 + (size_t)k * L::TILE;
+            cplx r1[ITP], r2[ITP];                               // rows kk and N-kk after the split
+#pragma unroll
+            for (int i2 = 0; i2 < ITP; i2++) {
+                const int kk = tl + i2 * T;
+                if (kk > N / 2) continue;
+                const cplx p1 = buf[C::pad(kk) * CB + c], p2 = buf[C::pad(kk ? N - kk : 0) * CB + c];
+                if (kk == 0 || (!NEU && (2 * kk == N || !mine))) { r1[i2] = p1; r2[i2] = p2; continue; }
                 cplx A = cmake(0.5 * (p1.re + p2.re), 0.5 * (p1.im - p2.im));       // (P1 + conj P2)/2
                 cplx D = cmake(p1.re - p2.re, p1.im + p2.im);
                 cplx B = cmake(0.5 * D.im, -0.5 * D.re);                            // (P1 - conj P2)/(2i)
                 if (NEU) {
                     const cplx wk = tdct[kk];
                     const cplx ta = cmul(A, wk), tb = cmul(B, wk);
-                    buf[C::pad(kk) * CB + c] = cmake(ta.re, tb.re);
-                    if (2 * kk != N) buf[C::pad(N - kk) * CB + c] = cmake(-ta.im, -tb.im);
-                } else {
-                    buf[C::pad(kk) * CB + c] = A;
-                    buf[C::pad(N - kk) * CB + c] = B;
+                    r1[i2] = cmake(ta.re, tb.re); r2[i2] = cmake(-ta.im, -tb.im);
+                } else { r1[i2] = A; r2[i2] = B; }
+            }
+#pragma unroll
+            for (int i2 = 0; i2 < ITP; i2++) {
+                const int kk = tl + i2 * T;
+                if (kk > N / 2) continue;
+                const bool two = kk != 0 && 2 * kk != N;        // row N-kk is a different row
+                if (tile == 0 && c == 0) {                      // right-hand sides of the special columns
+                    if (kk == 0) P.special_in[k] = r1[i2];
+                    else if (P.pp && 2 * kk == N) P.special_in[nz + k] = r1[i2];
                 }
-            }
-            FSEI_SYNC();
-        }
-        // forward elimination of plane k; element e of the tile = (row e / CB, slot c0 + e % CB).
-        // Loads first, then arithmetic, then stores: the compiler cannot reorder shared-memory accesses itself.
-        {
-            const double a = a_k;
-            a_k = more ? coef[k + kstep] : 0.0;             // next plane's coefficient: latency hidden by this plane
-            cplx* gk = tile0 + (size_t)k * L::TILE;
-            cplx d[EPT];
-#pragma unroll
-            for (int m = 0; m < EPT; m++) {
-                const int e = tid + m * NT;
-                const int row = e / CB, cc = e - row * CB;
-                d[m] = buf[C::pad(row) * CB + cc];
-            }
-            if (tile == 0) {                                    // rows 0 and N/2 of slot 0 (elements 0 and N CB / 2)
-#pragma unroll
-                for (int m = 0; m < EPT; m++) {
-                    const int e = tid + m * NT;
-                    if (e == 0) P.special_in[k] = d[m];
-                    else if (P.pp && e == (N / 2) * CB) P.special_in[nz + k] = d[m];
+                cplx& c1 = carry[2 * i2];
+                c1 = cmake((r1[i2].re - a * c1.re) * ipv[2 * i2][0], (r1[i2].im - a * c1.im) * ipv[2 * i2][NCOMP - 1]);
+                gk[kk * CB + c] = c1;
+                if (gm) gm[kk * CB + c] = c1;
+                if (two) {
+                    cplx& c2 = carry[2 * i2 + 1];
+                    c2 = cmake((r2[i2].re - a * c2.re) * ipv[2 * i2 + 1][0], (r2[i2].im - a * c2.im) * ipv[2 * i2 + 1][NCOMP - 1]);
+                    gk[(N - kk) * CB + c] = c2;
+                    if (gm) gm[(N - kk) * CB + c] = c2;
                 }
-            }
-#pragma unroll
-            for (int m = 0; m < EPT; m++) {
-                const double ipr = ipv[m][0], ipi = ipv[m][NCOMP - 1];
-                carry[m] = cmake((d[m].re - a * carry[m].re) * ipr, (d[m].im - a * carry[m].im) * ipi);
-            }
-#pragma unroll
-            for (int m = 0; m < EPT; m++) gk[tid + m * NT] = carry[m];
-            if (gm) {
-#pragma unroll
-                for (int m = 0; m < EPT; m++) gm[tid + m * NT] = carry[m];
             }
         }
         FSEI_SYNC();
@@ -262,9 +257,11 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
     if (tid == 0 && kcount > 0) issue(kfirst, kcount > 1);
     unsigned parity = 0;
 
-    cplx carry[EPT];                                             // x of the plane just left, per element of this thread
+    constexpr int ITP = N / (2 * T) + 1;                             // two-spectra tiles: row pairs (kk, N-kk), kk = tl + i T
+    constexpr int NCARRY = (EPT > 2 * ITP) ? EPT : 2 * ITP;
+    cplx carry[NCARRY];                                          // x of the plane just left, per element of this thread
 #pragma unroll
-    for (int m = 0; m < EPT; m++) carry[m] = cmake(0.0, 0.0);
+    for (int m = 0; m < NCARRY; m++) carry[m] = cmake(0.0, 0.0);
     if (P.ktw < nz) {
         // Twisted factorisation: the two eliminations met between planes m-1 and m,
         //   x_{m-1} + cp x_m = d'_{m-1},   ap x_{m-1} + x_m = e'_m      (cp = c_{m-1} / piv_{m-1}, ap = a_m / piv_m)
@@ -277,8 +274,12 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
         const double* ipm1 = ip0 + (size_t)(m - 1) * L::IPT;
         const double* iqm = ip0 + (size_t)m * L::IPT;
 #pragma unroll
-        for (int s = 0; s < EPT; s++) {
-            const int e = pairing ? tid + s * NT : (tl + (s / R0) * T + (s % R0) * (N / R0)) * CB + c;
+        for (int s = 0; s < NCARRY; s++) {
+            // element of carry slot s: pair slots (row kk or N-kk) on two-spectra tiles, first-pass input slots otherwise
+            const int kk = tl + (s >> 1) * T;
+            const bool ok = pairing ? (kk <= N / 2 && (!(s & 1) || (kk != 0 && 2 * kk != N))) : (s < EPT);
+            if (!ok) continue;
+            const int e = pairing ? ((s & 1) ? N - kk : kk) * CB + c : (tl + (s / R0) * T + (s % R0) * (N / R0)) * CB + c;
             const cplx d1 = dm1[e], e0 = em[e];
             double x[2];
 #pragma unroll
@@ -325,41 +326,45 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
             FSEI_SYNC();
             continue;
         }
+        // Tiles whose columns carry two spectra: ONE pass per thread over its row pairs (kk, N-kk): substitution with
+        // x_{k+1} carried per pair slot, special columns, merge (+ quarter-wave twiddle) into the staging buffer.
         {
             const double cz = c_k;
             c_k = more ? coef[k + kstep] : 0.0;
-            cplx dp[EPT];
-            double ipv[EPT][NCOMP];
+            cplx dp1[ITP], dp2[ITP];
+            double ip1[ITP][NCOMP], ip2[ITP][NCOMP];
 #pragma unroll
-            for (int m = 0; m < EPT; m++) {
-                const int e = tid + m * NT;
-                dp[m] = land[e];
+            for (int i2 = 0; i2 < ITP; i2++) {
+                const int kk = tl + i2 * T;
+                if (kk > N / 2) continue;
+                const int e1 = kk * CB + c, e2 = (kk ? N - kk : 0) * CB + c;
+                dp1[i2] = land[e1]; dp2[i2] = land[e2];
 #pragma unroll
-                for (int q = 0; q < NCOMP; q++) ipv[m][q] = ipb[e * NCOMP + q];
+                for (int q = 0; q < NCOMP; q++) { ip1[i2][q] = ipb[e1 * NCOMP + q]; ip2[i2][q] = ipb[e2 * NCOMP + q]; }
             }
 #pragma unroll
-            for (int m = 0; m < EPT; m++)
-                carry[m] = cmake(dp[m].re - (cz * ipv[m][0]) * carry[m].re, dp[m].im - (cz * ipv[m][NCOMP - 1]) * carry[m].im);
-#pragma unroll
-            for (int m = 0; m < EPT; m++) {
-                const int e = tid + m * NT;
-                const int row = e / CB, cc = e - row * CB;
-                cplx x = carry[m];
-                if (tile == 0 && cc == 0) {
-                    if (row == 0) { const cplx sv = P.special[k]; x.re = sv.re; if (P.pp) x.im = sv.im; }
-                    else if (P.pp && 2 * row == N) x = P.special[nz + k];
+            for (int i2 = 0; i2 < ITP; i2++) {
+                const int kk = tl + i2 * T;
+                if (kk > N / 2) continue;
+                const bool two = kk != 0 && 2 * kk != N;
+                cplx& c1 = carry[2 * i2];
+                c1 = cmake(dp1[i2].re - (cz * ip1[i2][0]) * c1.re, dp1[i2].im - (cz * ip1[i2][NCOMP - 1]) * c1.im);
+                cplx a = c1, b = cmake(0.0, 0.0);
+                if (two) {
+                    cplx& c2 = carry[2 * i2 + 1];
+                    c2 = cmake(dp2[i2].re - (cz * ip2[i2][0]) * c2.re, dp2[i2].im - (cz * ip2[i2][NCOMP - 1]) * c2.im);
+                    b = c2;
                 }
-                buf[C::pad(row) * CB + cc] = x;
-            }
-        }
-        FSEI_SYNC();
-        if (tid == 0 && more) issue(k + kstep, it + 2 < kcount); // landing tiles consumed: prefetch the next plane
-        if (pairing) {
-            for (int kk = tl; kk <= N / 2; kk += T) {
-                if (kk == 0 || (!NEU && (2 * kk == N || !mine))) continue;
-                cplx a = buf[C::pad(kk) * CB + c];
+                if (tile == 0 && c == 0) {                      // separately solved columns
+                    if (kk == 0) { const cplx sv = P.special[k]; a.re = sv.re; if (P.pp) a.im = sv.im; }
+                    else if (P.pp && 2 * kk == N) a = P.special[nz + k];
+                }
+                if (kk == 0 || (!NEU && (2 * kk == N || !mine))) {
+                    buf[C::pad(kk) * CB + c] = a;
+                    if (two) buf[C::pad(N - kk) * CB + c] = b;
+                    continue;
+                }
                 if (NEU && 2 * kk == N) { buf[C::pad(kk) * CB + c] = cmake(a.re * SQ2, a.im * SQ2); continue; }
-                cplx b = buf[C::pad(N - kk) * CB + c];
                 if (NEU) {
                     const cplx wk = tdct[kk];
                     const cplx ta = cmulc(cmake(a.re, -b.re), wk);     // V^a_k
@@ -369,8 +374,9 @@ FSEI_GLOBAL(C::T * CB, 1) k_yz_backward(YZFused P, cplx* spec)
                 buf[C::pad(kk) * CB + c] = cmake(a.re - b.im, a.im + b.re);          // A + i B
                 buf[C::pad(N - kk) * CB + c] = cmake(a.re + b.im, -a.im + b.re);     // conj A + i conj B
             }
-            FSEI_SYNC();
         }
+        FSEI_SYNC();
+        if (tid == 0 && more) issue(k + kstep, it + 2 < kcount); // landing tiles consumed: prefetch the next plane
         cplx* gk = tile0 + (size_t)k * L::TILE;
         auto out = [&](int n, cplx z, int) { gk[(NEU ? dct_perm(n, N) : n) * CB + c] = z; };
         auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, YIn<C, CB>{buf, c}, v0); };
