@@ -47,6 +47,7 @@ struct fsei_plan {
     XParams X; YParams Y; ZParams Z; SParams S;
     bool fast = false;                 // register-resident Stockham path (xfast / yfast / zfast), natural-order spectrum
     XFast XF; YFast YF; ZFast ZF;
+    int kchunk_inv = 16;               // planes per CTA of the x-inverse kernel (XF.kchunk: of the x-forward kernel)
     bool fused = false;                // fast path on the blocked spectrum layout with the z sweeps fused into the y kernels
     YZFused YZ; TmaMap3D xi_map; cplx* work = nullptr;   // work: plan-owned spectrum field (blocked layout)
     std::vector<void*> owned;          // device allocations freed with the plan
@@ -274,7 +275,10 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             const int lpb = xfast_lines_per_block(nx / 2, bcx == BC_NEUMANN);
             const long jblocks = (ny + lpb - 1) / lpb;
             long kc = (jblocks * nz) / (4L * nsm);
-            XF.kchunk = (int)(kc < 1 ? 1 : (kc > 16 ? 16 : kc));
+            // measured at configs[3]: the fused forward kernel likes long marches (w reuse, fewer table fills), the inverse
+            // kernel shorter ones
+            XF.kchunk = (int)(kc < 1 ? 1 : (kc > 64 ? 64 : kc));
+            P->kchunk_inv = (int)(kc < 1 ? 1 : (kc > 32 ? 32 : kc));
         }
         YF.nxc = T.nxc; YF.ny = ny; YF.nz = nz; YF.tw = Y.tw; YF.tw_dct = Y.tw_dct;
         YF.untangle = (bcy == BC_PERIODIC) ? (bcx == BC_PERIODIC ? 1 : T.nxc) : 0;
@@ -446,7 +450,7 @@ static int fast_spectral_solve(fsei_plan* P, cplx* spec, cudaStream_t st)
     }
     CU(cudaGetLastError());
     { LaunchTimer t(P, K_YI, st); CU(launch_y_fast(P->YF, true, ny_neu, spec, st)); }
-    { LaunchTimer t(P, K_XI, st); CU(launch_xi_fast(P->XF, T.bcx == BC_NEUMANN, spec, reinterpret_cast<double*>(spec), st)); }
+    { LaunchTimer t(P, K_XI, st); XFast xi = P->XF; xi.kchunk = P->kchunk_inv; CU(launch_xi_fast(xi, T.bcx == BC_NEUMANN, spec, reinterpret_cast<double*>(spec), st)); }
     return FSEI_OK;
 }
 
@@ -459,7 +463,7 @@ static int fused_spectral_solve(fsei_plan* P, double* phi, cudaStream_t st)
     { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, P->work); }
     CU(cudaGetLastError());
     { LaunchTimer t(P, K_YZB, st); CU(launch_yz_backward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
-    { LaunchTimer t(P, K_XI, st); CU(launch_xi_fast(P->XF, T.bcx == BC_NEUMANN, P->work, phi, st, &P->xi_map)); }
+    { LaunchTimer t(P, K_XI, st); XFast xi = P->XF; xi.kchunk = P->kchunk_inv; CU(launch_xi_fast(xi, T.bcx == BC_NEUMANN, P->work, phi, st, &P->xi_map)); }
     return FSEI_OK;
 }
 
