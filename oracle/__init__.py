@@ -19,6 +19,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fsei_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "fsei_fluid_oracle.c")]   # projection; viscous step + explicit terms
 BC_PERIODIC, BC_NEUMANN = 0, 1
 
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -32,10 +33,10 @@ def build(force: bool = False) -> None:
     """gcc -O2 -ffp-contract=off -fopenmp, once per flavour (rebuilt when the source is newer)."""
     for kind, defs in (("ld", ["-DORACLE_LONG_DOUBLE"]), ("d", [])):
         out = lib_path(kind)
-        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= max(os.path.getmtime(f) for f in _SRCS):
             continue
         cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-               "-Wall", "-Wextra", *defs, _SRC, "-o", out, "-lm"]
+               "-Wall", "-Wextra", *defs, *_SRCS, "-o", out, "-lm"]
         subprocess.run(cmd, check=True)
 
 
@@ -66,6 +67,13 @@ class Oracle:
         L.oracle_zcoef.argtypes = [i, _dp, _dp, _dp, _dp, _dp]
         L.oracle_gauge_column.argtypes = [i, _dp, _dp, _dp]
         L.oracle_modified_wavenumbers.argtypes = [i, d, i, _dp]
+        # fsei_fluid_oracle.c: implicit viscous step (NEXT-1) and explicit terms (NEXT-2)
+        L.oracle_viscous_step.argtypes = grid + [_dp] * 6 + [d]
+        L.oracle_viscous_sweep.argtypes = grid + [i, i, d, _dp]
+        L.oracle_cyclic_thomas.argtypes = [i, _dp, _dp, _dp, _dp, _dp]
+        L.oracle_convective.argtypes = grid + [_dp] * 3 + [ctypes.c_void_p] * 3 + [_dp] * 3
+        L.oracle_velocity_laplacian.argtypes = grid + [i, _dp, _dp]
+        L.oracle_explicit_terms.argtypes = grid + [_dp] * 4 + [ctypes.c_void_p] * 3 + [_dp] * 6 + [d, d, d, d]
 
     # -- grid tuple helper: g = (nx, ny, nz, Lx, Ly, zc, bc_x, bc_y) ------------------------
     @staticmethod
@@ -111,6 +119,54 @@ class Oracle:
         self._chk(self.lib.oracle_pressure_projection(*a, _ptr(u), _ptr(v), _ptr(w), _ptr(p), _ptr(phi),
                                                       float(alpha_dt), float(beta)), "pressure_projection")
         return phi
+
+    # -- fluid substep: explicit terms, implicit viscous step ----------------------------------
+    def viscous_step(self, g, u, v, w, ru, rv, rw, beta):
+        """In place on u, v, w: q += [(1-b dxx)(1-b dyy)(1-b dzz)]^-1 rhs_q."""
+        a, keep = self._g(g)
+        self._chk(self.lib.oracle_viscous_step(*a, _ptr(u), _ptr(v), _ptr(w), _ptr(ru), _ptr(rv), _ptr(rw),
+                                               float(beta)), "viscous_step")
+
+    def viscous_sweep(self, g, comp, direction, beta, f):
+        """Returns [(1 - beta d2_dir)]^-1 f for component comp (0,1,2 = u,v,w), direction 0,1,2 = x,y,z."""
+        a, keep = self._g(g)
+        out = np.ascontiguousarray(f, dtype=np.float64).copy()
+        self._chk(self.lib.oracle_viscous_sweep(*a, int(comp), int(direction), float(beta), _ptr(out)), "viscous_sweep")
+        return out
+
+    def cyclic_thomas(self, a, b, c, d):
+        a, b, c, d = (np.ascontiguousarray(t, dtype=np.float64) for t in (a, b, c, d))
+        x = np.empty_like(d)
+        self.lib.oracle_cyclic_thomas(d.shape[0], _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x))
+        return x
+
+    @staticmethod
+    def _opt(a):
+        return None if a is None else a.ctypes.data
+
+    def convective(self, g, u, v, w, f=(None, None, None)):
+        """H = -div(uu) (+ f): returns hu, hv, hw."""
+        a, keep = self._g(g)
+        h = [np.empty_like(u) for _ in range(3)]
+        self._chk(self.lib.oracle_convective(*a, _ptr(u), _ptr(v), _ptr(w), *[self._opt(x) for x in f],
+                                             *[_ptr(x) for x in h]), "convective")
+        return h
+
+    def velocity_laplacian(self, g, comp, q):
+        a, keep = self._g(g)
+        out = np.empty_like(q)
+        self._chk(self.lib.oracle_velocity_laplacian(*a, int(comp), _ptr(q), _ptr(out)), "velocity_laplacian")
+        return out
+
+    def explicit_terms(self, g, u, v, w, p, hu, hv, hw, gamma_dt, rho_dt, alpha_dt, beta, f=(None, None, None)):
+        """hu, hv, hw: H^{n-1} in, H^n out (in place).  Returns ru, rv, rw."""
+        a, keep = self._g(g)
+        r = [np.empty_like(u) for _ in range(3)]
+        self._chk(self.lib.oracle_explicit_terms(*a, _ptr(u), _ptr(v), _ptr(w), _ptr(p), *[self._opt(x) for x in f],
+                                                 _ptr(hu), _ptr(hv), _ptr(hw), *[_ptr(x) for x in r],
+                                                 float(gamma_dt), float(rho_dt), float(alpha_dt), float(beta)),
+                  "explicit_terms")
+        return r
 
     # -- building blocks ---------------------------------------------------------------------
     def dft(self, x: np.ndarray, sign: int) -> np.ndarray:
