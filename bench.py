@@ -10,8 +10,8 @@ configs[3] (1024x1024x768, the size the north-star target is quoted on; it fits 
 The path is single-GPU ("replicas only"): for N > 1 every rank runs an
 independent replica and `value` is the sum over ranks / max-over-ranks time.
 
-`--impl reference` times the CPU oracle (as it stands, `double` build) on a bounded sample of
-the same workload; rank 0 only.
+`--impl reference` times the CPU oracle (as it stands, `double` build) on the same full-size
+workload (at most 3 timed projections of ~12 s each); rank 0 only.
 
 Prints ONE JSON line.
 """
@@ -31,15 +31,21 @@ if ROOT not in sys.path:
 
 METRIC = "Mcell/s per fp64 pressure projection"
 UNIT = "Mcell/s"
-# algorithmic bytes per cell per launch of each kernel
+# algorithmic bytes per cell per launch of each kernel = the bytes that launch has to MOVE:
+# fields read + fields written + the reciprocal-pivot table where a kernel streams it.  `achieved` figures are
+# computed from these, so they can never exceed the copy bandwidth; the unfused 7-kernel yardstick of SURVEY.md
+# sec. 8(d) (184 B/cell) is reported separately as `unfused_equivalent_GBps`.
 ALGO_BYTES_PER_CELL = {
-    "divergence": 32.0, "x_forward": 16.0, "div_x_forward": 32.0, "y_forward": 16.0, "z_direct": 16.0,
-    "z_paired": 16.0, "z_solve": 16.0, "y_inverse": 16.0, "x_inverse": 16.0, "project": 72.0, "z_gauge": 0.0,
-    # fused path: a3 + first Thomas sweep, second sweep + a5 (y 16 + half of the z step's 16 each)
-    "yz_forward": 24.0, "yz_backward": 24.0,
+    "divergence": 32.0, "x_forward": 16.0, "div_x_forward": 32.0, "y_forward": 16.0, "z_direct": 36.0,
+    "z_paired": 32.0, "y_inverse": 16.0, "x_inverse": 16.0, "project": 72.0, "z_gauge": 0.0,
+    # fused path: spectrum in + out (16) + one reciprocal pivot per complex element (4; 8 on Neumann grids)
+    "yz_forward": 20.0, "yz_backward": 20.0,
+    # fluid substep: u,v,w,p + 3 Hprev in, 3 H + 3 rhs out; generic sweeps in place,
+    # forward + backward pass each (the z sweep also reads and writes the velocity component)
+    "explicit_terms": 104.0, "visc_x": 32.0, "visc_y": 32.0, "visc_z": 40.0, "visc_factor": 0.0,
 }
-A_REF = 184.0          # reference accounting of one projection, B/cell
-SAMPLE_NY = 256        # CPU legs: the workload's grid with ny cut to this many rows
+A_REF = 184.0          # unfused reference accounting of one projection, B/cell
+SLAB_NY = 64           # single-thread CPU leg: the workload's grid with ny cut to this many rows
 
 
 def _peaks():
@@ -145,18 +151,30 @@ def _workload_name(case) -> str:
 # ------------------------------------------------------------------------------------------------
 # CPU legs: the oracle (double build, as it stands) on a bounded sample of the workload
 # ------------------------------------------------------------------------------------------------
-def _oracle_sample(cfg: int, reps: int, warm: int = 0):
-    """Times `reps` oracle projections on the config's grid with ny cut to SAMPLE_NY rows (same nx, nz, zc,
-    bc, value distribution).  Returns (Mcell/s, cores, sample description, seconds per projection)."""
+def _cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def _oracle_time(cfg: int, shape, reps: int, warm: int = 0, fields=None):
+    """Times `reps` oracle projections (double build, as it stands) on the config's recipe at `shape`.
+    Returns (Mcell/s, seconds per projection)."""
     import numpy as np
     from paper_2103_15187_b200 import inputs
     from oracle import Oracle
-    nx, ny, nz = inputs.CONFIGS[cfg]["shape"]
-    shape = (nx, min(ny, SAMPLE_NY), nz)
-    case = inputs.make_case(cfg, shape=shape)
+    if fields is None:
+        case = inputs.make_case(cfg, shape=shape)
+        u, v, w = case.u, case.v, case.w
+    else:
+        case = inputs.make_case(cfg, shape=shape, fields=False)
+        u, v, w = fields
     orc = Oracle("d")
-    cores = int(os.environ.get("OMP_NUM_THREADS", 0)) or len(os.sched_getaffinity(0))
-    u, v, w = case.u.copy(), case.v.copy(), case.w.copy()
     p = np.zeros_like(u)
     for _ in range(warm):
         orc.pressure_projection(case.grid, u, v, w, p, case.alpha_dt, 0.0)
@@ -164,21 +182,58 @@ def _oracle_sample(cfg: int, reps: int, warm: int = 0):
     for _ in range(reps):
         orc.pressure_projection(case.grid, u, v, w, p, case.alpha_dt, 0.0)
     dt = (time.perf_counter() - t0) / reps
-    sample = (f"{reps} oracle projection(s) of a {shape[0]}x{shape[1]}x{shape[2]} slab of the workload grid "
-              f"(ny cut to {shape[1]}; same nx, nz, z-grid, bc, N(0,1)/smooth recipe), OpenMP over lines/columns")
-    return case.cells / dt / 1e6, cores, sample, dt
+    return case.cells / dt / 1e6, dt
+
+
+def _oracle_single_thread(cfg: int):
+    """One oracle projection with OMP_NUM_THREADS=1 on a slab of the workload (ny cut to SLAB_NY), in a child
+    process (the OpenMP runtime reads the variable once).  Returns (Mcell/s, sample description) or (None, why)."""
+    from paper_2103_15187_b200 import inputs
+    nx, ny, nz = inputs.CONFIGS[cfg]["shape"]
+    shape = (nx, min(ny, SLAB_NY), nz)
+    code = ("import sys, json; sys.path.insert(0, %r); import bench; "
+            "print(json.dumps(bench._oracle_time(%d, %r, 1)))" % (ROOT, cfg, shape))
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        val, dt = json.loads(out.stdout.strip().splitlines()[-1])
+    except Exception as e:  # noqa: BLE001 -- reported, not fatal
+        return None, f"single-thread leg failed: {e}"
+    return val, (f"1 oracle projection of a {shape[0]}x{shape[1]}x{shape[2]} slab of the workload grid (ny cut to {shape[1]}; "
+                 f"the full grid would take ~{dt * ny / shape[1]:.0f} s on one thread), OMP_NUM_THREADS=1")
+
+
+def _cpu_baseline(cfg: int, reps: int, warm: int = 0, fields=None, single: bool = True) -> dict:
+    """The oracle on the box's host cores at the FULL benchmark configuration (all cores), plus a single-thread
+    figure on a stated slab."""
+    from paper_2103_15187_b200 import inputs
+    shape = inputs.CONFIGS[cfg]["shape"]
+    cores = int(os.environ.get("OMP_NUM_THREADS", 0)) or len(os.sched_getaffinity(0))
+    need = 8 * shape[0] * shape[1] * shape[2] * (7 if fields is not None else 10) / 1e9
+    if _mem_available_gb() < need + 4:
+        return {"value": None, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": _cpu_model(),
+                "sample": f"skipped: the full-size oracle needs ~{need:.0f} GB of host memory, {_mem_available_gb():.0f} GB available"}
+    val, dt = _oracle_time(cfg, shape, reps, warm, fields)
+    out = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": _cpu_model(), "s_per_projection": dt,
+           "sample": (f"{reps} oracle projection(s) of the FULL {shape[0]}x{shape[1]}x{shape[2]} workload (double build, "
+                      f"OpenMP over lines/columns, {cores} threads)")}
+    if single:
+        v1, s1 = _oracle_single_thread(cfg)
+        out["threads1"] = {"value": v1, "unit": UNIT, "sample": s1}
+    return out
 
 
 def run_reference(args) -> dict:
     from paper_2103_15187_b200 import inputs
     case = inputs.make_case(args.config, fields=False)
-    val, cores, sample, dt = _oracle_sample(args.config, args.steps, args.warmup)
+    cpu = _cpu_baseline(args.config, args.steps, args.warmup, single=False)
+    val = cpu["value"]
     return {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": _workload_name(case), "sample": sample},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "warmup": args.warmup, "ms_per_step": cpu.get("s_per_projection", 0.0) * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": _workload_name(case), "cells": case.cells},
+        "cpu_baseline": cpu,
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -263,6 +318,9 @@ def run_ours(args) -> dict:
         kernels[name] = {"ms_per_launch": round(per, 4), "launches_per_step": cnt / args.steps,
                          "algo_GBps": round(ab / (per * 1e-3) / 1e9, 1) if per > 0 else None,
                          "share": round(ms / ms_total, 4)}
+    # whole step on the bytes the launches actually move (sum over the kernels of one step)
+    moved = sum(ALGO_BYTES_PER_CELL.get(name, 0.0) * cnt / args.steps for name, (ms, cnt) in prof.items())
+    moved_gbps = moved * case.cells / (ms_step * 1e-3) / 1e9
     top = max(prof, key=lambda k: prof[k][0])
     top_ms = prof[top][0] / prof[top][1]
     achieved = ALGO_BYTES_PER_CELL.get(top, 0.0) * case.cells / (top_ms * 1e-3) / 1e9
@@ -271,8 +329,10 @@ def run_ours(args) -> dict:
                 "frac": round(achieved / peak, 4), "traffic": traffic, "peak_source": peak_src,
                 "algo_bytes_per_launch": ALGO_BYTES_PER_CELL.get(top, 0.0) * case.cells,
                 "ms_per_launch": round(top_ms, 4),
-                "whole_step": {"algo_bytes_per_cell": A_REF, "achieved": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9, 1),
-                               "frac": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9 / peak, 4)},
+                "whole_step": {"moved_bytes_per_cell": round(moved, 2), "achieved": round(moved_gbps, 1),
+                               "frac": round(moved_gbps / peak, 4), "frac_of_8TBps": round(moved_gbps / 8000.0, 4),
+                               "unfused_bytes_per_cell": A_REF,
+                               "unfused_equivalent_GBps": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9, 1)},
                 "kernels": kernels}
 
     # ---- end to end: HOST buffers through the C ABI, H2D + D2H inside the timed region -------------------
@@ -303,8 +363,7 @@ def run_ours(args) -> dict:
     # ---- CPU baseline: the oracle as it stands, rank 0 at N = 1 only --------------------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        val, cores, sample, _ = _oracle_sample(args.config, 5)
-        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        cpu = _cpu_baseline(args.config, 1, 0, fields=[h.numpy() for h in host])
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -316,7 +375,7 @@ def run_ours(args) -> dict:
                          else "fields fit in L2 (small config; no flush)",
                    "parallelism": "replicas only" if world > 1 else "single GPU", "input_gen_s": round(t_gen, 1)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-        "hbm_GBps_vs_8TBps": round(A_REF * case.cells / (ms_step * 1e-3) / 1e9 / 8000.0, 4),
+        "hbm_GBps_vs_8TBps": round(moved_gbps / 8000.0, 4),
     }
     if world > 1:
         dist.destroy_process_group()
@@ -336,7 +395,7 @@ def main():
     if args.impl == "reference":
         if int(os.environ.get("RANK", 0)) != 0:
             return
-        args.steps = min(args.steps, 5)
+        args.steps = min(args.steps, 3)          # ~12 s per full-size projection on the box's cores
         args.warmup = min(args.warmup, 1)
         out = run_reference(args)
     else:

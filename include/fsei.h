@@ -115,6 +115,50 @@ int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double*
                                   double alpha_dt, double beta, void* cuda_stream);
 
 /*
+ * ---- The two steps that precede the projection in one fluid substep ----------
+ * Eq. 3:  (u^{n+1}-u^n)/dt + [gamma div(uu)^n + rho div(uu)^{n-1}] = -grad p + (1/(2Re)) lap(u^{n+1}+u^n) + f,
+ * "explicit Adams-Bashforth ... for the nonlinear convective term and an implicit Crank-Nicolson method for the
+ * viscous terms", gamma = 3/2, rho = -1/2, or the weights of a three-stage Runge-Kutta scheme; the
+ * substep l has alpha_l = gamma_l + rho_l and beta = alpha_l dt/(2 Re).  Discrete operators: DESIGN.md V1..V12.
+ *
+ * fsei_explicit_terms (NEXT-2): second-order central, divergence-form convective term on the staggered mesh
+ *   H_q   = -div(u q) (+ f_q)                at the position of each component q = u, v, w
+ *   rhs_q = ((gamma_dt*H_q + rho_dt*Hprev_q) - alpha_dt*(G p)_q) + (2 beta)*(lap q)
+ *   Hprev_q <- H_q
+ * evaluated in IEEE double in that fixed order, no FMA: bit-identical to the definition.
+ *   u, v, w, p     : in (read only).  fu, fv, fw: body force (e.g. the IB forcing), each may be NULL.
+ *   hu, hv, hw     : in: H of the previous substep (zeros on the first); out: H of this substep.
+ *   ru, rv, rw     : out.  No output may alias an input or another output           else FSEI_ERR_ARG
+ *   Wall-face rows (w at k = 0; u at i = 0 / v at j = 0 on a wall-bounded box) get H = rhs = 0.
+ */
+int fsei_explicit_terms(fsei_plan* plan, const double* u, const double* v, const double* w, const double* p,
+                        const double* fu, const double* fv, const double* fw, double* hu, double* hv, double* hw,
+                        double* ru, double* rv, double* rw, double gamma_dt, double rho_dt, double alpha_dt,
+                        double beta, void* cuda_stream);
+
+/*
+ * fsei_viscous_step (NEXT-1; sec. 3.1, Eq. 3): the implicit viscous step by approximate factorisation,
+ *   q += [(1 - beta dxx)(1 - beta dyy)(1 - beta dzz)]^-1 rhs_q          for q = u, v, w, in place,
+ * one tridiagonal system per grid line and direction (Thomas), cyclic in a periodic direction (the paper: Sherman-
+ * Morrison; here the equivalent bordered elimination).  dxx, dyy, dzz are the second differences at
+ * the staggered position of each component with no-slip walls (V3-V6); wall faces are never modified.
+ *   ru, rv, rw : in: right-hand sides; DESTROYED (used as scratch).  beta >= 0 finite    else FSEI_ERR_ARG
+ *   No field may alias another.  Any nx, ny, nz the plan accepts; both boundary types.
+ * The factorisation tables for `beta` are rebuilt on the device (one extra small launch) whenever beta differs from
+ * the previous call on this plan.
+ */
+int fsei_viscous_step(fsei_plan* plan, double* u, double* v, double* w, double* ru, double* rv, double* rw,
+                      double beta, void* cuda_stream);
+
+/*
+ * One whole fluid substep on a box without immersed bodies: fsei_explicit_terms -> fsei_viscous_step ->
+ * fsei_pressure_projection (with the same alpha_dt, beta), enqueued back to back.  ru, rv, rw, phi are scratch fields.
+ */
+int fsei_fluid_substep(fsei_plan* plan, double* u, double* v, double* w, double* p, const double* fu, const double* fv,
+                       const double* fw, double* hu, double* hv, double* hw, double* ru, double* rv, double* rw,
+                       double* phi, double gamma_dt, double rho_dt, double alpha_dt, double beta, void* cuda_stream);
+
+/*
  * Kernel-level timing aid for bench.py: number of kernels enqueued by the last
  * fsei_pressure_projection / fsei_poisson_solve call on this plan.
  */

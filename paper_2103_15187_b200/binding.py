@@ -17,7 +17,8 @@ OK, ERR_ARG, ERR_SIZE, ERR_GRID, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4, 5
 EXPORTS = ("fsei_plan_create", "fsei_plan_destroy", "fsei_last_error", "fsei_last_error_code",
            "fsei_plan_workspace_bytes", "fsei_divergence", "fsei_poisson_solve", "fsei_project",
            "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
-           "fsei_plan_profile", "fsei_plan_profile_read")
+           "fsei_plan_profile", "fsei_plan_profile_read",
+           "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep")
 
 _lib = None
 _vp, _d, _i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
@@ -68,6 +69,12 @@ def lib() -> ctypes.CDLL:
     L.fsei_plan_profile.argtypes = [_vp, _i]
     L.fsei_plan_profile_read.restype = _i
     L.fsei_plan_profile_read.argtypes = [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_long), ctypes.POINTER(ctypes.c_char_p)]
+    L.fsei_explicit_terms.restype = _i
+    L.fsei_explicit_terms.argtypes = [_vp] * 14 + [_d] * 4 + [_vp]
+    L.fsei_viscous_step.restype = _i
+    L.fsei_viscous_step.argtypes = [_vp] * 7 + [_d, _vp]
+    L.fsei_fluid_substep.restype = _i
+    L.fsei_fluid_substep.argtypes = [_vp] * 15 + [_d] * 4 + [_vp]
     _lib = L
     return L
 
@@ -81,6 +88,10 @@ def _ptr(t) -> int:
         return t.data_ptr()
     assert t.flags["C_CONTIGUOUS"] and t.itemsize == 8
     return t.ctypes.data
+
+
+def _optr(t):
+    return None if t is None else _ptr(t)
 
 
 def _stream(stream) -> int:
@@ -164,3 +175,19 @@ class Plan:
         """u, v, w, p: HOST float64 arrays/tensors (pinned for speed), updated in place; synchronous."""
         _chk(lib().fsei_pressure_projection_host(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), float(alpha_dt),
                                                  float(beta), _stream(stream)))
+
+    def explicit_terms(self, u, v, w, p, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, beta, f=(None, None, None),
+                       stream=None):
+        _chk(lib().fsei_explicit_terms(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), *[_optr(t) for t in f], _ptr(hu), _ptr(hv),
+                                       _ptr(hw), _ptr(ru), _ptr(rv), _ptr(rw), float(gamma_dt), float(rho_dt), float(alpha_dt),
+                                       float(beta), _stream(stream)))
+
+    def viscous_step(self, u, v, w, ru, rv, rw, beta, stream=None):
+        _chk(lib().fsei_viscous_step(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(ru), _ptr(rv), _ptr(rw), float(beta),
+                                     _stream(stream)))
+
+    def fluid_substep(self, u, v, w, p, hu, hv, hw, ru, rv, rw, phi, gamma_dt, rho_dt, alpha_dt, beta, f=(None, None, None),
+                      stream=None):
+        _chk(lib().fsei_fluid_substep(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), *[_optr(t) for t in f], _ptr(hu), _ptr(hv),
+                                      _ptr(hw), _ptr(ru), _ptr(rv), _ptr(rw), _ptr(phi), float(gamma_dt), float(rho_dt),
+                                      float(alpha_dt), float(beta), _stream(stream)))

@@ -21,6 +21,8 @@
 #include "fast_configs.hpp"
 #include "zfast.cuh"
 #include "stencil_fast.cuh"
+#include "fluid.cuh"
+#include <cmath>
 #include <cstdlib>
 
 using namespace fsei;
@@ -40,7 +42,7 @@ static int cuda_fail(cudaError_t e, const char* what)
 // ------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------
-enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, FSEI_NKERNELS };
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, FSEI_NKERNELS };
 
 struct fsei_plan {
     HostTables T;
@@ -55,6 +57,7 @@ struct fsei_plan {
     int LX = 1, CY = 1;                // tile shapes
     size_t smem_x = 0, smem_y = 0;
     int last_launches = 0;
+    double* vtab = nullptr; int vnmax = 0; double visc_beta = NAN;   // implicit viscous step: factorisation tables of the last beta
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
     // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
     bool profiling = false;
@@ -66,7 +69,8 @@ struct fsei_plan {
 };
 
 static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
-                                                   "y_inverse", "x_inverse", "project", "div_x_forward", "yz_forward", "yz_backward"};
+                                                   "y_inverse", "x_inverse", "project", "div_x_forward", "yz_forward", "yz_backward",
+                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z"};
 
 // record an event pair around one launch when profiling is on
 struct LaunchTimer {
@@ -263,6 +267,12 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     S.nx = nx; S.ny = ny; S.nz = nz; S.bcx = bcx; S.bcy = bcy; S.rdx = T.rdx; S.rdy = T.rdy;
     if ((rc = upload(P, T.rdzc, &S.rdzc))) return rc;
     if ((rc = upload(P, T.rdzm, &S.rdzm))) return rc;
+    {
+        P->vnmax = nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz);
+        void* q = nullptr;
+        if ((rc = dalloc(P, sizeof(double) * 9 * vtab_set_doubles(P->vnmax), &q))) return rc;
+        P->vtab = static_cast<double*>(q);
+    }
 
     if (fast) {
         XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
@@ -594,6 +604,111 @@ extern "C" int fsei_pressure_projection_host(fsei_plan* P, double* u, double* v,
     if (rc) return rc;
     for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(h[f], P->hostpath[f], bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return FSEI_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// fluid substep: explicit terms, implicit viscous step
+// ------------------------------------------------------------------------------------------
+extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* v, const double* w, const double* p,
+                                   const double* fu, const double* fv, const double* fw, double* hu, double* hv, double* hw,
+                                   double* ru, double* rv, double* rw, double gamma_dt, double rho_dt, double alpha_dt,
+                                   double beta, void* cuda_stream)
+{
+    if (!P || !u || !v || !w || !p || !hu || !hv || !hw || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: NULL argument");
+    if (gamma_dt != gamma_dt || rho_dt != rho_dt || alpha_dt != alpha_dt || !(beta >= 0.0)) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: NaN parameter or beta < 0");
+    const double* in[4] = {u, v, w, p};
+    double* out[6] = {hu, hv, hw, ru, rv, rw};
+    for (int a = 0; a < 6; a++) {
+        for (int b = 0; b < 4; b++) if (out[a] == in[b]) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: outputs must not alias u, v, w, p");
+        for (int b = a + 1; b < 6; b++) if (out[a] == out[b]) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: outputs must not alias each other");
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta};
+    const size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
+    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
+}
+
+static VTab visc_tab(const fsei_plan* P, int comp, int dir)
+{
+    const HostTables& T = P->T;
+    const double* t = P->vtab + (size_t)(comp * 3 + dir) * vtab_set_doubles(P->vnmax);
+    const size_t m = (size_t)P->vnmax;
+    VTab V;
+    V.ip = t; V.am = t + m; V.cp = t + 2 * m; V.wc = t + 3 * m; V.er = t + 4 * m; V.ipl = t + 5 * m;
+    V.n = dir == DIR_X ? T.nx : (dir == DIR_Y ? T.ny : T.nz);
+    V.cyclic = (dir == DIR_X && T.bcx == BC_PERIODIC) || (dir == DIR_Y && T.bcy == BC_PERIODIC);
+    V.fixed0 = (dir == DIR_X && comp == COMP_U && T.bcx != BC_PERIODIC) || (dir == DIR_Y && comp == COMP_V && T.bcy != BC_PERIODIC) ||
+               (dir == DIR_Z && comp == COMP_W);
+    return V;
+}
+
+extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, double* ru, double* rv, double* rw,
+                                 double beta, void* cuda_stream)
+{
+    if (!P || !u || !v || !w || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_viscous_step: NULL argument");
+    if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_viscous_step: beta must be finite and >= 0");
+    double* q[3] = {u, v, w};
+    double* r[3] = {ru, rv, rw};
+    for (int a = 0; a < 3; a++)
+        for (int b = 0; b < 3; b++) if (r[a] == q[b] || (a != b && (r[a] == r[b] || q[a] == q[b]))) return fail(FSEI_ERR_ARG, "fsei_viscous_step: fields must not alias");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const HostTables& T = P->T;
+    int launches = 0;
+    // factorisation tables for this beta (kept while beta does not change)
+    if (!(P->visc_beta == beta)) {
+        VFactorArgs A{P->S, beta, P->vtab, P->vnmax};
+        { LaunchTimer t(P, K_VFACT, st); k_visc_factor<<<9, 32, 0, st>>>(A); }
+        CU(cudaGetLastError());
+        P->visc_beta = beta; launches++;
+    }
+    const long nlx = (long)T.ny * T.nz, nly = (long)T.nx * T.nz, nlz = (long)T.nx * T.ny;
+    const size_t plane = (size_t)T.nx * T.ny;
+    for (int c = 0; c < 3; c++) {
+        {
+            VTab V = visc_tab(P, c, DIR_X);
+            LaunchTimer t(P, K_VX, st);
+            const unsigned g = (unsigned)((nlx + 127) / 128);
+            if (V.cyclic) k_visc_sweep_x<true, false><<<g, 128, 0, st>>>(V, r[c], nullptr, nlx);
+            else k_visc_sweep_x<false, false><<<g, 128, 0, st>>>(V, r[c], nullptr, nlx);
+        }
+        CU(cudaGetLastError());
+        {
+            VTab V = visc_tab(P, c, DIR_Y);
+            LaunchTimer t(P, K_VY, st);
+            const unsigned g = (unsigned)((nly + 127) / 128);
+            if (V.cyclic) k_visc_sweep_strided<true, false><<<g, 128, 0, st>>>(V, r[c], nullptr, T.nx, (size_t)T.nx, plane, nly);
+            else k_visc_sweep_strided<false, false><<<g, 128, 0, st>>>(V, r[c], nullptr, T.nx, (size_t)T.nx, plane, nly);
+        }
+        CU(cudaGetLastError());
+        {
+            VTab V = visc_tab(P, c, DIR_Z);
+            LaunchTimer t(P, K_VZ, st);
+            k_visc_sweep_strided<false, true><<<(unsigned)((nlz + 127) / 128), 128, 0, st>>>(V, r[c], q[c], (int)nlz, plane, 0, nlz);
+        }
+        CU(cudaGetLastError());
+        launches += 3;
+    }
+    P->last_launches = launches;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_fluid_substep(fsei_plan* P, double* u, double* v, double* w, double* p, const double* fu, const double* fv,
+                                  const double* fw, double* hu, double* hv, double* hw, double* ru, double* rv, double* rw,
+                                  double* phi, double gamma_dt, double rho_dt, double alpha_dt, double beta, void* cuda_stream)
+{
+    int rc, n = 0;
+    if (!P) return fail(FSEI_ERR_ARG, "fsei_fluid_substep: NULL plan");
+    if ((rc = fsei_explicit_terms(P, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, beta, cuda_stream))) return rc;
+    n += P->last_launches;
+    if ((rc = fsei_viscous_step(P, u, v, w, ru, rv, rw, beta, cuda_stream))) return rc;
+    n += P->last_launches;
+    if ((rc = fsei_pressure_projection(P, u, v, w, p, phi, alpha_dt, beta, cuda_stream))) return rc;
+    n += P->last_launches;
+    P->last_launches = n;
     return FSEI_OK;
 }
 

@@ -1,0 +1,169 @@
+"""GPU parity of the fluid-substep steps that precede the projection against the oracle,
+through the C ABI (include/fsei.h: fsei_explicit_terms, fsei_viscous_step, fsei_fluid_substep).
+
+Gates:
+  explicit terms : BIT-EXACT (np.array_equal) -- stencils in a fixed IEEE-double order on both sides;
+  viscous step   : max|q_gpu - q_oracle| <= 1e-12 * max|dq| + 2 ulp(max|q|) against the long-double oracle (the second
+                   term is the rounding of the final q + dq in double on one side and long double on the other).
+                   Derivation: each factor
+                   (1 - beta d2) is an M-matrix with condition number <= 1 + 4 beta / h_min^2 (~2.5e3 for the wall cells
+                   of configs[3] at Re = 3000, dt = 1e-3); the bordered / plain Thomas elimination is backward stable on
+                   it, so the fp64 error is ~ eps * cond ~ 3e-13 relative to |dq|.
+"""
+import numpy as np
+import pytest
+
+from paper_2103_15187_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+P, W = 0, 1
+EPS = 2.0 ** -52
+ALL_BC = [(P, P), (W, W), (P, W), (W, P)]
+SHAPES = [(32, 32, 32), (48, 24, 20), (36, 16, 33), (64, 12, 7)]
+
+
+def _case(shape, bc, seed=40, s=2.5, n=10):
+    nx, ny, nz = shape
+    g = (nx, ny, nz, 1.0, 1.5, inputs.tanh_grid(nz, s), bc[0], bc[1])
+    f = [inputs.normal_field(seed, i, (nz, ny, nx)) for i in range(n)]
+    u, v, w = f[:3]
+    w[0] = 0
+    if bc[0] == W: u[:, :, 0] = 0
+    if bc[1] == W: v[:, 0, :] = 0
+    return g, f
+
+
+def _dev(arrs):
+    import torch
+    return [torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0") for a in arrs]
+
+
+def _plan(g):
+    from paper_2103_15187_b200.binding import Plan
+    return Plan.from_grid(g)
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("force", [False, True])
+def test_explicit_terms_bit_exact(oracle_ld, shape, bc, force):
+    import torch
+    g, f = _case(shape, bc)
+    u, v, w, p, h0, h1, h2, f0, f1, f2 = f
+    gdt, rdt, adt, beta = 1.5e-3, -0.5e-3, 1e-3, 1e-3 / (2 * 300.0)
+    ff = (f0, f1, f2) if force else (None, None, None)
+    ho = [h0.copy(), h1.copy(), h2.copy()]
+    ro = oracle_ld.explicit_terms(g, u, v, w, p, *ho, gdt, rdt, adt, beta, f=ff)
+    plan = _plan(g)
+    du, dv, dw, dp, dh0, dh1, dh2 = _dev([u, v, w, p, h0, h1, h2])
+    dr = [torch.empty_like(du) for _ in range(3)]
+    df = _dev(ff) if force else (None, None, None)
+    plan.explicit_terms(du, dv, dw, dp, dh0, dh1, dh2, *dr, gdt, rdt, adt, beta, f=df)
+    torch.cuda.synchronize()
+    for c in range(3):
+        assert np.array_equal(dr[c].cpu().numpy(), ro[c]), ("rhs", c)
+        assert np.array_equal((dh0, dh1, dh2)[c].cpu().numpy(), ho[c]), ("H", c)
+    assert np.array_equal(du.cpu().numpy(), u) and np.array_equal(dp.cpu().numpy(), p)      # inputs untouched
+    plan.destroy()
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("beta", [1e-3 / 6000.0, 2e-3, 0.5])
+def test_viscous_step_vs_oracle(oracle_ld, shape, bc, beta):
+    import torch
+    g, f = _case(shape, bc, seed=41)
+    u, v, w, ru, rv, rw = f[:6]
+    uo, vo, wo = u.copy(), v.copy(), w.copy()
+    oracle_ld.viscous_step(g, uo, vo, wo, ru, rv, rw, beta)
+    plan = _plan(g)
+    d = _dev([u, v, w, ru, rv, rw])
+    plan.viscous_step(*d, beta)
+    torch.cuda.synchronize()
+    for c, (q0, qo) in enumerate(((u, uo), (v, vo), (w, wo))):
+        got = d[c].cpu().numpy()
+        scale = np.abs(qo - q0).max()
+        assert np.abs(got - qo).max() <= 1e-12 * scale + 2 * EPS * np.abs(qo).max(), (c, np.abs(got - qo).max() / scale)
+    # wall faces never move
+    assert np.array_equal(d[2].cpu().numpy()[0], w[0])
+    if bc[0] == W: assert np.array_equal(d[0].cpu().numpy()[:, :, 0], u[:, :, 0])
+    if bc[1] == W: assert np.array_equal(d[1].cpu().numpy()[:, 0, :], v[:, 0, :])
+    # a second call with another beta rebuilds the tables
+    d2 = _dev([u, v, w, ru, rv, rw])
+    plan.viscous_step(*d2, beta * 3)
+    torch.cuda.synchronize()
+    uo2, vo2, wo2 = u.copy(), v.copy(), w.copy()
+    oracle_ld.viscous_step(g, uo2, vo2, wo2, ru, rv, rw, beta * 3)
+    assert np.abs(d2[0].cpu().numpy() - uo2).max() <= 1e-12 * np.abs(uo2 - u).max() + 2 * EPS * np.abs(uo2).max()
+    plan.destroy()
+
+
+def test_viscous_step_config_grid_wall_cells(oracle_ld):
+    """configs[3]'s z-grid (clustering 3.5, nz = 768) at reduced x,y and a physiological beta: the wall cells have
+    beta/dz^2 ~ 3e2 ... the stiffest factor of the headline workload."""
+    import torch
+    g = inputs.make_grid(4, shape=(64, 32, 768))
+    f = [inputs.normal_field(42, i, (768, 32, 64)) for i in range(6)]
+    u, v, w, ru, rv, rw = f
+    w[0] = 0
+    beta = 1e-3 / (2 * 3000.0)
+    uo, vo, wo = u.copy(), v.copy(), w.copy()
+    oracle_ld.viscous_step(g, uo, vo, wo, ru, rv, rw, beta)
+    plan = _plan(g)
+    d = _dev(f)
+    plan.viscous_step(*d, beta)
+    torch.cuda.synchronize()
+    for c, (q0, qo) in enumerate(((u, uo), (v, vo), (w, wo))):
+        assert np.abs(d[c].cpu().numpy() - qo).max() <= 1e-12 * np.abs(qo - q0).max() + 2 * EPS * np.abs(qo).max(), c
+    plan.destroy()
+
+
+@pytest.mark.parametrize("bc", [(P, P), (W, W)])
+def test_fluid_substep_chain_vs_oracle(oracle_ld, bc):
+    """Three RK3 substeps (explicit terms -> viscous step -> projection) enqueued with no host sync."""
+    import torch
+    shape = (48, 24, 20)
+    g, f = _case(shape, bc, seed=43)
+    u, v, w = [0.1 * t for t in f[:3]]
+    p = np.zeros_like(u)
+    h = [np.zeros_like(u) for _ in range(3)]
+    dt, Re = 2e-3, 200.0
+    gam, rho = (8 / 15, 5 / 12, 3 / 4), (0.0, -17 / 60, -5 / 12)
+    plan = _plan(g)
+    d = _dev([u, v, w, p] + h)
+    scratch = [torch.empty_like(d[0]) for _ in range(4)]
+    uo, vo, wo, po = u.copy(), v.copy(), w.copy(), p.copy()
+    ho = [t.copy() for t in h]
+    for l in range(3):
+        al = gam[l] + rho[l]
+        beta = al * dt / (2 * Re)
+        plan.fluid_substep(*d[:4], *d[4:], *scratch, gam[l] * dt, rho[l] * dt, al * dt, beta)
+        r = oracle_ld.explicit_terms(g, uo, vo, wo, po, *ho, gam[l] * dt, rho[l] * dt, al * dt, beta)
+        oracle_ld.viscous_step(g, uo, vo, wo, *r, beta)
+        oracle_ld.pressure_projection(g, uo, vo, wo, po, al * dt, beta)
+    torch.cuda.synchronize()
+    for c, ref in enumerate((uo, vo, wo, po)):
+        got = d[c].cpu().numpy()
+        assert np.abs(got - ref).max() <= 1e-11 * max(1.0, np.abs(ref).max()), (c, np.abs(got - ref).max())
+    div = np.abs(oracle_ld.divergence(g, *[d[c].cpu().numpy() for c in range(3)], 1.0)).max()
+    assert div <= 1e-10, div
+    plan.destroy()
+
+
+def test_fluid_error_codes():
+    import torch
+    from paper_2103_15187_b200.binding import FseiError, ERR_ARG
+    g, f = _case((32, 32, 32), (P, P))
+    plan = _plan(g)
+    d = _dev(f[:7])
+    r = [torch.empty_like(d[0]) for _ in range(3)]
+    with pytest.raises(FseiError) as e:
+        plan.viscous_step(d[0], d[1], d[2], d[0], r[1], r[2], 1e-3)             # rhs aliases u
+    assert e.value.code == ERR_ARG
+    with pytest.raises(FseiError) as e:
+        plan.viscous_step(d[0], d[1], d[2], *r, -1.0)                            # beta < 0
+    assert e.value.code == ERR_ARG
+    with pytest.raises(FseiError) as e:
+        plan.explicit_terms(*d[:4], d[4], d[5], d[6], d[0], r[1], r[2], 1e-3, 0.0, 1e-3, 0.0)   # output aliases input
+    assert e.value.code == ERR_ARG
+    plan.destroy()
