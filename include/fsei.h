@@ -24,7 +24,11 @@
  * by the caller.  `cuda_stream` is a cudaStream_t cast to void* (NULL = default stream).
  *
  * Execution.  Calls enqueue kernels on `cuda_stream` and return; they never synchronise
- * the device and never allocate after plan creation.  Calls on different plans may run
+ * the device and never allocate after plan creation (two documented exceptions, neither on the
+ * compute path: fsei_pressure_projection_host allocates its staging fields on first use unless
+ * the plan was created with FSEI_PLAN_HOST_FIELDS, and synchronises the stream before it returns;
+ * fsei_plan_profile(plan, 1) creates its CUDA events when it is switched on).  A field pointer that
+ * is not 16-byte aligned is rejected with FSEI_ERR_ARG.  Calls on different plans may run
  * concurrently; calls on ONE plan must be issued from one thread at a time and on one
  * stream at a time (the plan owns the factorisation tables, the scratch of the gauge
  * column and, on large grids, one workspace field that holds the spectrum in a blocked
@@ -61,6 +65,21 @@ enum { FSEI_OK = 0, FSEI_ERR_ARG = 1, FSEI_ERR_SIZE = 2, FSEI_ERR_GRID = 3, FSEI
  */
 fsei_plan*  fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly,
                              const double* zc /* HOST, nz+1 */, int bc_x, int bc_y);
+/*
+ * Same, with per-plan options (no process-global state steers a plan):
+ *   FSEI_PLAN_PATH_GENERIC | _FAST | _FUSED : force the kernel family instead of the plan's own choice (
+ *       a family that has no instantiation for the size falls back to the next simpler one; FUSED with a line length
+ *       whose landing tile exceeds the TMA box limit fails with FSEI_ERR_CUDA)
+ *   FSEI_PLAN_TWIST_OFF / FSEI_PLAN_TWIST_ON : the twisted factorisation of the fused family
+ *   FSEI_PLAN_HOST_FIELDS : allocate, now, the five device fields fsei_pressure_projection_host stages through
+ * Unknown flag bits -> FSEI_ERR_ARG.  fsei_plan_create(...) == fsei_plan_create_ex(..., 0).
+ */
+enum { FSEI_PLAN_PATH_GENERIC = 1, FSEI_PLAN_PATH_FAST = 2, FSEI_PLAN_PATH_FUSED = 3, FSEI_PLAN_PATH_MASK = 3,
+       FSEI_PLAN_TWIST_OFF = 4, FSEI_PLAN_TWIST_ON = 8, FSEI_PLAN_HOST_FIELDS = 16 };
+fsei_plan*  fsei_plan_create_ex(int nx, int ny, int nz, double Lx, double Ly, const double* zc /* HOST, nz+1 */,
+                                int bc_x, int bc_y, unsigned flags);
+/* Kernel family the plan chose: 0 generic, 1 fast, 2 fused; +4 when the twisted factorisation is on; < 0: -FSEI_ERR_ARG. */
+int         fsei_plan_kernel_family(const fsei_plan* plan);
 void        fsei_plan_destroy(fsei_plan* plan);
 const char* fsei_last_error(void);
 int         fsei_last_error_code(void);
@@ -108,8 +127,8 @@ int fsei_pressure_projection(fsei_plan* plan, double* u, double* v, double* w, d
 /*
  * Host-buffer convenience used for end-to-end timing: u,v,w,p are HOST pointers (pinned for
  * full speed); copies them to plan-owned device fields, runs fsei_pressure_projection, copies
- * u,v,w,p back and synchronises the stream.  Allocates the device fields on first use
- * (5 fields; freed with the plan).
+ * u,v,w,p back and synchronises the stream.  The 5 staging fields are allocated at plan creation
+ * when the plan was made with FSEI_PLAN_HOST_FIELDS, else on first use; freed with the plan.
  */
 int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double* w, double* p,
                                   double alpha_dt, double beta, void* cuda_stream);
@@ -168,8 +187,9 @@ int fsei_plan_last_launch_count(const fsei_plan* plan);
  * Per-kernel device timing for the roofline report: while enabled, every launch the calls
  * above enqueue is bracketed by a pair of CUDA events on the caller's stream.
  * fsei_plan_profile_read waits for the recorded events, returns how many kernel kinds there are
- * (<= max_kernels) and fills, per kind, the summed milliseconds and launch count since the last
- * read (and, if names != NULL, static name strings); it resets the sums.
+ * (<= max_kernels; a NEGATIVE value -FSEI_ERR_* on failure) and fills, per kind, the summed
+ * milliseconds and launch count since the last read (and, if names != NULL, static name strings);
+ * it resets the sums.  fsei_plan_profile(plan, 1) creates the event pool (2048 launches between reads).
  */
 int fsei_plan_profile(fsei_plan* plan, int enable);
 int fsei_plan_profile_read(fsei_plan* plan, int max_kernels, double* ms_sum, long* count, const char** names);

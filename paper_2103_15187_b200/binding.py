@@ -14,7 +14,9 @@ from . import build as _build
 BC_PERIODIC, BC_NEUMANN = 0, 1
 OK, ERR_ARG, ERR_SIZE, ERR_GRID, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4, 5
 
-EXPORTS = ("fsei_plan_create", "fsei_plan_destroy", "fsei_last_error", "fsei_last_error_code",
+PATH_GENERIC, PATH_FAST, PATH_FUSED, TWIST_OFF, TWIST_ON, HOST_FIELDS = 1, 2, 3, 4, 8, 16     # fsei_plan_create_ex flags
+
+EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family", "fsei_plan_destroy", "fsei_last_error", "fsei_last_error_code",
            "fsei_plan_workspace_bytes", "fsei_divergence", "fsei_poisson_solve", "fsei_project",
            "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
            "fsei_plan_profile", "fsei_plan_profile_read",
@@ -39,12 +41,17 @@ def lib() -> ctypes.CDLL:
     if _build.stale():
         try:
             _build.build()
-        except Exception as e:  # no nvcc on this box: use the shipped .so if there is one
+        except RuntimeError as e:  # raised by build._nvcc(): no nvcc on this box -> use the shipped .so if there is one
             if not os.path.exists(path):
                 raise RuntimeError(f"libfsei.so is missing and cannot be built ({e}); there is no CPU fallback") from e
+        # a compile error (subprocess.CalledProcessError) propagates: never run a stale binary against new sources
     L = ctypes.CDLL(path)
     L.fsei_plan_create.restype = _vp
     L.fsei_plan_create.argtypes = [_i, _i, _i, _d, _d, _vp, _i, _i]
+    L.fsei_plan_create_ex.restype = _vp
+    L.fsei_plan_create_ex.argtypes = [_i, _i, _i, _d, _d, _vp, _i, _i, ctypes.c_uint]
+    L.fsei_plan_kernel_family.restype = _i
+    L.fsei_plan_kernel_family.argtypes = [_vp]
     L.fsei_plan_destroy.restype = None
     L.fsei_plan_destroy.argtypes = [_vp]
     L.fsei_last_error.restype = ctypes.c_char_p
@@ -113,7 +120,7 @@ def _chk(rc: int):
 class Plan:
     """fsei_plan_create(nx, ny, nz, Lx, Ly, zc[], bc_x, bc_y); zc is a host float64 array of nz+1 faces."""
 
-    def __init__(self, nx, ny, nz, Lx, Ly, zc, bc_x=BC_PERIODIC, bc_y=BC_PERIODIC):
+    def __init__(self, nx, ny, nz, Lx, Ly, zc, bc_x=BC_PERIODIC, bc_y=BC_PERIODIC, flags=0):
         import numpy as np
         L = lib()
         zc = np.ascontiguousarray(zc, dtype=np.float64)
@@ -121,14 +128,23 @@ class Plan:
             raise FseiError(ERR_ARG, f"zc must hold nz+1 = {nz + 1} face coordinates")
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.shape = (self.nz, self.ny, self.nx)
-        self._h = L.fsei_plan_create(self.nx, self.ny, self.nz, float(Lx), float(Ly), zc.ctypes.data, int(bc_x), int(bc_y))
+        if flags:
+            self._h = L.fsei_plan_create_ex(self.nx, self.ny, self.nz, float(Lx), float(Ly), zc.ctypes.data, int(bc_x), int(bc_y),
+                                            int(flags))
+        else:
+            self._h = L.fsei_plan_create(self.nx, self.ny, self.nz, float(Lx), float(Ly), zc.ctypes.data, int(bc_x), int(bc_y))
         if not self._h:
             raise FseiError(L.fsei_last_error_code(), last_error())
 
     @classmethod
-    def from_grid(cls, grid):
+    def from_grid(cls, grid, flags=0):
         nx, ny, nz, Lx, Ly, zc, bcx, bcy = grid
-        return cls(nx, ny, nz, Lx, Ly, zc, bcx, bcy)
+        return cls(nx, ny, nz, Lx, Ly, zc, bcx, bcy, flags)
+
+    @property
+    def kernel_family(self) -> int:
+        """0 generic, 1 fast, 2 fused; +4 with the twisted factorisation."""
+        return int(lib().fsei_plan_kernel_family(self._h))
 
     def destroy(self):
         if getattr(self, "_h", None):
@@ -150,11 +166,11 @@ class Plan:
 
     def profile_read(self) -> dict:
         """{kernel name: (summed ms, launches)} since the last read (waits for the recorded events)."""
-        n = 16
+        n = 32
         ms, cnt, names = (_d * n)(), (ctypes.c_long * n)(), (ctypes.c_char_p * n)()
         k = lib().fsei_plan_profile_read(self._h, n, ms, cnt, names)
         if k < 0:
-            raise FseiError(ERR_CUDA, last_error())
+            raise FseiError(-k, last_error())
         return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(k) if cnt[i] > 0}
 
     def divergence(self, u, v, w, alpha_dt, rhs, stream=None):

@@ -218,103 +218,21 @@ FSEI_GLOBAL(128, 1) k_visc_sweep_x(VTab T, double* __restrict__ f, double* __res
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// explicit terms: one thread per cell, every operation individually rounded in the order of the definition
+// explicit terms.  CTA = 32 x 8 threads on a tile of 32 x-cells by 8 y-rows, marching KZ planes along z: a thread owns
+// one (i, j) column segment.  Every neighbour index and wall flag is computed once per thread; per plane a thread
+// issues 23 loads (the centre column and the two w neighbours of the upper face roll over from the plane before),
+// x/y neighbours are L1 hits of the same tile, the k-1 plane of the first step and the k+1 plane of every step are the
+// only new DRAM traffic.  Every floating-point operation is individually rounded in the order of the definition
+// (oracle/fsei_fluid_oracle.c states it), so the results are bit-identical.
+//
+// Boundary conventions (V7): periodic wrap; beyond a wall the wall-normal component is 0 (face n) and a
+// tangential component is its ghost -q (no slip, wall midway); a convective flux through a wall face is 0; wall-face
+// rows (u at i = 0, v at j = 0 on a wall-bounded box; w at k = 0) get H = rhs = 0.
 // ---------------------------------------------------------------------------------------------------------------
-template <int COMP> FSEI_DEV double vfetch(const SParams& S, const double* __restrict__ q, int i, int j, int k)
-{
-    bool neg = false;
-    if (i < 0 || i >= S.nx) {
-        if (S.bcx == BC_PERIODIC) i = i < 0 ? i + S.nx : i - S.nx;
-        else if (COMP == COMP_U) return 0.0;
-        else { i = i < 0 ? 0 : S.nx - 1; neg = !neg; }
-    }
-    if (j < 0 || j >= S.ny) {
-        if (S.bcy == BC_PERIODIC) j = j < 0 ? j + S.ny : j - S.ny;
-        else if (COMP == COMP_V) return 0.0;
-        else { j = j < 0 ? 0 : S.ny - 1; neg = !neg; }
-    }
-    if (k < 0 || k >= S.nz) {
-        if (COMP == COMP_W) return 0.0;
-        k = k < 0 ? 0 : S.nz - 1; neg = !neg;
-    }
-    const double val = q[sidx(S, i, j, k)];
-    return neg ? -val : val;
-}
-
 FSEI_DEV double avg2(double a, double b) { return FSEI_MUL(0.5, FSEI_ADD(a, b)); }
-FSEI_DEV bool xwall(const SParams& S, int i) { return S.bcx != BC_PERIODIC && (i <= 0 || i >= S.nx); }
-FSEI_DEV bool ywall(const SParams& S, int j) { return S.bcy != BC_PERIODIC && (j <= 0 || j >= S.ny); }
-FSEI_DEV bool zwall(const SParams& S, int k) { return k <= 0 || k >= S.nz; }
-
-template <int COMP> FSEI_DEV bool wall_row(const SParams& S, int i, int j, int k)
-{
-    return (COMP == COMP_U && S.bcx != BC_PERIODIC && i == 0) || (COMP == COMP_V && S.bcy != BC_PERIODIC && j == 0) ||
-           (COMP == COMP_W && k == 0);
-}
-
-// lap q = (dxx q + dyy q) + dzz q, second differences as differences of face gradients
-template <int COMP> FSEI_DEV double vel_lap(const SParams& S, const double* __restrict__ q, int i, int j, int k)
-{
-    const double c0 = q[sidx(S, i, j, k)];
-    double gp = FSEI_MUL(FSEI_SUB(vfetch<COMP>(S, q, i + 1, j, k), c0), S.rdx), gm = FSEI_MUL(FSEI_SUB(c0, vfetch<COMP>(S, q, i - 1, j, k)), S.rdx);
-    const double dxx = FSEI_MUL(FSEI_SUB(gp, gm), S.rdx);
-    gp = FSEI_MUL(FSEI_SUB(vfetch<COMP>(S, q, i, j + 1, k), c0), S.rdy); gm = FSEI_MUL(FSEI_SUB(c0, vfetch<COMP>(S, q, i, j - 1, k)), S.rdy);
-    const double dyy = FSEI_MUL(FSEI_SUB(gp, gm), S.rdy);
-    double dzz;
-    if (COMP != COMP_W) {
-        const double rc = S.rdzc[k];
-        gp = (k + 1 < S.nz) ? FSEI_MUL(FSEI_SUB(q[sidx(S, i, j, k + 1)], c0), S.rdzm[k + 1]) : FSEI_MUL(FSEI_SUB(0.0, c0), FSEI_MUL(2.0, rc));
-        gm = (k > 0) ? FSEI_MUL(FSEI_SUB(c0, q[sidx(S, i, j, k - 1)]), S.rdzm[k]) : FSEI_MUL(FSEI_SUB(c0, 0.0), FSEI_MUL(2.0, rc));
-        dzz = FSEI_MUL(FSEI_SUB(gp, gm), rc);
-    } else {
-        const double wp = (k + 1 < S.nz) ? q[sidx(S, i, j, k + 1)] : 0.0;
-        gp = FSEI_MUL(FSEI_SUB(wp, c0), S.rdzc[k]); gm = FSEI_MUL(FSEI_SUB(c0, q[sidx(S, i, j, k - 1)]), S.rdzc[k - 1]);
-        dzz = FSEI_MUL(FSEI_SUB(gp, gm), S.rdzm[k]);
-    }
-    return FSEI_ADD(FSEI_ADD(dxx, dyy), dzz);
-}
-
+FSEI_DEV double sq_diff(double a, double b, double r) { return FSEI_MUL(FSEI_SUB(FSEI_MUL(a, a), FSEI_MUL(b, b)), r); }
+FSEI_DEV double d2_grad(double qp, double c0, double qm, double r) { return FSEI_MUL(FSEI_SUB(FSEI_MUL(FSEI_SUB(qp, c0), r), FSEI_MUL(FSEI_SUB(c0, qm), r)), r); }
 FSEI_DEV double neg3(double fx, double fy, double fz) { return -FSEI_ADD(FSEI_ADD(fx, fy), fz); }
-
-FSEI_DEV double conv_u(const SParams& S, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w, int i, int j, int k)
-{
-    const double c0 = u[sidx(S, i, j, k)];
-    const double ucp = avg2(c0, vfetch<COMP_U>(S, u, i + 1, j, k)), ucm = avg2(vfetch<COMP_U>(S, u, i - 1, j, k), c0);
-    const double fx = FSEI_MUL(FSEI_SUB(FSEI_MUL(ucp, ucp), FSEI_MUL(ucm, ucm)), S.rdx);
-    const double fa = ywall(S, j + 1) ? 0.0 : FSEI_MUL(avg2(c0, vfetch<COMP_U>(S, u, i, j + 1, k)), avg2(vfetch<COMP_V>(S, v, i - 1, j + 1, k), vfetch<COMP_V>(S, v, i, j + 1, k)));
-    const double fb = ywall(S, j) ? 0.0 : FSEI_MUL(avg2(vfetch<COMP_U>(S, u, i, j - 1, k), c0), avg2(vfetch<COMP_V>(S, v, i - 1, j, k), vfetch<COMP_V>(S, v, i, j, k)));
-    const double fy = FSEI_MUL(FSEI_SUB(fa, fb), S.rdy);
-    const double ga = zwall(S, k + 1) ? 0.0 : FSEI_MUL(avg2(c0, vfetch<COMP_U>(S, u, i, j, k + 1)), avg2(vfetch<COMP_W>(S, w, i - 1, j, k + 1), vfetch<COMP_W>(S, w, i, j, k + 1)));
-    const double gb = zwall(S, k) ? 0.0 : FSEI_MUL(avg2(vfetch<COMP_U>(S, u, i, j, k - 1), c0), avg2(vfetch<COMP_W>(S, w, i - 1, j, k), vfetch<COMP_W>(S, w, i, j, k)));
-    const double fz = FSEI_MUL(FSEI_SUB(ga, gb), S.rdzc[k]);
-    return neg3(fx, fy, fz);
-}
-FSEI_DEV double conv_v(const SParams& S, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w, int i, int j, int k)
-{
-    const double c0 = v[sidx(S, i, j, k)];
-    const double fa = xwall(S, i + 1) ? 0.0 : FSEI_MUL(avg2(c0, vfetch<COMP_V>(S, v, i + 1, j, k)), avg2(vfetch<COMP_U>(S, u, i + 1, j - 1, k), vfetch<COMP_U>(S, u, i + 1, j, k)));
-    const double fb = xwall(S, i) ? 0.0 : FSEI_MUL(avg2(vfetch<COMP_V>(S, v, i - 1, j, k), c0), avg2(vfetch<COMP_U>(S, u, i, j - 1, k), vfetch<COMP_U>(S, u, i, j, k)));
-    const double fx = FSEI_MUL(FSEI_SUB(fa, fb), S.rdx);
-    const double vcp = avg2(c0, vfetch<COMP_V>(S, v, i, j + 1, k)), vcm = avg2(vfetch<COMP_V>(S, v, i, j - 1, k), c0);
-    const double fy = FSEI_MUL(FSEI_SUB(FSEI_MUL(vcp, vcp), FSEI_MUL(vcm, vcm)), S.rdy);
-    const double ga = zwall(S, k + 1) ? 0.0 : FSEI_MUL(avg2(c0, vfetch<COMP_V>(S, v, i, j, k + 1)), avg2(vfetch<COMP_W>(S, w, i, j - 1, k + 1), vfetch<COMP_W>(S, w, i, j, k + 1)));
-    const double gb = zwall(S, k) ? 0.0 : FSEI_MUL(avg2(vfetch<COMP_V>(S, v, i, j, k - 1), c0), avg2(vfetch<COMP_W>(S, w, i, j - 1, k), vfetch<COMP_W>(S, w, i, j, k)));
-    const double fz = FSEI_MUL(FSEI_SUB(ga, gb), S.rdzc[k]);
-    return neg3(fx, fy, fz);
-}
-FSEI_DEV double conv_w(const SParams& S, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w, int i, int j, int k)
-{
-    const double c0 = w[sidx(S, i, j, k)];
-    const double fa = xwall(S, i + 1) ? 0.0 : FSEI_MUL(avg2(c0, vfetch<COMP_W>(S, w, i + 1, j, k)), avg2(vfetch<COMP_U>(S, u, i + 1, j, k - 1), vfetch<COMP_U>(S, u, i + 1, j, k)));
-    const double fb = xwall(S, i) ? 0.0 : FSEI_MUL(avg2(vfetch<COMP_W>(S, w, i - 1, j, k), c0), avg2(vfetch<COMP_U>(S, u, i, j, k - 1), vfetch<COMP_U>(S, u, i, j, k)));
-    const double fx = FSEI_MUL(FSEI_SUB(fa, fb), S.rdx);
-    const double ga = ywall(S, j + 1) ? 0.0 : FSEI_MUL(avg2(c0, vfetch<COMP_W>(S, w, i, j + 1, k)), avg2(vfetch<COMP_V>(S, v, i, j + 1, k - 1), vfetch<COMP_V>(S, v, i, j + 1, k)));
-    const double gb = ywall(S, j) ? 0.0 : FSEI_MUL(avg2(vfetch<COMP_W>(S, w, i, j - 1, k), c0), avg2(vfetch<COMP_V>(S, v, i, j, k - 1), vfetch<COMP_V>(S, v, i, j, k)));
-    const double fy = FSEI_MUL(FSEI_SUB(ga, gb), S.rdy);
-    const double wcp = avg2(c0, vfetch<COMP_W>(S, w, i, j, k + 1)), wcm = avg2(vfetch<COMP_W>(S, w, i, j, k - 1), c0);
-    const double fz = FSEI_MUL(FSEI_SUB(FSEI_MUL(wcp, wcp), FSEI_MUL(wcm, wcm)), S.rdzm[k]);
-    return neg3(fx, fy, fz);
-}
 
 struct ExplicitArgs {
     SParams S;
@@ -329,37 +247,108 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
     return FSEI_ADD(FSEI_SUB(FSEI_ADD(FSEI_MUL(A.gdt, H), FSEI_MUL(A.rdt, Hp)), FSEI_MUL(A.adt, gp)), FSEI_MUL(A.tb, lap));
 }
 
-// grid ceil(nx ny nz / 256), block 256, x fastest
-FSEI_GLOBAL(256, 1) k_explicit_terms(ExplicitArgs A)
+#define FSEI_EXPL_KZ 8
+
+// grid (ceil(nx/32), ceil(ny/8), ceil(nz/KZ)), block (32, 8)
+FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
 {
     const SParams& S = A.S;
-    const size_t t = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (t >= (size_t)S.nx * S.ny * S.nz) return;
-    const int i = (int)(t % S.nx); const size_t r = t / S.nx; const int j = (int)(r % S.ny), k = (int)(r / S.ny);
-    const double c0 = A.p[t];
-    if (wall_row<COMP_U>(S, i, j, k)) { A.hu[t] = 0.0; A.ru[t] = 0.0; }
-    else {
-        double H = conv_u(S, A.u, A.v, A.w, i, j, k);
-        if (A.fu) H = FSEI_ADD(H, A.fu[t]);
-        const double gp = FSEI_MUL(FSEI_SUB(c0, A.p[sidx(S, i > 0 ? i - 1 : S.nx - 1, j, k)]), S.rdx);
-        A.ru[t] = rhs_assemble(H, A.hu[t], gp, vel_lap<COMP_U>(S, A.u, i, j, k), A);
-        A.hu[t] = H;
-    }
-    if (wall_row<COMP_V>(S, i, j, k)) { A.hv[t] = 0.0; A.rv[t] = 0.0; }
-    else {
-        double H = conv_v(S, A.u, A.v, A.w, i, j, k);
-        if (A.fv) H = FSEI_ADD(H, A.fv[t]);
-        const double gp = FSEI_MUL(FSEI_SUB(c0, A.p[sidx(S, i, j > 0 ? j - 1 : S.ny - 1, k)]), S.rdy);
-        A.rv[t] = rhs_assemble(H, A.hv[t], gp, vel_lap<COMP_V>(S, A.v, i, j, k), A);
-        A.hv[t] = H;
-    }
-    if (wall_row<COMP_W>(S, i, j, k)) { A.hw[t] = 0.0; A.rw[t] = 0.0; }
-    else {
-        double H = conv_w(S, A.u, A.v, A.w, i, j, k);
-        if (A.fw) H = FSEI_ADD(H, A.fw[t]);
-        const double gp = FSEI_MUL(FSEI_SUB(c0, A.p[sidx(S, i, j, k - 1)]), S.rdzm[k]);
-        A.rw[t] = rhs_assemble(H, A.hw[t], gp, vel_lap<COMP_W>(S, A.w, i, j, k), A);
-        A.hw[t] = H;
+    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
+    if (i >= S.nx || j >= S.ny) return;
+    const bool xper = S.bcx == BC_PERIODIC, yper = S.bcy == BC_PERIODIC;
+    const bool xlo = !xper && i == 0, xhi = !xper && i == S.nx - 1;      // x-face i / i+1 is a wall
+    const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
+    const int im = i > 0 ? i - 1 : (xper ? S.nx - 1 : 0), ip = i + 1 < S.nx ? i + 1 : (xper ? 0 : i);
+    const int jm = j > 0 ? j - 1 : (yper ? S.ny - 1 : 0), jp = j + 1 < S.ny ? j + 1 : (yper ? 0 : j);
+    const size_t plane = (size_t)S.nx * S.ny;
+    const size_t o00 = (size_t)j * S.nx + i, oP0 = (size_t)j * S.nx + ip, oM0 = (size_t)j * S.nx + im;
+    const size_t o0P = (size_t)jp * S.nx + i, o0M = (size_t)jm * S.nx + i, oPM = (size_t)jm * S.nx + ip, oMP = (size_t)jp * S.nx + im;
+    const double* __restrict__ u = A.u; const double* __restrict__ v = A.v; const double* __restrict__ w = A.w;
+    const double* __restrict__ p = A.p;
+    const double rdx = S.rdx, rdy = S.rdy;
+    const int k0 = blockIdx.z * FSEI_EXPL_KZ, k1 = (k0 + FSEI_EXPL_KZ < S.nz) ? k0 + FSEI_EXPL_KZ : S.nz;
+
+    // rolling values of the centre column and of the w neighbours of the upper face
+    size_t b = (size_t)k0 * plane;
+    double u00 = u[b + o00], v00 = v[b + o00], w00 = w[b + o00], p00 = p[b + o00];
+    double wM0r = w[b + oM0], w0Mr = w[b + o0M];
+    double u_km = 0.0, v_km = 0.0, w_km = 0.0, p_km = 0.0;
+    if (k0 > 0) { u_km = u[b - plane + o00]; v_km = v[b - plane + o00]; w_km = w[b - plane + o00]; p_km = p[b - plane + o00]; }
+
+    for (int k = k0; k < k1; k++, b += plane) {
+        const bool zlo = k == 0, zhi = k == S.nz - 1;
+        const size_t bp = zhi ? b : b + plane, bm = zlo ? b : b - plane;
+        // ---- this plane
+        const double uP0 = xhi ? 0.0 : u[b + oP0], uM0 = u[b + oM0];
+        double u0P = u[b + o0P], u0M = u[b + o0M];
+        const double uPM = u[b + oPM];
+        double vP0 = v[b + oP0], vM0 = v[b + oM0];
+        const double v0P = yhi ? 0.0 : v[b + o0P], v0M = v[b + o0M], vMP = v[b + oMP];
+        double wP0 = w[b + oP0], w0P = w[b + o0P], wM0 = wM0r, w0M = w0Mr;
+        const double pM0 = p[b + oM0], p0M = p[b + o0M];
+        // ---- plane above (fluxes through the upper face; clamped loads are never used on the top plane) and below
+        const double u_kp = u[bp + o00], v_kp = v[bp + o00], w_kp = zhi ? 0.0 : w[bp + o00], p_kp = p[bp + o00];
+        const double wM_kp = w[bp + oM0], w0M_kp = w[bp + o0M];
+        const double uP_km = xhi ? 0.0 : u[bm + oP0], v0P_km = yhi ? 0.0 : v[bm + o0P];
+        // ghosts of the tangential components beyond a wall
+        if (ylo) u0M = -u00; if (yhi) u0P = -u00;
+        if (xlo) vM0 = -v00; if (xhi) vP0 = -v00;
+        if (xlo) wM0 = -w00; if (xhi) wP0 = -w00;
+        if (ylo) w0M = -w00; if (yhi) w0P = -w00;
+        const double rc = S.rdzc[k], rm = S.rdzm[k];
+        const size_t t = b + o00;
+
+        // ---- u
+        if (xlo) { A.hu[t] = 0.0; A.ru[t] = 0.0; }
+        else {
+            const double fx = sq_diff(avg2(u00, uP0), avg2(uM0, u00), rdx);
+            const double fa = yhi ? 0.0 : FSEI_MUL(avg2(u00, u0P), avg2(vMP, v0P));
+            const double fb = ylo ? 0.0 : FSEI_MUL(avg2(u0M, u00), avg2(vM0, v00));
+            const double ga = zhi ? 0.0 : FSEI_MUL(avg2(u00, u_kp), avg2(wM_kp, w_kp));
+            const double gb = zlo ? 0.0 : FSEI_MUL(avg2(u_km, u00), avg2(wM0, w00));
+            double H = neg3(fx, FSEI_MUL(FSEI_SUB(fa, fb), rdy), FSEI_MUL(FSEI_SUB(ga, gb), rc));
+            if (A.fu) H = FSEI_ADD(H, A.fu[t]);
+            const double gzp = zhi ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), S.rdzm[k + 1]);
+            const double gzm = zlo ? FSEI_MUL(FSEI_SUB(u00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u00, u_km), rm);
+            const double lap = FSEI_ADD(FSEI_ADD(d2_grad(uP0, u00, uM0, rdx), d2_grad(u0P, u00, u0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
+            A.ru[t] = rhs_assemble(H, A.hu[t], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
+            A.hu[t] = H;
+        }
+        // ---- v
+        if (ylo) { A.hv[t] = 0.0; A.rv[t] = 0.0; }
+        else {
+            const double fa = xhi ? 0.0 : FSEI_MUL(avg2(v00, vP0), avg2(uPM, uP0));
+            const double fb = xlo ? 0.0 : FSEI_MUL(avg2(vM0, v00), avg2(u0M, u00));
+            const double fy = sq_diff(avg2(v00, v0P), avg2(v0M, v00), rdy);
+            const double ga = zhi ? 0.0 : FSEI_MUL(avg2(v00, v_kp), avg2(w0M_kp, w_kp));
+            const double gb = zlo ? 0.0 : FSEI_MUL(avg2(v_km, v00), avg2(w0M, w00));
+            double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), fy, FSEI_MUL(FSEI_SUB(ga, gb), rc));
+            if (A.fv) H = FSEI_ADD(H, A.fv[t]);
+            const double gzp = zhi ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), S.rdzm[k + 1]);
+            const double gzm = zlo ? FSEI_MUL(FSEI_SUB(v00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v00, v_km), rm);
+            const double lap = FSEI_ADD(FSEI_ADD(d2_grad(vP0, v00, vM0, rdx), d2_grad(v0P, v00, v0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
+            A.rv[t] = rhs_assemble(H, A.hv[t], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
+            A.hv[t] = H;
+        }
+        // ---- w
+        if (zlo) { A.hw[t] = 0.0; A.rw[t] = 0.0; }
+        else {
+            const double fa = xhi ? 0.0 : FSEI_MUL(avg2(w00, wP0), avg2(uP_km, uP0));
+            const double fb = xlo ? 0.0 : FSEI_MUL(avg2(wM0, w00), avg2(u_km, u00));
+            const double ga = yhi ? 0.0 : FSEI_MUL(avg2(w00, w0P), avg2(v0P_km, v0P));
+            const double gb = ylo ? 0.0 : FSEI_MUL(avg2(w0M, w00), avg2(v_km, v00));
+            const double fz = sq_diff(avg2(w00, w_kp), avg2(w_km, w00), rm);
+            double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), FSEI_MUL(FSEI_SUB(ga, gb), rdy), fz);
+            if (A.fw) H = FSEI_ADD(H, A.fw[t]);
+            const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), S.rdzc[k - 1]);
+            const double lap = FSEI_ADD(FSEI_ADD(d2_grad(wP0, w00, wM0, rdx), d2_grad(w0P, w00, w0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rm));
+            A.rw[t] = rhs_assemble(H, A.hw[t], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
+            A.hw[t] = H;
+        }
+        // ---- roll to the next plane
+        u_km = u00; v_km = v00; w_km = w00; p_km = p00;
+        u00 = u_kp; v00 = v_kp; w00 = zhi ? 0.0 : w_kp; p00 = p_kp;
+        wM0r = wM_kp; w0Mr = w0M_kp;
     }
 }
 

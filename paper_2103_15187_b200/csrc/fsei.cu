@@ -37,6 +37,7 @@ static int cuda_fail(cudaError_t e, const char* what)
 {
     return fail(FSEI_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
+static bool misaligned(const void* p) { return (reinterpret_cast<size_t>(p) & 15u) != 0; }
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
 
 // ------------------------------------------------------------------------------------------
@@ -77,9 +78,7 @@ struct LaunchTimer {
     fsei_plan* P; cudaStream_t st; bool on;
     LaunchTimer(fsei_plan* P_, int kid, cudaStream_t st_) : P(P_), st(st_), on(P_->profiling) {
         if (!on) return;
-        if (P->ev_used + 2 > P->ev_pool.size()) {
-            for (int i = 0; i < 64; i++) { cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; } P->ev_pool.push_back(e); }
-        }
+        if (P->ev_used + 2 > P->ev_pool.size()) { on = false; return; }      // pool exhausted (2048 launches since the last read): stop recording
         P->ev_kid.push_back(kid);
         cudaEventRecord(P->ev_pool[P->ev_used], st);
     }
@@ -225,15 +224,16 @@ __global__ void __launch_bounds__(NT) k_z_gauge(ZParams Z, const cplx* spec, dou
 // ------------------------------------------------------------------------------------------
 // plan creation
 // ------------------------------------------------------------------------------------------
-static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy)
+static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy, unsigned flags)
 {
     int code = 0;
     // fast path: line lengths with a register-resident Stockham instantiation, special columns fit in shared memory
     // fused path: the fast path on the blocked layout, where one CTA per x-slot tile marches along z -- for grids
-    // with enough tiles to fill the GPU.  FSEI_PATH = generic | fast | fused overrides the choice (tests).
-    const char* force = std::getenv("FSEI_FORCE_GENERIC");
-    const char* path = std::getenv("FSEI_PATH");
-    const std::string want = path ? path : ((force && force[0] == '1') ? "generic" : "");
+    // with enough tiles to fill the GPU.  flags (fsei_plan_create_ex) may override the choice, per plan.
+    if (flags & ~(unsigned)(FSEI_PLAN_PATH_MASK | FSEI_PLAN_TWIST_OFF | FSEI_PLAN_TWIST_ON | FSEI_PLAN_HOST_FIELDS)) return fail(FSEI_ERR_ARG, "fsei_plan_create_ex: unknown flag");
+    if ((flags & FSEI_PLAN_TWIST_OFF) && (flags & FSEI_PLAN_TWIST_ON)) return fail(FSEI_ERR_ARG, "fsei_plan_create_ex: TWIST_OFF and TWIST_ON are exclusive");
+    const unsigned pf = flags & FSEI_PLAN_PATH_MASK;
+    const std::string want = pf == FSEI_PLAN_PATH_GENERIC ? "generic" : (pf == FSEI_PLAN_PATH_FAST ? "fast" : (pf == FSEI_PLAN_PATH_FUSED ? "fused" : ""));
     const bool fast = want != "generic" && nx >= 4 && ny >= 2 && xfast_supported(nx / 2) && yfast_supported(ny) &&
                       (size_t)nz * 4 * sizeof(cplx) <= 200 * 1024;
     const bool fused_ok = fast && xblocked_supported(nx / 2) && yzfused_supported(ny) && (nx / 2) % FSEI_CB == 0;
@@ -302,12 +302,12 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         ZF.cpw = static_cast<double*>(q);
         ZF.cb = fused ? FSEI_CB : 0; ZF.special_in = nullptr;
         // Twisted factorisation (two CTAs per tile sweeping towards each other) where one CTA per tile would leave SMs
-        // idle: fewer tiles than SMs.  FSEI_TWIST = 0 | 1 overrides (tests).
+        // idle: fewer tiles than SMs.  FSEI_PLAN_TWIST_OFF / _ON override.
         int nsm = 148;
         { int dev = 0; CU(cudaGetDevice(&dev)); CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev)); }
         // ... or three-warp CTAs (ny = 3 2^a) that cannot fill their SM even two at a time (configs[4]: 23.5 -> 22.1 ms)
         bool twist = fused && nz >= 4 && (T.nxc / FSEI_CB <= nsm || (yzfused_block_threads(ny) < 128 && T.nxc / FSEI_CB <= 2 * nsm));
-        if (const char* tw = std::getenv("FSEI_TWIST")) twist = fused && nz >= 4 && tw[0] == '1';
+        if (flags & (FSEI_PLAN_TWIST_OFF | FSEI_PLAN_TWIST_ON)) twist = fused && nz >= 4 && (flags & FSEI_PLAN_TWIST_ON);
         ZF.ktw = twist ? nz / 2 : nz;
         if (fused) {
             if ((rc = dalloc(P, sizeof(cplx) * 2 * nz, &q))) return rc;
@@ -402,14 +402,40 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     return FSEI_OK;
 }
 
-extern "C" fsei_plan* fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bc_x, int bc_y)
+static int host_fields(fsei_plan* P)
+{
+    const size_t bytes = sizeof(double) * (size_t)P->T.nx * P->T.ny * P->T.nz;
+    for (int f = 0; f < 5; f++)
+        if (!P->hostpath[f]) {
+            cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&P->hostpath[f]), bytes);
+            if (e != cudaSuccess) { cudaGetLastError(); P->hostpath[f] = nullptr; return fail(FSEI_ERR_ALLOC, "cudaMalloc of a device field failed"); }
+            P->bytes += bytes;
+        }
+    return FSEI_OK;
+}
+
+extern "C" fsei_plan* fsei_plan_create_ex(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bc_x, int bc_y,
+                                          unsigned flags)
 {
     fsei_plan* P = new (std::nothrow) fsei_plan();
     if (!P) { fail(FSEI_ERR_ALLOC, "out of host memory"); return nullptr; }
-    int rc = plan_build(P, nx, ny, nz, Lx, Ly, zc, bc_x, bc_y);
-    if (rc != FSEI_OK) { fsei_plan_destroy(P); g_err_code = rc; return nullptr; }
+    int rc = plan_build(P, nx, ny, nz, Lx, Ly, zc, bc_x, bc_y, flags);
+    if (rc == FSEI_OK && (flags & FSEI_PLAN_HOST_FIELDS)) rc = host_fields(P);
+    if (rc != FSEI_OK) { const std::string msg = g_err; fsei_plan_destroy(P); g_err = msg; g_err_code = rc; return nullptr; }
     g_err_code = FSEI_OK; g_err.clear();
     return P;
+}
+
+extern "C" fsei_plan* fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bc_x, int bc_y)
+{
+    return fsei_plan_create_ex(nx, ny, nz, Lx, Ly, zc, bc_x, bc_y, 0u);
+}
+
+// 0: generic, 1: fast, 2: fused (+4 when the twisted factorisation is on)
+extern "C" int fsei_plan_kernel_family(const fsei_plan* P)
+{
+    if (!P) return -FSEI_ERR_ARG;
+    return (P->fused ? 2 : (P->fast ? 1 : 0)) + ((P->fused && P->ZF.ktw != P->T.nz) ? 4 : 0);
 }
 
 extern "C" void fsei_plan_destroy(fsei_plan* P)
@@ -435,6 +461,7 @@ extern "C" int fsei_divergence(fsei_plan* P, const double* u, const double* v, c
     if (!P || !u || !v || !w || !rhs) return fail(FSEI_ERR_ARG, "fsei_divergence: NULL argument");
     if (alpha_dt == 0.0 || alpha_dt != alpha_dt) return fail(FSEI_ERR_ARG, "fsei_divergence: alpha_dt must be non-zero");
     if (rhs == u || rhs == v || rhs == w) return fail(FSEI_ERR_ARG, "fsei_divergence: rhs must not alias u, v, w");
+    if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(rhs)) return fail(FSEI_ERR_ARG, "fsei_divergence: field pointers must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
     { LaunchTimer t(P, K_DIV, st); k_divergence_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, 1.0 / alpha_dt, rhs); }
@@ -480,6 +507,7 @@ static int fused_spectral_solve(fsei_plan* P, double* phi, cudaStream_t st)
 extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, void* cuda_stream)
 {
     if (!P || !rhs || !phi) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: NULL argument");
+    if (misaligned(rhs) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: field pointers must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const HostTables& T = P->T;
     const long nlines = (long)T.ny * T.nz;
@@ -552,6 +580,7 @@ extern "C" int fsei_project(fsei_plan* P, double* u, double* v, double* w, doubl
     if (!P || !u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_project: NULL argument");
     if (alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_project: NaN parameter");
     if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_project: phi must not alias u, v, w, p");
+    if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(p) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_project: field pointers must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
     { LaunchTimer t(P, K_PROJ, st); k_project_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, p, phi, alpha_dt, beta); }
@@ -568,6 +597,7 @@ extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, doub
         if (!u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: NULL argument");
         if (alpha_dt == 0.0 || alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: alpha_dt must be non-zero, beta not NaN");
         if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: phi must not alias u, v, w, p");
+        if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(p) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: field pointers must be 16-byte aligned");
         cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
         cplx* spec = P->fused ? P->work : reinterpret_cast<cplx*>(phi);
         { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, P->T.bcx == BC_NEUMANN, true, u, v, w, 1.0 / alpha_dt, spec, st, P->fused)); }
@@ -592,11 +622,7 @@ extern "C" int fsei_pressure_projection_host(fsei_plan* P, double* u, double* v,
     if (!P || !u || !v || !w || !p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection_host: NULL argument");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t bytes = sizeof(double) * (size_t)P->T.nx * P->T.ny * P->T.nz;
-    for (int f = 0; f < 5; f++)
-        if (!P->hostpath[f]) {
-            cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&P->hostpath[f]), bytes);
-            if (e != cudaSuccess) { cudaGetLastError(); P->hostpath[f] = nullptr; return fail(FSEI_ERR_ALLOC, "cudaMalloc of a device field failed"); }
-        }
+    { int rc0 = host_fields(P); if (rc0) return rc0; }          // no-op when the plan was created with FSEI_PLAN_HOST_FIELDS
     double* h[4] = {u, v, w, p};
     for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(P->hostpath[f], h[f], bytes, cudaMemcpyHostToDevice, st));
     int rc = fsei_pressure_projection(P, P->hostpath[0], P->hostpath[1], P->hostpath[2], P->hostpath[3], P->hostpath[4],
@@ -625,8 +651,8 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta};
-    const size_t n = (size_t)P->T.nx * P->T.ny * P->T.nz;
-    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A); }
+    const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (P->T.nz + FSEI_EXPL_KZ - 1) / FSEI_EXPL_KZ);
+    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), 0, st>>>(A); }
     CU(cudaGetLastError());
     P->last_launches = 1;
     return FSEI_OK;
@@ -718,17 +744,22 @@ extern "C" int fsei_fluid_substep(fsei_plan* P, double* u, double* v, double* w,
 extern "C" int fsei_plan_profile(fsei_plan* P, int enable)
 {
     if (!P) return fail(FSEI_ERR_ARG, "fsei_plan_profile: NULL plan");
+    if (enable && P->ev_pool.size() < 4096) {                    // all events are created here, none inside a timed loop
+        P->ev_pool.reserve(4096); P->ev_kid.reserve(2048);
+        while (P->ev_pool.size() < 4096) { cudaEvent_t e; CU(cudaEventCreate(&e)); P->ev_pool.push_back(e); }
+    }
     P->profiling = enable != 0;
     return FSEI_OK;
 }
 
 extern "C" int fsei_plan_profile_read(fsei_plan* P, int max_kernels, double* ms_sum, long* count, const char** names)
 {
-    if (!P || !ms_sum || !count) return fail(FSEI_ERR_ARG, "fsei_plan_profile_read: NULL argument");
+    if (!P || !ms_sum || !count) return -fail(FSEI_ERR_ARG, "fsei_plan_profile_read: NULL argument");
     for (size_t i = 0; i < P->ev_kid.size(); i++) {
-        CU(cudaEventSynchronize(P->ev_pool[2 * i + 1]));
+        cudaError_t e = cudaEventSynchronize(P->ev_pool[2 * i + 1]);
         float ms = 0.f;
-        CU(cudaEventElapsedTime(&ms, P->ev_pool[2 * i], P->ev_pool[2 * i + 1]));
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, P->ev_pool[2 * i], P->ev_pool[2 * i + 1]);
+        if (e != cudaSuccess) return -cuda_fail(e, "fsei_plan_profile_read");
         P->prof_ms[P->ev_kid[i]] += ms; P->prof_n[P->ev_kid[i]]++;
     }
     P->ev_kid.clear(); P->ev_used = 0;

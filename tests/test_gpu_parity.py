@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 from paper_2103_15187_b200 import inputs
-from tests.util import div_gate, gpu_fields, gpu_projection, oracle_projection, rel_l2
+from tests.util import div_gate, gpu_fields, gpu_projection, make_plan, oracle_projection, rel_l2
 
 pytestmark = pytest.mark.gpu
 P, N = 0, 1
@@ -38,7 +38,7 @@ def test_divergence_bit_exact(oracle_ld, bc, shape):
     torch = _torch()
     from paper_2103_15187_b200.binding import Plan
     case = inputs.make_case(1, shape=shape, bc=bc)
-    plan = Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     u, v, w = (torch.from_numpy(a).cuda() for a in (case.u, case.v, case.w))
     rhs = torch.empty_like(u)
     plan.divergence(u, v, w, case.alpha_dt, rhs)
@@ -57,7 +57,7 @@ def test_project_bit_exact(oracle_ld, bc, shape, beta):
     nz, ny, nx = case.u.shape
     phi = inputs.normal_field(77, 0, (nz, ny, nx))
     p0 = inputs.normal_field(77, 1, (nz, ny, nx))
-    plan = Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     u, v, w, p, ph = (torch.from_numpy(a.copy()).cuda() for a in (case.u, case.v, case.w, p0, phi))
     plan.project(u, v, w, p, ph, case.alpha_dt, beta)
     torch.cuda.synchronize()
@@ -104,7 +104,7 @@ def test_poisson_out_of_place_and_manufactured(oracle_ld):
     dzc = np.diff(grid[5])[:, None, None]
     phi_true -= (phi_true * dzc).sum() / (dzc.sum() * nx * ny)
     rhs = oracle_ld.laplacian(grid, phi_true)
-    plan = Plan.from_grid(grid)
+    plan = make_plan(grid)
     r = torch.from_numpy(rhs).cuda()
     out = torch.empty_like(r)
     plan.poisson_solve(r, out)
@@ -147,7 +147,7 @@ def test_config3_three_substeps_reduced(oracle_ld, oracle_d):
     from paper_2103_15187_b200.binding import Plan
     shape = (128, 128, 384)
     cases = [inputs.make_case(3, shape=shape, substep=s) for s in range(3)]
-    plan = Plan.from_grid(cases[0].grid)
+    plan = make_plan(cases[0].grid)
     p = torch.zeros(cases[0].u.shape, dtype=torch.float64, device="cuda")
     phi = torch.empty_like(p)
     dev = [[torch.from_numpy(a).cuda() for a in (c.u, c.v, c.w)] for c in cases]
@@ -213,7 +213,7 @@ def test_runtime_argument_errors():
     torch = _torch()
     from paper_2103_15187_b200 import binding
     case = inputs.make_case(1, shape=(8, 8, 8))
-    plan = binding.Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     u = torch.zeros(case.u.shape, dtype=torch.float64, device="cuda")
     with pytest.raises(binding.FseiError) as e:
         plan.divergence(u, u, u, 0.0, torch.empty_like(u))
@@ -231,7 +231,7 @@ def test_host_buffer_entry(oracle_ld):
     torch = _torch()
     from paper_2103_15187_b200.binding import Plan
     case = inputs.make_case(1)
-    plan = Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     h = [torch.from_numpy(a.copy()).pin_memory() for a in (case.u, case.v, case.w, np.zeros_like(case.u))]
     plan.pressure_projection_host(*h, case.alpha_dt, 0.0)
     ref = gpu_projection(case)
@@ -242,7 +242,7 @@ def test_host_buffer_entry(oracle_ld):
 # ---------------------------------------------------------------------------------------------
 # fused path (blocked spectrum, Thomas sweeps inside the z-marching y kernels): chosen automatically for
 # grids with >= 128 x-slot tiles (configs[2..4] at full size); forced here on shapes the oracle finishes
-# in seconds through FSEI_PATH, which fsei_plan_create reads
+# in seconds through the flags of fsei_plan_create_ex (tests/util.plan_flags maps FSEI_PATH / FSEI_TWIST to them)
 # ---------------------------------------------------------------------------------------------
 @pytest.fixture
 def fused_path(monkeypatch):
@@ -258,7 +258,7 @@ def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
     from paper_2103_15187_b200.binding import Plan
     for cfg, beta in ((1, 0.0), (2, 1e-4)):
         case = inputs.make_case(cfg, shape=shape, bc=bc)
-        plan = Plan.from_grid(case.grid)
+        plan = make_plan(case.grid)
         got = gpu_projection(case, beta, plan=plan)
         assert plan.last_launch_count == 6                      # div+x, y+z fwd, special, z+y bwd, x inverse, project
         plan.destroy()
@@ -313,7 +313,7 @@ def test_fused_config5_grid_reduced(oracle_ld, oracle_d, fused_path):
 def test_fused_is_the_default_on_large_grids():
     from paper_2103_15187_b200.binding import Plan
     case = inputs.make_case(3, shape=(512, 512, 8))
-    plan = Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     got = gpu_projection(case, plan=plan)
     assert plan.last_launch_count == 6
     plan.destroy()
@@ -338,7 +338,7 @@ def _full_size_check(oracle_ld, cfg, launches):
     if avail < 120:
         pytest.skip(f"full-size oracle needs about 100 GB of host memory, {avail:.0f} GB available")
     case = inputs.make_case(cfg)
-    plan = Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     u, v, w = (torch.from_numpy(a).cuda() for a in (case.u, case.v, case.w))
     p = torch.zeros_like(u)
     phi = torch.empty_like(u)
@@ -394,7 +394,7 @@ def test_cuda_graph_capture_and_replay(monkeypatch, cfg, shape, path):
     if path:
         monkeypatch.setenv("FSEI_PATH", path)
     case = inputs.make_case(cfg, shape=shape)
-    plan = Plan.from_grid(case.grid)
+    plan = make_plan(case.grid)
     eager = gpu_projection(case, plan=plan)
     u0, v0, w0 = gpu_fields(case)
     u, v, w = u0.clone(), v0.clone(), w0.clone()
@@ -457,10 +457,10 @@ def test_deterministic_and_concurrent_plans(monkeypatch):
     from paper_2103_15187_b200.binding import Plan
     monkeypatch.setenv("FSEI_PATH", "fused")
     ca = inputs.make_case(2, shape=(512, 384, 16))
-    pa = Plan.from_grid(ca.grid)
+    pa = make_plan(ca.grid)
     monkeypatch.delenv("FSEI_PATH")
     cb = inputs.make_case(1, shape=(96, 72, 40), bc=(N, P))
-    pb = Plan.from_grid(cb.grid)
+    pb = make_plan(cb.grid)
     assert pa.workspace_bytes >= 8 * ca.cells                  # fused path: the blocked spectrum field is plan-owned
     ref_a, ref_b = gpu_projection(ca, plan=pa), gpu_projection(cb, plan=pb)
     again = gpu_projection(ca, plan=pa)

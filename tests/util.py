@@ -106,6 +106,23 @@ def div_gate(case, phi_absmax):
 
 
 # ---- CUDA path -----------------------------------------------------------------------------------
+def plan_flags() -> int:
+    """Test-only switches, read HERE (the library itself reads no environment variable): FSEI_PATH = generic|fast|fused
+    and FSEI_TWIST = 0|1 become flags of fsei_plan_create_ex."""
+    from paper_2103_15187_b200 import binding as b
+    f = {"generic": b.PATH_GENERIC, "fast": b.PATH_FAST, "fused": b.PATH_FUSED}.get(os.environ.get("FSEI_PATH", ""), 0)
+    tw = os.environ.get("FSEI_TWIST")
+    if tw is not None:
+        f |= b.TWIST_ON if tw == "1" else b.TWIST_OFF
+    return f
+
+
+def make_plan(grid):
+    from paper_2103_15187_b200.binding import Plan
+    return Plan.from_grid(grid, plan_flags())
+
+
+
 def gpu_fields(case):
     import torch
     dev = torch.device("cuda:0")
@@ -117,7 +134,7 @@ def gpu_projection(case, beta=0.0, plan=None, p=None, split=False):
     import torch
     from paper_2103_15187_b200.binding import Plan
     own = plan is None
-    plan = plan or Plan.from_grid(case.grid)
+    plan = plan or Plan.from_grid(case.grid, plan_flags())
     u, v, w = gpu_fields(case)
     p = torch.zeros_like(u) if p is None else p
     phi = torch.empty_like(u)
