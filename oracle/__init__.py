@@ -19,7 +19,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fsei_oracle.c")
-_SRCS = [_SRC, os.path.join(_HERE, "fsei_fluid_oracle.c")]   # projection; viscous step + explicit terms
+_SRCS = [_SRC, os.path.join(_HERE, "fsei_fluid_oracle.c"),    # projection; viscous step + explicit terms;
+         os.path.join(_HERE, "fsei_ibm_oracle.c")]            # IB-MLS transfer operators
 BC_PERIODIC, BC_NEUMANN = 0, 1
 
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -167,6 +168,53 @@ class Oracle:
                                                  float(gamma_dt), float(rho_dt), float(alpha_dt), float(beta)),
                   "explicit_terms")
         return r
+
+    # -- IB-MLS transfer operators (fsei_ibm_oracle.c) --------------------------------------------
+    def mls_weights(self, g, comp, xb, yb, zb):
+        """(idx[27], phi[27]) of one marker for component comp."""
+        a, keep = self._g(g)
+        idx = np.empty(27, dtype=np.int64); phi = np.empty(27)
+        self.lib.oracle_mls_weights.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 2 + [_dp] + [ctypes.c_int] * 3 + \
+            [ctypes.c_double] * 3 + [ctypes.c_void_p, _dp]
+        self._chk(self.lib.oracle_mls_weights(*a, int(comp), float(xb), float(yb), float(zb), idx.ctypes.data, _ptr(phi)), "mls_weights")
+        return idx, phi
+
+    def _markers(self, xm, ym, zm):
+        m = [np.ascontiguousarray(t, dtype=np.float64) for t in (xm, ym, zm)]
+        return m, ctypes.c_long(m[0].shape[0])
+
+    def mls_interpolate(self, g, xm, ym, zm, u, v, w):
+        a, keep = self._g(g)
+        m, n = self._markers(xm, ym, zm)
+        out = [np.empty(n.value) for _ in range(3)]
+        self.lib.oracle_mls_interpolate.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 2 + [_dp] + [ctypes.c_int] * 2 + \
+            [ctypes.c_long] + [_dp] * 9
+        self._chk(self.lib.oracle_mls_interpolate(*a, n, *[_ptr(t) for t in m], _ptr(u), _ptr(v), _ptr(w), *[_ptr(t) for t in out]),
+                  "mls_interpolate")
+        return out
+
+    def mls_spread(self, g, xm, ym, zm, area, F, f):
+        """f (3 fields) += spread of the marker forces F (3 arrays), in place."""
+        a, keep = self._g(g)
+        m, n = self._markers(xm, ym, zm)
+        area = np.ascontiguousarray(area, dtype=np.float64)
+        self.lib.oracle_mls_spread.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 2 + [_dp] + [ctypes.c_int] * 2 + \
+            [ctypes.c_long] + [_dp] * 10
+        self._chk(self.lib.oracle_mls_spread(*a, n, *[_ptr(t) for t in m], _ptr(area), *[_ptr(np.ascontiguousarray(t)) for t in F],
+                                             *[_ptr(t) for t in f]), "mls_spread")
+
+    def ibm_forcing(self, g, xm, ym, zm, area, V, u, v, w, inv_dt, f):
+        """f (3 fields) += IB forcing; returns the marker forces F (3 arrays)."""
+        a, keep = self._g(g)
+        m, n = self._markers(xm, ym, zm)
+        area = np.ascontiguousarray(area, dtype=np.float64)
+        F = [np.empty(n.value) for _ in range(3)]
+        self.lib.oracle_ibm_forcing.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 2 + [_dp] + [ctypes.c_int] * 2 + \
+            [ctypes.c_long] + [_dp] * 10 + [ctypes.c_double] + [_dp] * 6
+        self._chk(self.lib.oracle_ibm_forcing(*a, n, *[_ptr(t) for t in m], _ptr(area), *[_ptr(np.ascontiguousarray(t)) for t in V],
+                                              _ptr(u), _ptr(v), _ptr(w), float(inv_dt), *[_ptr(t) for t in F], *[_ptr(t) for t in f]),
+                  "ibm_forcing")
+        return F
 
     # -- building blocks ---------------------------------------------------------------------
     def dft(self, x: np.ndarray, sign: int) -> np.ndarray:

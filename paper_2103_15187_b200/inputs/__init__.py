@@ -142,6 +142,27 @@ def smooth_field(seed: int, stream: int, comp: str, grid, K: int, M: int = 48, o
 
 
 # --------------------------------------------------------------------------------------------
+# synthetic Lagrangian markers (stand-in for the paper's triangulated wet surfaces)
+# --------------------------------------------------------------------------------------------
+def sphere_markers(n: int, centre, radius: float, seed: int = 0, omega=(0.3, -0.2, 0.5), vel=(0.1, 0.0, -0.05)):
+    """n markers on a sphere (golden-angle spiral, rotated by a seeded phase): positions xm, ym, zm, the area each
+    marker stands for (4 pi R^2 / n, the paper's triangle areas) and the velocity of a rigid body (translation `vel` +
+    rotation `omega` about the centre) at each marker.  Returns (xm, ym, zm, area, (Vu, Vv, Vw)) as float64 arrays."""
+    rng = _Scalar(seed, 900)
+    ph0 = 2 * math.pi * rng.uniform()
+    l = np.arange(n, dtype=np.float64)
+    ct = 1.0 - 2.0 * (l + 0.5) / n
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = ph0 + l * math.pi * (3.0 - math.sqrt(5.0))
+    rx, ry, rz = radius * st * np.cos(ph), radius * st * np.sin(ph), radius * ct
+    xm, ym, zm = centre[0] + rx, centre[1] + ry, centre[2] + rz
+    area = np.full(n, 4.0 * math.pi * radius * radius / n)
+    V = (vel[0] + omega[1] * rz - omega[2] * ry, vel[1] + omega[2] * rx - omega[0] * rz, vel[2] + omega[0] * ry - omega[1] * rx)
+    return (np.ascontiguousarray(xm), np.ascontiguousarray(ym), np.ascontiguousarray(zm), area,
+            tuple(np.ascontiguousarray(t) for t in V))
+
+
+# --------------------------------------------------------------------------------------------
 # BASELINE.json configs (recipe table of DESIGN.md sec. 4)
 # --------------------------------------------------------------------------------------------
 RK3_ALPHA = (8.0 / 15.0, 2.0 / 15.0, 1.0 / 3.0)      # reading R10
