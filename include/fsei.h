@@ -178,6 +178,38 @@ int fsei_fluid_substep(fsei_plan* plan, double* u, double* v, double* w, double*
                        double* phi, double gamma_dt, double rho_dt, double alpha_dt, double beta, void* cuda_stream);
 
 /*
+ * ---- IB-MLS transfer operators (Eq. 4, Fig. 2; sec. 3.2) -----------------
+ * "A three-dimensional support domain consisting of N_e = n x n x n Eulerian nodes (n = 3 ...) is created around each
+ * Lagrangian marker, and the fluid velocity at the body position is computed interpolating ...
+ *      u_i(x_b) = sum_{k=1..N_e} phi_i^k(x_b) u_i(x_k)                                              (Eq. 4)
+ * ... a linear basis function is used, p^T(x) = [1, x, y, z], with an exponential weight function centered at the
+ * location of the Lagrangian marker.  The interpolated velocity is used to compute the IB force at the exact location
+ * of the marker which is then transferred back to the Eulerian grid-points as a distributed forcing ... for the three
+ * velocity components."  Support, weight, force and spreading scale: readings M1..M8 of DESIGN.md sec. 3.
+ *
+ * Markers: n >= 0 markers as DEVICE arrays xm, ym, zm (coordinates; taken modulo the period in a periodic direction;
+ * in a wall direction the support is clamped inside the box), area (the surface area each marker stands for).
+ * Marker values (ub.., Fu.., Vu..) are DEVICE arrays of n doubles per component.  nz >= 3            else FSEI_ERR_SIZE
+ *
+ *   fsei_mls_interpolate : ub[l] = sum_k phi^k u(x_k) on u's staggered nodes; vb, wb alike.               (Eq. 4)
+ *   fsei_mls_spread      : fu(x_k) += c_l phi^k Fu[l], c_l = area[l] h_l / sum_k phi^k dV_k (total force conserved);
+ *                          fv, fw alike.  fp64 atomic adds: the sum over markers has no fixed order.
+ *   fsei_ibm_forcing     : Fu[l] = (Vu[l] - ub[l]) * inv_dt (out), then the spreading of Fu into fu (+=); v, w alike:
+ *                          the IB forcing f of Eq. 3 that fsei_explicit_terms takes as fu, fv, fw.  One kernel.
+ * The forcing fields must not alias the velocity fields                                              else FSEI_ERR_ARG
+ */
+int fsei_mls_interpolate(fsei_plan* plan, long n, const double* xm, const double* ym, const double* zm,
+                         const double* u, const double* v, const double* w, double* ub, double* vb, double* wb,
+                         void* cuda_stream);
+int fsei_mls_spread(fsei_plan* plan, long n, const double* xm, const double* ym, const double* zm, const double* area,
+                    const double* Fu, const double* Fv, const double* Fw, double* fu, double* fv, double* fw,
+                    void* cuda_stream);
+int fsei_ibm_forcing(fsei_plan* plan, long n, const double* xm, const double* ym, const double* zm, const double* area,
+                     const double* Vu, const double* Vv, const double* Vw, const double* u, const double* v, const double* w,
+                     double inv_dt, double* Fu, double* Fv, double* Fw, double* fu, double* fv, double* fw,
+                     void* cuda_stream);
+
+/*
  * Kernel-level timing aid for bench.py: number of kernels enqueued by the last
  * fsei_pressure_projection / fsei_poisson_solve call on this plan.
  */

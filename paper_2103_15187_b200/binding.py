@@ -20,7 +20,8 @@ EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family",
            "fsei_plan_workspace_bytes", "fsei_divergence", "fsei_poisson_solve", "fsei_project",
            "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
            "fsei_plan_profile", "fsei_plan_profile_read",
-           "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep")
+           "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep",
+           "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing")
 
 _lib = None
 _vp, _d, _i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
@@ -82,6 +83,12 @@ def lib() -> ctypes.CDLL:
     L.fsei_viscous_step.argtypes = [_vp] * 7 + [_d, _vp]
     L.fsei_fluid_substep.restype = _i
     L.fsei_fluid_substep.argtypes = [_vp] * 15 + [_d] * 4 + [_vp]
+    L.fsei_mls_interpolate.restype = _i
+    L.fsei_mls_interpolate.argtypes = [_vp, ctypes.c_long] + [_vp] * 9 + [_vp]
+    L.fsei_mls_spread.restype = _i
+    L.fsei_mls_spread.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_vp]
+    L.fsei_ibm_forcing.restype = _i
+    L.fsei_ibm_forcing.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_d] + [_vp] * 6 + [_vp]
     _lib = L
     return L
 
@@ -207,3 +214,16 @@ class Plan:
         _chk(lib().fsei_fluid_substep(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), *[_optr(t) for t in f], _ptr(hu), _ptr(hv),
                                       _ptr(hw), _ptr(ru), _ptr(rv), _ptr(rw), _ptr(phi), float(gamma_dt), float(rho_dt),
                                       float(alpha_dt), float(beta), _stream(stream)))
+
+    def mls_interpolate(self, n, xm, ym, zm, u, v, w, ub, vb, wb, stream=None):
+        _chk(lib().fsei_mls_interpolate(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(u), _ptr(v), _ptr(w), _ptr(ub),
+                                        _ptr(vb), _ptr(wb), _stream(stream)))
+
+    def mls_spread(self, n, xm, ym, zm, area, Fu, Fv, Fw, fu, fv, fw, stream=None):
+        _chk(lib().fsei_mls_spread(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(area), _ptr(Fu), _ptr(Fv), _ptr(Fw),
+                                   _ptr(fu), _ptr(fv), _ptr(fw), _stream(stream)))
+
+    def ibm_forcing(self, n, xm, ym, zm, area, Vu, Vv, Vw, u, v, w, inv_dt, Fu, Fv, Fw, fu, fv, fw, stream=None):
+        _chk(lib().fsei_ibm_forcing(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(area), _ptr(Vu), _ptr(Vv), _ptr(Vw),
+                                    _ptr(u), _ptr(v), _ptr(w), float(inv_dt), _ptr(Fu), _ptr(Fv), _ptr(Fw), _ptr(fu), _ptr(fv),
+                                    _ptr(fw), _stream(stream)))

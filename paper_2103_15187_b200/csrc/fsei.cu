@@ -22,6 +22,7 @@
 #include "zfast.cuh"
 #include "stencil_fast.cuh"
 #include "fluid.cuh"
+#include "ibm.cuh"
 #include <cmath>
 #include <cstdlib>
 
@@ -43,7 +44,7 @@ static bool misaligned(const void* p) { return (reinterpret_cast<size_t>(p) & 15
 // ------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------
-enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, FSEI_NKERNELS };
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, K_MLS, FSEI_NKERNELS };
 
 struct fsei_plan {
     HostTables T;
@@ -58,6 +59,7 @@ struct fsei_plan {
     int LX = 1, CY = 1;                // tile shapes
     size_t smem_x = 0, smem_y = 0;
     int last_launches = 0;
+    const double* zc_dev = nullptr;      // z-face coordinates (IB-MLS node positions)
     double* vtab = nullptr; int vnmax = 0; double visc_beta = NAN;   // implicit viscous step: factorisation tables of the last beta
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
     // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
@@ -71,7 +73,7 @@ struct fsei_plan {
 
 static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
                                                    "y_inverse", "x_inverse", "project", "div_x_forward", "yz_forward", "yz_backward",
-                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z"};
+                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z", "ib_mls"};
 
 // record an event pair around one launch when profiling is on
 struct LaunchTimer {
@@ -267,6 +269,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     S.nx = nx; S.ny = ny; S.nz = nz; S.bcx = bcx; S.bcy = bcy; S.rdx = T.rdx; S.rdy = T.rdy;
     if ((rc = upload(P, T.rdzc, &S.rdzc))) return rc;
     if ((rc = upload(P, T.rdzm, &S.rdzm))) return rc;
+    { std::vector<double> zcv(zc, zc + nz + 1); if ((rc = upload(P, zcv, &P->zc_dev))) return rc; }
     {
         P->vnmax = nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz);
         void* q = nullptr;
@@ -736,6 +739,62 @@ extern "C" int fsei_fluid_substep(fsei_plan* P, double* u, double* v, double* w,
     n += P->last_launches;
     P->last_launches = n;
     return FSEI_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// IB-MLS transfer operators
+// ------------------------------------------------------------------------------------------
+static MlsGrid mls_grid(const fsei_plan* P)
+{
+    const HostTables& T = P->T;
+    MlsGrid G;
+    G.nx = T.nx; G.ny = T.ny; G.nz = T.nz; G.bcx = T.bcx; G.bcy = T.bcy;
+    G.dx = T.Lx / T.nx; G.dy = T.Ly / T.ny; G.Lx = T.Lx; G.Ly = T.Ly; G.zc = P->zc_dev;
+    return G;
+}
+
+template <int MODE> static int mls_launch(fsei_plan* P, const MlsArgs& A, cudaStream_t st)
+{
+    if (A.n == 0) { P->last_launches = 0; return FSEI_OK; }
+    { LaunchTimer t(P, K_MLS, st); k_mls<MODE><<<(unsigned)((3 * A.n + 127) / 128), 128, 0, st>>>(A); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_mls_interpolate(fsei_plan* P, long n, const double* xm, const double* ym, const double* zm,
+                                    const double* u, const double* v, const double* w, double* ub, double* vb, double* wb,
+                                    void* cuda_stream)
+{
+    if (!P || n < 0 || (n > 0 && (!xm || !ym || !zm || !u || !v || !w || !ub || !vb || !wb))) return fail(FSEI_ERR_ARG, "fsei_mls_interpolate: NULL argument or n < 0");
+    if (P->T.nz < 3) return fail(FSEI_ERR_SIZE, "fsei_mls_interpolate: the 27-node support needs nz >= 3");
+    MlsArgs A{mls_grid(P), n, xm, ym, zm, nullptr, {u, v, w}, {nullptr, nullptr, nullptr}, {ub, vb, wb}, {nullptr, nullptr, nullptr}, 0.0};
+    return mls_launch<0>(P, A, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int fsei_mls_spread(fsei_plan* P, long n, const double* xm, const double* ym, const double* zm, const double* area,
+                               const double* Fu, const double* Fv, const double* Fw, double* fu, double* fv, double* fw,
+                               void* cuda_stream)
+{
+    if (!P || n < 0 || (n > 0 && (!xm || !ym || !zm || !area || !Fu || !Fv || !Fw || !fu || !fv || !fw))) return fail(FSEI_ERR_ARG, "fsei_mls_spread: NULL argument or n < 0");
+    if (P->T.nz < 3) return fail(FSEI_ERR_SIZE, "fsei_mls_spread: the 27-node support needs nz >= 3");
+    MlsArgs A{mls_grid(P), n, xm, ym, zm, area, {nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr},
+              {const_cast<double*>(Fu), const_cast<double*>(Fv), const_cast<double*>(Fw)}, {fu, fv, fw}, 0.0};
+    return mls_launch<2>(P, A, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int fsei_ibm_forcing(fsei_plan* P, long n, const double* xm, const double* ym, const double* zm, const double* area,
+                                const double* Vu, const double* Vv, const double* Vw, const double* u, const double* v,
+                                const double* w, double inv_dt, double* Fu, double* Fv, double* Fw, double* fu, double* fv,
+                                double* fw, void* cuda_stream)
+{
+    if (!P || n < 0 || (n > 0 && (!xm || !ym || !zm || !area || !Vu || !Vv || !Vw || !u || !v || !w || !Fu || !Fv || !Fw || !fu || !fv || !fw)))
+        return fail(FSEI_ERR_ARG, "fsei_ibm_forcing: NULL argument or n < 0");
+    if (inv_dt != inv_dt) return fail(FSEI_ERR_ARG, "fsei_ibm_forcing: NaN inv_dt");
+    if (fu == u || fu == v || fu == w || fv == u || fv == v || fv == w || fw == u || fw == v || fw == w) return fail(FSEI_ERR_ARG, "fsei_ibm_forcing: the forcing fields must not alias the velocity");
+    if (P->T.nz < 3) return fail(FSEI_ERR_SIZE, "fsei_ibm_forcing: the 27-node support needs nz >= 3");
+    MlsArgs A{mls_grid(P), n, xm, ym, zm, area, {u, v, w}, {Vu, Vv, Vw}, {Fu, Fv, Fw}, {fu, fv, fw}, inv_dt};
+    return mls_launch<1>(P, A, static_cast<cudaStream_t>(cuda_stream));
 }
 
 // ------------------------------------------------------------------------------------------
