@@ -43,6 +43,8 @@ ALGO_BYTES_PER_CELL = {
     # fluid substep: u,v,w,p + 3 Hprev in, 3 H + 3 rhs out; generic sweeps in place,
     # forward + backward pass each (the z sweep also reads and writes the velocity component)
     "explicit_terms": 104.0, "visc_x": 32.0, "visc_y": 32.0, "visc_z": 40.0, "visc_factor": 0.0,
+    # fast viscous family, three components per launch: rhs -> d' in place (3 x 16); d' + q in, q out (3 x 24)
+    "visc_xz": 48.0, "visc_zy": 72.0, "ib_mls": 0.0,
 }
 A_REF = 184.0          # unfused reference accounting of one projection, B/cell
 SLAB_NY = 64           # single-thread CPU leg: the workload's grid with ny cut to this many rows

@@ -71,11 +71,12 @@ fsei_plan*  fsei_plan_create(int nx, int ny, int nz, double Lx, double Ly,
  *       a family that has no instantiation for the size falls back to the next simpler one; FUSED with a line length
  *       whose landing tile exceeds the TMA box limit fails with FSEI_ERR_CUDA)
  *   FSEI_PLAN_TWIST_OFF / FSEI_PLAN_TWIST_ON : the twisted factorisation of the fused family
+ *   FSEI_PLAN_VISC_GENERIC : fsei_viscous_step uses its generic kernels even where the fast family applies
  *   FSEI_PLAN_HOST_FIELDS : allocate, now, the five device fields fsei_pressure_projection_host stages through
  * Unknown flag bits -> FSEI_ERR_ARG.  fsei_plan_create(...) == fsei_plan_create_ex(..., 0).
  */
 enum { FSEI_PLAN_PATH_GENERIC = 1, FSEI_PLAN_PATH_FAST = 2, FSEI_PLAN_PATH_FUSED = 3, FSEI_PLAN_PATH_MASK = 3,
-       FSEI_PLAN_TWIST_OFF = 4, FSEI_PLAN_TWIST_ON = 8, FSEI_PLAN_HOST_FIELDS = 16 };
+       FSEI_PLAN_TWIST_OFF = 4, FSEI_PLAN_TWIST_ON = 8, FSEI_PLAN_HOST_FIELDS = 16, FSEI_PLAN_VISC_GENERIC = 32 };
 fsei_plan*  fsei_plan_create_ex(int nx, int ny, int nz, double Lx, double Ly, const double* zc /* HOST, nz+1 */,
                                 int bc_x, int bc_y, unsigned flags);
 /* Kernel family the plan chose: 0 generic, 1 fast, 2 fused; +4 when the twisted factorisation is on; < 0: -FSEI_ERR_ARG. */
@@ -163,8 +164,10 @@ int fsei_explicit_terms(fsei_plan* plan, const double* u, const double* v, const
  * the staggered position of each component with no-slip walls (V3-V6); wall faces are never modified.
  *   ru, rv, rw : in: right-hand sides; DESTROYED (used as scratch).  beta >= 0 finite    else FSEI_ERR_ARG
  *   No field may alias another.  Any nx, ny, nz the plan accepts; both boundary types.
- * The factorisation tables for `beta` are rebuilt on the device (one extra small launch) whenever beta differs from
- * the previous call on this plan.
+ * The factorisation tables for `beta` are rebuilt (one extra small launch, plus a few microseconds of host work)
+ * whenever beta differs from the previous call on this plan.  Two kernel families: periodic x
+ * and y with nx/32 in {2,4,8,12,16,24,32} and ny/32 in {2,3,4,6,8,12,16,24,32} run two fused launches for the three
+ * components (40 B/cell each); any other grid runs the generic sweeps (nine launches).
  */
 int fsei_viscous_step(fsei_plan* plan, double* u, double* v, double* w, double* ru, double* rv, double* rw,
                       double beta, void* cuda_stream);

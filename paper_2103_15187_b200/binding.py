@@ -14,7 +14,7 @@ from . import build as _build
 BC_PERIODIC, BC_NEUMANN = 0, 1
 OK, ERR_ARG, ERR_SIZE, ERR_GRID, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4, 5
 
-PATH_GENERIC, PATH_FAST, PATH_FUSED, TWIST_OFF, TWIST_ON, HOST_FIELDS = 1, 2, 3, 4, 8, 16     # fsei_plan_create_ex flags
+PATH_GENERIC, PATH_FAST, PATH_FUSED, TWIST_OFF, TWIST_ON, HOST_FIELDS, VISC_GENERIC = 1, 2, 3, 4, 8, 16, 32     # fsei_plan_create_ex flags
 
 EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family", "fsei_plan_destroy", "fsei_last_error", "fsei_last_error_code",
            "fsei_plan_workspace_bytes", "fsei_divergence", "fsei_poisson_solve", "fsei_project",

@@ -41,6 +41,14 @@ cudaError_t launch_xf_fast(const XFast& P, const SParams& S, bool neu, bool fuse
                            const double* w, double inv_adt, cplx* spec, cudaStream_t st, bool blocked = false);
 cudaError_t launch_xi_fast(const XFast& P, bool neu, const cplx* spec, double* phi, cudaStream_t st,
                            const TmaMap3D* map = nullptr);
+// fast family of the implicit viscous step (visc_fast.cuh): periodic x and y, nx/32 and ny/32 instantiated
+struct VFastLine; struct VFastArgs;
+bool visc_fast_supported(int nx, int ny);
+cudaError_t visc_fast_init();
+void visc_fast_line(int n, double h_recip, double beta, VFastLine* out);
+cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st);
+cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st);
+
 // a3 / a5, in place
 cudaError_t launch_y_fast(const YFast& P, bool inv, bool neu, cplx* spec, cudaStream_t st);
 

@@ -1,0 +1,114 @@
+// fast_visc.cu -- instantiations, host-side line tables and launchers of the fast viscous family (visc_fast.cuh).
+#include <cuda_runtime.h>
+#include <cmath>
+#include "visc_fast.cuh"
+#include "fast_launch.hpp"
+
+namespace fsei {
+
+// chunk lengths with an instantiation: pass A needs M % 4 == 0 (conflict-free 128-bit slots; 2 for small test grids)
+#define FSEI_VA_LIST(X) X(2) X(4) X(8) X(12) X(16) X(24) X(32)
+#define FSEI_VB_LIST(X) X(2) X(3) X(4) X(6) X(8) X(12) X(16) X(24) X(32)
+
+bool visc_fast_supported(int nx, int ny)
+{
+    if (nx % 32 || ny % 32 || nx % 8) return false;
+    bool a = false, b = false;
+#define X(M) if (nx / 32 == M) a = true;
+    FSEI_VA_LIST(X)
+#undef X
+#define X(M) if (ny / 32 == M) b = true;
+    FSEI_VB_LIST(X)
+#undef X
+    return a && b;
+}
+
+static size_t va_smem(int M) { return (size_t)FSEI_VA_WPB * (FSEI_VA_STAGES * 32 * (8 * M + 16) + 64); }
+
+cudaError_t visc_fast_init()
+{
+    cudaError_t e = cudaSuccess;
+#define X(M) if (e == cudaSuccess) e = kernel_smem(k_visc_xz<M>, (int)va_smem(M));
+    FSEI_VA_LIST(X)
+#undef X
+    return e;
+}
+
+// Tables of one uniform periodic line of n = 32 M unknowns, (1 + 2r) on the diagonal and -r beside it, in long double
+void visc_fast_line(int n, double h_recip, double beta, VFastLine* out)
+{
+    const int M = n / 32, Mi = M - 1;
+    const long double r = (long double)beta * (long double)h_recip * (long double)h_recip, b = 1.0L + 2.0L * r;
+    long double ip[32], cp[32], ls[32], rs[32];
+    // interior factorisation: piv_0 = b, piv_i = b - (-r) c'_{i-1}, c'_i = -r / piv_i
+    for (int i = 0; i < Mi; i++) {
+        const long double piv = i == 0 ? b : b + r * cp[i - 1];
+        ip[i] = 1.0L / piv; cp[i] = -r * ip[i];
+    }
+    // spikes: T ls = r e_0, T rs = r e_{Mi-1}
+    for (int which = 0; which < 2; which++) {
+        long double y[32];
+        for (int i = 0; i < Mi; i++) {
+            const long double d = ((which == 0 && i == 0) || (which == 1 && i == Mi - 1)) ? r : 0.0L;
+            y[i] = (i == 0 ? d : d + r * y[i - 1]) * ip[i];
+        }
+        for (int i = Mi - 2; i >= 0; i--) y[i] -= cp[i] * y[i + 1];
+        for (int i = 0; i < Mi; i++) (which == 0 ? ls : rs)[i] = y[i];
+    }
+    // separator system: circulant tridiagonal, diag sd, off-diagonals so (both sides); dense solve S z = e_0
+    long double sd = b, so = -r;
+    if (Mi > 0) { sd = b - r * (rs[Mi - 1] + ls[0]); so = -r * ls[Mi - 1]; }
+    long double S[32][33];
+    for (int p = 0; p < 32; p++) {
+        for (int q = 0; q < 33; q++) S[p][q] = 0.0L;
+        S[p][p] += sd; S[p][(p + 1) & 31] += so; S[p][(p + 31) & 31] += so;
+    }
+    S[0][32] = 1.0L;
+    for (int c = 0; c < 32; c++) {
+        int piv = c;
+        for (int p = c + 1; p < 32; p++) if (fabsl(S[p][c]) > fabsl(S[piv][c])) piv = p;
+        if (piv != c) for (int q = 0; q < 33; q++) { const long double t = S[c][q]; S[c][q] = S[piv][q]; S[piv][q] = t; }
+        for (int p = c + 1; p < 32; p++) {
+            const long double m = S[p][c] / S[c][c];
+            if (m != 0.0L) for (int q = c; q < 33; q++) S[p][q] -= m * S[c][q];
+        }
+    }
+    long double z[32];
+    for (int c = 31; c >= 0; c--) {
+        long double s = S[c][32];
+        for (int q = c + 1; q < 32; q++) s -= S[c][q] * z[q];
+        z[c] = s / S[c][c];
+    }
+    out->r = (double)r;
+    for (int i = 0; i < 31; i++) {
+        out->ip[i] = i < Mi ? (double)ip[i] : 0.0; out->cp[i] = i < Mi ? (double)cp[i] : 0.0;
+        out->ls[i] = i < Mi ? (double)ls[i] : 0.0; out->rs[i] = i < Mi ? (double)rs[i] : 0.0;
+    }
+    for (int s = 0; s < 32; s++) out->sinv[s] = (double)z[s];      // S^-1[p][q] = z[(p - q) mod 32]
+}
+
+cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st)
+{
+    const dim3 grid((A.ny + FSEI_VA_WPB - 1) / FSEI_VA_WPB, 3);
+    switch (A.nx / 32) {
+#define X(M) case M: k_visc_xz<M><<<grid, 32 * FSEI_VA_WPB, va_smem(M), st>>>(A); break;
+        FSEI_VA_LIST(X)
+#undef X
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st)
+{
+    const dim3 grid(A.nx / 8, 3);
+    switch (A.ny / 32) {
+#define X(M) case M: k_visc_zy<M><<<grid, 256, 0, st>>>(A); break;
+        FSEI_VB_LIST(X)
+#undef X
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace fsei

@@ -19,7 +19,6 @@
 
 namespace fsei {
 
-enum { COMP_U = 0, COMP_V = 1, COMP_W = 2, DIR_X = 0, DIR_Y = 1, DIR_Z = 2 };
 
 // ---------------------------------------------------------------------------------------------------------------
 // implicit step: factorisation tables of one (component, direction)

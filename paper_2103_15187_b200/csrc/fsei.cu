@@ -23,6 +23,7 @@
 #include "stencil_fast.cuh"
 #include "fluid.cuh"
 #include "ibm.cuh"
+#include "visc_fast.cuh"
 #include <cmath>
 #include <cstdlib>
 
@@ -44,7 +45,7 @@ static bool misaligned(const void* p) { return (reinterpret_cast<size_t>(p) & 15
 // ------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------
-enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, K_MLS, FSEI_NKERNELS };
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, K_MLS, K_VXZ, K_VZY, FSEI_NKERNELS };
 
 struct fsei_plan {
     HostTables T;
@@ -60,6 +61,7 @@ struct fsei_plan {
     size_t smem_x = 0, smem_y = 0;
     int last_launches = 0;
     const double* zc_dev = nullptr;      // z-face coordinates (IB-MLS node positions)
+    bool visc_fast = false; VFastLine vline_x, vline_y;   // fast viscous family: host-built line tables of the last beta
     double* vtab = nullptr; int vnmax = 0; double visc_beta = NAN;   // implicit viscous step: factorisation tables of the last beta
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
     // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
@@ -73,7 +75,7 @@ struct fsei_plan {
 
 static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
                                                    "y_inverse", "x_inverse", "project", "div_x_forward", "yz_forward", "yz_backward",
-                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z", "ib_mls"};
+                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z", "ib_mls", "visc_xz", "visc_zy"};
 
 // record an event pair around one launch when profiling is on
 struct LaunchTimer {
@@ -232,7 +234,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     // fast path: line lengths with a register-resident Stockham instantiation, special columns fit in shared memory
     // fused path: the fast path on the blocked layout, where one CTA per x-slot tile marches along z -- for grids
     // with enough tiles to fill the GPU.  flags (fsei_plan_create_ex) may override the choice, per plan.
-    if (flags & ~(unsigned)(FSEI_PLAN_PATH_MASK | FSEI_PLAN_TWIST_OFF | FSEI_PLAN_TWIST_ON | FSEI_PLAN_HOST_FIELDS)) return fail(FSEI_ERR_ARG, "fsei_plan_create_ex: unknown flag");
+    if (flags & ~(unsigned)(FSEI_PLAN_PATH_MASK | FSEI_PLAN_TWIST_OFF | FSEI_PLAN_TWIST_ON | FSEI_PLAN_HOST_FIELDS | FSEI_PLAN_VISC_GENERIC)) return fail(FSEI_ERR_ARG, "fsei_plan_create_ex: unknown flag");
     if ((flags & FSEI_PLAN_TWIST_OFF) && (flags & FSEI_PLAN_TWIST_ON)) return fail(FSEI_ERR_ARG, "fsei_plan_create_ex: TWIST_OFF and TWIST_ON are exclusive");
     const unsigned pf = flags & FSEI_PLAN_PATH_MASK;
     const std::string want = pf == FSEI_PLAN_PATH_GENERIC ? "generic" : (pf == FSEI_PLAN_PATH_FAST ? "fast" : (pf == FSEI_PLAN_PATH_FUSED ? "fused" : ""));
@@ -275,6 +277,8 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         void* q = nullptr;
         if ((rc = dalloc(P, sizeof(double) * 9 * vtab_set_doubles(P->vnmax), &q))) return rc;
         P->vtab = static_cast<double*>(q);
+        P->visc_fast = !(flags & FSEI_PLAN_VISC_GENERIC) && bcx == BC_PERIODIC && bcy == BC_PERIODIC && visc_fast_supported(nx, ny);
+        if (P->visc_fast) CU(visc_fast_init());
     }
 
     if (fast) {
@@ -692,7 +696,25 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
         VFactorArgs A{P->S, beta, P->vtab, P->vnmax};
         { LaunchTimer t(P, K_VFACT, st); k_visc_factor<<<9, 32, 0, st>>>(A); }
         CU(cudaGetLastError());
+        if (P->visc_fast) {
+            visc_fast_line(T.nx, P->S.rdx, beta, &P->vline_x);
+            visc_fast_line(T.ny, P->S.rdy, beta, &P->vline_y);
+        }
         P->visc_beta = beta; launches++;
+    }
+    if (P->visc_fast) {
+        VFastArgs A;
+        for (int c = 0; c < 3; c++) {
+            const VTab V = visc_tab(P, c, DIR_Z);
+            A.zam[c] = V.am; A.zip[c] = V.ip; A.zcp[c] = V.cp; A.r[c] = r[c]; A.q[c] = q[c];
+        }
+        A.nx = T.nx; A.ny = T.ny; A.nz = T.nz;
+        A.L = P->vline_x;
+        { LaunchTimer t(P, K_VXZ, st); CU(launch_visc_xz(A, st)); }
+        A.L = P->vline_y;
+        { LaunchTimer t(P, K_VZY, st); CU(launch_visc_zy(A, st)); }
+        P->last_launches = launches + 2;
+        return FSEI_OK;
     }
     const long nlx = (long)T.ny * T.nz, nly = (long)T.nx * T.nz, nlz = (long)T.nx * T.ny;
     const size_t plane = (size_t)T.nx * T.ny;

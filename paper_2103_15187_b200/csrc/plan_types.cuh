@@ -6,6 +6,7 @@
 namespace fsei {
 
 enum { BC_PERIODIC = 0, BC_NEUMANN = 1 };
+enum { COMP_U = 0, COMP_V = 1, COMP_W = 2, DIR_X = 0, DIR_Y = 1, DIR_Z = 2 };   // velocity components, directions
 
 // Transform along x: real lines of n = nx values handled as N = nx/2 complex values.
 //   periodic: real-to-complex FFT, slot pos[k] holds X_k (k = 1..N-1), slot 0 holds (X_0, X_N) (both real)

@@ -1,0 +1,210 @@
+// visc_fast.cuh -- fast family of the implicit viscous step (Eq. 3) for the paper's own
+// case: periodic, uniform x and y ("Thomas' algorithm with a Sherman-Morrison perturbation in the two periodic
+// dimensions"), stretched wall-normal z.
+//
+//   q += [(1 - beta dxx)(1 - beta dyy)(1 - beta dzz)]^-1 rhs      (the three factors commute: each acts on its own index)
+//
+// TWO launches move each component 40 B/cell (the generic family: six passes, 104 B/cell):
+//   pass A  k_visc_xz : one WARP owns one x-line and marches k = 0 .. nz-1.  Per plane the line arrives by 32 bulk
+//           copies (cp.async.bulk, one 8M-byte chunk per lane into a padded slot: conflict-free 128-bit reads), is solved
+//           in REGISTERS (lane = chunk of M = nx/32 unknowns) and goes straight through the forward elimination of the
+//           z system, whose previous row d'(k-1) is carried in registers; d' leaves by bulk stores.  rhs -> d' in place.
+//   pass B  k_visc_zy : one CTA owns 8 adjacent columns x all ny rows and marches k = nz-1 .. 0: back substitution of
+//           the z system with x(k+1) carried in registers, then the periodic y-solve of the tile (thread = one column x
+//           one chunk of M = ny/32 rows, lanes along x: 64-byte row segments), then q += result.
+//
+// A periodic line of n = 32 M unknowns is solved by a PARTITION method instead of a serial sweep: each of the 32 chunks
+// eliminates its M-1 interior unknowns against its two separators with a local Thomas solve (the matrix has constant
+// coefficients, so factorisation and spikes are the same for every chunk: warp-uniform constants in the kernel
+// parameter bank), the 32 separators obey a circulant tridiagonal system whose inverse is ONE row of 32 numbers (built on
+// the host per beta, in long double), applied by 32 shuffles (x) or 32 shared-memory reads (y), and the interiors are
+// corrected with the two spikes.  Exact up to rounding (no truncation of the decay), ~7 FMA per unknown.
+#pragma once
+#include "kernel_env.cuh"
+#include "plan_types.cuh"
+
+namespace fsei {
+
+// uniform periodic line: a = c = -r, b = 1 + 2r (r = beta / h^2); M = n / 32 unknowns per chunk, the last one the separator
+struct VFastLine {
+    double r;
+    double ip[31], cp[31];      // interior Thomas factorisation: reciprocal pivots, c'_i      (entries < M-1)
+    double ls[31], rs[31];      // spikes: interior response to a unit left / right separator  (entries < M-1)
+    double sinv[32];            // first row of the inverse of the 32 x 32 circulant separator system
+};
+
+struct VFastArgs {
+    VFastLine L;                // x line (pass A) or y line (pass B)
+    const double* zam[3];       // z tables of u, v, w (device): sub-diagonal, reciprocal pivot, c'
+    const double* zip[3];
+    const double* zcp[3];
+    double* r[3];               // right-hand sides: rhs -> d' (pass A, in place); d' read by pass B
+    double* q[3];               // velocity components (pass B)
+    int nx, ny, nz;
+};
+
+#if defined(__CUDACC__)
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// interior solve of one chunk, in place: x[0 .. M-2] -> y = T^-1 x   (T: constant-coefficient tridiagonal of size M-1)
+template <int M> __device__ __forceinline__ void chunk_interior(const VFastLine& L, double (&x)[M])
+{
+    x[0] *= L.ip[0];
+#pragma unroll
+    for (int i = 1; i < M - 1; i++) x[i] = fma(L.r, x[i - 1], x[i]) * L.ip[i];
+#pragma unroll
+    for (int i = M - 3; i >= 0; i--) x[i] = fma(-L.cp[i], x[i + 1], x[i]);
+}
+// interiors corrected with the separators to their left (xl) and right (xs); the separator itself stored last
+template <int M> __device__ __forceinline__ void chunk_correct(const VFastLine& L, double (&x)[M], double xl, double xs)
+{
+#pragma unroll
+    for (int i = 0; i < M - 1; i++) x[i] = fma(L.rs[i], xs, fma(L.ls[i], xl, x[i]));
+    x[M - 1] = xs;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pass A: grid (ny / WPB, 3), block 32 * WPB.  Dynamic shared memory: WPB * (S * 32 * (8 M + 16) + 8 S) bytes.
+// ---------------------------------------------------------------------------------------------------------------
+#define FSEI_VA_STAGES 3
+#define FSEI_VA_WPB 2
+
+template <int M>
+FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
+{
+    constexpr int S = FSEI_VA_STAGES, PITCH = 8 * M + 16, STAGE = 32 * PITCH;
+    FSEI_DYN_SMEM(smraw);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, comp = blockIdx.y;
+    const int j = blockIdx.x * FSEI_VA_WPB + wid;
+    if (j >= A.ny) return;
+    unsigned char* buf = smraw + (size_t)wid * (S * STAGE + 64);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(buf + S * STAGE);
+    const size_t plane = (size_t)A.nx * A.ny;
+    double* f = A.r[comp] + (size_t)j * A.nx + (size_t)lane * M;          // this lane's chunk of line j at plane 0
+    const double* __restrict__ zam = A.zam[comp];
+    const double* __restrict__ zip = A.zip[comp];
+    const VFastLine& L = A.L;
+    if (lane == 0) for (int s = 0; s < S; s++) abar_init(bar + s);
+    __syncwarp();
+    // prologue: planes 0 .. S-2 in flight
+    for (int s = 0; s < S - 1 && s < A.nz; s++) {
+        if (lane == 0) abar_expect(bar + s, 32 * 8 * M);
+        __syncwarp();
+        bulk_g2s(buf + s * STAGE + lane * PITCH, f + (size_t)s * plane, 8 * M, bar + s);
+    }
+    double dprev[M];
+#pragma unroll
+    for (int i = 0; i < M; i++) dprev[i] = 0.0;
+    const bool wfix = comp == COMP_W;                                       // w: plane 0 is the wall (row fixed)
+    for (int k = 0; k < A.nz; k++) {
+        const int st = k % S;
+        abar_wait(bar + st, (k / S) & 1);
+        double x[M];
+        const double2* src = reinterpret_cast<const double2*>(buf + st * STAGE + lane * PITCH);
+#pragma unroll
+        for (int i = 0; i < M / 2; i++) { const double2 t = src[i]; x[2 * i] = t.x; x[2 * i + 1] = t.y; }
+        // ---- periodic x-solve of the line
+        const double sep = x[M - 1];
+        chunk_interior<M>(L, x);
+        const double y0n = __shfl_sync(0xffffffffu, x[0], (lane + 1) & 31);
+        const double g = fma(L.r, x[M - 2] + y0n, sep);
+        double xs0 = 0.0, xs1 = 0.0;
+#pragma unroll
+        for (int s = 0; s < 32; s += 2) {
+            xs0 = fma(L.sinv[s], __shfl_sync(0xffffffffu, g, (lane - s) & 31), xs0);
+            xs1 = fma(L.sinv[s + 1], __shfl_sync(0xffffffffu, g, (lane - s - 1) & 31), xs1);
+        }
+        const double xs = xs0 + xs1;
+        const double xl = __shfl_sync(0xffffffffu, xs, (lane - 1) & 31);
+        chunk_correct<M>(L, x, xl, xs);
+        // ---- forward elimination of the z system: d'_k = (x_k - a_k d'_{k-1}) / piv_k
+        const double am = zam[k], ipk = zip[k];
+#pragma unroll
+        for (int i = 0; i < M; i++) { dprev[i] = (wfix && k == 0) ? 0.0 : fma(-am, dprev[i], x[i]) * ipk; }
+        // ---- out: through the same slot
+        double2* dst = reinterpret_cast<double2*>(buf + st * STAGE + lane * PITCH);
+#pragma unroll
+        for (int i = 0; i < M / 2; i++) dst[i] = make_double2(dprev[2 * i], dprev[2 * i + 1]);
+        fence_async_smem();
+        bulk_s2g(f + (size_t)k * plane, dst, 8 * M);
+        bulk_commit();
+        // ---- next load into the slot of plane k-1 once its store has been read out
+        const int kn = k + S - 1;
+        if (kn < A.nz) {
+            const int sn = kn % S;
+            bulk_wait_read<1>();
+            if (lane == 0) abar_expect(bar + sn, 32 * 8 * M);
+            __syncwarp();
+            bulk_g2s(buf + sn * STAGE + lane * PITCH, f + (size_t)kn * plane, 8 * M, bar + sn);
+        }
+    }
+    bulk_wait_all<0>();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pass B: grid (nx / 8, 3), block 256: thread = (column i = tid & 7, chunk c = tid >> 3)
+// ---------------------------------------------------------------------------------------------------------------
+template <int M>
+FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A)
+{
+    __shared__ double sm_y0[2][32][8], sm_g[2][32][8], sm_x[2][32][8];
+    const int i = threadIdx.x & 7, c = threadIdx.x >> 3, comp = blockIdx.y;
+    const size_t plane = (size_t)A.nx * A.ny, nx = (size_t)A.nx;
+    const size_t off0 = (size_t)(c * M) * nx + (size_t)blockIdx.x * 8 + i;
+    const double* __restrict__ d = A.r[comp];
+    double* __restrict__ q = A.q[comp];
+    const double* __restrict__ zcp = A.zcp[comp];
+    const VFastLine& L = A.L;
+    double carry[M];
+#pragma unroll
+    for (int m = 0; m < M; m++) carry[m] = 0.0;
+    for (int k = A.nz - 1; k >= 0; k--) {
+        const size_t base = (size_t)k * plane + off0;
+        const int pb = k & 1;
+        double x[M];
+#pragma unroll
+        for (int m = 0; m < M; m++) x[m] = d[base + m * nx];
+        if (k >= 2) {                                          // plane k-2 of d' and q towards L2: the 8 column threads share the rows
+#pragma unroll
+            for (int m = 0; m < M; m += 8)
+                if (m + i < M) { prefetch_l2(d + base - 2 * plane + (m + i) * nx - i); prefetch_l2(q + base - 2 * plane + (m + i) * nx - i); }
+        }
+        // ---- back substitution of the z system: x_k = d'_k - c'_k x_{k+1}
+        const double cpk = zcp[k];
+#pragma unroll
+        for (int m = 0; m < M; m++) { x[m] = fma(-cpk, carry[m], x[m]); carry[m] = x[m]; }
+        // ---- periodic y-solve of the tile
+        const double sep = x[M - 1];
+        chunk_interior<M>(L, x);
+        sm_y0[pb][c][i] = x[0];
+        __syncthreads();
+        const double g = fma(L.r, x[M - 2] + sm_y0[pb][(c + 1) & 31][i], sep);
+        sm_g[pb][c][i] = g;
+        __syncthreads();
+        double xs0 = 0.0, xs1 = 0.0;
+#pragma unroll
+        for (int s = 0; s < 32; s += 2) {
+            xs0 = fma(L.sinv[s], sm_g[pb][(c - s) & 31][i], xs0);
+            xs1 = fma(L.sinv[s + 1], sm_g[pb][(c - s - 1) & 31][i], xs1);
+        }
+        const double xs = xs0 + xs1;
+        sm_x[pb][c][i] = xs;
+        __syncthreads();
+        const double xl = sm_x[pb][(c - 1) & 31][i];
+        chunk_correct<M>(L, x, xl, xs);
+        // ---- q += dq
+#pragma unroll
+        for (int m = 0; m < M; m++) q[base + m * nx] += x[m];
+    }
+}
+#endif  // __CUDACC__
+
+}  // namespace fsei

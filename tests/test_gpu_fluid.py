@@ -167,3 +167,44 @@ def test_fluid_error_codes():
         plan.explicit_terms(*d[:4], d[4], d[5], d[6], d[0], r[1], r[2], 1e-3, 0.0, 1e-3, 0.0)   # output aliases input
     assert e.value.code == ERR_ARG
     plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# fast family of the viscous step (periodic x, y; partition solves in registers; two fused launches)
+# ---------------------------------------------------------------------------------------------
+FAST_SHAPES = [(64, 64, 9), (128, 96, 12), (256, 192, 7), (384, 256, 5), (512, 384, 5), (768, 512, 4), (1024, 768, 3),
+               (1024, 1024, 2), (64, 1024, 40), (1024, 64, 33)]
+
+
+@pytest.mark.parametrize("shape", FAST_SHAPES)
+@pytest.mark.parametrize("beta", [1e-3 / 6000.0, 3e-4])
+def test_viscous_fast_family_vs_oracle(oracle_ld, shape, beta):
+    """beta/dx^2 spans 0.0007 (decoupled chunks) .. 300 (every unknown of a line coupled to every other)."""
+    import torch
+    from paper_2103_15187_b200 import binding
+    g, f = _case(shape, (P, P), seed=44, n=6)
+    u, v, w, ru, rv, rw = f
+    uo, vo, wo = u.copy(), v.copy(), w.copy()
+    oracle_ld.viscous_step(g, uo, vo, wo, ru, rv, rw, beta)
+    plan = _plan(g)
+    d = _dev(f)
+    plan.viscous_step(*d, beta)
+    torch.cuda.synchronize()
+    assert plan.last_launch_count == 3                              # factorisation tables + two fused passes
+    for c, (q0, qo) in enumerate(((u, uo), (v, vo), (w, wo))):
+        got = d[c].cpu().numpy()
+        scale = np.abs(qo - q0).max()
+        assert np.abs(got - qo).max() <= 1e-12 * scale + 2 * EPS * np.abs(qo).max(), (c, np.abs(got - qo).max() / scale)
+    assert np.array_equal(d[2].cpu().numpy()[0], w[0])
+    plan.viscous_step(*d, beta)                                      # same beta again: the tables are kept
+    assert plan.last_launch_count == 2
+    plan.destroy()
+    # the generic family on the same grid (forced per plan) agrees to rounding
+    pg = binding.Plan.from_grid(g, binding.VISC_GENERIC)
+    dg = _dev(f)
+    pg.viscous_step(*dg, beta)
+    torch.cuda.synchronize()
+    assert pg.last_launch_count == 10
+    for c, qo in enumerate((uo, vo, wo)):
+        assert np.abs(dg[c].cpu().numpy() - qo).max() <= 1e-12 * np.abs(qo - f[c]).max() + 2 * EPS * np.abs(qo).max()
+    pg.destroy()
