@@ -3,6 +3,7 @@
 #include <cmath>
 #include "visc_fast.cuh"
 #include "fast_launch.hpp"
+#include "tma_host.hpp"
 
 namespace fsei {
 
@@ -23,6 +24,7 @@ bool visc_fast_supported(int nx, int ny)
     return a && b;
 }
 
+static size_t vb_smem(int M) { return 128 + (size_t)2 * 32 * M * 64 + (size_t)M * 256 * 8; }
 static size_t va_smem(int M) { return (size_t)FSEI_VA_WPB * (FSEI_VA_STAGES * 32 * (8 * M + 16) + 64); }
 
 cudaError_t visc_fast_init()
@@ -30,6 +32,9 @@ cudaError_t visc_fast_init()
     cudaError_t e = cudaSuccess;
 #define X(M) if (e == cudaSuccess) e = kernel_smem(k_visc_xz<M>, (int)va_smem(M));
     FSEI_VA_LIST(X)
+#undef X
+#define X(M) if (e == cudaSuccess) e = kernel_smem(k_visc_zy<M>, (int)vb_smem(M));
+    FSEI_VB_LIST(X)
 #undef X
     return e;
 }
@@ -99,11 +104,33 @@ cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// 2-D fp64 view of a field: inner dimension nx doubles, outer ny nz rows; box = 8 doubles x box_rows rows
+static cudaError_t field_map(const VFastArgs& A, int box_rows, double* f, TmaMap2D* out)
+{
+    EncodeTiledFn fn = tma_encode_fn();
+    if (!fn) return cudaErrorNotSupported;
+    cuuint64_t dims[2] = {(cuuint64_t)A.nx, (cuuint64_t)A.ny * A.nz};
+    cuuint64_t strides[1] = {(cuuint64_t)A.nx * sizeof(double)};
+    cuuint32_t box[2] = {8u, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(&out->m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, f, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st)
 {
     const dim3 grid(A.nx / 8, 3);
+    VFastMaps Mp;
+    Mp.box_rows = 256;
+    while (A.ny % Mp.box_rows) Mp.box_rows--;                   // largest divisor of ny that fits a TMA box
+    for (int c = 0; c < 3; c++) {
+        cudaError_t e = field_map(A, Mp.box_rows, A.r[c], &Mp.d[c]);
+        if (e == cudaSuccess) e = field_map(A, Mp.box_rows, A.q[c], &Mp.q[c]);
+        if (e != cudaSuccess) return e;
+    }
     switch (A.ny / 32) {
-#define X(M) case M: k_visc_zy<M><<<grid, 256, 0, st>>>(A); break;
+#define X(M) case M: k_visc_zy<M><<<grid, 256, vb_smem(M), st>>>(A, Mp); break;
         FSEI_VB_LIST(X)
 #undef X
         default: return cudaErrorInvalidValue;

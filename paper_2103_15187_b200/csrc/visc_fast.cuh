@@ -150,37 +150,58 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// pass B: grid (nx / 8, 3), block 256: thread = (column i = tid & 7, chunk c = tid >> 3)
+// pass B: grid (nx / 8, 3), block 256: thread = (column i = tid & 7, chunk c = tid >> 3).
+// The (ny x 8) tile of d' of plane k-1 lands by 2-D TMA boxes in one of two shared-memory tiles while plane k is being
+// solved in the other; the result goes back into its tile and leaves as a TMA REDUCE-ADD onto q (the addition q + dq is
+// done by the L2: the SM never loads q), so the LSU only sees shared memory.  x(k+1) of the z back substitution is
+// carried in a third shared-memory tile [M][256].  Dynamic shared memory: 128 + 2 * ny * 64 + M * 256 * 8 bytes.
 // ---------------------------------------------------------------------------------------------------------------
+struct VFastMaps { TmaMap2D d[3], q[3]; int box_rows; };      // 2-D fp64 views [nz * ny rows][nx], box 8 x box_rows
+
+__device__ __forceinline__ void tma_reduce_add_2d(const TmaMap2D* map, int x0, int y0, const void* src)
+{
+    asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(map), "r"(x0), "r"(y0), "r"(smem_u32(src)) : "memory");
+}
+
 template <int M>
-FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A)
+FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_GRID_CONSTANT VFastMaps Mp)
 {
     __shared__ double sm_y0[2][32][8], sm_g[2][32][8], sm_x[2][32][8];
-    const int i = threadIdx.x & 7, c = threadIdx.x >> 3, comp = blockIdx.y;
-    const size_t plane = (size_t)A.nx * A.ny, nx = (size_t)A.nx;
-    const size_t off0 = (size_t)(c * M) * nx + (size_t)blockIdx.x * 8 + i;
-    const double* __restrict__ d = A.r[comp];
-    double* __restrict__ q = A.q[comp];
+    FSEI_DYN_SMEM(smraw);
+    constexpr int NY = 32 * M;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
+    double* tile0 = reinterpret_cast<double*>(smraw + 128);     // [2][NY][8]
+    double* carry = tile0 + 2 * NY * 8 + threadIdx.x;           // [M][256]
+    const int tid = threadIdx.x, i = tid & 7, c = tid >> 3, comp = blockIdx.y;
+    const int col0 = blockIdx.x * 8, nb = NY / Mp.box_rows;
     const double* __restrict__ zcp = A.zcp[comp];
     const VFastLine& L = A.L;
-    double carry[M];
+    const TmaMap2D* dmap = &Mp.d[comp];
+    const TmaMap2D* qmap = &Mp.q[comp];
+    auto issue = [&](int k) {
+        double* t = tile0 + (k & 1) * NY * 8;
+        abar_expect(bar + (k & 1), (unsigned)(NY * 64));
+        for (int b = 0; b < nb; b++) tma_load_2d(t + b * Mp.box_rows * 8, dmap, col0, k * NY + b * Mp.box_rows, bar + (k & 1));
+    };
+    if (tid == 0) { abar_init(bar); abar_init(bar + 1); }
 #pragma unroll
-    for (int m = 0; m < M; m++) carry[m] = 0.0;
+    for (int m = 0; m < M; m++) carry[m * 256] = 0.0;
+    __syncthreads();
+    if (tid == 0) issue(A.nz - 1);
+    unsigned ph[2] = {0u, 0u};
     for (int k = A.nz - 1; k >= 0; k--) {
-        const size_t base = (size_t)k * plane + off0;
         const int pb = k & 1;
+        double* tl = tile0 + pb * NY * 8 + (c * M) * 8 + i;
+        if (tid == 0 && k > 0) { bulk_wait_read<0>(); issue(k - 1); }   // the other tile: its reduce-store (plane k+1) has been read out
+        abar_wait(bar + pb, ph[pb]); ph[pb] ^= 1u;
         double x[M];
 #pragma unroll
-        for (int m = 0; m < M; m++) x[m] = d[base + m * nx];
-        if (k >= 2) {                                          // plane k-2 of d' and q towards L2: the 8 column threads share the rows
-#pragma unroll
-            for (int m = 0; m < M; m += 8)
-                if (m + i < M) { prefetch_l2(d + base - 2 * plane + (m + i) * nx - i); prefetch_l2(q + base - 2 * plane + (m + i) * nx - i); }
-        }
+        for (int m = 0; m < M; m++) x[m] = tl[m * 8];
         // ---- back substitution of the z system: x_k = d'_k - c'_k x_{k+1}
         const double cpk = zcp[k];
 #pragma unroll
-        for (int m = 0; m < M; m++) { x[m] = fma(-cpk, carry[m], x[m]); carry[m] = x[m]; }
+        for (int m = 0; m < M; m++) { x[m] = fma(-cpk, carry[m * 256], x[m]); carry[m * 256] = x[m]; }
         // ---- periodic y-solve of the tile
         const double sep = x[M - 1];
         chunk_interior<M>(L, x);
@@ -200,10 +221,18 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A)
         __syncthreads();
         const double xl = sm_x[pb][(c - 1) & 31][i];
         chunk_correct<M>(L, x, xl, xs);
-        // ---- q += dq
+        // ---- q += dq: the increments go back into the tile and leave as a reduce-add
 #pragma unroll
-        for (int m = 0; m < M; m++) q[base + m * nx] += x[m];
+        for (int m = 0; m < M; m++) tl[m * 8] = x[m];
+        fence_async_smem();
+        __syncthreads();
+        if (tid == 0) {
+            const double* t = tile0 + pb * NY * 8;
+            for (int b = 0; b < nb; b++) tma_reduce_add_2d(qmap, col0, k * NY + b * Mp.box_rows, t + b * Mp.box_rows * 8);
+            bulk_commit();
+        }
     }
+    if (tid == 0) bulk_wait_all<0>();
 }
 #endif  // __CUDACC__
 
