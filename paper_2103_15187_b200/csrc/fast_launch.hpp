@@ -46,6 +46,7 @@ struct VFastLine; struct VFastArgs;
 bool visc_fast_supported(int nx, int ny);
 cudaError_t visc_fast_init();
 void visc_fast_line(int n, double h_recip, double beta, VFastLine* out);
+int visc_fast_nsig(const VFastLine& L);
 cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st);
 cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st);
 

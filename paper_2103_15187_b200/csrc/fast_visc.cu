@@ -89,7 +89,19 @@ void visc_fast_line(int n, double h_recip, double beta, VFastLine* out)
         out->ip[i] = i < Mi ? (double)ip[i] : 0.0; out->cp[i] = i < Mi ? (double)cp[i] : 0.0;
         out->ls[i] = i < Mi ? (double)ls[i] : 0.0; out->rs[i] = i < Mi ? (double)rs[i] : 0.0;
     }
-    for (int s = 0; s < 32; s++) out->sinv[s] = (double)z[s];      // S^-1[p][q] = z[(p - q) mod 32]
+    for (int s = 0; s < 32; s++) out->sinv[s] = (double)z[s];      // S^-1[p][q] = z[(p - q) mod 32]; z[s] = z[32 - s]
+}
+
+// number of terms of sinv on either side of s = 0 that can reach the last bit of sum_s sinv[s] g_{p-s}:
+// |sinv[s]| decays geometrically away from s = 0; terms below 2^-70 of the largest are dropped (exact to rounding:
+// with |g| bounded by 32 max|g| cancellation such a term is < 2^-65 ulp-relative of the separator value)
+int visc_fast_nsig(const VFastLine& L)
+{
+    double mx = 0.0;
+    for (int s = 0; s < 32; s++) mx = std::fmax(mx, std::fabs(L.sinv[s]));
+    int n = 0;
+    for (int s = 1; s <= 16; s++) if (std::fabs(L.sinv[s]) > mx * 0x1p-70) n = s;
+    return n;
 }
 
 cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st)
@@ -120,7 +132,7 @@ static cudaError_t field_map(const VFastArgs& A, int box_rows, double* f, TmaMap
 
 cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st)
 {
-    const dim3 grid(A.nx / 8, 3);
+    const dim3 grid(A.nx / 8);
     VFastMaps Mp;
     Mp.box_rows = 256;
     while (A.ny % Mp.box_rows) Mp.box_rows--;                   // largest divisor of ny that fits a TMA box

@@ -709,9 +709,9 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
             A.zam[c] = V.am; A.zip[c] = V.ip; A.zcp[c] = V.cp; A.r[c] = r[c]; A.q[c] = q[c];
         }
         A.nx = T.nx; A.ny = T.ny; A.nz = T.nz;
-        A.L = P->vline_x;
+        A.L = P->vline_x; A.nsig = visc_fast_nsig(A.L);
         { LaunchTimer t(P, K_VXZ, st); CU(launch_visc_xz(A, st)); }
-        A.L = P->vline_y;
+        A.L = P->vline_y; A.nsig = visc_fast_nsig(A.L);
         { LaunchTimer t(P, K_VZY, st); CU(launch_visc_zy(A, st)); }
         P->last_launches = launches + 2;
         return FSEI_OK;

@@ -41,6 +41,7 @@ struct VFastArgs {
     double* r[3];               // right-hand sides: rhs -> d' (pass A, in place); d' read by pass B
     double* q[3];               // velocity components (pass B)
     int nx, ny, nz;
+    int nsig;                   // terms of sinv kept on either side of s = 0 (16 = all)
 };
 
 #if defined(__CUDACC__)
@@ -92,10 +93,10 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
     const double* __restrict__ zam = A.zam[comp];
     const double* __restrict__ zip = A.zip[comp];
     const VFastLine& L = A.L;
+    const int nz = A.nz, nsig = A.nsig;
     if (lane == 0) for (int s = 0; s < S; s++) abar_init(bar + s);
     __syncwarp();
-    // prologue: planes 0 .. S-2 in flight
-    for (int s = 0; s < S - 1 && s < A.nz; s++) {
+    for (int s = 0; s < S - 1 && s < nz; s++) {                  // prologue: planes 0 .. S-2 in flight
         if (lane == 0) abar_expect(bar + s, 32 * 8 * M);
         __syncwarp();
         bulk_g2s(buf + s * STAGE + lane * PITCH, f + (size_t)s * plane, 8 * M, bar + s);
@@ -104,9 +105,11 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
 #pragma unroll
     for (int i = 0; i < M; i++) dprev[i] = 0.0;
     const bool wfix = comp == COMP_W;                                       // w: plane 0 is the wall (row fixed)
-    for (int k = 0; k < A.nz; k++) {
-        const int st = k % S;
-        abar_wait(bar + st, (k / S) & 1);
+    int st = 0; unsigned par = 0;
+    double* fk = f;                                                         // plane k
+    double* fn = f + (size_t)(S - 1) * plane;                               // plane k + S - 1
+    for (int k = 0; k < nz; k++, fk += plane, fn += plane) {
+        abar_wait(bar + st, par);
         double x[M];
         const double2* src = reinterpret_cast<const double2*>(buf + st * STAGE + lane * PITCH);
 #pragma unroll
@@ -116,41 +119,42 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
         chunk_interior<M>(L, x);
         const double y0n = __shfl_sync(0xffffffffu, x[0], (lane + 1) & 31);
         const double g = fma(L.r, x[M - 2] + y0n, sep);
-        double xs0 = 0.0, xs1 = 0.0;
-#pragma unroll
-        for (int s = 0; s < 32; s += 2) {
-            xs0 = fma(L.sinv[s], __shfl_sync(0xffffffffu, g, (lane - s) & 31), xs0);
-            xs1 = fma(L.sinv[s + 1], __shfl_sync(0xffffffffu, g, (lane - s - 1) & 31), xs1);
+        // separators: xs_p = sum_s sinv[s] g_{p-s}; sinv[s] = sinv[32-s] decays away from s = 0 and only the nsig terms on
+        // either side that can reach the last bit of the sum are kept (nsig = 16: all of them)
+        double xs = L.sinv[0] * g;
+        for (int s = 1; s <= nsig; s++) {
+            const double gm = __shfl_sync(0xffffffffu, g, (lane - s) & 31), gp = __shfl_sync(0xffffffffu, g, (lane + s) & 31);
+            xs = fma(L.sinv[s], s == 16 ? gm : gm + gp, xs);
         }
-        const double xs = xs0 + xs1;
         const double xl = __shfl_sync(0xffffffffu, xs, (lane - 1) & 31);
         chunk_correct<M>(L, x, xl, xs);
         // ---- forward elimination of the z system: d'_k = (x_k - a_k d'_{k-1}) / piv_k
         const double am = zam[k], ipk = zip[k];
+        const bool zero = wfix && k == 0;
 #pragma unroll
-        for (int i = 0; i < M; i++) { dprev[i] = (wfix && k == 0) ? 0.0 : fma(-am, dprev[i], x[i]) * ipk; }
+        for (int i = 0; i < M; i++) dprev[i] = zero ? 0.0 : fma(-am, dprev[i], x[i]) * ipk;
         // ---- out: through the same slot
         double2* dst = reinterpret_cast<double2*>(buf + st * STAGE + lane * PITCH);
 #pragma unroll
         for (int i = 0; i < M / 2; i++) dst[i] = make_double2(dprev[2 * i], dprev[2 * i + 1]);
         fence_async_smem();
-        bulk_s2g(f + (size_t)k * plane, dst, 8 * M);
+        bulk_s2g(fk, dst, 8 * M);
         bulk_commit();
         // ---- next load into the slot of plane k-1 once its store has been read out
-        const int kn = k + S - 1;
-        if (kn < A.nz) {
-            const int sn = kn % S;
+        const int sn = st == 0 ? S - 1 : st - 1;
+        if (k + S - 1 < nz) {
             bulk_wait_read<1>();
             if (lane == 0) abar_expect(bar + sn, 32 * 8 * M);
             __syncwarp();
-            bulk_g2s(buf + sn * STAGE + lane * PITCH, f + (size_t)kn * plane, 8 * M, bar + sn);
+            bulk_g2s(buf + sn * STAGE + lane * PITCH, fn, 8 * M, bar + sn);
         }
+        if (++st == S) { st = 0; par ^= 1u; }
     }
     bulk_wait_all<0>();
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// pass B: grid (nx / 8, 3), block 256: thread = (column i = tid & 7, chunk c = tid >> 3).
+// pass B: grid nx / 8, block 256 (the CTA walks its tile through u, v, w): thread = (column i = tid & 7, chunk c = tid >> 3).
 // The (ny x 8) tile of d' of plane k-1 lands by 2-D TMA boxes in one of two shared-memory tiles while plane k is being
 // solved in the other; the result goes back into its tile and leaves as a TMA REDUCE-ADD onto q (the addition q + dq is
 // done by the L2: the SM never loads q), so the LSU only sees shared memory.  x(k+1) of the z back substitution is
@@ -173,35 +177,36 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
     uint64_t* bar = reinterpret_cast<uint64_t*>(smraw);
     double* tile0 = reinterpret_cast<double*>(smraw + 128);     // [2][NY][8]
     double* carry = tile0 + 2 * NY * 8 + threadIdx.x;           // [M][256]
-    const int tid = threadIdx.x, i = tid & 7, c = tid >> 3, comp = blockIdx.y;
-    const int col0 = blockIdx.x * 8, nb = NY / Mp.box_rows;
-    const double* __restrict__ zcp = A.zcp[comp];
+    const int tid = threadIdx.x, i = tid & 7, c = tid >> 3;
+    const int col0 = blockIdx.x * 8, nb = NY / Mp.box_rows, nz = A.nz, nit = 3 * nz;
     const VFastLine& L = A.L;
-    const TmaMap2D* dmap = &Mp.d[comp];
-    const TmaMap2D* qmap = &Mp.q[comp];
-    auto issue = [&](int k) {
-        double* t = tile0 + (k & 1) * NY * 8;
-        abar_expect(bar + (k & 1), (unsigned)(NY * 64));
-        for (int b = 0; b < nb; b++) tma_load_2d(t + b * Mp.box_rows * 8, dmap, col0, k * NY + b * Mp.box_rows, bar + (k & 1));
+    // items it = comp * nz + (nz - 1 - k): the tile walks down each component in turn; item it uses tile it & 1
+    auto issue = [&](int it) {
+        const int cc = it / nz, k = nz - 1 - (it - cc * nz);
+        double* t = tile0 + (it & 1) * NY * 8;
+        abar_expect(bar + (it & 1), (unsigned)(NY * 64));
+        for (int b = 0; b < nb; b++) tma_load_2d(t + b * Mp.box_rows * 8, &Mp.d[cc], col0, k * NY + b * Mp.box_rows, bar + (it & 1));
     };
     if (tid == 0) { abar_init(bar); abar_init(bar + 1); }
-#pragma unroll
-    for (int m = 0; m < M; m++) carry[m * 256] = 0.0;
     __syncthreads();
-    if (tid == 0) issue(A.nz - 1);
-    unsigned ph[2] = {0u, 0u};
-    for (int k = A.nz - 1; k >= 0; k--) {
-        const int pb = k & 1;
+    if (tid == 0) issue(0);
+    for (int it = 0; it < nit; it++) {
+        const int comp = it / nz, k = nz - 1 - (it - comp * nz), pb = it & 1;
         double* tl = tile0 + pb * NY * 8 + (c * M) * 8 + i;
-        if (tid == 0 && k > 0) { bulk_wait_read<0>(); issue(k - 1); }   // the other tile: its reduce-store (plane k+1) has been read out
-        abar_wait(bar + pb, ph[pb]); ph[pb] ^= 1u;
+        if (tid == 0 && it + 1 < nit) { bulk_wait_read<0>(); issue(it + 1); }   // the other tile: its reduce-store has been read out
+        abar_wait(bar + pb, (it >> 1) & 1);
         double x[M];
 #pragma unroll
         for (int m = 0; m < M; m++) x[m] = tl[m * 8];
-        // ---- back substitution of the z system: x_k = d'_k - c'_k x_{k+1}
-        const double cpk = zcp[k];
+        // ---- back substitution of the z system: x_k = d'_k - c'_k x_{k+1}   (top plane: nothing above)
+        const double cpk = A.zcp[comp][k];
+        if (k == nz - 1) {
 #pragma unroll
-        for (int m = 0; m < M; m++) { x[m] = fma(-cpk, carry[m * 256], x[m]); carry[m * 256] = x[m]; }
+            for (int m = 0; m < M; m++) carry[m * 256] = x[m];
+        } else {
+#pragma unroll
+            for (int m = 0; m < M; m++) { x[m] = fma(-cpk, carry[m * 256], x[m]); carry[m * 256] = x[m]; }
+        }
         // ---- periodic y-solve of the tile
         const double sep = x[M - 1];
         chunk_interior<M>(L, x);
@@ -210,13 +215,11 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
         const double g = fma(L.r, x[M - 2] + sm_y0[pb][(c + 1) & 31][i], sep);
         sm_g[pb][c][i] = g;
         __syncthreads();
-        double xs0 = 0.0, xs1 = 0.0;
-#pragma unroll
-        for (int s = 0; s < 32; s += 2) {
-            xs0 = fma(L.sinv[s], sm_g[pb][(c - s) & 31][i], xs0);
-            xs1 = fma(L.sinv[s + 1], sm_g[pb][(c - s - 1) & 31][i], xs1);
+        double xs = L.sinv[0] * g;
+        for (int s = 1; s <= A.nsig; s++) {
+            const double gm = sm_g[pb][(c - s) & 31][i], gp = sm_g[pb][(c + s) & 31][i];
+            xs = fma(L.sinv[s], s == 16 ? gm : gm + gp, xs);
         }
-        const double xs = xs0 + xs1;
         sm_x[pb][c][i] = xs;
         __syncthreads();
         const double xl = sm_x[pb][(c - 1) & 31][i];
@@ -228,7 +231,7 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
         __syncthreads();
         if (tid == 0) {
             const double* t = tile0 + pb * NY * 8;
-            for (int b = 0; b < nb; b++) tma_reduce_add_2d(qmap, col0, k * NY + b * Mp.box_rows, t + b * Mp.box_rows * 8);
+            for (int b = 0; b < nb; b++) tma_reduce_add_2d(&Mp.q[comp], col0, k * NY + b * Mp.box_rows, t + b * Mp.box_rows * 8);
             bulk_commit();
         }
     }
