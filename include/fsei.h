@@ -213,6 +213,37 @@ int fsei_ibm_forcing(fsei_plan* plan, long n, const double* xm, const double* ym
                      void* cuda_stream);
 
 /*
+ * ---- Multi-GPU slab decomposition of the projection: per-rank stages -------------------------
+ * "the Cartesian domain is split into slabs ... at most one halo layer is required on each side of a slab";
+ * "all-to-all communications ... needed to solve both the equation for the provisional velocity and for the elliptic
+ * equation".  One process per GPU.  A rank owns
+ *   planes [k0, k1) of u, v, w, p, phi (a z-slab)            for a1-a3 and a5-a7, and
+ *   x-slots [s0, s1) of the nx/2 packed wavenumber slots, for every row and EVERY plane (full z columns), for a4.
+ * Between fsei_slab_forward and fsei_pencil_solve, and between fsei_pencil_solve and fsei_slab_backward, the spectrum
+ * changes hands by an all-to-all (paper_2103_15187_b200/slab.py, torch.distributed).
+ * Periodic x and y only; nx/2 and ny in the fast family's lengths                          else FSEI_ERR_ARG / _SIZE
+ *
+ * Layouts (DEVICE pointers, 16-byte aligned).  nzl = k1 - k0, nsl = s1 - s0.
+ *   slab field   : [nzl][ny][nx] doubles.  w must be followed in memory by plane k1 (the neighbour's first plane) unless
+ *                  k1 == nz; phi passed to fsei_slab_project must be preceded by plane k0-1 unless k0 == 0, and, when
+ *                  beta != 0, followed by plane k1 unless k1 == nz.  (The pointer is the address of local plane 0.)
+ *   slab spectrum: [nzl][ny][nx/2] complex (re, im), the packed natural-order layout of DESIGN.md sec. 2.
+ *   pencil       : [nz][ny][nsl] complex: element (k, row, s0 + s) of the spectrum.
+ */
+fsei_plan* fsei_slab_plan_create(int nx, int ny, int nz, double Lx, double Ly, const double* zc /* HOST, nz+1, GLOBAL */,
+                                 int bc_x, int bc_y, int k0, int k1, int s0, int s1);
+/* a1-a3 on the slab: spec = y-transform of x-transform of D(u,v,w)/alpha_dt.  spec must not alias u, v, w. */
+int fsei_slab_forward(fsei_plan* plan, const double* u, const double* v, const double* w, double alpha_dt,
+                      double* spec, void* cuda_stream);
+/* a4 on the pencil, in place (the rank with s0 == 0 also solves the gauge column). */
+int fsei_pencil_solve(fsei_plan* plan, double* pencil, void* cuda_stream);
+/* a5, a6 on the slab: phi = inverse transforms of spec (phi may alias spec). */
+int fsei_slab_backward(fsei_plan* plan, double* spec, double* phi, void* cuda_stream);
+/* a7 on the slab (halo planes of phi as described above). */
+int fsei_slab_project(fsei_plan* plan, double* u, double* v, double* w, double* p, const double* phi,
+                      double alpha_dt, double beta, void* cuda_stream);
+
+/*
  * Kernel-level timing aid for bench.py: number of kernels enqueued by the last
  * fsei_pressure_projection / fsei_poisson_solve call on this plan.
  */

@@ -21,7 +21,8 @@ EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family",
            "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
            "fsei_plan_profile", "fsei_plan_profile_read",
            "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep",
-           "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing")
+           "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing",
+           "fsei_slab_plan_create", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project")
 
 _lib = None
 _vp, _d, _i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
@@ -89,6 +90,16 @@ def lib() -> ctypes.CDLL:
     L.fsei_mls_spread.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_vp]
     L.fsei_ibm_forcing.restype = _i
     L.fsei_ibm_forcing.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_d] + [_vp] * 6 + [_vp]
+    L.fsei_slab_plan_create.restype = _vp
+    L.fsei_slab_plan_create.argtypes = [_i, _i, _i, _d, _d, _vp, _i, _i, _i, _i, _i, _i]
+    L.fsei_slab_forward.restype = _i
+    L.fsei_slab_forward.argtypes = [_vp, _vp, _vp, _vp, _d, _vp, _vp]
+    L.fsei_pencil_solve.restype = _i
+    L.fsei_pencil_solve.argtypes = [_vp, _vp, _vp]
+    L.fsei_slab_backward.restype = _i
+    L.fsei_slab_backward.argtypes = [_vp, _vp, _vp, _vp]
+    L.fsei_slab_project.restype = _i
+    L.fsei_slab_project.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _d, _d, _vp]
     _lib = L
     return L
 
@@ -227,3 +238,35 @@ class Plan:
         _chk(lib().fsei_ibm_forcing(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(area), _ptr(Vu), _ptr(Vv), _ptr(Vw),
                                     _ptr(u), _ptr(v), _ptr(w), float(inv_dt), _ptr(Fu), _ptr(Fv), _ptr(Fw), _ptr(fu), _ptr(fv),
                                     _ptr(fw), _stream(stream)))
+
+
+class SlabPlan(Plan):
+    """fsei_slab_plan_create: this rank's share of a multi-GPU projection -- planes [k0, k1) and x-slots [s0, s1)."""
+
+    def __init__(self, grid, k0, k1, s0, s1):
+        import numpy as np
+        nx, ny, nz, Lx, Ly, zc, bcx, bcy = grid
+        L = lib()
+        zc = np.ascontiguousarray(zc, dtype=np.float64)
+        if zc.shape != (nz + 1,):
+            raise FseiError(ERR_ARG, f"zc must hold nz+1 = {nz + 1} face coordinates")
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.k0, self.k1, self.s0, self.s1 = int(k0), int(k1), int(s0), int(s1)
+        self.shape = (self.k1 - self.k0, self.ny, self.nx)
+        self._h = L.fsei_slab_plan_create(self.nx, self.ny, self.nz, float(Lx), float(Ly), zc.ctypes.data, int(bcx), int(bcy),
+                                          self.k0, self.k1, self.s0, self.s1)
+        if not self._h:
+            raise FseiError(L.fsei_last_error_code(), last_error())
+
+    def slab_forward(self, u, v, w, alpha_dt, spec, stream=None):
+        _chk(lib().fsei_slab_forward(self._h, _ptr(u), _ptr(v), _ptr(w), float(alpha_dt), _ptr(spec), _stream(stream)))
+
+    def pencil_solve(self, pencil, stream=None):
+        _chk(lib().fsei_pencil_solve(self._h, _ptr(pencil), _stream(stream)))
+
+    def slab_backward(self, spec, phi, stream=None):
+        _chk(lib().fsei_slab_backward(self._h, _ptr(spec), _ptr(phi), _stream(stream)))
+
+    def slab_project(self, u, v, w, p, phi, alpha_dt, beta=0.0, stream=None):
+        _chk(lib().fsei_slab_project(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), _ptr(phi), float(alpha_dt), float(beta),
+                                     _stream(stream)))

@@ -246,10 +246,15 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
     return FSEI_ADD(FSEI_SUB(FSEI_ADD(FSEI_MUL(A.gdt, H), FSEI_MUL(A.rdt, Hp)), FSEI_MUL(A.adt, gp)), FSEI_MUL(A.tb, lap));
 }
 
+#ifndef FSEI_EXPL_KZ
 #define FSEI_EXPL_KZ 8
+#endif
+#ifndef FSEI_EXPL_MINB
+#define FSEI_EXPL_MINB 2
+#endif
 
 // grid (ceil(nx/32), ceil(ny/8), ceil(nz/KZ)), block (32, 8)
-FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
+FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
 {
     const SParams& S = A.S;
     const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;

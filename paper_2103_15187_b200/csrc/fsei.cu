@@ -61,6 +61,7 @@ struct fsei_plan {
     size_t smem_x = 0, smem_y = 0;
     int last_launches = 0;
     const double* zc_dev = nullptr;      // z-face coordinates (IB-MLS node positions)
+    bool slab = false; int k0 = 0, k1 = 0, s0 = 0, s1 = 0;   // z-slab / x-slot-pencil share of a multi-GPU decomposition (fsei_slab_plan_create)
     bool visc_fast = false; VFastLine vline_x, vline_y;   // fast viscous family: host-built line tables of the last beta
     double* vtab = nullptr; int vnmax = 0; double visc_beta = NAN;   // implicit viscous step: factorisation tables of the last beta
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
@@ -465,6 +466,7 @@ extern "C" int fsei_plan_last_launch_count(const fsei_plan* P) { return P ? P->l
 extern "C" int fsei_divergence(fsei_plan* P, const double* u, const double* v, const double* w, double alpha_dt,
                                double* rhs, void* cuda_stream)
 {
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_divergence: this is a slab plan (use the fsei_slab_* calls)");
     if (!P || !u || !v || !w || !rhs) return fail(FSEI_ERR_ARG, "fsei_divergence: NULL argument");
     if (alpha_dt == 0.0 || alpha_dt != alpha_dt) return fail(FSEI_ERR_ARG, "fsei_divergence: alpha_dt must be non-zero");
     if (rhs == u || rhs == v || rhs == w) return fail(FSEI_ERR_ARG, "fsei_divergence: rhs must not alias u, v, w");
@@ -513,6 +515,7 @@ static int fused_spectral_solve(fsei_plan* P, double* phi, cudaStream_t st)
 
 extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, void* cuda_stream)
 {
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: this is a slab plan (use the fsei_slab_* calls)");
     if (!P || !rhs || !phi) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: NULL argument");
     if (misaligned(rhs) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_poisson_solve: field pointers must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -584,6 +587,7 @@ extern "C" int fsei_poisson_solve(fsei_plan* P, const double* rhs, double* phi, 
 extern "C" int fsei_project(fsei_plan* P, double* u, double* v, double* w, double* p, const double* phi,
                             double alpha_dt, double beta, void* cuda_stream)
 {
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_project: this is a slab plan (use the fsei_slab_* calls)");
     if (!P || !u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_project: NULL argument");
     if (alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_project: NaN parameter");
     if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_project: phi must not alias u, v, w, p");
@@ -599,6 +603,7 @@ extern "C" int fsei_project(fsei_plan* P, double* u, double* v, double* w, doubl
 extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, double* w, double* p, double* phi,
                                         double alpha_dt, double beta, void* cuda_stream)
 {
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: this is a slab plan (use the fsei_slab_* calls)");
     int rc, n = 0;
     if (P && P->fast) {
         if (!u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: NULL argument");
@@ -648,6 +653,7 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
                                    double* ru, double* rv, double* rw, double gamma_dt, double rho_dt, double alpha_dt,
                                    double beta, void* cuda_stream)
 {
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: this is a slab plan (use the fsei_slab_* calls)");
     if (!P || !u || !v || !w || !p || !hu || !hv || !hw || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: NULL argument");
     if (gamma_dt != gamma_dt || rho_dt != rho_dt || alpha_dt != alpha_dt || !(beta >= 0.0)) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: NaN parameter or beta < 0");
     const double* in[4] = {u, v, w, p};
@@ -682,6 +688,7 @@ static VTab visc_tab(const fsei_plan* P, int comp, int dir)
 extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, double* ru, double* rv, double* rw,
                                  double beta, void* cuda_stream)
 {
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_viscous_step: this is a slab plan (use the fsei_slab_* calls)");
     if (!P || !u || !v || !w || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_viscous_step: NULL argument");
     if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_viscous_step: beta must be finite and >= 0");
     double* q[3] = {u, v, w};
@@ -817,6 +824,158 @@ extern "C" int fsei_ibm_forcing(fsei_plan* P, long n, const double* xm, const do
     if (P->T.nz < 3) return fail(FSEI_ERR_SIZE, "fsei_ibm_forcing: the 27-node support needs nz >= 3");
     MlsArgs A{mls_grid(P), n, xm, ym, zm, area, {u, v, w}, {Vu, Vv, Vw}, {Fu, Fv, Fw}, {fu, fv, fw}, inv_dt};
     return mls_launch<1>(P, A, static_cast<cudaStream_t>(cuda_stream));
+}
+
+// ------------------------------------------------------------------------------------------
+// multi-GPU slab decomposition of the projection: the per-rank stages.
+// A rank owns planes [k0, k1) of the fields (a z-slab with one halo plane) for a1-a3 and a5-a7, and x-slots [s0, s1) of
+// every (ky, k) -- full z columns -- for a4.  The two exchanges between them are the all-to-all of P:L248, done by
+// paper_2103_15187_b200/slab.py over torch.distributed; these calls are the local work on either side of it.
+// ------------------------------------------------------------------------------------------
+static int slab_plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bcx, int bcy,
+                           int k0, int k1, int s0, int s1)
+{
+    int code = 0, rc;
+    if (bcx != BC_PERIODIC || bcy != BC_PERIODIC) return fail(FSEI_ERR_ARG, "fsei_slab_plan_create: periodic x and y only (the paper's decomposition, P:L240)");
+    if (nx < 4 || nx % 4 || k0 < 0 || k1 <= k0 || k1 > nz || s0 < 0 || s1 <= s0 || s1 > nx / 2) return fail(FSEI_ERR_ARG, "fsei_slab_plan_create: empty or out-of-range share [k0,k1) x [s0,s1)");
+    std::string msg = build_tables(P->T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code, true);
+    if (code) return fail(code, msg);
+    if (!(xfast_supported(nx / 2) && yfast_supported(ny) && (size_t)nz * 4 * sizeof(cplx) <= 200 * 1024))
+        return fail(FSEI_ERR_SIZE, "fsei_slab_plan_create: nx/2 and ny need a register-resident transform (16..1024, 3*2^a up to 768), nz <= 3200");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FSEI_ERR_CUDA, "no CUDA device: libfsei has no CPU fallback"); }
+    HostTables& T = P->T;
+    P->slab = true; P->fast = true; P->k0 = k0; P->k1 = k1; P->s0 = s0; P->s1 = s1;
+    const int nzl = k1 - k0, nsl = s1 - s0;
+    XParams& X = P->X; YParams& Y = P->Y; ZParams& Z = P->Z; SParams& S = P->S;
+    if ((rc = upload(P, T.twx, &X.tw))) return rc;
+    if ((rc = upload(P, T.twx_r2c, &X.tw_r2c))) return rc;
+    if ((rc = upload(P, T.twx_dct, &X.tw_dct))) return rc;
+    if ((rc = upload(P, T.twy, &Y.tw))) return rc;
+    if ((rc = upload(P, T.twy_dct, &Y.tw_dct))) return rc;
+    if ((rc = upload(P, T.za, &Z.za))) return rc;
+    if ((rc = upload(P, T.zcc, &Z.zcc))) return rc;
+    if ((rc = upload(P, T.dzc, &Z.dzc))) return rc;
+    if ((rc = upload(P, T.dzm, &Z.dzm))) return rc;
+    if ((rc = upload(P, T.lamx, &Z.lamx))) return rc;
+    if ((rc = upload(P, T.lamy, &Z.lamy))) return rc;
+    S.nx = nx; S.ny = ny; S.nz = nzl; S.bcx = bcx; S.bcy = bcy; S.rdx = T.rdx; S.rdy = T.rdy;
+    if ((rc = upload(P, T.rdzc, &S.rdzc))) return rc;
+    if ((rc = upload(P, T.rdzm, &S.rdzm))) return rc;
+    S.kofs = k0; S.halo_lo = k0 > 0; S.halo_hi = k1 < nz;
+    XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
+    XF.nx = nx; XF.ny = ny; XF.nz = nzl; XF.N = nx / 2; XF.tw = X.tw; XF.tw_r2c = X.tw_r2c; XF.tw_dct = X.tw_dct; XF.scale = T.scale;
+    {
+        int dev = 0, nsm = 148;
+        cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        const int lpb = xfast_lines_per_block(nx / 2, false);
+        long kc = ((long)((ny + lpb - 1) / lpb) * nzl) / (4L * nsm);
+        XF.kchunk = (int)(kc < 1 ? 1 : (kc > 64 ? 64 : kc));
+        P->kchunk_inv = (int)(kc < 1 ? 1 : (kc > 32 ? 32 : kc));
+    }
+    YF.nxc = T.nxc; YF.ny = ny; YF.nz = nzl; YF.tw = Y.tw; YF.tw_dct = Y.tw_dct; YF.untangle = 1;
+    ZF.nxc = nsl; ZF.ny = ny; ZF.nz = nz; ZF.bcx = bcx; ZF.bcy = bcy; ZF.ncomp = 1; ZF.s0 = s0;
+    ZF.za = Z.za; ZF.zcc = Z.zcc; ZF.lamx = Z.lamx + 2 * (size_t)s0; ZF.lamy = Z.lamy; ZF.dzc = Z.dzc; ZF.dzm = Z.dzm;
+    ZF.ktw = nz; ZF.cb = 0; ZF.special_in = nullptr;
+    void* q = nullptr;
+    if ((rc = dalloc(P, sizeof(cplx) * 2 * nz, &q))) return rc;
+    ZF.special = static_cast<cplx*>(q);
+    if ((rc = dalloc(P, sizeof(double) * 8 * nz, &q))) return rc;
+    ZF.cpw = static_cast<double*>(q);
+    if ((rc = dalloc(P, sizeof(double) * (size_t)nz * ny * nsl, &q))) return rc;
+    ZF.ipiv = static_cast<const double*>(q);
+    const size_t cols = (size_t)ny * nsl;
+    k_zf_factor<<<(unsigned)((cols + 255) / 256), 256>>>(ZF, static_cast<double*>(q));
+    CU(cudaGetLastError());
+    if (s0 == 0) { k_z_special_factor<<<1, 32>>>(ZF); CU(cudaGetLastError()); }
+    CU(cudaDeviceSynchronize());
+    CU(xfast_init());
+    CU(yfast_init());
+    CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz + 16)));
+    return FSEI_OK;
+}
+
+extern "C" fsei_plan* fsei_slab_plan_create(int nx, int ny, int nz, double Lx, double Ly, const double* zc, int bc_x, int bc_y,
+                                            int k0, int k1, int s0, int s1)
+{
+    fsei_plan* P = new (std::nothrow) fsei_plan();
+    if (!P) { fail(FSEI_ERR_ALLOC, "out of host memory"); return nullptr; }
+    int rc = slab_plan_build(P, nx, ny, nz, Lx, Ly, zc, bc_x, bc_y, k0, k1, s0, s1);
+    if (rc != FSEI_OK) { const std::string msg = g_err; fsei_plan_destroy(P); g_err = msg; g_err_code = rc; return nullptr; }
+    g_err_code = FSEI_OK; g_err.clear();
+    return P;
+}
+
+#define SLAB_ONLY(name) if (!P || !P->slab) return fail(FSEI_ERR_ARG, name ": not a slab plan")
+
+extern "C" int fsei_slab_forward(fsei_plan* P, const double* u, const double* v, const double* w, double alpha_dt,
+                                 double* spec, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_slab_forward");
+    if (!u || !v || !w || !spec) return fail(FSEI_ERR_ARG, "fsei_slab_forward: NULL argument");
+    if (alpha_dt == 0.0 || alpha_dt != alpha_dt) return fail(FSEI_ERR_ARG, "fsei_slab_forward: alpha_dt must be non-zero");
+    if (spec == u || spec == v || spec == w) return fail(FSEI_ERR_ARG, "fsei_slab_forward: spec must not alias u, v, w");
+    if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(spec)) return fail(FSEI_ERR_ARG, "fsei_slab_forward: field pointers must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t n = (size_t)P->T.nx * P->T.ny * (P->k1 - P->k0);
+    { LaunchTimer t(P, K_DIV, st); k_divergence_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, 1.0 / alpha_dt, spec); }
+    CU(cudaGetLastError());
+    cplx* sp = reinterpret_cast<cplx*>(spec);
+    { LaunchTimer t(P, K_XF, st); CU(launch_xf_fast(P->XF, P->S, false, false, spec, nullptr, nullptr, 0.0, sp, st)); }
+    { LaunchTimer t(P, K_YF, st); CU(launch_y_fast(P->YF, false, false, sp, st)); }
+    P->last_launches = 3;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_pencil_solve(fsei_plan* P, double* pencil, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_pencil_solve");
+    if (!pencil || misaligned(pencil)) return fail(FSEI_ERR_ARG, "fsei_pencil_solve: NULL or misaligned pencil");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const HostTables& T = P->T;
+    cplx* sp = reinterpret_cast<cplx*>(pencil);
+    int launches = 0;
+    if (P->s0 == 0) {
+        { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, sp); }
+        CU(cudaGetLastError()); launches++;
+    }
+    {
+        LaunchTimer t(P, K_ZD, st);
+        const size_t nthr = (size_t)(P->s1 - P->s0) * T.ny;
+        if (T.nz <= 32) k_zf_pcr<<<(unsigned)((nthr * 32 + 127) / 128), 128, 0, st>>>(P->ZF, sp);
+        else k_zf_sweep<1><<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(P->ZF, sp);
+    }
+    CU(cudaGetLastError());
+    P->last_launches = launches + 1;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_slab_backward(fsei_plan* P, double* spec, double* phi, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_slab_backward");
+    if (!spec || !phi || misaligned(spec) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_slab_backward: NULL or misaligned argument");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cplx* sp = reinterpret_cast<cplx*>(spec);
+    { LaunchTimer t(P, K_YI, st); CU(launch_y_fast(P->YF, true, false, sp, st)); }
+    { LaunchTimer t(P, K_XI, st); XFast xi = P->XF; xi.kchunk = P->kchunk_inv; CU(launch_xi_fast(xi, false, sp, phi, st)); }
+    P->last_launches = 2;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_slab_project(fsei_plan* P, double* u, double* v, double* w, double* p, const double* phi,
+                                 double alpha_dt, double beta, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_slab_project");
+    if (!u || !v || !w || !p || !phi) return fail(FSEI_ERR_ARG, "fsei_slab_project: NULL argument");
+    if (alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_slab_project: NaN parameter");
+    if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(p) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_slab_project: field pointers must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t n = (size_t)P->T.nx * P->T.ny * (P->k1 - P->k0);
+    { LaunchTimer t(P, K_PROJ, st); k_project_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, p, phi, alpha_dt, beta); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
 }
 
 // ------------------------------------------------------------------------------------------

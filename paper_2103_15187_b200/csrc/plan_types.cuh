@@ -59,6 +59,10 @@ struct SParams {
     double rdx, rdy;
     const double* rdzc;   // 1/(zc[k+1]-zc[k])
     const double* rdzm;   // 1/(zm[k]-zm[k-1]), rdzm[0] = 0
+    // z-slab view (multi-GPU decomposition, slab.py): the fields hold planes [kofs, kofs + nz) of the global grid; the
+    // metric tables stay global (indexed k + kofs); halo_lo / halo_hi: the plane below the first / above the last one
+    // is present in memory (a neighbour's plane) instead of being a wall
+    int kofs = 0, halo_lo = 0, halo_hi = 0;
 };
 
 FSEI_HD int padx(int n) { return n + (n >> 3); }

@@ -41,8 +41,8 @@ FSEI_GLOBAL(256, 1) k_divergence_fast(SParams S, const double* __restrict__ u, c
     cplx vv = sld2(v + c);
     cplx vp = (j + 1 < S.ny) ? sld2(v + c + S.nx) : (S.bcy == BC_PERIODIC ? sld2(v + c - (size_t)(S.ny - 1) * S.nx) : cmake(0.0, 0.0));
     cplx ww = sld2(w + c);
-    cplx wp = (k + 1 < S.nz) ? sld2(w + c + plane) : cmake(0.0, 0.0);
-    const double rdz = S.rdzc[k];
+    cplx wp = (k + 1 < S.nz || S.halo_hi) ? sld2(w + c + plane) : cmake(0.0, 0.0);
+    const double rdz = S.rdzc[k + S.kofs];
     sst2(rhs + c, cmake(div_cell(uu.re, uu.im, vv.re, vp.re, ww.re, wp.re, S.rdx, S.rdy, rdz, inv_adt),
                         div_cell(uu.im, un, vv.im, vp.im, ww.im, wp.im, S.rdx, S.rdy, rdz, inv_adt)));
 }
@@ -58,7 +58,7 @@ FSEI_GLOBAL(256, 1) k_project_fast(SParams S, double* __restrict__ u, double* __
     const int t = (int)(pr % hx); const size_t r = pr / hx; const int j = (int)(r % S.ny), k = (int)(r / S.ny);
     const size_t line = r * S.nx, c = line + 2 * t, plane = (size_t)S.nx * S.ny;
     const bool xper = S.bcx == BC_PERIODIC, yper = S.bcy == BC_PERIODIC;
-    const bool xlo0 = (t > 0) || xper, ylo = (j > 0) || yper, zlo = k > 0;
+    const bool xlo0 = (t > 0) || xper, ylo = (j > 0) || yper, zlo = k > 0 || S.halo_lo;
     const cplx z0 = cmake(0.0, 0.0);
 
     const cplx c0 = sld2(phi + c);
@@ -66,7 +66,7 @@ FSEI_GLOBAL(256, 1) k_project_fast(SParams S, double* __restrict__ u, double* __
     const cplx pym = ylo ? sld2(phi + (j > 0 ? c - S.nx : c + (size_t)(S.ny - 1) * S.nx)) : z0;
     const cplx pzm = zlo ? sld2(phi + c - plane) : z0;
     cplx uu = sld2(u + c), vv = sld2(v + c), ww = sld2(w + c), pp = sld2(p + c);
-    const double rzm = S.rdzm[k];
+    const double rzm = S.rdzm[k + S.kofs];
 
     if (xlo0) uu.re = corr_face(uu.re, c0.re, pxm, S.rdx, adt);
     uu.im = corr_face(uu.im, c0.im, c0.re, S.rdx, adt);
@@ -75,11 +75,11 @@ FSEI_GLOBAL(256, 1) k_project_fast(SParams S, double* __restrict__ u, double* __
     if (beta == 0.0) {
         pp.re = FSEI_ADD(pp.re, c0.re); pp.im = FSEI_ADD(pp.im, c0.im);
     } else {
-        const bool xhi1 = (2 * t + 2 < S.nx) || xper, yhi = (j + 1 < S.ny) || yper, zhi = k + 1 < S.nz;
+        const bool xhi1 = (2 * t + 2 < S.nx) || xper, yhi = (j + 1 < S.ny) || yper, zhi = k + 1 < S.nz || S.halo_hi;
         const double pxp = (2 * t + 2 < S.nx) ? phi[c + 2] : (xper ? phi[line] : 0.0);
         const cplx pyp = yhi ? sld2(phi + (j + 1 < S.ny ? c + S.nx : c - (size_t)(S.ny - 1) * S.nx)) : z0;
         const cplx pzp = zhi ? sld2(phi + c + plane) : z0;
-        const double rzp = zhi ? S.rdzm[k + 1] : 0.0, rzc = S.rdzc[k];
+        const double rzp = zhi ? S.rdzm[k + 1 + S.kofs] : 0.0, rzc = S.rdzc[k + S.kofs];
         pp.re = pressure_cell(S, pp.re, c0.re, pxm, c0.im, pym.re, pyp.re, pzm.re, pzp.re, xlo0, true, ylo, yhi, zlo, zhi, rzm, rzp, rzc, beta);
         pp.im = pressure_cell(S, pp.im, c0.im, c0.re, pxp, pym.im, pyp.im, pzm.im, pzp.im, true, xhi1, ylo, yhi, zlo, zhi, rzm, rzp, rzc, beta);
     }

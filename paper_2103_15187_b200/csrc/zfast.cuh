@@ -27,6 +27,7 @@ struct ZFast {
     const cplx* special_in;   // fused path: [2][nz] right-hand sides of the special columns (else read from the spectrum)
     double* cpw;          // [8][nz] plan-time factorisation of the special columns: c'_k of component t at [t][k],
                           // reciprocal pivots at [4 + t][k]   (t = 2 col + comp; k_z_special_factor)
+    int s0 = 0;           // pencil view (slab.py): local slot s is global slot s + s0 (lamx already points at slot s0)
 };
 
 FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot)
@@ -41,7 +42,7 @@ FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot)
 FSEI_HD double z_lambda(const ZFast& Z, int row, int slot, int comp)
 {
     int cx = comp;
-    if (Z.bcy == BC_PERIODIC && (slot == 0 || Z.bcx == BC_NEUMANN)) {
+    if (Z.bcy == BC_PERIODIC && (slot + Z.s0 == 0 || Z.bcx == BC_NEUMANN)) {
         const int h = Z.ny >> 1;
         if (row != 0 && row != h) cx = (row < h) ? 0 : 1;
     }
@@ -55,7 +56,7 @@ FSEI_HD double z_lambda(const ZFast& Z, int row, int slot, int comp)
 FSEI_HD int z_special(const ZFast& Z, int row, int slot, int& mask)
 {
     mask = 0;
-    if (slot != 0) return -1;
+    if (slot + Z.s0 != 0) return -1;
     const bool pp = (Z.bcx == BC_PERIODIC && Z.bcy == BC_PERIODIC);
     if (row == 0) { mask = pp ? 3 : 1; return 0; }
     if (pp && row == (Z.ny >> 1)) { mask = 3; return 1; }

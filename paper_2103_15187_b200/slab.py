@@ -1,0 +1,206 @@
+"""Multi-GPU slab decomposition of the pressure projection.
+
+The paper splits the Cartesian domain into slabs with one halo layer and solves the implicit and the elliptic
+problems across ranks with all-to-all transposes, staged through the host.  Here: one process per
+GPU over `torch.distributed` (NCCL across NVLink / NVSwitch), device buffers only.  A rank owns
+
+  * planes [k0, k1) of u, v, w, p, phi (a z-slab)  -> divergence, x and y transforms, correction are local (a1-a3, a5-a7);
+    the divergence needs the neighbour's first w plane, the correction the neighbour's last phi plane (one halo layer);
+  * x-slots [s0, s1) of the packed spectrum for every row and every plane -> the z tridiagonals are local (a4).
+
+Between the two sits one exchange each way.  In the slab spectrum [nzl][ny][N] a destination's slots are a strided slice
+(packed once); in the pencil [nz][ny][nsl] a source's planes are CONTIGUOUS, so received chunks land in place and the way
+back sends views without packing.
+
+This module holds only plumbing: index ranges, buffers, packing copies, send/recv lists.  Every arithmetic step runs in
+the kernels of libfsei behind `binding.SlabPlan` (fsei_slab_forward / fsei_pencil_solve / fsei_slab_backward /
+fsei_slab_project).  `DistComm` runs the exchanges over a process group; `LocalComm` delivers them by copies between
+the ranks of ONE process that are stepped stage by stage (no kernel of one rank ever waits on another's) -- used to
+check the decomposition against the single-plan projection on one GPU.
+"""
+from __future__ import annotations
+
+from typing import List, Sequence, Tuple
+
+
+def split(n: int, world: int) -> List[Tuple[int, int]]:
+    """Balanced contiguous ranges [lo, hi) of n items over `world` ranks (every rank non-empty needs n >= world)."""
+    return [(n * r // world, n * (r + 1) // world) for r in range(world)]
+
+
+class SlabExchange:
+    """Buffers and send/recv lists of one rank.  Pure torch: usable on CPU tensors (gloo tests) and on the GPU."""
+
+    def __init__(self, nx: int, ny: int, nz: int, rank: int, world: int, device, dtype=None):
+        import torch
+        if nz < world or nx // 2 < world:
+            raise ValueError("every rank needs at least one plane and one x-slot")
+        self.nx, self.ny, self.nz, self.N = nx, ny, nz, nx // 2
+        self.rank, self.world = rank, world
+        self.kr, self.sr = split(nz, world), split(self.N, world)
+        self.k0, self.k1 = self.kr[rank]
+        self.s0, self.s1 = self.sr[rank]
+        self.nzl, self.nsl = self.k1 - self.k0, self.s1 - self.s0
+        dt = dtype or torch.float64
+        mk = lambda *shape: torch.zeros(shape, dtype=dt, device=device)
+        self.spec = mk(self.nzl, ny, self.N, 2)                       # slab spectrum (also the rhs of the x transform)
+        self.pencil = mk(nz, ny, self.nsl, 2)                         # full z columns of this rank's slots
+        self.send = [mk(self.nzl, ny, s1 - s0, 2) for (s0, s1) in self.sr]          # slab -> pencil: packed slices
+        self.recv = [mk(self.nzl, ny, s1 - s0, 2) for (s0, s1) in self.sr]          # pencil -> slab: chunks per source
+        self.w_ext = mk(self.nzl + 1, ny, nx)                         # w with the plane above (zeros at the top wall)
+        self.phi_ext = mk(self.nzl + 2, ny, nx)                       # phi with the planes below and above
+
+    # ---- halo of w (before a1): my first plane goes down, the neighbour's first plane arrives on top ----------
+    def w_halo(self):
+        sends = [(self.w_ext[0], self.rank - 1)] if self.rank > 0 else []
+        recvs = [(self.w_ext[self.nzl], self.rank + 1)] if self.rank + 1 < self.world else []
+        return sends, recvs
+
+    # ---- slab spectrum -> pencils (between a3 and a4) ----------------------------------------------------------
+    def to_pencils(self):
+        sends, recvs = [], []
+        for d, (s0, s1) in enumerate(self.sr):
+            self.send[d].copy_(self.spec[:, :, s0:s1, :])
+            sends.append((self.send[d], d))
+        for s, (k0, k1) in enumerate(self.kr):
+            recvs.append((self.pencil[k0:k1], s))                     # contiguous: lands in place
+        return sends, recvs
+
+    # ---- pencils -> slab spectrum (between a4 and a5) ------------------------------------------------------------
+    def to_slabs(self):
+        sends = [(self.pencil[k0:k1], d) for d, (k0, k1) in enumerate(self.kr)]   # contiguous views, no packing
+        recvs = [(self.recv[s], s) for s in range(self.world)]
+        return sends, recvs
+
+    def unpack_slabs(self):
+        for s, (s0, s1) in enumerate(self.sr):
+            self.spec[:, :, s0:s1, :].copy_(self.recv[s])
+
+    # ---- halo of phi (before a7): my last plane goes up; with beta != 0 my first plane also goes down ---------
+    def phi_halo(self, both: bool):
+        sends, recvs = [], []
+        if self.rank + 1 < self.world:
+            sends.append((self.phi_ext[self.nzl], self.rank + 1))
+        if self.rank > 0:
+            recvs.append((self.phi_ext[0], self.rank - 1))
+        if both:
+            if self.rank > 0:
+                sends.append((self.phi_ext[1], self.rank - 1))
+            if self.rank + 1 < self.world:
+                recvs.append((self.phi_ext[self.nzl + 1], self.rank + 1))
+        return sends, recvs
+
+
+class DistComm:
+    """Exchanges over a torch.distributed process group: grouped point-to-point operations (NCCL fuses a batch into one
+    all-to-all-like launch over NVLink / NVSwitch; gloo runs them on CPU tensors in the tests)."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+
+    def exchange(self, sends, recvs):
+        ops = []
+        for t, src in recvs:
+            if src == self.rank:
+                continue
+            ops.append(self.dist.P2POp(self.dist.irecv, t, src, self.group))
+        for t, dst in sends:
+            if dst == self.rank:                                        # my own share: a local copy
+                mine = [r for r, src in recvs if src == self.rank]
+                mine[0].copy_(t)
+                continue
+            ops.append(self.dist.P2POp(self.dist.isend, t, dst, self.group))
+        if ops:
+            for req in self.dist.batch_isend_irecv(ops):
+                req.wait()
+
+
+class LocalComm:
+    """All ranks live in this process and are stepped stage by stage; an exchange is a set of copies.  For checking the
+    decomposition on one GPU -- not a way to run it: the ranks run one after the other."""
+
+    @staticmethod
+    def exchange_all(lists: Sequence[Tuple[list, list]]):
+        """lists[r] = (sends, recvs) of rank r.  Message from s to d = the next unmatched send of s addressed to d."""
+        world = len(lists)
+        queues = {(s, d): [t for t, dst in lists[s][0] if dst == d] for s in range(world) for d in range(world)}
+        for d in range(world):
+            for t, src in lists[d][1]:
+                t.copy_(queues[(src, d)].pop(0))
+        assert all(len(q) == 0 for q in queues.values()), "unmatched send"
+
+
+class SlabProjection:
+    """One rank of the decomposed projection: fields of the local slab + the stages around the exchanges."""
+
+    def __init__(self, grid, rank: int, world: int, device="cuda"):
+        import torch
+        from .binding import SlabPlan
+        nx, ny, nz = grid[0], grid[1], grid[2]
+        self.x = SlabExchange(nx, ny, nz, rank, world, device)
+        self.plan = SlabPlan(grid, self.x.k0, self.x.k1, self.x.s0, self.x.s1)
+        nzl = self.x.nzl
+        self.u = torch.zeros((nzl, ny, nx), dtype=torch.float64, device=device)
+        self.v = torch.zeros_like(self.u)
+        self.p = torch.zeros_like(self.u)
+        self.w = self.x.w_ext[:nzl]                                   # the halo plane follows it in memory
+        self.phi = self.x.phi_ext[1:nzl + 1]                          # the halo planes surround it in memory
+        self.launches = 0
+
+    def load(self, u, v, w, p=None):
+        """Local planes [k0, k1) of global (or already local) host / device arrays."""
+        import torch
+        k0, k1 = self.x.k0, self.x.k1
+        for dst, src in ((self.u, u), (self.v, v), (self.w, w), (self.p, p)):
+            if src is None:
+                dst.zero_()
+                continue
+            t = torch.as_tensor(src)
+            dst.copy_(t[k0:k1] if t.shape[0] == self.x.nz else t)
+
+    # stages: each returns the (sends, recvs) that must be exchanged before the next one
+    def stage_w_halo(self):
+        return self.x.w_halo()
+
+    def stage_forward(self, alpha_dt, stream=None):
+        self.plan.slab_forward(self.u, self.v, self.w, alpha_dt, self.x.spec, stream)
+        self.launches += self.plan.last_launch_count
+        return self.x.to_pencils()
+
+    def stage_solve(self, stream=None):
+        self.plan.pencil_solve(self.x.pencil, stream)
+        self.launches += self.plan.last_launch_count
+        return self.x.to_slabs()
+
+    def stage_backward(self, beta, stream=None):
+        self.x.unpack_slabs()
+        self.plan.slab_backward(self.x.spec, self.phi, stream)
+        self.launches += self.plan.last_launch_count
+        return self.x.phi_halo(both=beta != 0.0)
+
+    def stage_project(self, alpha_dt, beta, stream=None):
+        self.plan.slab_project(self.u, self.v, self.w, self.p, self.phi, alpha_dt, beta, stream)
+        self.launches += self.plan.last_launch_count
+
+    def project(self, comm: DistComm, alpha_dt, beta=0.0, stream=None):
+        """The whole projection of this rank, exchanges over `comm` (all ranks call it together)."""
+        comm.exchange(*self.stage_w_halo())
+        comm.exchange(*self.stage_forward(alpha_dt, stream))
+        comm.exchange(*self.stage_solve(stream))
+        comm.exchange(*self.stage_backward(beta, stream))
+        self.stage_project(alpha_dt, beta, stream)
+
+    def destroy(self):
+        self.plan.destroy()
+
+
+def project_local(ranks: Sequence[SlabProjection], alpha_dt, beta=0.0):
+    """All ranks in one process, stage by stage (LocalComm)."""
+    LocalComm.exchange_all([r.stage_w_halo() for r in ranks])
+    LocalComm.exchange_all([r.stage_forward(alpha_dt) for r in ranks])
+    LocalComm.exchange_all([r.stage_solve() for r in ranks])
+    LocalComm.exchange_all([r.stage_backward(beta) for r in ranks])
+    for r in ranks:
+        r.stage_project(alpha_dt, beta)
