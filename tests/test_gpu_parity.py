@@ -383,6 +383,36 @@ def test_config3_full_size(oracle_ld):
     _full_size_check(oracle_ld, 3, 6)                       # 512x512x384, first substep, fused path (128 tiles)
 
 
+def test_config3_full_size_three_substeps(oracle_ld):
+    """configs[2] as BASELINE.json states it: 512x512x384, three RK substeps of projection back to back -- three
+    independent provisional triples (R14), ONE shared p, no host sync between the projections; fused path."""
+    torch = _torch()
+    if torch.cuda.get_device_properties(0).total_memory < 60e9:
+        pytest.skip("needs a GPU with >= 60 GB")
+    cases = [inputs.make_case(3, substep=s) for s in range(3)]
+    plan = make_plan(cases[0].grid)
+    p = torch.zeros(cases[0].u.shape, dtype=torch.float64, device="cuda")
+    phi = torch.empty_like(p)
+    dev = [[torch.from_numpy(a).cuda() for a in (c.u, c.v, c.w)] for c in cases]
+    for c, (u, v, w) in zip(cases, dev):
+        plan.pressure_projection(u, v, w, p, phi, c.alpha_dt, 0.0)
+    torch.cuda.synchronize()
+    assert plan.last_launch_count == 6
+    po = np.zeros(cases[0].u.shape)
+    for c, (u, v, w) in zip(cases, dev):
+        ref = oracle_projection(oracle_ld, c, 0.0, p=po)
+        got = [t.cpu().numpy() for t in (u, v, w)]
+        for g, r in zip(got, ref[:3]):
+            assert np.abs(g - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
+        pd = _post_div(oracle_ld, c, *got)
+        gate = div_gate(c, np.abs(ref[4]).max())
+        print(f"cfg 3 FULL substep alpha_dt={c.alpha_dt:.3e}: post-div {pd:.2e} (gate {gate:.2e})")
+        assert pd <= gate
+    assert rel_l2(p.cpu().numpy(), po) <= PHI_TOL               # the pressure accumulated over the three substeps
+    assert rel_l2(phi.cpu().numpy(), ref[4]) <= PHI_TOL
+    plan.destroy()
+
+
 # ---------------------------------------------------------------------------------------------
 # the calls never synchronise or allocate, so a whole projection can be captured in a CUDA graph
 # (small grids are launch-latency-bound: configs[0] is 7 launches of a few microseconds each)
