@@ -244,6 +244,66 @@ def run_reference(args) -> dict:
 # ------------------------------------------------------------------------------------------------
 # GPU leg
 # ------------------------------------------------------------------------------------------------
+def _config_table(main_cfg, dev, peak, steps_small=20):
+    """Device-resident projection time of the OTHER BASELINE.json configs (compact: ms, Mcell/s, moved GB/s, kernel
+    family), so that the one JSON line covers all five.  Inputs: N(0,1) fields generated on the device (the method is
+    direct: its cost does not depend on the data; parity of these configs is the tests' job, with the seeded recipe)."""
+    import torch
+    from paper_2103_15187_b200 import inputs
+    from paper_2103_15187_b200.binding import Plan
+    fam = {0: "generic", 1: "fast", 2: "fused", 6: "fused+twisted"}
+    out = {}
+    for cfg in (1, 2, 3, 5):
+        if cfg == main_cfg:
+            continue
+        case = inputs.make_case(cfg, fields=False)
+        free, _ = torch.cuda.mem_get_info()
+        if free < 8.0 * case.cells * 8:
+            out[f"configs[{cfg - 1}]"] = {"skipped": "not enough device memory"}
+            continue
+        shp = (case.nz, case.ny, case.nx)
+        g = torch.Generator(device=dev).manual_seed(cfg)
+        u, v, w = (torch.randn(shp, dtype=torch.float64, device=dev, generator=g) for _ in range(3))
+        w[0] = 0
+        if case.bc_x:
+            u[:, :, 0] = 0
+        if case.bc_y:
+            v[:, 0, :] = 0
+        p, phi = torch.zeros_like(u), torch.empty_like(u)
+        plan = Plan.from_grid(case.grid)
+        steps = steps_small if case.cells < 3e8 else 5
+        for _ in range(3):
+            plan.pressure_projection(u, v, w, p, phi, case.alpha_dt, 0.0)
+        plan.profile(True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            plan.pressure_projection(u, v, w, p, phi, case.alpha_dt, 0.0)
+        e1.record()
+        torch.cuda.synchronize()
+        plan.profile(False)
+        ms = e0.elapsed_time(e1) / steps
+        prof = plan.profile_read()
+        ncomp2 = 2 if (case.bc_x or case.bc_y) else 1
+        moved = 0.0
+        for name, (kms, cnt) in prof.items():
+            b = ALGO_BYTES_PER_CELL.get(name, 0.0)
+            if name in ("yz_forward", "yz_backward"):
+                b = 16.0 + 4.0 * ncomp2
+            moved += b * cnt / steps
+        out[f"configs[{cfg - 1}]"] = {
+            "grid": f"{case.nx}x{case.ny}x{case.nz}", "bc": "PN"[case.bc_x] + "PN"[case.bc_y], "ms": round(ms, 4),
+            "Mcell_per_s": round(case.cells / ms / 1e3, 1), "kernel_family": fam.get(plan.kernel_family, str(plan.kernel_family)),
+            "launches_per_step": plan.last_launch_count, "moved_bytes_per_cell": round(moved, 1),
+            "moved_GBps": round(moved * case.cells / (ms * 1e-3) / 1e9, 1), "frac_of_copy": round(moved * case.cells / (ms * 1e-3) / 1e9 / peak, 3),
+            "kernels_ms": {k: round(v[0] / v[1], 4) for k, v in prof.items()}, "steps": steps}
+        plan.destroy()
+        del u, v, w, p, phi
+        torch.cuda.empty_cache()
+    return out
+
+
 def _fluid_leg(plan, case, fields, stream, barrier, dev, peak, world, steps=3):
     """One whole fluid substep (fsei_fluid_substep) on the same workload: ms, per-kernel breakdown and a roofline entry for
     the implicit viscous step.  Extra device fields: 3 H + 3 rhs."""
@@ -429,10 +489,18 @@ def run_ours(args) -> dict:
         fluid, nl = _fluid_leg(plan, case, (u, v, w, p, phi), stream, barrier, dev, peak, world)
         launches += nl
 
+    # ---- the other BASELINE.json configs, compact ------------------------------------------------------------
+    all_cfg = None
+    if rank == 0 and world == 1 and not args.no_all_configs:
+        del u, v, w, p, phi
+        torch.cuda.empty_cache()
+        all_cfg = _config_table(args.config, dev, peak)
+        u = v = w = p = phi = None
+
     # ---- end to end: HOST buffers through the C ABI, H2D + D2H inside the timed region -------------------
     e2e = None
     if want_e2e:
-        del u, v, w, p, phi
+        u = v = w = p = phi = None
         torch.cuda.empty_cache()
         hp = torch.zeros(shp, dtype=torch.float64, pin_memory=True)
         hu, hv, hw = host
@@ -472,7 +540,7 @@ def run_ours(args) -> dict:
         "beta_nonzero": {"beta": beta_nz, "ms_per_step": round(ms_beta, 4), "Mcell_per_s": round(replica_throughput(case.cells, world, ms_beta), 1),
                          "note": "headline value is timed with beta = 0 (BASELINE configs state no Re); this is the same step with "
                                  "beta = alpha dt/(2 Re), Re = 3000"},
-        "fluid_substep": fluid,
+        "fluid_substep": fluid, "all_configs": all_cfg,
         "hbm_GBps_vs_8TBps": round(moved_gbps / 8000.0, 4),
     }
     if world > 1:
@@ -490,6 +558,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fluid", action="store_true", help="skip the whole-fluid-substep leg")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the compact table of the other configs")
     args = ap.parse_args()
     if args.impl == "reference":
         if int(os.environ.get("RANK", 0)) != 0:

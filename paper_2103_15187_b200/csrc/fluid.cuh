@@ -217,16 +217,17 @@ FSEI_GLOBAL(128, 1) k_visc_sweep_x(VTab T, double* __restrict__ f, double* __res
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// explicit terms.  CTA = 32 x 8 threads on a tile of 32 x-cells by 8 y-rows, marching KZ planes along z: a thread owns
-// one (i, j) column segment.  Every neighbour index and wall flag is computed once per thread; per plane a thread
-// issues 23 loads (the centre column and the two w neighbours of the upper face roll over from the plane before),
-// x/y neighbours are L1 hits of the same tile, the k-1 plane of the first step and the k+1 plane of every step are the
-// only new DRAM traffic.  Every floating-point operation is individually rounded in the order of the definition
+// explicit terms.  CTA = 32 x 8 threads on a tile of 32 x-cells by 8 y-rows, marching KZ planes along z (2.5-D
+// blocking): the (34 x 10) halo tiles of u, v, w, p and the tile of the three H_prev fields of plane k+3 are on their way
+// to a five-slot shared-memory ring (cp.async, 8-byte copies, one commit group per plane) while plane k is evaluated
+// from slots k-1, k, k+1 -- so the bytes in flight per SM do not depend on how many registers a thread can spare, every
+// input plane is read from L2/DRAM once per CTA (+ halo), and the only global accesses of the compute phase are the six
+// coalesced stores.  Every floating-point operation is individually rounded in the order of the definition
 // (oracle/fsei_fluid_oracle.c states it), so the results are bit-identical.
 //
-// Boundary conventions (V7): periodic wrap; beyond a wall the wall-normal component is 0 (face n) and a
-// tangential component is its ghost -q (no slip, wall midway); a convective flux through a wall face is 0; wall-face
-// rows (u at i = 0, v at j = 0 on a wall-bounded box; w at k = 0) get H = rhs = 0.
+// Boundary conventions (V7): periodic wrap (by the loader's source index); beyond a wall the wall-normal
+// component is 0 (face n) and a tangential component is its ghost -q (no slip, wall midway); a convective flux through
+// a wall face is 0; wall-face rows (u at i = 0, v at j = 0 on a wall-bounded box; w at k = 0) get H = rhs = 0.
 // ---------------------------------------------------------------------------------------------------------------
 FSEI_DEV double avg2(double a, double b) { return FSEI_MUL(0.5, FSEI_ADD(a, b)); }
 FSEI_DEV double sq_diff(double a, double b, double r) { return FSEI_MUL(FSEI_SUB(FSEI_MUL(a, a), FSEI_MUL(b, b)), r); }
@@ -247,113 +248,183 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
 }
 
 #ifndef FSEI_EXPL_KZ
-#define FSEI_EXPL_KZ 8
+#define FSEI_EXPL_KZ 32
 #endif
-#ifndef FSEI_EXPL_MINB
-#define FSEI_EXPL_MINB 2
-#endif
+#define FSEI_EXPL_TX 32
+#define FSEI_EXPL_TY 8
+#define FSEI_EXPL_RING 5
+#define FSEI_EXPL_PW (FSEI_EXPL_TX + 2)
+#define FSEI_EXPL_TILE (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
+// doubles per ring slot: four halo tiles (u, v, w, p) and three plain tiles (H_prev of u, v, w)
+#define FSEI_EXPL_SLOT (4 * FSEI_EXPL_TILE + 3 * FSEI_EXPL_TX * FSEI_EXPL_TY)
+#define FSEI_EXPL_SMEM (FSEI_EXPL_RING * FSEI_EXPL_SLOT * 8)
 
-// grid (ceil(nx/32), ceil(ny/8), ceil(nz/KZ)), block (32, 8)
-FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
+#if defined(__CUDACC__)
+__device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc)
 {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sdst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// one cell of the three components from the ring slots of planes k-1 (sm), k (s0), k+1 (sp).  EDGE = false: a cell with
+// no wall or z boundary among its neighbours (every cell of a periodic box except on its bottom and top planes): the
+// wall selects compile away.  The arithmetic of the two variants is the same, operation for operation.
+template <bool EDGE>
+__device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const double* __restrict__ s0, const double* __restrict__ sm,
+                                              const double* __restrict__ sp, int c, int hidx, size_t t, int k,
+                                              bool xlo, bool xhi, bool ylo, bool yhi, bool zlo, bool zhi)
+{
+    constexpr int PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE, NT = FSEI_EXPL_TX * FSEI_EXPL_TY;
     const SParams& S = A.S;
-    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
-    if (i >= S.nx || j >= S.ny) return;
-    const bool xper = S.bcx == BC_PERIODIC, yper = S.bcy == BC_PERIODIC;
-    const bool xlo = !xper && i == 0, xhi = !xper && i == S.nx - 1;      // x-face i / i+1 is a wall
-    const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
-    const int im = i > 0 ? i - 1 : (xper ? S.nx - 1 : 0), ip = i + 1 < S.nx ? i + 1 : (xper ? 0 : i);
-    const int jm = j > 0 ? j - 1 : (yper ? S.ny - 1 : 0), jp = j + 1 < S.ny ? j + 1 : (yper ? 0 : j);
-    const size_t plane = (size_t)S.nx * S.ny;
-    const size_t o00 = (size_t)j * S.nx + i, oP0 = (size_t)j * S.nx + ip, oM0 = (size_t)j * S.nx + im;
-    const size_t o0P = (size_t)jp * S.nx + i, o0M = (size_t)jm * S.nx + i, oPM = (size_t)jm * S.nx + ip, oMP = (size_t)jp * S.nx + im;
-    const double* __restrict__ u = A.u; const double* __restrict__ v = A.v; const double* __restrict__ w = A.w;
-    const double* __restrict__ p = A.p;
     const double rdx = S.rdx, rdy = S.rdy;
-    const int k0 = blockIdx.z * FSEI_EXPL_KZ, k1 = (k0 + FSEI_EXPL_KZ < S.nz) ? k0 + FSEI_EXPL_KZ : S.nz;
-
-    // rolling values of the centre column and of the w neighbours of the upper face
-    size_t b = (size_t)k0 * plane;
-    double u00 = u[b + o00], v00 = v[b + o00], w00 = w[b + o00], p00 = p[b + o00];
-    double wM0r = w[b + oM0], w0Mr = w[b + o0M];
-    double u_km = 0.0, v_km = 0.0, w_km = 0.0, p_km = 0.0;
-    if (k0 > 0) { u_km = u[b - plane + o00]; v_km = v[b - plane + o00]; w_km = w[b - plane + o00]; p_km = p[b - plane + o00]; }
-
-    for (int k = k0; k < k1; k++, b += plane) {
-        const bool zlo = k == 0, zhi = k == S.nz - 1;
-        const size_t bp = zhi ? b : b + plane, bm = zlo ? b : b - plane;
-        // ---- this plane
-        const double uP0 = xhi ? 0.0 : u[b + oP0], uM0 = u[b + oM0];
-        double u0P = u[b + o0P], u0M = u[b + o0M];
-        const double uPM = u[b + oPM];
-        double vP0 = v[b + oP0], vM0 = v[b + oM0];
-        const double v0P = yhi ? 0.0 : v[b + o0P], v0M = v[b + o0M], vMP = v[b + oMP];
-        double wP0 = w[b + oP0], w0P = w[b + o0P], wM0 = wM0r, w0M = w0Mr;
-        const double pM0 = p[b + oM0], p0M = p[b + o0M];
-        // ---- plane above (fluxes through the upper face; clamped loads are never used on the top plane) and below
-        const double u_kp = u[bp + o00], v_kp = v[bp + o00], w_kp = zhi ? 0.0 : w[bp + o00], p_kp = p[bp + o00];
-        const double wM_kp = w[bp + oM0], w0M_kp = w[bp + o0M];
-        const double uP_km = xhi ? 0.0 : u[bm + oP0], v0P_km = yhi ? 0.0 : v[bm + o0P];
-        // ghosts of the tangential components beyond a wall
+    const double *U0 = s0, *V0 = s0 + TILE, *W0 = s0 + 2 * TILE, *P0 = s0 + 3 * TILE;
+    const double *Um = sm, *Vm = sm + TILE, *Wm = sm + 2 * TILE, *Pm = sm + 3 * TILE;
+    const double *Up = sp, *Vp = sp + TILE, *Wp = sp + 2 * TILE;
+    const double u00 = U0[c], v00 = V0[c], w00 = W0[c], p00 = P0[c];
+    const double uP0 = (EDGE && xhi) ? 0.0 : U0[c + 1], uM0 = U0[c - 1], uPM = U0[c - PW + 1];
+    double u0P = U0[c + PW], u0M = U0[c - PW];
+    double vP0 = V0[c + 1], vM0 = V0[c - 1];
+    const double v0P = (EDGE && yhi) ? 0.0 : V0[c + PW], v0M = V0[c - PW], vMP = V0[c + PW - 1];
+    double wP0 = W0[c + 1], w0P = W0[c + PW], wM0 = W0[c - 1], w0M = W0[c - PW];
+    const double pM0 = P0[c - 1], p0M = P0[c - PW];
+    // plane above (fluxes through the upper face; never used on the top plane) and below (never used on the bottom one)
+    const double u_kp = Up[c], v_kp = Vp[c], w_kp = (EDGE && zhi) ? 0.0 : Wp[c], wM_kp = Wp[c - 1], w0M_kp = Wp[c - PW];
+    const double u_km = Um[c], v_km = Vm[c], w_km = Wm[c], p_km = Pm[c];
+    const double uP_km = (EDGE && xhi) ? 0.0 : Um[c + 1], v0P_km = (EDGE && yhi) ? 0.0 : Vm[c + PW];
+    if (EDGE) {                                      // ghosts of the tangential components beyond a wall
         if (ylo) u0M = -u00; if (yhi) u0P = -u00;
         if (xlo) vM0 = -v00; if (xhi) vP0 = -v00;
         if (xlo) wM0 = -w00; if (xhi) wP0 = -w00;
         if (ylo) w0M = -w00; if (yhi) w0P = -w00;
-        const double rc = S.rdzc[k], rm = S.rdzm[k];
-        const size_t t = b + o00;
+    }
+    const double rc = S.rdzc[k], rm = S.rdzm[k];
+    const double* hp = s0 + 4 * TILE + hidx;
 
-        // ---- u
-        if (xlo) { A.hu[t] = 0.0; A.ru[t] = 0.0; }
-        else {
-            const double fx = sq_diff(avg2(u00, uP0), avg2(uM0, u00), rdx);
-            const double fa = yhi ? 0.0 : FSEI_MUL(avg2(u00, u0P), avg2(vMP, v0P));
-            const double fb = ylo ? 0.0 : FSEI_MUL(avg2(u0M, u00), avg2(vM0, v00));
-            const double ga = zhi ? 0.0 : FSEI_MUL(avg2(u00, u_kp), avg2(wM_kp, w_kp));
-            const double gb = zlo ? 0.0 : FSEI_MUL(avg2(u_km, u00), avg2(wM0, w00));
-            double H = neg3(fx, FSEI_MUL(FSEI_SUB(fa, fb), rdy), FSEI_MUL(FSEI_SUB(ga, gb), rc));
-            if (A.fu) H = FSEI_ADD(H, A.fu[t]);
-            const double gzp = zhi ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), S.rdzm[k + 1]);
-            const double gzm = zlo ? FSEI_MUL(FSEI_SUB(u00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u00, u_km), rm);
-            const double lap = FSEI_ADD(FSEI_ADD(d2_grad(uP0, u00, uM0, rdx), d2_grad(u0P, u00, u0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
-            A.ru[t] = rhs_assemble(H, A.hu[t], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
-            A.hu[t] = H;
-        }
-        // ---- v
-        if (ylo) { A.hv[t] = 0.0; A.rv[t] = 0.0; }
-        else {
-            const double fa = xhi ? 0.0 : FSEI_MUL(avg2(v00, vP0), avg2(uPM, uP0));
-            const double fb = xlo ? 0.0 : FSEI_MUL(avg2(vM0, v00), avg2(u0M, u00));
-            const double fy = sq_diff(avg2(v00, v0P), avg2(v0M, v00), rdy);
-            const double ga = zhi ? 0.0 : FSEI_MUL(avg2(v00, v_kp), avg2(w0M_kp, w_kp));
-            const double gb = zlo ? 0.0 : FSEI_MUL(avg2(v_km, v00), avg2(w0M, w00));
-            double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), fy, FSEI_MUL(FSEI_SUB(ga, gb), rc));
-            if (A.fv) H = FSEI_ADD(H, A.fv[t]);
-            const double gzp = zhi ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), S.rdzm[k + 1]);
-            const double gzm = zlo ? FSEI_MUL(FSEI_SUB(v00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v00, v_km), rm);
-            const double lap = FSEI_ADD(FSEI_ADD(d2_grad(vP0, v00, vM0, rdx), d2_grad(v0P, v00, v0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
-            A.rv[t] = rhs_assemble(H, A.hv[t], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
-            A.hv[t] = H;
-        }
-        // ---- w
-        if (zlo) { A.hw[t] = 0.0; A.rw[t] = 0.0; }
-        else {
-            const double fa = xhi ? 0.0 : FSEI_MUL(avg2(w00, wP0), avg2(uP_km, uP0));
-            const double fb = xlo ? 0.0 : FSEI_MUL(avg2(wM0, w00), avg2(u_km, u00));
-            const double ga = yhi ? 0.0 : FSEI_MUL(avg2(w00, w0P), avg2(v0P_km, v0P));
-            const double gb = ylo ? 0.0 : FSEI_MUL(avg2(w0M, w00), avg2(v_km, v00));
-            const double fz = sq_diff(avg2(w00, w_kp), avg2(w_km, w00), rm);
-            double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), FSEI_MUL(FSEI_SUB(ga, gb), rdy), fz);
-            if (A.fw) H = FSEI_ADD(H, A.fw[t]);
-            const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), S.rdzc[k - 1]);
-            const double lap = FSEI_ADD(FSEI_ADD(d2_grad(wP0, w00, wM0, rdx), d2_grad(w0P, w00, w0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rm));
-            A.rw[t] = rhs_assemble(H, A.hw[t], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
-            A.hw[t] = H;
-        }
-        // ---- roll to the next plane
-        u_km = u00; v_km = v00; w_km = w00; p_km = p00;
-        u00 = u_kp; v00 = v_kp; w00 = zhi ? 0.0 : w_kp; p00 = p_kp;
-        wM0r = wM_kp; w0Mr = w0M_kp;
+    // ---- u
+    if (EDGE && xlo) { A.hu[t] = 0.0; A.ru[t] = 0.0; }
+    else {
+        const double fx = sq_diff(avg2(u00, uP0), avg2(uM0, u00), rdx);
+        const double fa = (EDGE && yhi) ? 0.0 : FSEI_MUL(avg2(u00, u0P), avg2(vMP, v0P));
+        const double fb = (EDGE && ylo) ? 0.0 : FSEI_MUL(avg2(u0M, u00), avg2(vM0, v00));
+        const double ga = (EDGE && zhi) ? 0.0 : FSEI_MUL(avg2(u00, u_kp), avg2(wM_kp, w_kp));
+        const double gb = (EDGE && zlo) ? 0.0 : FSEI_MUL(avg2(u_km, u00), avg2(wM0, w00));
+        double H = neg3(fx, FSEI_MUL(FSEI_SUB(fa, fb), rdy), FSEI_MUL(FSEI_SUB(ga, gb), rc));
+        if (A.fu) H = FSEI_ADD(H, A.fu[t]);
+        const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), S.rdzm[k + 1]);
+        const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(u00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u00, u_km), rm);
+        const double lap = FSEI_ADD(FSEI_ADD(d2_grad(uP0, u00, uM0, rdx), d2_grad(u0P, u00, u0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
+        A.ru[t] = rhs_assemble(H, hp[0], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
+        A.hu[t] = H;
+    }
+    // ---- v
+    if (EDGE && ylo) { A.hv[t] = 0.0; A.rv[t] = 0.0; }
+    else {
+        const double fa = (EDGE && xhi) ? 0.0 : FSEI_MUL(avg2(v00, vP0), avg2(uPM, uP0));
+        const double fb = (EDGE && xlo) ? 0.0 : FSEI_MUL(avg2(vM0, v00), avg2(u0M, u00));
+        const double fy = sq_diff(avg2(v00, v0P), avg2(v0M, v00), rdy);
+        const double ga = (EDGE && zhi) ? 0.0 : FSEI_MUL(avg2(v00, v_kp), avg2(w0M_kp, w_kp));
+        const double gb = (EDGE && zlo) ? 0.0 : FSEI_MUL(avg2(v_km, v00), avg2(w0M, w00));
+        double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), fy, FSEI_MUL(FSEI_SUB(ga, gb), rc));
+        if (A.fv) H = FSEI_ADD(H, A.fv[t]);
+        const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), S.rdzm[k + 1]);
+        const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(v00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v00, v_km), rm);
+        const double lap = FSEI_ADD(FSEI_ADD(d2_grad(vP0, v00, vM0, rdx), d2_grad(v0P, v00, v0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
+        A.rv[t] = rhs_assemble(H, hp[NT], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
+        A.hv[t] = H;
+    }
+    // ---- w
+    if (EDGE && zlo) { A.hw[t] = 0.0; A.rw[t] = 0.0; }
+    else {
+        const double fa = (EDGE && xhi) ? 0.0 : FSEI_MUL(avg2(w00, wP0), avg2(uP_km, uP0));
+        const double fb = (EDGE && xlo) ? 0.0 : FSEI_MUL(avg2(wM0, w00), avg2(u_km, u00));
+        const double ga = (EDGE && yhi) ? 0.0 : FSEI_MUL(avg2(w00, w0P), avg2(v0P_km, v0P));
+        const double gb = (EDGE && ylo) ? 0.0 : FSEI_MUL(avg2(w0M, w00), avg2(v_km, v00));
+        const double fz = sq_diff(avg2(w00, w_kp), avg2(w_km, w00), rm);
+        double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), FSEI_MUL(FSEI_SUB(ga, gb), rdy), fz);
+        if (A.fw) H = FSEI_ADD(H, A.fw[t]);
+        const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), S.rdzc[k - 1]);
+        const double lap = FSEI_ADD(FSEI_ADD(d2_grad(wP0, w00, wM0, rdx), d2_grad(w0P, w00, w0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rm));
+        A.rw[t] = rhs_assemble(H, hp[2 * NT], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
+        A.hw[t] = H;
     }
 }
+
+// grid (ceil(nx/32), ceil(ny/8), ceil(nz/KZ)), block (32, 8), dynamic shared memory FSEI_EXPL_SMEM
+FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
+{
+    constexpr int TX = FSEI_EXPL_TX, TY = FSEI_EXPL_TY, PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE, R = FSEI_EXPL_RING, SLOT = FSEI_EXPL_SLOT;
+    FSEI_DYN_SMEM(smraw);
+    double* ring = reinterpret_cast<double*>(smraw);
+    const SParams& S = A.S;
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
+    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, i = i0 + tx, j = j0 + ty;
+    const bool in = i < S.nx && j < S.ny;
+    const bool xper = S.bcx == BC_PERIODIC, yper = S.bcy == BC_PERIODIC;
+    const bool xlo = !xper && i == 0, xhi = !xper && i == S.nx - 1;      // x-face i / i+1 is a wall
+    const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
+    const bool xyedge = xlo || xhi || ylo || yhi;
+    const size_t plane = (size_t)S.nx * S.ny;
+    const int k0 = blockIdx.z * FSEI_EXPL_KZ, k1 = (k0 + FSEI_EXPL_KZ < S.nz) ? k0 + FSEI_EXPL_KZ : S.nz;
+
+    // loader: tile elements e = tid and tid + 256 of the halo tiles (source index wrapped in a periodic direction, clamped at
+    // a wall or a ragged edge) and this thread's own cell of the H_prev tiles; source pointers advance one plane per issue
+    const int e1 = tid + 256;
+    const bool has1 = e1 < TILE;
+    auto srcidx = [&](int e) {
+        const int jj = e / PW, ii = e - jj * PW;
+        int gi = i0 + ii - 1, gj = j0 + jj - 1;
+        if (xper) { gi = gi < 0 ? gi + S.nx : (gi >= S.nx ? gi - S.nx : gi); }
+        gi = gi < 0 ? 0 : (gi >= S.nx ? S.nx - 1 : gi);
+        if (yper) { gj = gj < 0 ? gj + S.ny : (gj >= S.ny ? gj - S.ny : gj); }
+        gj = gj < 0 ? 0 : (gj >= S.ny ? S.ny - 1 : gj);
+        return (size_t)gj * S.nx + gi;
+    };
+    const int kfirst = k0 - 1;                       // first plane the loader is asked for
+    size_t o0 = srcidx(tid) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
+    size_t o1 = srcidx(has1 ? e1 : tid) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
+    size_t oh = (size_t)(j < S.ny ? j : S.ny - 1) * S.nx + (i < S.nx ? i : S.nx - 1) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
+    int kk = kfirst, slot = (kfirst + R) % R;
+    auto issue = [&]() {                             // next plane kk -> its ring slot (nothing for a plane outside the grid)
+        if (kk >= 0 && kk < S.nz) {
+            double* sl = ring + slot * SLOT;
+            cp_async8(sl + tid, A.u + o0); cp_async8(sl + TILE + tid, A.v + o0);
+            cp_async8(sl + 2 * TILE + tid, A.w + o0); cp_async8(sl + 3 * TILE + tid, A.p + o0);
+            if (has1) {
+                cp_async8(sl + e1, A.u + o1); cp_async8(sl + TILE + e1, A.v + o1);
+                cp_async8(sl + 2 * TILE + e1, A.w + o1); cp_async8(sl + 3 * TILE + e1, A.p + o1);
+            }
+            if (kk >= k0 && kk < k1) {
+                double* h = sl + 4 * TILE + tid;
+                cp_async8(h, A.hu + oh); cp_async8(h + TX * TY, A.hv + oh); cp_async8(h + 2 * TX * TY, A.hw + oh);
+            }
+            o0 += plane; o1 += plane; oh += plane;
+        }
+        cp_async_commit();
+        kk++; slot = slot + 1 == R ? 0 : slot + 1;
+    };
+    issue(); issue(); issue(); issue();              // planes k0-1 .. k0+2
+    const int c = (ty + 1) * PW + tx + 1;
+    int sc = k0 % R;                                 // slot of plane k
+    size_t t = (size_t)k0 * plane + (size_t)j * S.nx + i;
+
+    for (int k = k0; k < k1; k++, t += plane) {
+        cp_async_wait<1>();                          // everything but the newest group (plane k+2): planes <= k+1 have landed
+        __syncthreads();                             // ... for every thread; and every thread is done with slot (k-2) mod R
+        issue();                                     // plane k+3 -> slot (k+3) mod R = (k-2) mod R
+        const int sm_ = sc == 0 ? R - 1 : sc - 1, sp_ = sc + 1 == R ? 0 : sc + 1;
+        if (in) {
+            const double* s0 = ring + sc * SLOT;
+            const double* sm = ring + sm_ * SLOT;
+            const double* sp = ring + sp_ * SLOT;
+            const bool zlo = k == 0, zhi = k == S.nz - 1;
+            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, tid, t, k, xlo, xhi, ylo, yhi, zlo, zhi);
+            else explicit_cell<false>(A, s0, sm, sp, c, tid, t, k, false, false, false, false, false, false);
+        }
+        sc = sp_;
+    }
+    cp_async_wait<0>();
+}
+#endif  // __CUDACC__
 
 }  // namespace fsei

@@ -278,6 +278,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         void* q = nullptr;
         if ((rc = dalloc(P, sizeof(double) * 9 * vtab_set_doubles(P->vnmax), &q))) return rc;
         P->vtab = static_cast<double*>(q);
+        CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM));
         P->visc_fast = !(flags & FSEI_PLAN_VISC_GENERIC) && bcx == BC_PERIODIC && bcy == BC_PERIODIC && visc_fast_supported(nx, ny);
         if (P->visc_fast) CU(visc_fast_init());
     }
@@ -366,7 +367,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
             CU(yzfused_init());
             CU(make_xi_blocked_map(XF, bcx == BC_NEUMANN, P->work, &P->xi_map));
         }
-        CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz + 16)));
+        CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)z_special_smem(nz, z_special_staged(nz))));
         return FSEI_OK;
     }
 
@@ -485,7 +486,7 @@ static int fast_spectral_solve(fsei_plan* P, cplx* spec, cudaStream_t st)
     const HostTables& T = P->T;
     const bool ny_neu = T.bcy == BC_NEUMANN;
     { LaunchTimer t(P, K_YF, st); CU(launch_y_fast(P->YF, false, ny_neu, spec, st)); }
-    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, spec); }
+    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, z_special_smem(T.nz, z_special_staged(T.nz)), st>>>(P->ZF, spec, z_special_staged(T.nz)); }
     CU(cudaGetLastError());
     {
         LaunchTimer t(P, K_ZD, st);
@@ -506,7 +507,7 @@ static int fused_spectral_solve(fsei_plan* P, double* phi, cudaStream_t st)
     const HostTables& T = P->T;
     const bool ny_neu = T.bcy == BC_NEUMANN;
     { LaunchTimer t(P, K_YZF, st); CU(launch_yz_forward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
-    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, P->work); }
+    { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, z_special_smem(T.nz, z_special_staged(T.nz)), st>>>(P->ZF, P->work, z_special_staged(T.nz)); }
     CU(cudaGetLastError());
     { LaunchTimer t(P, K_YZB, st); CU(launch_yz_backward(P->YZ, ny_neu, P->ZF.ncomp, P->work, st)); }
     { LaunchTimer t(P, K_XI, st); XFast xi = P->XF; xi.kchunk = P->kchunk_inv; CU(launch_xi_fast(xi, T.bcx == BC_NEUMANN, P->work, phi, st, &P->xi_map)); }
@@ -665,7 +666,7 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta};
     const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (P->T.nz + FSEI_EXPL_KZ - 1) / FSEI_EXPL_KZ);
-    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), 0, st>>>(A); }
+    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), FSEI_EXPL_SMEM, st>>>(A); }
     CU(cudaGetLastError());
     P->last_launches = 1;
     return FSEI_OK;
@@ -892,7 +893,7 @@ static int slab_plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, doub
     CU(cudaDeviceSynchronize());
     CU(xfast_init());
     CU(yfast_init());
-    CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4 * sizeof(cplx) * nz + 16)));
+    CU(cudaFuncSetAttribute(k_z_special, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)z_special_smem(nz, z_special_staged(nz))));
     return FSEI_OK;
 }
 
@@ -937,7 +938,7 @@ extern "C" int fsei_pencil_solve(fsei_plan* P, double* pencil, void* cuda_stream
     cplx* sp = reinterpret_cast<cplx*>(pencil);
     int launches = 0;
     if (P->s0 == 0) {
-        { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, 4 * sizeof(cplx) * T.nz + 16, st>>>(P->ZF, sp); }
+        { LaunchTimer t(P, K_GAUGE, st); k_z_special<<<1, 128, z_special_smem(T.nz, z_special_staged(T.nz)), st>>>(P->ZF, sp, z_special_staged(T.nz)); }
         CU(cudaGetLastError()); launches++;
     }
     {

@@ -147,7 +147,8 @@ FSEI_HD void zf_sweep_column(const ZFast& Z, cplx* S, int row, int slot)
 // issued before its dependent chain (the compiler cannot reorder loads over the stores of x itself).
 #define FSEI_ZCH 16
 // Returns the volume-weighted mean; the caller subtracts it from x (in parallel).
-FSEI_HD double zf_gauge_serial(const ZFast& Z, const double* FSEI_RESTRICT d, double* FSEI_RESTRICT x)
+FSEI_HD double zf_gauge_serial(const ZFast& Z, const double* FSEI_RESTRICT d, double* FSEI_RESTRICT x,
+                               const double* FSEI_RESTRICT dzc, const double* FSEI_RESTRICT dzm)
 {
     const int nz = Z.nz;
     double F = 0.0, acc = 0.0, vol = 0.0, xp = 0.0;
@@ -157,7 +158,7 @@ FSEI_HD double zf_gauge_serial(const ZFast& Z, const double* FSEI_RESTRICT d, do
 #pragma unroll
         for (int j = 0; j < FSEI_ZCH; j++) {
             const int k = (k0 + j < nz) ? k0 + j : nz - 1;
-            dd[j] = d[2 * (k - 1)]; wc[j] = Z.dzc[k - 1]; wm[j] = Z.dzm[k];
+            dd[j] = d[2 * (k - 1)]; wc[j] = dzc[k - 1]; wm[j] = dzm[k];
         }
 #pragma unroll
         for (int j = 0; j < FSEI_ZCH; j++) {
@@ -171,7 +172,7 @@ FSEI_HD double zf_gauge_serial(const ZFast& Z, const double* FSEI_RESTRICT d, do
 #pragma unroll
         for (int j = 0; j < FSEI_ZCH; j++) {
             const int k = (k0 + j < nz) ? k0 + j : nz - 1;
-            xx[j] = x[2 * k]; wc[j] = Z.dzc[k];
+            xx[j] = x[2 * k]; wc[j] = dzc[k];
         }
 #pragma unroll
         for (int j = 0; j < FSEI_ZCH; j++) if (k0 + j < nz) { acc += xx[j] * wc[j]; vol += wc[j]; }
@@ -192,7 +193,7 @@ FSEI_HD void zf_special_factor(const ZFast& Z, double lam, double* cp, double* i
 
 // Thomas on one component of a column held in shared memory, factorisation from the plan's tables
 FSEI_HD void zf_thomas_serial(const ZFast& Z, const double* FSEI_RESTRICT d, double* FSEI_RESTRICT x,
-                              const double* FSEI_RESTRICT cp, const double* FSEI_RESTRICT ip)
+                              const double* FSEI_RESTRICT cp, const double* FSEI_RESTRICT ip, const double* FSEI_RESTRICT za)
 {
     const int nz = Z.nz;
     double prev = 0.0;
@@ -201,7 +202,7 @@ FSEI_HD void zf_thomas_serial(const ZFast& Z, const double* FSEI_RESTRICT d, dou
 #pragma unroll
         for (int j = 0; j < FSEI_ZCH; j++) {
             const int k = (k0 + j < nz) ? k0 + j : nz - 1;
-            dd[j] = d[2 * k]; aa[j] = Z.za[k]; ii[j] = ip[k];
+            dd[j] = d[2 * k]; aa[j] = za[k]; ii[j] = ip[k];
         }
 #pragma unroll
         for (int j = 0; j < FSEI_ZCH; j++) if (k0 + j < nz) { prev = (dd[j] - aa[j] * prev) * ii[j]; dd[j] = prev; }
@@ -223,14 +224,20 @@ FSEI_HD void zf_thomas_serial(const ZFast& Z, const double* FSEI_RESTRICT d, dou
     }
 }
 
-// grid 1, block 128, dynamic shared memory 2 * 2 * nz * sizeof(cplx) + 16: gathers the special columns, solves
-// them (one thread per component), leaves them in Z.special
-FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec)
+// dynamic shared memory of k_z_special: the columns (4 nz cplx + 16) and, when `staged`, the tables of the serial chains
+// (dzc, dzm, za and the 8 rows of cpw: 11 nz doubles) -- a chain that reads its coefficients from L2 spends most of its
+// time waiting for them
+FSEI_HD size_t z_special_smem(int nz, bool staged) { return 4 * sizeof(cplx) * (size_t)nz + 16 + (staged ? 11 * sizeof(double) * (size_t)nz : 0); }
+FSEI_HD bool z_special_staged(int nz) { return z_special_smem(nz, true) <= 200 * 1024; }
+
+// grid 1, block 128: gathers the special columns, solves them (one thread per component), leaves them in Z.special
+FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec, int staged)
 {
     FSEI_DYN_SMEM(smraw);
     cplx* d = reinterpret_cast<cplx*>(smraw);            // [2][nz]
     cplx* x = d + 2 * Z.nz;                              // [2][nz]
     double* mean = reinterpret_cast<double*>(x + 2 * Z.nz);
+    double* tab = mean + 2;                              // [11][nz] when staged
     const int nz = Z.nz, tid = threadIdx.x;
     const bool pp = (Z.bcx == BC_PERIODIC && Z.bcy == BC_PERIODIC);
     const int ncol = pp ? 2 : 1;
@@ -239,13 +246,19 @@ FSEI_GLOBAL(128, 1) k_z_special(ZFast Z, const cplx* spec)
         d[i] = Z.special_in ? Z.special_in[i] : spec[zf_idx(Z, k, col == 0 ? 0 : (Z.ny >> 1), 0)];
         x[i] = cmake(0.0, 0.0);
     }
+    const double *dzc = Z.dzc, *dzm = Z.dzm, *za = Z.za, *cpw = Z.cpw;
+    if (staged) {
+        for (int i = tid; i < nz; i += 128) { tab[i] = Z.dzc[i]; tab[nz + i] = Z.dzm[i]; tab[2 * nz + i] = Z.za[i]; }
+        if (pp) for (int i = tid; i < 8 * nz; i += 128) tab[3 * nz + i] = Z.cpw[i];
+        dzc = tab; dzm = tab + nz; za = tab + 2 * nz; cpw = tab + 3 * nz;
+    }
     FSEI_SYNC();
     if ((tid & 31) == 0 && (tid >> 5) < 2 * ncol) {          // component t on lane 0 of warp t: the four chains run side by side
         const int t = tid >> 5, col = t >> 1, comp = t & 1;
         const double* dd = reinterpret_cast<const double*>(d + col * nz) + comp;
         double* xx = reinterpret_cast<double*>(x + col * nz) + comp;
-        if (t == 0) mean[0] = zf_gauge_serial(Z, dd, xx);
-        else if (pp) zf_thomas_serial(Z, dd, xx, Z.cpw + (size_t)t * nz, Z.cpw + (size_t)(4 + t) * nz);
+        if (t == 0) mean[0] = zf_gauge_serial(Z, dd, xx, dzc, dzm);
+        else if (pp) zf_thomas_serial(Z, dd, xx, cpw + (size_t)t * nz, cpw + (size_t)(4 + t) * nz, za);
     }
     FSEI_SYNC();
     const double gm = mean[0];

@@ -190,7 +190,7 @@ void spectral_solve(Ctx& c, cplx* spec, bool pcr = false)
     const HostTables& T = c.T;
     const bool yneu = T.bcy == BC_NEUMANN;
     yf(c.YF, false, yneu, spec);
-    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz + 16, [&] { k_z_special(c.ZF, spec); });
+    cuda_shim::launch(1, 128, z_special_smem(T.nz, z_special_staged(T.nz)), [&] { k_z_special(c.ZF, spec, z_special_staged(T.nz)); });
     size_t nthr = (size_t)T.nxc * T.ny;
     if (pcr && T.nz <= 32) cuda_shim::launch((unsigned)((nthr * 32 + 127) / 128), 128, 0, [&] { k_zf_pcr(c.ZF, spec); });
     else if (c.ZF.ncomp == 1) cuda_shim::launch((unsigned)((nthr + 127) / 128), 128, 0, [&] { k_zf_sweep<1>(c.ZF, spec); });
@@ -212,7 +212,7 @@ void fused_spectral_solve(Ctx& c, cplx* work, double* phi)
     YZ.ktw = c.ZF.ktw; c.mid.assign((size_t)T.nxc * T.ny * 2, cmake(0, 0)); YZ.mid = c.mid.data();
     const bool yneu = T.bcy == BC_NEUMANN;
     yz(YZ, false, yneu, c.ZF.ncomp, work);
-    cuda_shim::launch(1, 128, 4 * sizeof(cplx) * T.nz + 16, [&] { k_z_special(c.ZF, work); });
+    cuda_shim::launch(1, 128, z_special_smem(T.nz, z_special_staged(T.nz)), [&] { k_z_special(c.ZF, work, z_special_staged(T.nz)); });
     yz(YZ, true, yneu, c.ZF.ncomp, work);
     xib(c.XF, T.bcx == BC_NEUMANN, work, phi);
 }
