@@ -250,13 +250,16 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
 #ifndef FSEI_EXPL_KZ
 #define FSEI_EXPL_KZ 32
 #endif
+#ifndef FSEI_EXPL_MINB
+#define FSEI_EXPL_MINB 2
+#endif
 #define FSEI_EXPL_TX 32
 #define FSEI_EXPL_TY 8
 #define FSEI_EXPL_RING 5
 #define FSEI_EXPL_PW (FSEI_EXPL_TX + 2)
 #define FSEI_EXPL_TILE (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
-// doubles per ring slot: four halo tiles (u, v, w, p) and three plain tiles (H_prev of u, v, w)
-#define FSEI_EXPL_SLOT (4 * FSEI_EXPL_TILE + 3 * FSEI_EXPL_TX * FSEI_EXPL_TY)
+// doubles per ring slot: four halo tiles (u, v, w, p); H_prev of the next plane waits in three registers
+#define FSEI_EXPL_SLOT (4 * FSEI_EXPL_TILE)
 #define FSEI_EXPL_SMEM (FSEI_EXPL_RING * FSEI_EXPL_SLOT * 8)
 
 #if defined(__CUDACC__)
@@ -272,10 +275,10 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // wall selects compile away.  The arithmetic of the two variants is the same, operation for operation.
 template <bool EDGE>
 __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const double* __restrict__ s0, const double* __restrict__ sm,
-                                              const double* __restrict__ sp, int c, int hidx, size_t t, int k,
+                                              const double* __restrict__ sp, int c, const double (&hprev)[3], size_t t, int k,
                                               bool xlo, bool xhi, bool ylo, bool yhi, bool zlo, bool zhi)
 {
-    constexpr int PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE, NT = FSEI_EXPL_TX * FSEI_EXPL_TY;
+    constexpr int PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE;
     const SParams& S = A.S;
     const double rdx = S.rdx, rdy = S.rdy;
     const double *U0 = s0, *V0 = s0 + TILE, *W0 = s0 + 2 * TILE, *P0 = s0 + 3 * TILE;
@@ -299,7 +302,6 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         if (ylo) w0M = -w00; if (yhi) w0P = -w00;
     }
     const double rc = S.rdzc[k], rm = S.rdzm[k];
-    const double* hp = s0 + 4 * TILE + hidx;
 
     // ---- u
     if (EDGE && xlo) { A.hu[t] = 0.0; A.ru[t] = 0.0; }
@@ -314,7 +316,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), S.rdzm[k + 1]);
         const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(u00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u00, u_km), rm);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(uP0, u00, uM0, rdx), d2_grad(u0P, u00, u0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
-        A.ru[t] = rhs_assemble(H, hp[0], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
+        A.ru[t] = rhs_assemble(H, hprev[0], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
         A.hu[t] = H;
     }
     // ---- v
@@ -330,7 +332,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), S.rdzm[k + 1]);
         const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(v00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v00, v_km), rm);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(vP0, v00, vM0, rdx), d2_grad(v0P, v00, v0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
-        A.rv[t] = rhs_assemble(H, hp[NT], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
+        A.rv[t] = rhs_assemble(H, hprev[1], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
         A.hv[t] = H;
     }
     // ---- w
@@ -345,13 +347,13 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         if (A.fw) H = FSEI_ADD(H, A.fw[t]);
         const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), S.rdzc[k - 1]);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(wP0, w00, wM0, rdx), d2_grad(w0P, w00, w0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rm));
-        A.rw[t] = rhs_assemble(H, hp[2 * NT], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
+        A.rw[t] = rhs_assemble(H, hprev[2], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
         A.hw[t] = H;
     }
 }
 
 // grid (ceil(nx/32), ceil(ny/8), ceil(nz/KZ)), block (32, 8), dynamic shared memory FSEI_EXPL_SMEM
-FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
+FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
 {
     constexpr int TX = FSEI_EXPL_TX, TY = FSEI_EXPL_TY, PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE, R = FSEI_EXPL_RING, SLOT = FSEI_EXPL_SLOT;
     FSEI_DYN_SMEM(smraw);
@@ -383,7 +385,6 @@ FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
     const int kfirst = k0 - 1;                       // first plane the loader is asked for
     size_t o0 = srcidx(tid) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
     size_t o1 = srcidx(has1 ? e1 : tid) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
-    size_t oh = (size_t)(j < S.ny ? j : S.ny - 1) * S.nx + (i < S.nx ? i : S.nx - 1) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
     int kk = kfirst, slot = (kfirst + R) % R;
     auto issue = [&]() {                             // next plane kk -> its ring slot (nothing for a plane outside the grid)
         if (kk >= 0 && kk < S.nz) {
@@ -394,11 +395,7 @@ FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
                 cp_async8(sl + e1, A.u + o1); cp_async8(sl + TILE + e1, A.v + o1);
                 cp_async8(sl + 2 * TILE + e1, A.w + o1); cp_async8(sl + 3 * TILE + e1, A.p + o1);
             }
-            if (kk >= k0 && kk < k1) {
-                double* h = sl + 4 * TILE + tid;
-                cp_async8(h, A.hu + oh); cp_async8(h + TX * TY, A.hv + oh); cp_async8(h + 2 * TX * TY, A.hw + oh);
-            }
-            o0 += plane; o1 += plane; oh += plane;
+            o0 += plane; o1 += plane;
         }
         cp_async_commit();
         kk++; slot = slot + 1 == R ? 0 : slot + 1;
@@ -407,8 +404,12 @@ FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
     const int c = (ty + 1) * PW + tx + 1;
     int sc = k0 % R;                                 // slot of plane k
     size_t t = (size_t)k0 * plane + (size_t)j * S.nx + i;
+    double hnext[3] = {0.0, 0.0, 0.0};
+    if (in) { hnext[0] = A.hu[t]; hnext[1] = A.hv[t]; hnext[2] = A.hw[t]; }
 
     for (int k = k0; k < k1; k++, t += plane) {
+        const double hprev[3] = {hnext[0], hnext[1], hnext[2]};
+        if (in && k + 1 < k1) { hnext[0] = A.hu[t + plane]; hnext[1] = A.hv[t + plane]; hnext[2] = A.hw[t + plane]; }
         cp_async_wait<1>();                          // everything but the newest group (plane k+2): planes <= k+1 have landed
         __syncthreads();                             // ... for every thread; and every thread is done with slot (k-2) mod R
         issue();                                     // plane k+3 -> slot (k+3) mod R = (k-2) mod R
@@ -418,8 +419,8 @@ FSEI_GLOBAL(256, 2) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
             const double* sm = ring + sm_ * SLOT;
             const double* sp = ring + sp_ * SLOT;
             const bool zlo = k == 0, zhi = k == S.nz - 1;
-            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, tid, t, k, xlo, xhi, ylo, yhi, zlo, zhi);
-            else explicit_cell<false>(A, s0, sm, sp, c, tid, t, k, false, false, false, false, false, false);
+            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, hprev, t, k, xlo, xhi, ylo, yhi, zlo, zhi);
+            else explicit_cell<false>(A, s0, sm, sp, c, hprev, t, k, false, false, false, false, false, false);
         }
         sc = sp_;
     }
