@@ -70,15 +70,15 @@ cudaError_t xblocked_init()
 }
 
 // 3-D fp64 view of the blocked spectrum [N / CB][nz][ny][CB] complex: (2 ny CB doubles, nz, N / CB);
-// box = (2 CB doubles of ONE line, 1 plane, xi_box_tiles(N / CB) tiles): the tiles of a line land one after the other
+// box = (2 LPB CB doubles, 1 plane, xi_box_tiles(N / CB) tiles)
 template <class C, bool NEU> static cudaError_t xi_map_one(const XFast& P, const cplx* spec, TmaMap3D* out)
 {
-    constexpr int CB = FSEI_CB, NXT = C::N / CB;
+    constexpr int LPB = XShape<C, NEU>::LPB, CB = FSEI_CB, NXT = C::N / CB;
     EncodeTiledFn fn = tma_encode_fn();
     if (!fn) return cudaErrorNotSupported;
     cuuint64_t dims[3] = {(cuuint64_t)2 * P.ny * CB, (cuuint64_t)P.nz, (cuuint64_t)NXT};
     cuuint64_t strides[2] = {(cuuint64_t)P.ny * CB * sizeof(cplx), (cuuint64_t)P.nz * P.ny * CB * sizeof(cplx)};
-    cuuint32_t box[3] = {(cuuint32_t)(2 * CB), 1u, (cuuint32_t)xi_box_tiles(NXT)};
+    cuuint32_t box[3] = {(cuuint32_t)(2 * LPB * CB), 1u, (cuuint32_t)xi_box_tiles(NXT)};
     cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = fn(&out->m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<cplx*>(spec), dims, strides, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,

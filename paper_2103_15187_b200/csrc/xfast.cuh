@@ -316,12 +316,14 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
 // a6: phi(line) = scale * C2R / DCT-III of spec(line), in place
 // ---------------------------------------------------------------------------------------------------
 // CB > 0: the spectrum is in the blocked layout and the landing tile is fetched through `map`, a 3-D view
-// (2 ny CB doubles, nz, N / CB) of it, with ONE BOX PER LINE, (2 CB, 1, xi_box_tiles(N / CB)): the tiles of one line land
-// one after the other, i.e. the landing tile is line-major [LPB][N] in either layout.  That is what lets the Hermitian
-// pair step (half spectrum -> Z) fold into the first pass' loads: a thread forms its R0 inputs Z(n) straight from
-// X(n), X(N-n) of the landing tile (unit stride across the threads of a line in both directions: no bank conflicts), so
-// the line never takes the extra shared-memory round trip and CTA barrier of a separate pair phase.  Each pair is then
-// evaluated by both of its owners -- a few more flops on an fp64 pipe that is a third busy.
+// (2 ny CB doubles, nz, N / CB) of it with boxes (2 LPB CB, 1, xi_box_tiles(N / CB)): landing tile [N / CB][LPB][CB].
+// CB = 0 (natural layout): the landing tile is line-major [LPB][N], and the Hermitian pair step (half spectrum -> Z) is
+// FOLDED into the first pass' loads: a thread forms its R0 inputs Z(m) straight from X(m), X(N-m) of the landing tile
+// (unit stride across the threads of a line in both directions: no bank conflicts), so the line skips the separate pair
+// phase with its shared-memory round trip and CTA barrier; each pair is then evaluated by both of its owners -- a few more
+// flops on an fp64 pipe that is a third busy (configs[1]: 0.066 -> 0.058 ms).  On the blocked layout a line-major landing
+// tile would need one TMA box per line with a 32-byte inner dimension, which the TMA engine serves at a third of the
+// speed of the 128-byte boxes (measured: x_inverse 2.65 -> 8.7 ms at configs[3]), so that path keeps the pair phase.
 template <class C, int LPB, bool NEU, int CB = 0>
 FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 : 1)) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D map, const cplx* spec, double* phi)
 {
@@ -350,17 +352,13 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
             abar_expect(bar, bytes);
             bulk_g2s(land, spec + ((size_t)k * ny + j0) * N, bytes, bar);
         } else {                                                   // whole boxes: rows past ny arrive as zeros
-            constexpr int CBq = CB ? CB : 1, NXT = N / CBq, BT = xi_box_tiles(NXT);
+            constexpr int NXT = N / (CB ? CB : 1), BT = xi_box_tiles(NXT);
             abar_expect(bar, (unsigned)(LPB * N * sizeof(cplx)));
 #pragma unroll
-            for (int l = 0; l < LPB; l++)
-#pragma unroll
-                for (int b = 0; b < NXT / BT; b++) tma_load_3d(land + (size_t)l * N + (size_t)b * BT * CBq, &map, 2 * (j0 + l) * CBq, k, b * BT, bar);
+            for (int b = 0; b < NXT / BT; b++) tma_load_3d(land + (size_t)b * BT * LPB * CB, &map, 2 * j0 * CB, k, b * BT, bar);
             if (k + 1 < k1) {                                      // the plane after: DRAM -> L2 now
 #pragma unroll
-                for (int l = 0; l < LPB; l++)
-#pragma unroll
-                    for (int b = 0; b < NXT / BT; b++) tma_prefetch_3d(&map, 2 * (j0 + l) * CBq, k + 1, b * BT);
+                for (int b = 0; b < NXT / BT; b++) tma_prefetch_3d(&map, 2 * j0 * CB, k + 1, b * BT);
             }
         }
     };
@@ -375,13 +373,10 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
     cplx* lbuf = buf + li * C::PITCH;
     double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
     const double scale = P.scale;
-    const cplx* FSEI_RESTRICT lland = land + (size_t)li * N;       // this line's packed half spectrum
-    const cplx* FSEI_RESTRICT tr2c_r = tr2c;
-    const cplx* FSEI_RESTRICT tdct_r = tdct;
 
-    // Z(m), m in [0, N): packed half spectrum -> the complex sequence whose inverse FFT is the real line (Hermitian pair
-    // step, preceded by the inverse quarter-wave twiddle on Neumann lines); element m and element N - m come from the
-    // same pair (X_p, X_{N-p}), p = min(m, N - m)
+    // Z(m), m in [0, N), of this thread's line from a line-major landing tile (CB == 0): element m and element N - m come
+    // from the same pair (X_p, X_{N-p}), p = min(m, N - m)
+    const cplx* FSEI_RESTRICT lland = land + (size_t)li * N;
     auto zin = [&](int m) -> cplx {
         if (m == 0) {
             const cplx s = lland[0];
@@ -392,27 +387,66 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
         const bool lo = 2 * m <= N;
         const int p = lo ? m : N - m;
         cplx xk = lland[p], xm = lland[N - p];
-        if (NEU) { xk = dct_tw_inv(xk, tdct_r[p]); xm = dct_tw_inv(xm, tdct_r[N - p]); }
+        if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
         const cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));    // (Xk + conj Xm)/2
         const cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));   // (Xk - conj Xm)/2
-        const cplx O = cmulc(Tt, tr2c_r[p]);
+        const cplx O = cmulc(Tt, tr2c[p]);
         return lo ? cmake(E.re - O.im, E.im + O.re)                            // E + i O
                   : cmake(E.re + O.im, -(E.im - O.re));                        // conj(E - i O)
     };
 
     for (int k = k0; k < k1; k++) {
         abar_wait(bar, parity); parity ^= 1;
-        auto next = [&]() { if (tid == 0 && k + 1 < k1) issue(k + 1); };       // landing tile consumed: fetch the next plane
+        // packed half spectrum -> Z (Hermitian pair step, preceded by the inverse quarter-wave twiddle)
+        // gl(p): slot p of line l2 in the landing tile; lb: that line's buffer
+        // (restrict: the landing tile and the tables are only read here, the line buffers only written, so the loads of
+        // the next pair may be issued before the stores of this one)
+        const cplx* FSEI_RESTRICT land_r = land;
+        const cplx* FSEI_RESTRICT tr2c_r = tr2c;
+        const cplx* FSEI_RESTRICT tdct_r = tdct;
+        auto pair_load = [&](int l2, cplx* FSEI_RESTRICT lb, int p) {
+            auto g = [&](int q) -> cplx { return CB ? land_r[((q / (CB ? CB : 1)) * LPB + l2) * CB + q % (CB ? CB : 1)] : land_r[l2 * N + q]; };
+            if (p == 0) {
+                cplx s = g(0);
+                double x0 = s.re, xn = s.im;
+                if (NEU) xn *= 1.41421356237309504880168872420969808;
+                lb[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
+            } else {
+                cplx xk = g(p), xm = g(N - p);
+                if (NEU) { xk = dct_tw_inv(xk, tdct_r[p]); xm = dct_tw_inv(xm, tdct_r[N - p]); }
+                cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
+                cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2
+                cplx O = cmulc(Tt, tr2c_r[p]);
+                lb[C::pad(p)] = cmake(E.re - O.im, E.im + O.re);               // E + i O
+                if (p != N - p) lb[C::pad(N - p)] = cmake(E.re + O.im, -(E.im - O.re));   // conj(E - i O)
+            }
+        };
+        if (CB != 0) {
+            // landing tile is [tile][line][CB]: adjacent threads read adjacent elements of it
+            constexpr int CBq = CB ? CB : 1, HP = N / 2 / CBq + 1, NW = HP * LPB * CBq, IT = (NW + T * LPB - 1) / (T * LPB);
+#pragma unroll
+            for (int it = 0; it < IT; it++) {
+                const int wi = tid + it * nt;
+                const int cc = wi % CBq, l2 = (wi / CBq) % LPB, p = (wi / (CBq * LPB)) * CBq + cc;
+                if (wi >= NW || p > N / 2 || l2 >= nl) continue;
+                pair_load(l2, buf + l2 * C::PITCH, p);
+            }
+        }
+        auto next = [&]() { if (tid == 0 && k + 1 < k1) issue(k + 1); };          // landing tile consumed: fetch the next plane
+        if (CB != 0) { FSEI_SYNC(); next(); }
         double* gl = phi + ((size_t)k * ny + j) * n;
-        auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, zin, v0); };
+        auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, SmIn<C>{lbuf}, v0); };
+        auto load0f = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, zin, v0); };
         if (!NEU) {
             auto out = [&](int t, cplx z, int) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
-            fft_line<C, true, false, false>(tl, act, lbuf, tws, load0, out, next, li);
+            if constexpr (CB == 0) fft_line<C, true, false, false>(tl, act, lbuf, tws, load0f, out, next, li);
+            else fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{}, li);
         } else {
             auto out = [&](int t, cplx z, int) {
                 lxs[xs_pad(makhoul(2 * t, n))] = z.re * scale; lxs[xs_pad(makhoul(2 * t + 1, n))] = z.im * scale;
             };
-            fft_line<C, true, false, false>(tl, act, lbuf, tws, load0, out, next, li);
+            if constexpr (CB == 0) fft_line<C, true, false, false>(tl, act, lbuf, tws, load0f, out, next, li);
+            else fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{}, li);
             FSEI_SYNC();
             if (act) {
 #pragma unroll

@@ -120,9 +120,9 @@ template <class C, bool NEU> void xib_one(const XFast& P, const cplx* spec, doub
 {
     constexpr int LPB = XShape<C, NEU>::LPB, CB = FSEI_CB, NXT = C::N / CB;
     dim3 grid((P.ny + LPB - 1) / LPB, (P.nz + P.kchunk - 1) / P.kchunk);
-    // the view make_xi_blocked_map (fast_x.cu) encodes: (2 ny CB doubles, nz, N / CB), one box per line (2 CB, 1, xi_box_tiles)
+    // the view make_xi_blocked_map (fast_x.cu) encodes: (2 ny CB doubles, nz, N / CB), boxes (2 LPB CB, 1, xi_box_tiles)
     TmaMap3D map{reinterpret_cast<const unsigned char*>(spec), (size_t)P.ny * CB * sizeof(cplx), (size_t)P.nz * P.ny * CB * sizeof(cplx),
-                 (unsigned)sizeof(double), 2u * P.ny * CB, (unsigned)P.nz, (unsigned)NXT, 2u * CB, 1u, (unsigned)xi_box_tiles(NXT)};
+                 (unsigned)sizeof(double), 2u * P.ny * CB, (unsigned)P.nz, (unsigned)NXT, 2u * LPB * CB, 1u, (unsigned)xi_box_tiles(NXT)};
     cuda_shim::launch(grid, C::T * LPB, XSmemLayout<C, LPB, NEU, LPB>::BYTES, [&] { k_xi_fast<C, LPB, NEU, FSEI_CB>(P, map, spec, phi); });
 }
 void xib(const XFast& P, bool neu, const cplx* spec, double* phi)
