@@ -164,8 +164,9 @@ int fsei_explicit_terms(fsei_plan* plan, const double* u, const double* v, const
  * the staggered position of each component with no-slip walls (V3-V6); wall faces are never modified.
  *   ru, rv, rw : in: right-hand sides; DESTROYED (used as scratch).  beta >= 0 finite    else FSEI_ERR_ARG
  *   No field may alias another.  Any nx, ny, nz the plan accepts; both boundary types.
- * The factorisation tables for `beta` are rebuilt (one extra small launch, plus a few microseconds of host work)
- * whenever beta differs from the previous call on this plan.  Two kernel families: periodic x
+ * The factorisation tables for `beta` are built on first use (one extra small launch, plus a few microseconds of host
+ * work) and kept for the last four values of beta used on this plan (a three-stage Runge-Kutta scheme cycles through
+ * three); under stream capture they are rebuilt inside the graph, so a replay never depends on cached state.  Two kernel families: periodic x
  * and y with nx/32 in {2,4,8,12,16,24,32} and ny/32 in {2,3,4,6,8,12,16,24,32} run two fused launches for the three
  * components (40 B/cell each); any other grid runs the generic sweeps (nine launches).
  */

@@ -223,7 +223,7 @@ FSEI_GLOBAL(128, 1) k_visc_sweep_x(VTab T, double* __restrict__ f, double* __res
 // from slots k-1, k, k+1 -- so the bytes in flight per SM do not depend on how many registers a thread can spare, every
 // input plane is read from L2/DRAM once per CTA (+ halo), and the only global accesses of the compute phase are the six
 // coalesced stores.  Every floating-point operation is individually rounded in the order of the definition
-// (oracle/fsei_fluid_oracle.c states it), so the results are bit-identical.
+// (V10 states it), so the results are bit-identical.
 //
 // Boundary conventions (V7): periodic wrap (by the loader's source index); beyond a wall the wall-normal
 // component is 0 (face n) and a tangential component is its ghost -q (no slip, wall midway); a convective flux through

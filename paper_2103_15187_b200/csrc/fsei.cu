@@ -45,6 +45,7 @@ static bool misaligned(const void* p) { return (reinterpret_cast<size_t>(p) & 15
 // ------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------
+#define FSEI_VSLOTS 4
 enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, K_MLS, K_VXZ, K_VZY, FSEI_NKERNELS };
 
 struct fsei_plan {
@@ -62,8 +63,10 @@ struct fsei_plan {
     int last_launches = 0;
     const double* zc_dev = nullptr;      // z-face coordinates (IB-MLS node positions)
     bool slab = false; int k0 = 0, k1 = 0, s0 = 0, s1 = 0;   // z-slab / x-slot-pencil share of a multi-GPU decomposition (fsei_slab_plan_create)
-    bool visc_fast = false; VFastLine vline_x, vline_y;   // fast viscous family: host-built line tables of the last beta
-    double* vtab = nullptr; int vnmax = 0; double visc_beta = NAN;   // implicit viscous step: factorisation tables of the last beta
+    // implicit viscous step: factorisation tables of the last FSEI_VSLOTS values of beta (a three-stage Runge-Kutta scheme
+    // cycles through three), device tables in vtab[slot], host-built line tables of the fast family beside them
+    bool visc_fast = false; VFastLine vline_x[FSEI_VSLOTS], vline_y[FSEI_VSLOTS]; int vnsig_x[FSEI_VSLOTS], vnsig_y[FSEI_VSLOTS];
+    double* vtab = nullptr; int vnmax = 0; double visc_beta[FSEI_VSLOTS] = {NAN, NAN, NAN, NAN}; int visc_next = 0;
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
     // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
     bool profiling = false;
@@ -276,7 +279,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     {
         P->vnmax = nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz);
         void* q = nullptr;
-        if ((rc = dalloc(P, sizeof(double) * 9 * vtab_set_doubles(P->vnmax), &q))) return rc;
+        if ((rc = dalloc(P, sizeof(double) * FSEI_VSLOTS * 9 * vtab_set_doubles(P->vnmax), &q))) return rc;
         P->vtab = static_cast<double*>(q);
         CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM));
         P->visc_fast = !(flags & FSEI_PLAN_VISC_GENERIC) && bcx == BC_PERIODIC && bcy == BC_PERIODIC && visc_fast_supported(nx, ny);
@@ -672,10 +675,10 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     return FSEI_OK;
 }
 
-static VTab visc_tab(const fsei_plan* P, int comp, int dir)
+static VTab visc_tab(const fsei_plan* P, int slot, int comp, int dir)
 {
     const HostTables& T = P->T;
-    const double* t = P->vtab + (size_t)(comp * 3 + dir) * vtab_set_doubles(P->vnmax);
+    const double* t = P->vtab + (size_t)(slot * 9 + comp * 3 + dir) * vtab_set_doubles(P->vnmax);
     const size_t m = (size_t)P->vnmax;
     VTab V;
     V.ip = t; V.am = t + m; V.cp = t + 2 * m; V.wc = t + 3 * m; V.er = t + 4 * m; V.ipl = t + 5 * m;
@@ -699,27 +702,38 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const HostTables& T = P->T;
     int launches = 0;
-    // factorisation tables for this beta (kept while beta does not change)
-    if (!(P->visc_beta == beta)) {
-        VFactorArgs A{P->S, beta, P->vtab, P->vnmax};
+    // factorisation tables for this beta: kept per value in FSEI_VSLOTS slots (round-robin replacement).  Under stream
+    // capture the device tables are rebuilt inside the graph even on a hit, so a replay never depends on a slot that an
+    // eager call with other betas has overwritten in the meantime (the host-built tables travel as kernel parameters).
+    int slot = -1;
+    for (int i = 0; i < FSEI_VSLOTS; i++) if (P->visc_beta[i] == beta) slot = i;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    CU(cudaStreamIsCapturing(st, &cap));
+    const bool miss = slot < 0;
+    if (miss) {
+        slot = P->visc_next; P->visc_next = (slot + 1) % FSEI_VSLOTS;
+        if (P->visc_fast) {
+            visc_fast_line(T.nx, P->S.rdx, beta, &P->vline_x[slot]); P->vnsig_x[slot] = visc_fast_nsig(P->vline_x[slot]);
+            visc_fast_line(T.ny, P->S.rdy, beta, &P->vline_y[slot]); P->vnsig_y[slot] = visc_fast_nsig(P->vline_y[slot]);
+        }
+        P->visc_beta[slot] = beta;
+    }
+    if (miss || cap != cudaStreamCaptureStatusNone) {
+        VFactorArgs A{P->S, beta, P->vtab + (size_t)slot * 9 * vtab_set_doubles(P->vnmax), P->vnmax};
         { LaunchTimer t(P, K_VFACT, st); k_visc_factor<<<9, 32, 0, st>>>(A); }
         CU(cudaGetLastError());
-        if (P->visc_fast) {
-            visc_fast_line(T.nx, P->S.rdx, beta, &P->vline_x);
-            visc_fast_line(T.ny, P->S.rdy, beta, &P->vline_y);
-        }
-        P->visc_beta = beta; launches++;
+        launches++;
     }
     if (P->visc_fast) {
         VFastArgs A;
         for (int c = 0; c < 3; c++) {
-            const VTab V = visc_tab(P, c, DIR_Z);
+            const VTab V = visc_tab(P, slot, c, DIR_Z);
             A.zam[c] = V.am; A.zip[c] = V.ip; A.zcp[c] = V.cp; A.r[c] = r[c]; A.q[c] = q[c];
         }
         A.nx = T.nx; A.ny = T.ny; A.nz = T.nz;
-        A.L = P->vline_x; A.nsig = visc_fast_nsig(A.L);
+        A.L = P->vline_x[slot]; A.nsig = P->vnsig_x[slot];
         { LaunchTimer t(P, K_VXZ, st); CU(launch_visc_xz(A, st)); }
-        A.L = P->vline_y; A.nsig = visc_fast_nsig(A.L);
+        A.L = P->vline_y[slot]; A.nsig = P->vnsig_y[slot];
         { LaunchTimer t(P, K_VZY, st); CU(launch_visc_zy(A, st)); }
         P->last_launches = launches + 2;
         return FSEI_OK;
@@ -728,7 +742,7 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
     const size_t plane = (size_t)T.nx * T.ny;
     for (int c = 0; c < 3; c++) {
         {
-            VTab V = visc_tab(P, c, DIR_X);
+            VTab V = visc_tab(P, slot, c, DIR_X);
             LaunchTimer t(P, K_VX, st);
             const unsigned g = (unsigned)((nlx + 127) / 128);
             if (V.cyclic) k_visc_sweep_x<true, false><<<g, 128, 0, st>>>(V, r[c], nullptr, nlx);
@@ -736,7 +750,7 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
         }
         CU(cudaGetLastError());
         {
-            VTab V = visc_tab(P, c, DIR_Y);
+            VTab V = visc_tab(P, slot, c, DIR_Y);
             LaunchTimer t(P, K_VY, st);
             const unsigned g = (unsigned)((nly + 127) / 128);
             if (V.cyclic) k_visc_sweep_strided<true, false><<<g, 128, 0, st>>>(V, r[c], nullptr, T.nx, (size_t)T.nx, plane, nly);
@@ -744,7 +758,7 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
         }
         CU(cudaGetLastError());
         {
-            VTab V = visc_tab(P, c, DIR_Z);
+            VTab V = visc_tab(P, slot, c, DIR_Z);
             LaunchTimer t(P, K_VZ, st);
             k_visc_sweep_strided<false, true><<<(unsigned)((nlz + 127) / 128), 128, 0, st>>>(V, r[c], q[c], (int)nlz, plane, 0, nlz);
         }

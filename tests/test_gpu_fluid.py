@@ -208,3 +208,46 @@ def test_viscous_fast_family_vs_oracle(oracle_ld, shape, beta):
     for c, qo in enumerate((uo, vo, wo)):
         assert np.abs(dg[c].cpu().numpy() - qo).max() <= 1e-12 * np.abs(qo - f[c]).max() + 2 * EPS * np.abs(qo).max()
     pg.destroy()
+
+
+def test_viscous_beta_cache_and_graph_capture(oracle_ld):
+    """The factorisation tables are kept for the last four betas (RK3 cycles through three); a whole fluid substep can be
+    captured in a CUDA graph (no call synchronises or allocates) and replays correctly after other betas have been used."""
+    import torch
+    shape = (64, 64, 16)
+    g, f = _case(shape, (P, P), seed=45, n=7)
+    u, v, w, p, ru, rv, rw = f
+    plan = _plan(g)
+    betas = [1e-4, 2e-4, 3e-4]
+    d = _dev([u, v, w, ru, rv, rw])
+    for b in betas:
+        plan.viscous_step(*d, b)
+        assert plan.last_launch_count == 3                          # first use: tables built
+    for b in betas:
+        plan.viscous_step(*d, b)
+        assert plan.last_launch_count == 2                          # cached
+    # --- graph capture of one fluid substep
+    dt, Re = 2e-3, 300.0
+    beta = dt / (2 * Re)
+    u0, v0, w0 = [0.1 * t for t in (u, v, w)]
+    fld = _dev([u0, v0, w0, np.zeros_like(u)] + [np.zeros_like(u) for _ in range(7)])
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        plan.fluid_substep(*fld, 1.5 * dt, -0.5 * dt, dt, beta)
+    torch.cuda.synchronize()
+    for b in (5e-4, 6e-4, 7e-4, 8e-4, 9e-4):                        # evict every slot
+        plan.viscous_step(*_dev([u, v, w, ru, rv, rw]), b)
+    for t, a in zip(fld, [u0, v0, w0, np.zeros_like(u)] + [np.zeros_like(u) for _ in range(7)]):
+        t.copy_(torch.from_numpy(a))
+    graph.replay()
+    torch.cuda.synchronize()
+    uo, vo, wo, po = u0.copy(), v0.copy(), w0.copy(), np.zeros_like(u)
+    ho = [np.zeros_like(u) for _ in range(3)]
+    r = oracle_ld.explicit_terms(g, uo, vo, wo, po, *ho, 1.5 * dt, -0.5 * dt, dt, beta)
+    oracle_ld.viscous_step(g, uo, vo, wo, *r, beta)
+    oracle_ld.pressure_projection(g, uo, vo, wo, po, dt, beta)
+    for c, ref in enumerate((uo, vo, wo, po)):
+        assert np.abs(fld[c].cpu().numpy() - ref).max() <= 1e-11 * max(1.0, np.abs(ref).max()), c
+    plan.destroy()
