@@ -551,6 +551,69 @@ def run_ours(args) -> dict:
     return out if rank == 0 else None
 
 
+def run_slab(args) -> dict:
+    """--parallel slab: ONE projection of the workload decomposed over the ranks: z-slabs for a1-a3 and
+    a5-a7, x-slot pencils for a4, two exchanges over torch.distributed (NCCL).  Strong scaling: total work fixed."""
+    import torch
+    import torch.distributed as dist
+    from paper_2103_15187_b200 import inputs, slab
+    rank = int(os.environ.get("RANK", 0)); local = int(os.environ.get("LOCAL_RANK", 0)); world = int(os.environ.get("WORLD_SIZE", 1))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libfsei has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if not dist.is_initialized():
+        if world > 1:
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group("gloo", init_method="tcp://127.0.0.1:29533", rank=0, world_size=1)
+    case = inputs.make_case(args.config, fields=False)
+    sp = slab.SlabProjection(case.grid, rank, world, device=dev)
+    g = torch.Generator(device=dev).manual_seed(100 + rank)
+    for t in (sp.u, sp.v, sp.w):
+        t.copy_(torch.randn(t.shape, dtype=torch.float64, device=dev, generator=g))
+    if rank == 0:
+        sp.w[0] = 0
+    comm = slab.DistComm()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        sp.project(comm, case.alpha_dt, 0.0)
+    barrier()
+    sampler = ClockSampler(local)
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sp.launches = 0
+    barrier()
+    t0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        sp.project(comm, case.alpha_dt, 0.0)
+    e1.record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms = max_over_ranks(e0.elapsed_time(e1), dev) / args.steps
+    x = sp.x
+    out = {"metric": METRIC, "value": case.cells / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": _workload_name(case), "cells": case.cells, "parallelism": f"z-slabs x{world} / x-slot pencils x{world}",
+                      "exchange_bytes_per_rank_per_step": 2 * 16 * x.nzl * x.ny * (x.N - x.nsl) + 0,
+                      "note": "unfused fast-family kernels per rank + 2 all-to-all exchanges (NCCL grouped send/recv); inputs N(0,1) "
+                              "generated on the device; fields larger than L2"},
+           "clocks": clocks, "gpu_launches": sp.launches,
+           "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "skipped": "slab mode times device-resident fields"}}
+    sp.destroy()
+    if dist.is_initialized():
+        dist.destroy_process_group()
+    return out if rank == 0 else None
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -562,7 +625,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fluid", action="store_true", help="skip the whole-fluid-substep leg")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the compact table of the other configs")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default; the headline path is single-GPU) or ONE projection decomposed into "
+                         "z-slabs / x-slot pencils over the N ranks (paper_2103_15187_b200/slab.py; strong scaling)")
     args = ap.parse_args()
+    if args.parallel == "slab" and args.impl != "reference":
+        out = run_slab(args)
+        if out is not None:
+            print(json.dumps(out), flush=True)
+        return
     if args.impl == "reference":
         if int(os.environ.get("RANK", 0)) != 0:
             return

@@ -141,3 +141,26 @@ def test_slab_plan_errors():
     with pytest.raises(FseiError):
         SlabPlan.pencil_solve(pl, t)                                    # slab call on an ordinary plan
     sp.destroy(); pl.destroy()
+
+
+@pytest.mark.gpu
+def test_dist_comm_path_single_rank_group(oracle_ld):
+    """SlabProjection.project over a real torch.distributed group (one rank: every exchange is a self-send) -- the code path
+    bench.py --parallel slab takes under torchrun -- against the single-plan projection."""
+    from tests.util import gpu_projection, rel_l2
+    case = inputs.make_case(2, shape=(128, 64, 40))
+    created = not dist.is_initialized()
+    if created:
+        dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{_free_port()}", rank=0, world_size=1)
+    try:
+        r = slab.SlabProjection(case.grid, 0, 1)
+        r.load(case.u, case.v, case.w)
+        r.project(slab.DistComm(), case.alpha_dt, 1e-4)
+        torch.cuda.synchronize()
+        one = gpu_projection(case, 1e-4)
+        assert rel_l2(r.phi.cpu().numpy(), one[4]) <= 1e-13
+        assert np.abs(r.u.cpu().numpy() - one[0]).max() <= 1e-12 and np.abs(r.p.cpu().numpy() - one[3]).max() <= 1e-12 * np.abs(one[3]).max()
+        r.destroy()
+    finally:
+        if created:
+            dist.destroy_process_group()
