@@ -575,6 +575,12 @@ def run_slab(args) -> dict:
     if rank == 0:
         sp.w[0] = 0
     comm = slab.DistComm()
+    if args.slab_peers:                                  # the exchanges happen in the kernels' epilogues (peer stores)
+        if world > 1:
+            pencils, specs = slab.DistComm.symmetric_buffers(sp.x)
+        else:
+            pencils, specs = [sp.x.pencil.data_ptr()], [sp.x.spec.data_ptr()]
+        sp.set_peers(pencils, specs)
 
     def barrier():
         if world > 1:
@@ -602,7 +608,7 @@ def run_slab(args) -> dict:
     out = {"metric": METRIC, "value": case.cells / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
-           "config": {"workload": _workload_name(case), "cells": case.cells, "parallelism": f"z-slabs x{world} / x-slot pencils x{world}",
+           "config": {"workload": _workload_name(case), "cells": case.cells, "parallelism": f"z-slabs x{world} / x-slot pencils x{world}" + (", peer-store exchange" if args.slab_peers else ", grouped send/recv"),
                       "exchange_bytes_per_rank_per_step": 2 * 16 * x.nzl * x.ny * (x.N - x.nsl) + 0,
                       "note": "unfused fast-family kernels per rank + 2 all-to-all exchanges (NCCL grouped send/recv); inputs N(0,1) "
                               "generated on the device; fields larger than L2"},
@@ -625,6 +631,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fluid", action="store_true", help="skip the whole-fluid-substep leg")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the compact table of the other configs")
+    ap.add_argument("--slab-peers", action="store_true", help="--parallel slab: exchanges by peer stores from the kernels' epilogues")
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default; the headline path is single-GPU) or ONE projection decomposed into "
                          "z-slabs / x-slot pencils over the N ranks (paper_2103_15187_b200/slab.py; strong scaling)")

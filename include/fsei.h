@@ -233,6 +233,16 @@ int fsei_ibm_forcing(fsei_plan* plan, long n, const double* xm, const double* ym
  */
 fsei_plan* fsei_slab_plan_create(int nx, int ny, int nz, double Lx, double Ly, const double* zc /* HOST, nz+1, GLOBAL */,
                                  int bc_x, int bc_y, int k0, int k1, int s0, int s1);
+/*
+ * Peer-store exchange (the all-to-all folded into the kernels' epilogues).  Gives the plan the
+ * pencil and the slab-spectrum buffer of EVERY rank (device pointers; on a multi-GPU node the peers' buffers mapped into
+ * this process, e.g. torch symmetric memory) with the plane ranges k0s[0..nranks] and slot ranges s0s[0..nranks]
+ * (nranks <= 8).  From then on fsei_slab_forward stores its result straight into the owners' pencils (its `spec`
+ * argument is scratch) and fsei_pencil_solve stores its result straight into the owners' slab spectra (its `pencil`
+ * keeps the forward-eliminated column); the caller orders the ranks (all forwards before any solve, all solves before
+ * any backward).  nranks = 0 switches back to local results + explicit exchange.
+ */
+int fsei_slab_set_peers(fsei_plan* plan, int nranks, void* const* pencils, void* const* specs, const int* k0s, const int* s0s);
 /* a1-a3 on the slab: spec = y-transform of x-transform of D(u,v,w)/alpha_dt.  spec must not alias u, v, w. */
 int fsei_slab_forward(fsei_plan* plan, const double* u, const double* v, const double* w, double alpha_dt,
                       double* spec, void* cuda_stream);

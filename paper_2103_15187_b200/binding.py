@@ -22,7 +22,7 @@ EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family",
            "fsei_plan_profile", "fsei_plan_profile_read",
            "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep",
            "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing",
-           "fsei_slab_plan_create", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project")
+           "fsei_slab_plan_create", "fsei_slab_set_peers", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project")
 
 _lib = None
 _vp, _d, _i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
@@ -92,6 +92,8 @@ def lib() -> ctypes.CDLL:
     L.fsei_ibm_forcing.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_d] + [_vp] * 6 + [_vp]
     L.fsei_slab_plan_create.restype = _vp
     L.fsei_slab_plan_create.argtypes = [_i, _i, _i, _d, _d, _vp, _i, _i, _i, _i, _i, _i]
+    L.fsei_slab_set_peers.restype = _i
+    L.fsei_slab_set_peers.argtypes = [_vp, _i, ctypes.POINTER(_vp), ctypes.POINTER(_vp), ctypes.POINTER(_i), ctypes.POINTER(_i)]
     L.fsei_slab_forward.restype = _i
     L.fsei_slab_forward.argtypes = [_vp, _vp, _vp, _vp, _d, _vp, _vp]
     L.fsei_pencil_solve.restype = _i
@@ -257,6 +259,16 @@ class SlabPlan(Plan):
                                           self.k0, self.k1, self.s0, self.s1)
         if not self._h:
             raise FseiError(L.fsei_last_error_code(), last_error())
+
+    def set_peers(self, pencils, specs, k0s, s0s):
+        """Device addresses (ints) of every rank's pencil and slab spectrum + the range tables; [] switches peers off."""
+        n = len(pencils)
+        if n == 0:
+            _chk(lib().fsei_slab_set_peers(self._h, 0, None, None, None, None))
+            return
+        pa, sa = (_vp * n)(*[int(x) for x in pencils]), (_vp * n)(*[int(x) for x in specs])
+        ka, xa = (_i * (n + 1))(*[int(x) for x in k0s]), (_i * (n + 1))(*[int(x) for x in s0s])
+        _chk(lib().fsei_slab_set_peers(self._h, n, pa, sa, ka, xa))
 
     def slab_forward(self, u, v, w, alpha_dt, spec, stream=None):
         _chk(lib().fsei_slab_forward(self._h, _ptr(u), _ptr(v), _ptr(w), float(alpha_dt), _ptr(spec), _stream(stream)))

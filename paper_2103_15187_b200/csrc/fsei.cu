@@ -924,6 +924,32 @@ extern "C" fsei_plan* fsei_slab_plan_create(int nx, int ny, int nz, double Lx, d
 
 #define SLAB_ONLY(name) if (!P || !P->slab) return fail(FSEI_ERR_ARG, name ": not a slab plan")
 
+// Peer-store exchange: after this call fsei_slab_forward writes its result straight into the pencils of the ranks that
+// own the slots, and fsei_pencil_solve writes its result straight into the slab spectra of the ranks that own the planes
+// (pointers may be peer-mapped device pointers of other GPUs; on one GPU they are ordinary device pointers).
+extern "C" int fsei_slab_set_peers(fsei_plan* P, int nranks, void* const* pencils, void* const* specs, const int* k0s, const int* s0s)
+{
+    SLAB_ONLY("fsei_slab_set_peers");
+    if (nranks == 0) { P->YF.npeer = 0; P->ZF.npeer = 0; return FSEI_OK; }
+    if (nranks < 0 || nranks > 8 || !pencils || !specs || !k0s || !s0s) return fail(FSEI_ERR_ARG, "fsei_slab_set_peers: 1 <= nranks <= 8 and non-NULL tables");
+    if (k0s[0] != 0 || k0s[nranks] != P->T.nz || s0s[0] != 0 || s0s[nranks] != P->T.nxc) return fail(FSEI_ERR_ARG, "fsei_slab_set_peers: the ranges must cover [0, nz) and [0, nx/2)");
+    bool mine = false;
+    for (int d = 0; d < nranks; d++) {
+        if (!pencils[d] || !specs[d] || misaligned(pencils[d]) || misaligned(specs[d]) || k0s[d + 1] <= k0s[d] || s0s[d + 1] <= s0s[d])
+            return fail(FSEI_ERR_ARG, "fsei_slab_set_peers: NULL / misaligned pointer or empty range");
+        mine = mine || (k0s[d] == P->k0 && k0s[d + 1] == P->k1 && s0s[d] == P->s0 && s0s[d + 1] == P->s1);
+    }
+    if (!mine) return fail(FSEI_ERR_ARG, "fsei_slab_set_peers: this plan's own share is not among the ranges");
+    YFast& YF = P->YF; ZFast& ZF = P->ZF;
+    YF.npeer = nranks; YF.kofs = P->k0; ZF.npeer = nranks; ZF.nxc_full = P->T.nxc;
+    for (int d = 0; d < nranks; d++) {
+        YF.peer_base[d] = static_cast<cplx*>(pencils[d]); YF.peer_s0[d] = s0s[d];
+        ZF.slab_base[d] = static_cast<cplx*>(specs[d]); ZF.slab_k0[d] = k0s[d];
+    }
+    YF.peer_s0[nranks] = s0s[nranks]; ZF.slab_k0[nranks] = k0s[nranks];
+    return FSEI_OK;
+}
+
 extern "C" int fsei_slab_forward(fsei_plan* P, const double* u, const double* v, const double* w, double alpha_dt,
                                  double* spec, void* cuda_stream)
 {

@@ -26,6 +26,13 @@ struct YFast {
     int untangle;               // periodic y: columns [0, untangle) are split / merged (0, 1 or nxc)
     const cplx* tw;             // e^{-2 pi i j / ny}
     const cplx* tw_dct;         // e^{-i pi k / (2 ny)}, k in [0, ny)   (Neumann only)
+    // multi-GPU slab decomposition, peer-store exchange (slab.py): when npeer > 0 the FORWARD transform
+    // does not write its result back to the local spectrum but straight into the pencils of the ranks that own the slots:
+    // element (k, row, slot) -> peer_base[d][((kofs + k) ny + row) nsl_d + slot - peer_s0[d]], peer_s0[d] <= slot < peer_s0[d+1]
+    // (peer_base[d] may be a peer-mapped pointer: the stores then travel over NVLink while the CTA transforms its next tile)
+    int npeer = 0, kofs = 0;
+    cplx* peer_base[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int peer_s0[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 };
 
 template <class C, int CY, bool NEU> struct YSmemLayout {
@@ -131,7 +138,14 @@ FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D ma
 
     for (int k = blockIdx.y; k < P.nz; k += kstep) {
         abar_wait(bar, parity); parity ^= 1;
-        cplx* g = spec + (size_t)k * N * nxc + col;            // row r of this column at g[r * nxc]
+        cplx* g = spec + (size_t)k * N * nxc + col;            // row r of this column at g[r * gs]
+        size_t gs = (size_t)nxc;
+        if (!INV && P.npeer > 0 && act) {                      // peer-store exchange: this column's rows go to the owner of its slot
+            int d = 0;
+            while (d + 1 < P.npeer && col >= P.peer_s0[d + 1]) d++;
+            gs = (size_t)(P.peer_s0[d + 1] - P.peer_s0[d]);
+            g = P.peer_base[d] + (size_t)(P.kofs + k) * N * gs + (col - P.peer_s0[d]);
+        }
         auto next = [&]() { if (tid == 0 && k + kstep < P.nz) issue(k + kstep); };
         if (!INV) {
             auto load0 = [&](cplx (*v0)[R0]) {
@@ -145,7 +159,7 @@ FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D ma
                 }
             };
             if (!pairing) {
-                auto out = [&](int n, cplx z, int) { g[(size_t)n * nxc] = z; };
+                auto out = [&](int n, cplx z, int) { g[(size_t)n * gs] = z; };
                 fft_column<C, CY, false, false, false>(tl, c, act, buf, tws, load0, out, next);
             } else {
                 fft_column<C, CY, false, false, true>(tl, c, act, buf, tws, load0, YOut<C, CY>{buf, c}, next);
@@ -154,8 +168,8 @@ FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D ma
                     for (int kk = tl; kk <= N / 2; kk += T) {
                         cplx p1 = buf[C::pad(kk) * CY + c];
                         if (kk == 0 || (!NEU && (2 * kk == N || !mine))) {
-                            g[(size_t)kk * nxc] = p1;
-                            if (kk != 0 && 2 * kk != N) g[(size_t)(N - kk) * nxc] = buf[C::pad(N - kk) * CY + c];
+                            g[(size_t)kk * gs] = p1;
+                            if (kk != 0 && 2 * kk != N) g[(size_t)(N - kk) * gs] = buf[C::pad(N - kk) * CY + c];
                             continue;
                         }
                         cplx p2 = buf[C::pad(N - kk) * CY + c];
@@ -165,17 +179,17 @@ FSEI_GLOBAL(C::T * CY, 1) k_y_fast(YFast P, const FSEI_GRID_CONSTANT TmaMap2D ma
                         if (NEU) {
                             cplx wk = tdct[kk];
                             cplx ta = cmul(A, wk), tb = cmul(B, wk);
-                            g[(size_t)kk * nxc] = cmake(ta.re, tb.re);
-                            if (2 * kk != N) g[(size_t)(N - kk) * nxc] = cmake(-ta.im, -tb.im);
+                            g[(size_t)kk * gs] = cmake(ta.re, tb.re);
+                            if (2 * kk != N) g[(size_t)(N - kk) * gs] = cmake(-ta.im, -tb.im);
                         } else {
-                            g[(size_t)kk * nxc] = A;
-                            g[(size_t)(N - kk) * nxc] = B;
+                            g[(size_t)kk * gs] = A;
+                            g[(size_t)(N - kk) * gs] = B;
                         }
                     }
                 }
             }
         } else {
-            auto out = [&](int n, cplx z, int) { g[(size_t)(NEU ? dct_perm(n, N) : n) * nxc] = z; };
+            auto out = [&](int n, cplx z, int) { g[(size_t)(NEU ? dct_perm(n, N) : n) * gs] = z; };
             if (!pairing) {
                 auto load0 = [&](cplx (*v0)[R0]) {
 #pragma unroll

@@ -28,7 +28,22 @@ struct ZFast {
     double* cpw;          // [8][nz] plan-time factorisation of the special columns: c'_k of component t at [t][k],
                           // reciprocal pivots at [4 + t][k]   (t = 2 col + comp; k_z_special_factor)
     int s0 = 0;           // pencil view (slab.py): local slot s is global slot s + s0 (lamx already points at slot s0)
+    // peer-store exchange (slab.py): when npeer > 0 the solved column does not go back into the pencil but straight into the
+    // slab spectra of the ranks that own the planes: (k, row, slot) -> slab_base[d][((k - slab_k0[d]) ny + row) nxc_full + s0 + slot]
+    int npeer = 0, nxc_full = 0;
+    cplx* slab_base[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int slab_k0[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 };
+
+FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot);
+// final store of a solved element: the pencil itself, or (peer-store exchange) the slab spectrum of the plane's owner
+FSEI_HD void zf_store_out(const ZFast& Z, cplx* S, int k, int row, int slot, cplx v)
+{
+    if (Z.npeer == 0) { S[zf_idx(Z, k, row, slot)] = v; return; }
+    int d = 0;
+    while (d + 1 < Z.npeer && k >= Z.slab_k0[d + 1]) d++;
+    Z.slab_base[d][((size_t)(k - Z.slab_k0[d]) * Z.ny + row) * Z.nxc_full + Z.s0 + slot] = v;
+}
 
 FSEI_HD size_t zf_idx(const ZFast& Z, int k, int row, int slot)
 {
@@ -137,7 +152,7 @@ FSEI_HD void zf_sweep_column(const ZFast& Z, cplx* S, int row, int slot)
             }
         }
 #pragma unroll
-        for (int j = 0; j < FSEI_ZSW; j++) if (k1 - j >= 0) S[zf_idx(Z, k1 - j, row, slot)] = d[j];
+        for (int j = 0; j < FSEI_ZSW; j++) if (k1 - j >= 0) zf_store_out(Z, S, k1 - j, row, slot, d[j]);
     }
 }
 
@@ -341,7 +356,7 @@ FSEI_GLOBAL(128, 1) k_zf_pcr(ZFast Z, cplx* spec)
             if (mask & 1) o.re = s.re;
             if (mask & 2) o.im = s.im;
         }
-        spec[i] = o;
+        zf_store_out(Z, spec, lane, row, slot, o);
     }
 }
 

@@ -116,6 +116,30 @@ class DistComm:
             for req in self.dist.batch_isend_irecv(ops):
                 req.wait()
 
+    def fence(self):
+        """All kernels enqueued so far on every rank have completed (peer stores included)."""
+        import torch
+        if torch.cuda.is_available():
+            torch.cuda.synchronize()
+        if self.world > 1:
+            self.dist.barrier(self.group)
+
+    @staticmethod
+    def symmetric_buffers(x: "SlabExchange", group=None):
+        """Re-allocate a rank's pencil and slab spectrum in torch symmetric memory and return (pencil_ptrs, spec_ptrs) of all
+        ranks as mapped into this process -- the arguments of SlabProjection.set_peers on a multi-GPU node."""
+        import torch
+        import torch.distributed._symmetric_memory as symm
+        name = group.group_name if group is not None else torch.distributed.group.WORLD.group_name
+        ptrs = []
+        for attr in ("pencil", "spec"):
+            old = getattr(x, attr)
+            t = symm.empty(old.shape, dtype=old.dtype, device=old.device)
+            h = symm.rendezvous(t, name)
+            setattr(x, attr, t)
+            ptrs.append([int(p) for p in h.buffer_ptrs])
+        return ptrs[0], ptrs[1]
+
 
 class LocalComm:
     """All ranks live in this process and are stepped stage by stage; an exchange is a set of copies.  For checking the
@@ -148,6 +172,14 @@ class SlabProjection:
         self.w = self.x.w_ext[:nzl]                                   # the halo plane follows it in memory
         self.phi = self.x.phi_ext[1:nzl + 1]                          # the halo planes surround it in memory
         self.launches = 0
+        self.peers = False
+
+    def set_peers(self, pencil_ptrs, spec_ptrs):
+        """Peer-store exchange: device addresses of every rank's pencil and slab spectrum (own buffers included; peers'
+        buffers as mapped into this process).  The two all-to-all exchanges then happen inside the kernels' epilogues."""
+        x = self.x
+        self.plan.set_peers(pencil_ptrs, spec_ptrs, [k for k, _ in x.kr] + [x.nz], [a for a, _ in x.sr] + [x.N])
+        self.peers = True
 
     def load(self, u, v, w, p=None):
         """Local planes [k0, k1) of global (or already local) host / device arrays."""
@@ -167,15 +199,16 @@ class SlabProjection:
     def stage_forward(self, alpha_dt, stream=None):
         self.plan.slab_forward(self.u, self.v, self.w, alpha_dt, self.x.spec, stream)
         self.launches += self.plan.last_launch_count
-        return self.x.to_pencils()
+        return ([], []) if self.peers else self.x.to_pencils()          # peers: the y-transform stored into the owners' pencils
 
     def stage_solve(self, stream=None):
         self.plan.pencil_solve(self.x.pencil, stream)
         self.launches += self.plan.last_launch_count
-        return self.x.to_slabs()
+        return ([], []) if self.peers else self.x.to_slabs()            # peers: the back substitution stored into the owners' spectra
 
     def stage_backward(self, beta, stream=None):
-        self.x.unpack_slabs()
+        if not self.peers:
+            self.x.unpack_slabs()
         self.plan.slab_backward(self.x.spec, self.phi, stream)
         self.launches += self.plan.last_launch_count
         return self.x.phi_halo(both=beta != 0.0)
@@ -188,7 +221,11 @@ class SlabProjection:
         """The whole projection of this rank, exchanges over `comm` (all ranks call it together)."""
         comm.exchange(*self.stage_w_halo())
         comm.exchange(*self.stage_forward(alpha_dt, stream))
+        if self.peers:
+            comm.fence()                                    # every rank's stores into my pencil have landed
         comm.exchange(*self.stage_solve(stream))
+        if self.peers:
+            comm.fence()                                    # ... and into my slab spectrum
         comm.exchange(*self.stage_backward(beta, stream))
         self.stage_project(alpha_dt, beta, stream)
 
@@ -196,8 +233,17 @@ class SlabProjection:
         self.plan.destroy()
 
 
+def local_peers(ranks: Sequence[SlabProjection]):
+    """All ranks in one process: every rank's buffers are ordinary device allocations of this process."""
+    pencils = [r.x.pencil.data_ptr() for r in ranks]
+    specs = [r.x.spec.data_ptr() for r in ranks]
+    for r in ranks:
+        r.set_peers(pencils, specs)
+
+
 def project_local(ranks: Sequence[SlabProjection], alpha_dt, beta=0.0):
-    """All ranks in one process, stage by stage (LocalComm)."""
+    """All ranks in one process, stage by stage (LocalComm).  With peers set, the forward and solve stages of ALL ranks store
+    into each other's buffers and the stage order is the fence."""
     LocalComm.exchange_all([r.stage_w_halo() for r in ranks])
     LocalComm.exchange_all([r.stage_forward(alpha_dt) for r in ranks])
     LocalComm.exchange_all([r.stage_solve() for r in ranks])
