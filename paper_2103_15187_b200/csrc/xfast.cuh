@@ -58,7 +58,7 @@ template <class C, bool NEU> struct XShape {
     static constexpr int N = C::N;
     static constexpr size_t tables = sizeof(cplx) * (C::TW + N / 2 + 1 + (NEU ? N + 1 : 0));
     static constexpr size_t bytes(int L) {
-        return 128 + sizeof(double) * (size_t)(4 * L + 1) * 2 * N + sizeof(cplx) * (size_t)L * C::PITCH + tables +
+        return 128 + sizeof(double) * (size_t)(4 * L + 1) * 2 * N + sizeof(cplx) * (size_t)L * (C::PITCH + 8) + tables +
                (NEU ? sizeof(double) * (size_t)L * (2 * N + (2 * N >> 2) + 2) : 0);
     }
     static constexpr int fit(int L) { return (L <= 1 || bytes(L) <= 200 * 1024) ? L : fit(L - 1); }
@@ -72,7 +72,7 @@ template <class C, bool NEU> struct XShape {
 template <class C, int LPB, bool NEU, int LL> struct XSmemLayout {
     static constexpr int N = C::N;
     static constexpr int LAND = LL * 2 * N;                     // doubles
-    static constexpr int BUF = LPB * C::PITCH;                  // complex
+    static constexpr int BUF = LPB * (C::PITCH + 8);            // complex (slack: the blocked x-inverse pads its line pitch to 2 mod 8)
     static constexpr int TWS = C::TW;
     static constexpr int R2C = N / 2 + 1;
     static constexpr int DCT = NEU ? N + 1 : 0;
@@ -323,7 +323,12 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
 // phase with its shared-memory round trip and CTA barrier; each pair is then evaluated by both of its owners -- a few more
 // flops on an fp64 pipe that is a third busy (configs[1]: 0.066 -> 0.058 ms).  On the blocked layout a line-major landing
 // tile would need one TMA box per line with a 32-byte inner dimension, which the TMA engine serves at a third of the
-// speed of the 128-byte boxes (measured: x_inverse 2.65 -> 8.7 ms at configs[3]), so that path keeps the pair phase.
+// speed of the 128-byte boxes (measured: x_inverse 2.65 -> 8.7 ms at configs[3]).  There the fold is done on the
+// [tile][line][CB] tile as it lands, with the THREADS remapped instead: eight consecutive threads are (slot-in-tile 0..1) x
+// (line 0..3) of one tile, so a quarter-warp reads 128 contiguous bytes of the landing tile for X(m) and -- the mirror
+// tiles of the two slots being neighbours -- a permutation of 128 contiguous bytes for X(N-m); the line buffers get a
+// pitch of 2 (mod 8) elements so that the same eight threads (two neighbouring butterflies of four lines) stay
+// conflict-free in every pass.  A warp then holds all four lines, so the passes meet at CTA barriers.
 template <class C, int LPB, bool NEU, int CB = 0>
 FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 : 1)) k_xi_fast(XFast P, const FSEI_GRID_CONSTANT TmaMap3D map, const cplx* spec, double* phi)
 {
@@ -340,7 +345,12 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
     cplx* tdct = tr2c + L::R2C;
     double* xs = reinterpret_cast<double*>(tdct + L::DCT);
     const int tid = threadIdx.x, nt = T * LPB;
-    const int li = tid / T, tl = tid - li * T;
+    constexpr int CBm = CB ? CB : 1;
+    // natural layout: thread = (line, butterfly) line-major.  Blocked layout: (slot in tile, line, tile) fastest-first
+    const int li = CB ? (tid / CBm) % LPB : tid / T;
+    const int tl = CB ? (tid / (CBm * LPB)) * CBm + tid % CBm : tid - li * T;
+    constexpr int XP = CB ? C::PITCH + ((10 - C::PITCH % 8) % 8) : C::PITCH;      // line-buffer pitch (blocked: 2 mod 8)
+    static_assert(CB == 0 || (T % CBm == 0 && XP <= C::PITCH + 8), "blocked x-inverse thread mapping");
     const int ny = P.ny, nz = P.nz;
     const int j0 = blockIdx.x * LPB, j = j0 + li;
     const int nl = (ny - j0 < LPB) ? ny - j0 : LPB;
@@ -370,83 +380,48 @@ FSEI_GLOBAL(C::T * LPB, (XSmemLayout<C, LPB, NEU, LPB>::BYTES <= 112 * 1024 ? 2 
     if (tid == 0 && k0 < k1) issue(k0);
     unsigned parity = 0;
 
-    cplx* lbuf = buf + li * C::PITCH;
+    cplx* lbuf = buf + li * XP;
     double* lxs = xs + (NEU ? li * xs_pitch(n) : 0);
     const double scale = P.scale;
 
-    // Z(m), m in [0, N), of this thread's line from a line-major landing tile (CB == 0): element m and element N - m come
-    // from the same pair (X_p, X_{N-p}), p = min(m, N - m)
-    const cplx* FSEI_RESTRICT lland = land + (size_t)li * N;
+    // Z(m), m in [0, N), of this thread's line from the landing tile (line-major, or [tile][line][CB] on the blocked
+    // layout): element m and element N - m come from the same pair (X_p, X_{N-p}), p = min(m, N - m)
+    const cplx* FSEI_RESTRICT land_r = land;
+    const cplx* FSEI_RESTRICT tr2c_r = tr2c;
+    const cplx* FSEI_RESTRICT tdct_r = tdct;
+    auto xat = [&](int q) -> cplx { return CB ? land_r[((q / CBm) * LPB + li) * CBm + q % CBm] : land_r[li * N + q]; };
     auto zin = [&](int m) -> cplx {
         if (m == 0) {
-            const cplx s = lland[0];
+            const cplx s = xat(0);
             double x0 = s.re, xn = s.im;
             if (NEU) xn *= 1.41421356237309504880168872420969808;
             return cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
         }
         const bool lo = 2 * m <= N;
         const int p = lo ? m : N - m;
-        cplx xk = lland[p], xm = lland[N - p];
-        if (NEU) { xk = dct_tw_inv(xk, tdct[p]); xm = dct_tw_inv(xm, tdct[N - p]); }
+        cplx xk = xat(p), xm = xat(N - p);
+        if (NEU) { xk = dct_tw_inv(xk, tdct_r[p]); xm = dct_tw_inv(xm, tdct_r[N - p]); }
         const cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));    // (Xk + conj Xm)/2
         const cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));   // (Xk - conj Xm)/2
-        const cplx O = cmulc(Tt, tr2c[p]);
+        const cplx O = cmulc(Tt, tr2c_r[p]);
         return lo ? cmake(E.re - O.im, E.im + O.re)                            // E + i O
                   : cmake(E.re + O.im, -(E.im - O.re));                        // conj(E - i O)
     };
+    const int gid = CB ? -1 : li;          // blocked layout: a warp holds all the lines of the CTA -> CTA barriers
 
     for (int k = k0; k < k1; k++) {
         abar_wait(bar, parity); parity ^= 1;
-        // packed half spectrum -> Z (Hermitian pair step, preceded by the inverse quarter-wave twiddle)
-        // gl(p): slot p of line l2 in the landing tile; lb: that line's buffer
-        // (restrict: the landing tile and the tables are only read here, the line buffers only written, so the loads of
-        // the next pair may be issued before the stores of this one)
-        const cplx* FSEI_RESTRICT land_r = land;
-        const cplx* FSEI_RESTRICT tr2c_r = tr2c;
-        const cplx* FSEI_RESTRICT tdct_r = tdct;
-        auto pair_load = [&](int l2, cplx* FSEI_RESTRICT lb, int p) {
-            auto g = [&](int q) -> cplx { return CB ? land_r[((q / (CB ? CB : 1)) * LPB + l2) * CB + q % (CB ? CB : 1)] : land_r[l2 * N + q]; };
-            if (p == 0) {
-                cplx s = g(0);
-                double x0 = s.re, xn = s.im;
-                if (NEU) xn *= 1.41421356237309504880168872420969808;
-                lb[0] = cmake(0.5 * (x0 + xn), 0.5 * (x0 - xn));
-            } else {
-                cplx xk = g(p), xm = g(N - p);
-                if (NEU) { xk = dct_tw_inv(xk, tdct_r[p]); xm = dct_tw_inv(xm, tdct_r[N - p]); }
-                cplx E = cmake(0.5 * (xk.re + xm.re), 0.5 * (xk.im - xm.im));   // (Xk + conj Xm)/2
-                cplx Tt = cmake(0.5 * (xk.re - xm.re), 0.5 * (xk.im + xm.im));  // (Xk - conj Xm)/2
-                cplx O = cmulc(Tt, tr2c_r[p]);
-                lb[C::pad(p)] = cmake(E.re - O.im, E.im + O.re);               // E + i O
-                if (p != N - p) lb[C::pad(N - p)] = cmake(E.re + O.im, -(E.im - O.re));   // conj(E - i O)
-            }
-        };
-        if (CB != 0) {
-            // landing tile is [tile][line][CB]: adjacent threads read adjacent elements of it
-            constexpr int CBq = CB ? CB : 1, HP = N / 2 / CBq + 1, NW = HP * LPB * CBq, IT = (NW + T * LPB - 1) / (T * LPB);
-#pragma unroll
-            for (int it = 0; it < IT; it++) {
-                const int wi = tid + it * nt;
-                const int cc = wi % CBq, l2 = (wi / CBq) % LPB, p = (wi / (CBq * LPB)) * CBq + cc;
-                if (wi >= NW || p > N / 2 || l2 >= nl) continue;
-                pair_load(l2, buf + l2 * C::PITCH, p);
-            }
-        }
         auto next = [&]() { if (tid == 0 && k + 1 < k1) issue(k + 1); };          // landing tile consumed: fetch the next plane
-        if (CB != 0) { FSEI_SYNC(); next(); }
         double* gl = phi + ((size_t)k * ny + j) * n;
-        auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, SmIn<C>{lbuf}, v0); };
-        auto load0f = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, zin, v0); };
+        auto load0 = [&](cplx (*v0)[R0]) { fft_pass_load<N, R0, 1, T>(tl, zin, v0); };
         if (!NEU) {
             auto out = [&](int t, cplx z, int) { st2(gl + 2 * t, cmake(z.re * scale, z.im * scale)); };
-            if constexpr (CB == 0) fft_line<C, true, false, false>(tl, act, lbuf, tws, load0f, out, next, li);
-            else fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{}, li);
+            fft_line<C, true, false, false>(tl, act, lbuf, tws, load0, out, next, gid);
         } else {
             auto out = [&](int t, cplx z, int) {
                 lxs[xs_pad(makhoul(2 * t, n))] = z.re * scale; lxs[xs_pad(makhoul(2 * t + 1, n))] = z.im * scale;
             };
-            if constexpr (CB == 0) fft_line<C, true, false, false>(tl, act, lbuf, tws, load0f, out, next, li);
-            else fft_line<C, true, true, false>(tl, act, lbuf, tws, load0, out, NoHook{}, li);
+            fft_line<C, true, false, false>(tl, act, lbuf, tws, load0, out, next, gid);
             FSEI_SYNC();
             if (act) {
 #pragma unroll
