@@ -142,8 +142,9 @@ int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double*
  * substep l has alpha_l = gamma_l + rho_l and beta = alpha_l dt/(2 Re).  Discrete operators: DESIGN.md V1..V12.
  *
  * fsei_explicit_terms (NEXT-2): second-order central, divergence-form convective term on the staggered mesh
- *   H_q   = -div(u q) (+ f_q)                at the position of each component q = u, v, w
- *   rhs_q = ((gamma_dt*H_q + rho_dt*Hprev_q) - alpha_dt*(G p)_q) + (2 beta)*(lap q)
+ *   H_q   = -div(u q)                        at the position of each component q = u, v, w
+ *   rhs_q = ((gamma_dt*H_q + rho_dt*Hprev_q) - alpha_dt*(G p)_q) + (2 beta)*(lap q)   [+ alpha_dt*f_q if a force is given:
+ *           in Eq. 3 the force f stands outside the [gamma .. rho ..] bracket, so it carries the substep's weight alpha_dt]
  *   Hprev_q <- H_q
  * evaluated in IEEE double in that fixed order, no FMA: bit-identical to the definition.
  *   u, v, w, p     : in (read only).  fu, fv, fw: body force (e.g. the IB forcing), each may be NULL.

@@ -72,7 +72,7 @@ class Oracle:
         L.oracle_viscous_step.argtypes = grid + [_dp] * 6 + [d]
         L.oracle_viscous_sweep.argtypes = grid + [i, i, d, _dp]
         L.oracle_cyclic_thomas.argtypes = [i, _dp, _dp, _dp, _dp, _dp]
-        L.oracle_convective.argtypes = grid + [_dp] * 3 + [ctypes.c_void_p] * 3 + [_dp] * 3
+        L.oracle_convective.argtypes = grid + [_dp] * 3 + [_dp] * 3
         L.oracle_velocity_laplacian.argtypes = grid + [i, _dp, _dp]
         L.oracle_explicit_terms.argtypes = grid + [_dp] * 4 + [ctypes.c_void_p] * 3 + [_dp] * 6 + [d, d, d, d]
 
@@ -145,12 +145,11 @@ class Oracle:
     def _opt(a):
         return None if a is None else a.ctypes.data
 
-    def convective(self, g, u, v, w, f=(None, None, None)):
-        """H = -div(uu) (+ f): returns hu, hv, hw."""
+    def convective(self, g, u, v, w):
+        """H = -div(uu): returns hu, hv, hw."""
         a, keep = self._g(g)
         h = [np.empty_like(u) for _ in range(3)]
-        self._chk(self.lib.oracle_convective(*a, _ptr(u), _ptr(v), _ptr(w), *[self._opt(x) for x in f],
-                                             *[_ptr(x) for x in h]), "convective")
+        self._chk(self.lib.oracle_convective(*a, _ptr(u), _ptr(v), _ptr(w), *[_ptr(x) for x in h]), "convective")
         return h
 
     def velocity_laplacian(self, g, comp, q):

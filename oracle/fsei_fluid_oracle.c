@@ -21,8 +21,9 @@
  * sec. 3 (the second-order staggered scheme of the paper's refs [12],[13],[14]):
  *
  *   substep with weights gamma_l, rho_l, alpha_l = gamma_l + rho_l, beta = alpha_l dt/(2 Re):
- *     H^n   = -div(u u)^n + f                                              (NEXT-2, explicit)
- *     rhs   = dt (gamma_l H^n + rho_l H^{n-1}) - alpha_l dt G p^n + 2 beta lap(q^n)
+ *     H^n   = -div(u u)^n                                                  (NEXT-2, explicit)
+ *     rhs   = dt (gamma_l H^n + rho_l H^{n-1}) - alpha_l dt G p^n + 2 beta lap(q^n) + alpha_l dt f
+ *             (f stands OUTSIDE the [gamma .. rho ..] bracket of Eq. 3: it carries the weight of the substep, alpha_l dt)
  *     (1 - beta dxx)(1 - beta dyy)(1 - beta dzz) dq = rhs                   (NEXT-1, implicit)
  *     q^    = q^n + dq          -> then the pressure projection of fsei_oracle.c
  *
@@ -278,6 +279,7 @@ int oracle_cyclic_thomas(int n, const double *a, const double *b, const double *
  * Viscous term: lap q = (dxx q + dyy q) + dzz q with the flux-form second differences of
  *  visc_rows (reading V3-V6) written out as gradient differences.
  *  rhs_q = ((gdt H + rdt Hprev) - adt G p) + (2 beta) lap q      (each operation rounded)
+ *  rhs_q = rhs_q + adt f_q                                        if a body force is given (Eq. 3: f outside the bracket)
  *  Hprev <- H.
  */
 typedef struct {
@@ -421,10 +423,9 @@ static int sgrid_init(sgrid *g, int nx, int ny, int nz, double Lx, double Ly, co
 }
 static void sgrid_free(sgrid *g) { free((void *)g->rdzc); free((void *)g->rdzm); }
 
-/* H = -div(u u) (+ f if given): the three components at their own positions; wall rows 0. */
+/* H = -div(u u): the three components at their own positions; wall rows 0. */
 int oracle_convective(int nx, int ny, int nz, double Lx, double Ly, const double *zc, int bc_x, int bc_y,
-                      const double *u, const double *v, const double *w,
-                      const double *fu, const double *fv, const double *fw, double *hu, double *hv, double *hw)
+                      const double *u, const double *v, const double *w, double *hu, double *hv, double *hw)
 {
     sgrid g;
     if (sgrid_init(&g, nx, ny, nz, Lx, Ly, zc, bc_x, bc_y)) return 4;
@@ -436,9 +437,6 @@ int oracle_convective(int nx, int ny, int nz, double Lx, double Ly, const double
                 double a = wall_row(&g, COMP_U, i, j, k) ? 0.0 : conv_u(&g, u, v, w, i, j, k);
                 double b = wall_row(&g, COMP_V, i, j, k) ? 0.0 : conv_v(&g, u, v, w, i, j, k);
                 double c = wall_row(&g, COMP_W, i, j, k) ? 0.0 : conv_w(&g, u, v, w, i, j, k);
-                if (fu && !wall_row(&g, COMP_U, i, j, k)) a = a + fu[t];
-                if (fv && !wall_row(&g, COMP_V, i, j, k)) b = b + fv[t];
-                if (fw && !wall_row(&g, COMP_W, i, j, k)) c = c + fw[t];
                 hu[t] = a; hv[t] = b; hw[t] = c;
             }
     sgrid_free(&g);
@@ -471,7 +469,7 @@ int oracle_explicit_terms(int nx, int ny, int nz, double Lx, double Ly, const do
     size_t N = (size_t)nx * ny * nz;
     double *nu = malloc(sizeof(double) * N), *nv = malloc(sizeof(double) * N), *nw = malloc(sizeof(double) * N);
     if (!nu || !nv || !nw) return 4;
-    int rc = oracle_convective(nx, ny, nz, Lx, Ly, zc, bc_x, bc_y, u, v, w, fu, fv, fw, nu, nv, nw);
+    int rc = oracle_convective(nx, ny, nz, Lx, Ly, zc, bc_x, bc_y, u, v, w, nu, nv, nw);
     if (rc) return rc;
     const double tb = 2.0 * beta;
 #pragma omp parallel for schedule(static)
@@ -484,16 +482,19 @@ int oracle_explicit_terms(int nx, int ny, int nz, double Lx, double Ly, const do
                 else {
                     double gp = (c0 - p[IDX(wrapi(i - 1, nx), j, k)]) * g.rdx;
                     ru[t] = ((gamma_dt * nu[t] + rho_dt * hu[t]) - alpha_dt * gp) + tb * vel_lap(&g, u, COMP_U, i, j, k);
+                    if (fu) ru[t] = ru[t] + alpha_dt * fu[t];
                 }
                 if (wall_row(&g, COMP_V, i, j, k)) rv[t] = 0.0;
                 else {
                     double gp = (c0 - p[IDX(i, wrapi(j - 1, ny), k)]) * g.rdy;
                     rv[t] = ((gamma_dt * nv[t] + rho_dt * hv[t]) - alpha_dt * gp) + tb * vel_lap(&g, v, COMP_V, i, j, k);
+                    if (fv) rv[t] = rv[t] + alpha_dt * fv[t];
                 }
                 if (wall_row(&g, COMP_W, i, j, k)) rw[t] = 0.0;
                 else {
                     double gp = (c0 - p[IDX(i, j, k - 1)]) * g.rdzm[k];
                     rw[t] = ((gamma_dt * nw[t] + rho_dt * hw[t]) - alpha_dt * gp) + tb * vel_lap(&g, w, COMP_W, i, j, k);
+                    if (fw) rw[t] = rw[t] + alpha_dt * fw[t];
                 }
             }
     memcpy(hu, nu, sizeof(double) * N); memcpy(hv, nv, sizeof(double) * N); memcpy(hw, nw, sizeof(double) * N);

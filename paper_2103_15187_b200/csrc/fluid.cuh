@@ -1,7 +1,7 @@
 // fluid.cuh -- the two steps that precede the pressure projection in one fluid substep:
 //
-//   explicit terms (Eq. 3):  H = -div(u u) + f,
-//        rhs_q = ((gdt H + rdt Hprev) - adt G p) + 2 beta lap q,   Hprev <- H
+//   explicit terms (Eq. 3):  H = -div(u u),
+//        rhs_q = ((gdt H + rdt Hprev) - adt G p) + 2 beta lap q (+ adt f),   Hprev <- H
 //   implicit viscous step:    q += [(1 - beta dxx)(1 - beta dyy)(1 - beta dzz)]^-1 rhs_q
 //        "approximate factorization yielding tridiagonal matrices (one for each direction) inverted using Thomas'
 //        algorithm with a Sherman-Morrison perturbation in the two periodic dimensions"
@@ -311,12 +311,12 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double fb = (EDGE && ylo) ? 0.0 : FSEI_MUL(avg2(u0M, u00), avg2(vM0, v00));
         const double ga = (EDGE && zhi) ? 0.0 : FSEI_MUL(avg2(u00, u_kp), avg2(wM_kp, w_kp));
         const double gb = (EDGE && zlo) ? 0.0 : FSEI_MUL(avg2(u_km, u00), avg2(wM0, w00));
-        double H = neg3(fx, FSEI_MUL(FSEI_SUB(fa, fb), rdy), FSEI_MUL(FSEI_SUB(ga, gb), rc));
-        if (A.fu) H = FSEI_ADD(H, fb3[0]);
+        const double H = neg3(fx, FSEI_MUL(FSEI_SUB(fa, fb), rdy), FSEI_MUL(FSEI_SUB(ga, gb), rc));
         const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), S.rdzm[k + 1]);
         const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(u00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u00, u_km), rm);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(uP0, u00, uM0, rdx), d2_grad(u0P, u00, u0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
-        A.ru[t] = rhs_assemble(H, hprev[0], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
+        const double r_ = rhs_assemble(H, hprev[0], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
+        A.ru[t] = A.fu ? FSEI_ADD(r_, FSEI_MUL(A.adt, fb3[0])) : r_;
         A.hu[t] = H;
     }
     // ---- v
@@ -327,12 +327,12 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double fy = sq_diff(avg2(v00, v0P), avg2(v0M, v00), rdy);
         const double ga = (EDGE && zhi) ? 0.0 : FSEI_MUL(avg2(v00, v_kp), avg2(w0M_kp, w_kp));
         const double gb = (EDGE && zlo) ? 0.0 : FSEI_MUL(avg2(v_km, v00), avg2(w0M, w00));
-        double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), fy, FSEI_MUL(FSEI_SUB(ga, gb), rc));
-        if (A.fv) H = FSEI_ADD(H, fb3[1]);
+        const double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), fy, FSEI_MUL(FSEI_SUB(ga, gb), rc));
         const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), S.rdzm[k + 1]);
         const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(v00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v00, v_km), rm);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(vP0, v00, vM0, rdx), d2_grad(v0P, v00, v0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
-        A.rv[t] = rhs_assemble(H, hprev[1], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
+        const double r_ = rhs_assemble(H, hprev[1], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
+        A.rv[t] = A.fv ? FSEI_ADD(r_, FSEI_MUL(A.adt, fb3[1])) : r_;
         A.hv[t] = H;
     }
     // ---- w
@@ -343,11 +343,11 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double ga = (EDGE && yhi) ? 0.0 : FSEI_MUL(avg2(w00, w0P), avg2(v0P_km, v0P));
         const double gb = (EDGE && ylo) ? 0.0 : FSEI_MUL(avg2(w0M, w00), avg2(v_km, v00));
         const double fz = sq_diff(avg2(w00, w_kp), avg2(w_km, w00), rm);
-        double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), FSEI_MUL(FSEI_SUB(ga, gb), rdy), fz);
-        if (A.fw) H = FSEI_ADD(H, fb3[2]);
+        const double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), FSEI_MUL(FSEI_SUB(ga, gb), rdy), fz);
         const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), S.rdzc[k - 1]);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(wP0, w00, wM0, rdx), d2_grad(w0P, w00, w0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rm));
-        A.rw[t] = rhs_assemble(H, hprev[2], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
+        const double r_ = rhs_assemble(H, hprev[2], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
+        A.rw[t] = A.fw ? FSEI_ADD(r_, FSEI_MUL(A.adt, fb3[2])) : r_;
         A.hw[t] = H;
     }
 }

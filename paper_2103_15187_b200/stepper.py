@@ -1,0 +1,64 @@
+"""Time stepping of the fluid solver on a box, as sequences of libfsei calls (plumbing only: no arithmetic here).
+
+One time step of the paper's scheme (Eq. 3; V1) is one substep (Adams-Bashforth, gamma = 3/2,
+rho = -1/2) or three (the low-storage third-order Runge-Kutta scheme of the paper's refs [12],[13]:
+gamma = (8/15, 5/12, 3/4), rho = (0, -17/60, -5/12), alpha_l = gamma_l + rho_l); a substep is
+
+    [IB forcing of the markers, if any: fsei_ibm_forcing]  ->  fsei_fluid_substep
+    (explicit terms -> implicit viscous step -> pressure projection)
+
+with beta_l = alpha_l dt / (2 Re).  The first Adams-Bashforth step has no H^{n-1} and runs as forward Euler
+(gamma = 1, rho = 0).  All fields live on the device; nothing synchronises, so a step can be captured in a CUDA graph.
+"""
+from __future__ import annotations
+
+SCHEMES = {
+    "ab2": ((1.5,), (-0.5,)),
+    "rk3": ((8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0), (0.0, -17.0 / 60.0, -5.0 / 12.0)),
+}
+
+
+class FluidStepper:
+    def __init__(self, plan, u, v, w, dt: float, Re: float, scheme: str = "rk3", markers=None):
+        """plan: binding.Plan; u, v, w: device float64 tensors [nz][ny][nx] (updated in place).
+        markers: optional dict of device tensors xm, ym, zm, area, Vu, Vv, Vw (an immersed body moving with velocity V)."""
+        import torch
+        if scheme not in SCHEMES:
+            raise ValueError(f"scheme must be one of {sorted(SCHEMES)}")
+        self.plan, self.dt, self.Re, self.scheme = plan, float(dt), float(Re), scheme
+        self.u, self.v, self.w = u, v, w
+        z = lambda: torch.zeros_like(u)
+        self.p, self.phi = z(), z()
+        self.h = [z(), z(), z()]                       # H of the previous substep
+        self.r = [z(), z(), z()]                       # scratch: right-hand sides
+        self.markers = markers
+        if markers is not None:
+            n = markers["xm"].shape[0]
+            self.f = [z(), z(), z()]
+            self.F = [torch.zeros(n, dtype=u.dtype, device=u.device) for _ in range(3)]
+        self.steps = 0
+        self.launches = 0
+
+    def substep(self, gamma: float, rho: float, stream=None):
+        dt, alpha = self.dt, gamma + rho
+        beta = alpha * dt / (2.0 * self.Re)
+        f = (None, None, None)
+        if self.markers is not None:
+            m = self.markers
+            for t in self.f:
+                t.zero_()
+            self.plan.ibm_forcing(m["xm"].shape[0], m["xm"], m["ym"], m["zm"], m["area"], m["Vu"], m["Vv"], m["Vw"],
+                                  self.u, self.v, self.w, 1.0 / (alpha * dt), *self.F, *self.f, stream=stream)
+            self.launches += self.plan.last_launch_count
+            f = tuple(self.f)
+        self.plan.fluid_substep(self.u, self.v, self.w, self.p, *self.h, *self.r, self.phi, gamma * dt, rho * dt, alpha * dt, beta,
+                                f=f, stream=stream)
+        self.launches += self.plan.last_launch_count
+
+    def step(self, stream=None):
+        gam, rho = SCHEMES[self.scheme]
+        if self.scheme == "ab2" and self.steps == 0:
+            gam, rho = (1.0,), (0.0,)                  # no H^{n-1} yet: forward Euler
+        for g, r in zip(gam, rho):
+            self.substep(g, r, stream)
+        self.steps += 1

@@ -493,12 +493,12 @@ def test_EP6_rhs_assembly_term_by_term(oracle_ld, bc):
     r = oracle_ld.explicit_terms(g, u, v, w, Z(), Z(), Z(), Z(), 0.0, 0.0, 0.0, 0.25)
     for c, q in enumerate((u, v, w)):
         assert np.allclose(r[c], 0.5 * oracle_ld.velocity_laplacian(g, c, q), rtol=1e-15, atol=0)
-    # (e) body force enters H
+    # (e) the body force stands outside the [gamma, rho] bracket of Eq. 3: weight alpha dt in the rhs, H unchanged
     f = [h0, h1, h2]
     hh = [Z(), Z(), Z()]
-    oracle_ld.explicit_terms(g, u, v, w, Z(), *hh, 1.0, 0.0, 0.0, 0.0, f=f)
+    r = oracle_ld.explicit_terms(g, u, v, w, Z(), *hh, 0.0, 0.0, 0.3, 0.0, f=f)
     for c in range(3):
-        assert np.allclose(hh[c], H[c] + f[c], rtol=1e-15, atol=1e-300)
+        assert np.array_equal(hh[c], H[c]) and np.allclose(r[c], 0.3 * f[c], rtol=1e-15, atol=0)
 
 
 # ------------------------------------------------------------------------------------------

@@ -1,0 +1,93 @@
+"""Whole time steps (paper_2103_15187_b200/stepper.py: RK3 and AB2 sequences of fsei_fluid_substep, with and without an
+immersed sphere) on the GPU against the same sequence of oracle calls, and the physics the scheme must respect:
+the velocity stays discretely solenoidal, and without forcing the kinetic energy of a viscous flow between no-slip walls
+does not grow."""
+import numpy as np
+import pytest
+
+from paper_2103_15187_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+P = 0
+
+
+def _setup(shape=(64, 64, 24), K=3, seed=8):
+    import torch
+    from paper_2103_15187_b200.binding import Plan
+    nx, ny, nz = shape
+    g = (nx, ny, nz, 1.0, 1.0, inputs.tanh_grid(nz, 2.0), P, P)
+    vel = [0.3 * inputs.smooth_field(seed, 200 + c, "uvw"[c], g, K) for c in range(3)]
+    vel[2][0] = 0
+    plan = Plan.from_grid(g)
+    dev = [torch.from_numpy(a.copy()).to("cuda:0") for a in vel]
+    return g, vel, plan, dev
+
+
+def _oracle_step(orc, g, st, gam, rho, dt, Re, markers=None):
+    u, v, w, p, h = st
+    for ga, ro in zip(gam, rho):
+        al = ga + ro
+        beta = al * dt / (2 * Re)
+        f = (None, None, None)
+        if markers is not None:
+            xm, ym, zm, area, V = markers
+            f = [np.zeros_like(u) for _ in range(3)]
+            orc.ibm_forcing(g, xm, ym, zm, area, V, u, v, w, 1.0 / (al * dt), f)
+        r = orc.explicit_terms(g, u, v, w, p, *h, ga * dt, ro * dt, al * dt, beta, f=f)
+        orc.viscous_step(g, u, v, w, *r, beta)
+        orc.pressure_projection(g, u, v, w, p, al * dt, beta)
+
+
+@pytest.mark.parametrize("scheme,nsteps", [("rk3", 3), ("ab2", 5)])
+def test_time_steps_vs_oracle(oracle_ld, scheme, nsteps):
+    import torch
+    from paper_2103_15187_b200.stepper import FluidStepper, SCHEMES
+    g, vel, plan, dev = _setup()
+    dt, Re = 2e-3, 150.0
+    fs = FluidStepper(plan, *dev, dt, Re, scheme)
+    st = [a.copy() for a in vel] + [np.zeros_like(vel[0]), [np.zeros_like(vel[0]) for _ in range(3)]]
+    dzc = np.diff(g[5])[:, None, None]
+    e_prev = None
+    for n in range(nsteps):
+        fs.step()
+        gam, rho = SCHEMES[scheme]
+        if scheme == "ab2" and n == 0:
+            gam, rho = (1.0,), (0.0,)
+        _oracle_step(oracle_ld, g, st, gam, rho, dt, Re)
+        torch.cuda.synchronize()
+        got = [t.cpu().numpy() for t in (fs.u, fs.v, fs.w, fs.p)]
+        for c, (a, b) in enumerate(zip(got, st[:4])):
+            assert np.abs(a - b).max() <= 1e-11 * max(1.0, np.abs(b).max()), (n, c, np.abs(a - b).max())
+        div = np.abs(oracle_ld.divergence(g, got[0], got[1], got[2], 1.0)).max()
+        assert div <= 1e-10, (n, div)
+        e = 0.5 * sum(((q * q) * dzc).sum() for q in got[:3])
+        if e_prev is not None:
+            assert e <= e_prev * (1 + 1e-9), (n, e, e_prev)             # no forcing, no-slip walls: energy does not grow
+        e_prev = e
+    assert fs.launches > 0
+    plan.destroy()
+
+
+def test_time_steps_with_immersed_sphere_vs_oracle(oracle_ld):
+    import torch
+    from paper_2103_15187_b200.stepper import FluidStepper, SCHEMES
+    g, vel, plan, dev = _setup(seed=9)
+    dt, Re, n = 2e-3, 150.0, 3200                          # marker spacing ~ grid spacing (4 pi R^2 / n ~ dx^2), as the paper's tiling ensures
+    xm, ym, zm, area, V = inputs.sphere_markers(n, (0.5, 0.5, 0.5), 0.25, seed=3)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+    mk = dict(xm=d(xm), ym=d(ym), zm=d(zm), area=d(area), Vu=d(V[0]), Vv=d(V[1]), Vw=d(V[2]))
+    fs = FluidStepper(plan, *dev, dt, Re, "rk3", markers=mk)
+    st = [a.copy() for a in vel] + [np.zeros_like(vel[0]), [np.zeros_like(vel[0]) for _ in range(3)]]
+    U0 = oracle_ld.mls_interpolate(g, xm, ym, zm, *st[:3])
+    for _ in range(2):
+        fs.step()
+        _oracle_step(oracle_ld, g, st, *SCHEMES["rk3"], dt, Re, markers=(xm, ym, zm, area, V))
+    torch.cuda.synchronize()
+    got = [t.cpu().numpy() for t in (fs.u, fs.v, fs.w, fs.p)]
+    for c, (a, b) in enumerate(zip(got, st[:4])):
+        assert np.abs(a - b).max() <= 1e-10 * max(1.0, np.abs(b).max()), (c, np.abs(a - b).max())
+    # the forcing pulls the fluid at the markers towards the body's velocity
+    U1 = oracle_ld.mls_interpolate(g, xm, ym, zm, *got[:3])
+    err0 = sum(np.abs(U0[c] - V[c]).mean() for c in range(3)); err1 = sum(np.abs(U1[c] - V[c]).mean() for c in range(3))
+    assert err1 < 0.8 * err0, (err0, err1)
+    plan.destroy()
