@@ -101,20 +101,29 @@ class DistComm:
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
 
     def exchange(self, sends, recvs):
-        ops = []
+        # gloo moves host memory only: device tensors are staged through host copies (the paper's own transport, P:L202-204;
+        # here only so that the multi-process path can be exercised on a box with one GPU).  NCCL takes device tensors as is.
+        stage = self.dist.get_backend(self.group) == "gloo"
+        ops, landed = [], []
         for t, src in recvs:
             if src == self.rank:
                 continue
-            ops.append(self.dist.P2POp(self.dist.irecv, t, src, self.group))
+            buf = t
+            if stage and t.is_cuda:
+                buf = t.new_empty(t.shape, device="cpu")
+                landed.append((t, buf))
+            ops.append(self.dist.P2POp(self.dist.irecv, buf, src, self.group))
         for t, dst in sends:
             if dst == self.rank:                                        # my own share: a local copy
                 mine = [r for r, src in recvs if src == self.rank]
                 mine[0].copy_(t)
                 continue
-            ops.append(self.dist.P2POp(self.dist.isend, t, dst, self.group))
+            ops.append(self.dist.P2POp(self.dist.isend, t.cpu() if (stage and t.is_cuda) else t, dst, self.group))
         if ops:
             for req in self.dist.batch_isend_irecv(ops):
                 req.wait()
+        for t, buf in landed:
+            t.copy_(buf)
 
     def fence(self):
         """All kernels enqueued so far on every rank have completed (peer stores included)."""

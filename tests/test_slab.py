@@ -200,3 +200,37 @@ def test_peer_store_exchange_vs_oracle(oracle_ld, world, shape, beta):
             assert torch.equal(getattr(a, f), getattr(b, f)), f
     for r in ranks + plain:
         r.destroy()
+
+
+def _gpu_worker(rank, world, port, shape, beta, out):
+    sys.path.insert(0, ROOT)
+    import numpy as _np
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    case = inputs.make_case(2, shape=shape)
+    r = slab.SlabProjection(case.grid, rank, world, device="cuda:0")
+    r.load(case.u, case.v, case.w)
+    r.project(slab.DistComm(), case.alpha_dt, beta)
+    torch.cuda.synchronize()
+    _np.savez(os.path.join(out, f"r{rank}.npz"), **{f: getattr(r, f).cpu().numpy() for f in ("u", "v", "w", "p", "phi")})
+    r.destroy()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world,shape,beta", [(2, (128, 64, 50), 2.5e-4), (3, (96, 48, 41), 0.0)])
+def test_real_process_group_ranks_on_one_gpu(tmp_path, oracle_ld, world, shape, beta):
+    """One PROCESS per rank, exchanges through torch.distributed point-to-point operations (gloo here: NCCL refuses two ranks
+    on one device) -- the code path of a multi-GPU run, with the ranks time-sharing the one GPU of this box.  No kernel of a
+    rank waits on another rank: the exchanges are host-side send/recv between kernel launches."""
+    from tests.util import oracle_projection, rel_l2
+    port = _free_port()
+    mp.spawn(_gpu_worker, args=(world, port, shape, beta, str(tmp_path)), nprocs=world, join=True)
+    parts = [np.load(os.path.join(tmp_path, f"r{r}.npz")) for r in range(world)]
+    got = {f: np.concatenate([p[f] for p in parts], axis=0) for f in ("u", "v", "w", "p", "phi")}
+    case = inputs.make_case(2, shape=shape)
+    ref = oracle_projection(oracle_ld, case, beta)
+    assert rel_l2(got["phi"], ref[4]) <= 1e-11
+    for f, r in zip(("u", "v", "w", "p"), ref[:4]):
+        assert np.abs(got[f] - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
