@@ -576,8 +576,8 @@ def run_slab(args) -> dict:
         sp.w[0] = 0
     comm = slab.DistComm()
     if args.slab_peers:                                  # the exchanges happen in the kernels' epilogues (peer stores)
-        if world > 1:
-            pencils, specs = slab.DistComm.symmetric_buffers(sp.x)
+        if world > 1:                                    # one node: CUDA IPC handles of every rank's buffers
+            pencils, specs = comm.ipc_buffers(sp.x)
         else:
             pencils, specs = [sp.x.pencil.data_ptr()], [sp.x.spec.data_ptr()]
         sp.set_peers(pencils, specs)
@@ -614,6 +614,9 @@ def run_slab(args) -> dict:
                               "generated on the device; fields larger than L2"},
            "clocks": clocks, "gpu_launches": sp.launches,
            "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "skipped": "slab mode times device-resident fields"}}
+    if args.slab_peers and world > 1:
+        comm.fence()
+        return out if rank == 0 else None
     sp.destroy()
     if dist.is_initialized():
         dist.destroy_process_group()
@@ -640,6 +643,9 @@ def main():
         out = run_slab(args)
         if out is not None:
             print(json.dumps(out), flush=True)
+        if args.slab_peers and int(os.environ.get("WORLD_SIZE", 1)) > 1:
+            sys.stdout.flush()
+            os._exit(0)              # CUDA-IPC-shared tensors: torch's teardown order at interpreter exit is undefined
         return
     if args.impl == "reference":
         if int(os.environ.get("RANK", 0)) != 0:

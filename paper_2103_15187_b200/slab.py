@@ -133,6 +133,22 @@ class DistComm:
         if self.world > 1:
             self.dist.barrier(self.group)
 
+    def ipc_buffers(self, x: "SlabExchange"):
+        """(pencil_ptrs, spec_ptrs) of all ranks of ONE NODE as mapped into this process through CUDA IPC handles (the
+        handles travel as pickled objects over the process group; torch opens them with cudaIpcOpenMemHandle).  The mapped
+        tensors are kept alive on `x`.  Arguments of SlabProjection.set_peers."""
+        from torch.multiprocessing.reductions import reduce_tensor
+        mine = [reduce_tensor(x.pencil), reduce_tensor(x.spec)]
+        allh = [None] * self.world
+        self.dist.all_gather_object(allh, mine, group=self.group)
+        keep, pencils, specs = [], [], []
+        for r, (hp, hs) in enumerate(allh):
+            tp, ts = (x.pencil, x.spec) if r == self.rank else (hp[0](*hp[1]), hs[0](*hs[1]))
+            keep += [tp, ts]
+            pencils.append(tp.data_ptr()); specs.append(ts.data_ptr())
+        x._ipc_keepalive = keep
+        return pencils, specs
+
     @staticmethod
     def symmetric_buffers(x: "SlabExchange", group=None):
         """Re-allocate a rank's pencil and slab spectrum in torch symmetric memory and return (pencil_ptrs, spec_ptrs) of all
