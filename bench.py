@@ -560,11 +560,14 @@ def run_slab(args) -> dict:
     rank = int(os.environ.get("RANK", 0)); local = int(os.environ.get("LOCAL_RANK", 0)); world = int(os.environ.get("WORLD_SIZE", 1))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; libfsei has no CPU fallback")
+    local = local % torch.cuda.device_count()        # (more ranks than GPUs only with --dist-backend gloo: a functional check)
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if not dist.is_initialized():
-        if world > 1:
+        if world > 1 and args.dist_backend == "nccl":
             dist.init_process_group("nccl", device_id=dev)
+        elif world > 1:
+            dist.init_process_group("gloo")
         else:
             dist.init_process_group("gloo", init_method="tcp://127.0.0.1:29533", rank=0, world_size=1)
     case = inputs.make_case(args.config, fields=False)
@@ -634,6 +637,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fluid", action="store_true", help="skip the whole-fluid-substep leg")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the compact table of the other configs")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="--parallel slab: process-group backend (gloo stages through the host and lets several ranks share one GPU)")
     ap.add_argument("--slab-peers", action="store_true", help="--parallel slab: exchanges by peer stores from the kernels' epilogues")
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default; the headline path is single-GPU) or ONE projection decomposed into "
