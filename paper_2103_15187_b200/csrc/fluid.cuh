@@ -275,7 +275,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // wall selects compile away.  The arithmetic of the two variants is the same, operation for operation.
 template <bool EDGE>
 __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const double* __restrict__ s0, const double* __restrict__ sm,
-                                              const double* __restrict__ sp, int c, const double (&hprev)[3], const double (&fb3)[3], size_t t, int k,
+                                              const double* __restrict__ sp, int c, const double (&hprev)[3], const double (&fb3)[3], const double (&zm4)[4], size_t t,
                                               bool xlo, bool xhi, bool ylo, bool yhi, bool zlo, bool zhi)
 {
     constexpr int PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE;
@@ -301,7 +301,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         if (xlo) wM0 = -w00; if (xhi) wP0 = -w00;
         if (ylo) w0M = -w00; if (yhi) w0P = -w00;
     }
-    const double rc = S.rdzc[k], rm = S.rdzm[k];
+    const double rc = zm4[1], rm = zm4[2], rm_up = zm4[3], rc_dn = zm4[0];      // rdzc[k], rdzm[k], rdzm[k+1], rdzc[k-1]
 
     // ---- u
     if (EDGE && xlo) { A.hu[t] = 0.0; A.ru[t] = 0.0; }
@@ -312,7 +312,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double ga = (EDGE && zhi) ? 0.0 : FSEI_MUL(avg2(u00, u_kp), avg2(wM_kp, w_kp));
         const double gb = (EDGE && zlo) ? 0.0 : FSEI_MUL(avg2(u_km, u00), avg2(wM0, w00));
         const double H = neg3(fx, FSEI_MUL(FSEI_SUB(fa, fb), rdy), FSEI_MUL(FSEI_SUB(ga, gb), rc));
-        const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), S.rdzm[k + 1]);
+        const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, u00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u_kp, u00), rm_up);
         const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(u00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(u00, u_km), rm);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(uP0, u00, uM0, rdx), d2_grad(u0P, u00, u0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
         const double r_ = rhs_assemble(H, hprev[0], FSEI_MUL(FSEI_SUB(p00, pM0), rdx), lap, A);
@@ -328,7 +328,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double ga = (EDGE && zhi) ? 0.0 : FSEI_MUL(avg2(v00, v_kp), avg2(w0M_kp, w_kp));
         const double gb = (EDGE && zlo) ? 0.0 : FSEI_MUL(avg2(v_km, v00), avg2(w0M, w00));
         const double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), fy, FSEI_MUL(FSEI_SUB(ga, gb), rc));
-        const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), S.rdzm[k + 1]);
+        const double gzp = (EDGE && zhi) ? FSEI_MUL(FSEI_SUB(0.0, v00), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v_kp, v00), rm_up);
         const double gzm = (EDGE && zlo) ? FSEI_MUL(FSEI_SUB(v00, 0.0), FSEI_MUL(2.0, rc)) : FSEI_MUL(FSEI_SUB(v00, v_km), rm);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(vP0, v00, vM0, rdx), d2_grad(v0P, v00, v0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rc));
         const double r_ = rhs_assemble(H, hprev[1], FSEI_MUL(FSEI_SUB(p00, p0M), rdy), lap, A);
@@ -344,7 +344,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
         const double gb = (EDGE && ylo) ? 0.0 : FSEI_MUL(avg2(w0M, w00), avg2(v_km, v00));
         const double fz = sq_diff(avg2(w00, w_kp), avg2(w_km, w00), rm);
         const double H = neg3(FSEI_MUL(FSEI_SUB(fa, fb), rdx), FSEI_MUL(FSEI_SUB(ga, gb), rdy), fz);
-        const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), S.rdzc[k - 1]);
+        const double gzp = FSEI_MUL(FSEI_SUB(w_kp, w00), rc), gzm = FSEI_MUL(FSEI_SUB(w00, w_km), rc_dn);
         const double lap = FSEI_ADD(FSEI_ADD(d2_grad(wP0, w00, wM0, rdx), d2_grad(w0P, w00, w0M, rdy)), FSEI_MUL(FSEI_SUB(gzp, gzm), rm));
         const double r_ = rhs_assemble(H, hprev[2], FSEI_MUL(FSEI_SUB(p00, p_km), rm), lap, A);
         A.rw[t] = A.fw ? FSEI_ADD(r_, FSEI_MUL(A.adt, fb3[2])) : r_;
@@ -413,10 +413,15 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         if (A.fw) fnext[2] = A.fw[tt];
     };
     if (in) fetch_hf(t);
+    // z metrics of plane k: rdzc[k-1], rdzc[k], rdzm[k], rdzm[k+1], rolled along the march; the two new ones of the next plane
+    // are loaded one iteration ahead of their use
+    double zq[4] = {k0 > 0 ? S.rdzc[k0 - 1] : 0.0, S.rdzc[k0], S.rdzm[k0], k0 + 1 < S.nz ? S.rdzm[k0 + 1] : 0.0};
 
     for (int k = k0; k < k1; k++, t += plane) {
         const double hprev[3] = {hnext[0], hnext[1], hnext[2]}, fb3[3] = {fnext[0], fnext[1], fnext[2]};
         if (in && k + 1 < k1) fetch_hf(t + plane);
+        const double zm4[4] = {zq[0], zq[1], zq[2], zq[3]};
+        if (k + 1 < k1) { zq[0] = zq[1]; zq[1] = S.rdzc[k + 1]; zq[2] = zq[3]; zq[3] = k + 2 < S.nz ? S.rdzm[k + 2] : 0.0; }
         cp_async_wait<1>();                          // everything but the newest group (plane k+2): planes <= k+1 have landed
         __syncthreads();                             // ... for every thread; and every thread is done with slot (k-2) mod R
         issue();                                     // plane k+3 -> slot (k+3) mod R = (k-2) mod R
@@ -426,8 +431,8 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
             const double* sm = ring + sm_ * SLOT;
             const double* sp = ring + sp_ * SLOT;
             const bool zlo = k == 0, zhi = k == S.nz - 1;
-            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, hprev, fb3, t, k, xlo, xhi, ylo, yhi, zlo, zhi);
-            else explicit_cell<false>(A, s0, sm, sp, c, hprev, fb3, t, k, false, false, false, false, false, false);
+            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, hprev, fb3, zm4, t, xlo, xhi, ylo, yhi, zlo, zhi);
+            else explicit_cell<false>(A, s0, sm, sp, c, hprev, fb3, zm4, t, false, false, false, false, false, false);
         }
         sc = sp_;
     }
