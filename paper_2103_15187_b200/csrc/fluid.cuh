@@ -240,6 +240,7 @@ struct ExplicitArgs {
     double *hu, *hv, *hw;                           // in: H of the previous substep, out: H of this one
     double *ru, *rv, *rw;                           // out: right-hand sides of the implicit step
     double gdt, rdt, adt, tb;                       // gamma dt, rho dt, alpha dt, 2 beta
+    int kz;                                         // planes per CTA (host: 64 on large grids, fewer when the grid would not fill the GPU)
 };
 
 FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const ExplicitArgs& A)
@@ -247,15 +248,15 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
     return FSEI_ADD(FSEI_SUB(FSEI_ADD(FSEI_MUL(A.gdt, H), FSEI_MUL(A.rdt, Hp)), FSEI_MUL(A.adt, gp)), FSEI_MUL(A.tb, lap));
 }
 
-#ifndef FSEI_EXPL_KZ
-#define FSEI_EXPL_KZ 32
-#endif
 #ifndef FSEI_EXPL_MINB
 #define FSEI_EXPL_MINB 2
 #endif
 #define FSEI_EXPL_TX 32
 #define FSEI_EXPL_TY 8
-#define FSEI_EXPL_RING 5
+#ifndef FSEI_EXPL_AHEAD
+#define FSEI_EXPL_AHEAD 2              // planes in flight beyond k+1
+#endif
+#define FSEI_EXPL_RING (3 + FSEI_EXPL_AHEAD)
 #define FSEI_EXPL_PW (FSEI_EXPL_TX + 2)
 #define FSEI_EXPL_TILE (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
 // doubles per ring slot: four halo tiles (u, v, w, p); H_prev of the next plane waits in three registers
@@ -352,7 +353,7 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
     }
 }
 
-// grid (ceil(nx/32), ceil(ny/8), ceil(nz/KZ)), block (32, 8), dynamic shared memory FSEI_EXPL_SMEM
+// grid (ceil(nx/32), ceil(ny/8), ceil(nz/kz)), block (32, 8), dynamic shared memory FSEI_EXPL_SMEM
 FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
 {
     constexpr int TX = FSEI_EXPL_TX, TY = FSEI_EXPL_TY, PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE, R = FSEI_EXPL_RING, SLOT = FSEI_EXPL_SLOT;
@@ -367,7 +368,7 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
     const bool xyedge = xlo || xhi || ylo || yhi;
     const size_t plane = (size_t)S.nx * S.ny;
-    const int k0 = blockIdx.z * FSEI_EXPL_KZ, k1 = (k0 + FSEI_EXPL_KZ < S.nz) ? k0 + FSEI_EXPL_KZ : S.nz;
+    const int k0 = blockIdx.z * A.kz, k1 = (k0 + A.kz < S.nz) ? k0 + A.kz : S.nz;
 
     // loader: tile elements e = tid and tid + 256 of the halo tiles (source index wrapped in a periodic direction, clamped at
     // a wall or a ragged edge) and this thread's own cell of the H_prev tiles; source pointers advance one plane per issue
@@ -400,7 +401,8 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         cp_async_commit();
         kk++; slot = slot + 1 == R ? 0 : slot + 1;
     };
-    issue(); issue(); issue(); issue();              // planes k0-1 .. k0+2
+#pragma unroll
+    for (int q = 0; q < FSEI_EXPL_AHEAD + 2; q++) issue();       // planes k0-1 .. k0+AHEAD
     const int c = (ty + 1) * PW + tx + 1;
     int sc = k0 % R;                                 // slot of plane k
     size_t t = (size_t)k0 * plane + (size_t)j * S.nx + i;
@@ -422,9 +424,9 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         if (in && k + 1 < k1) fetch_hf(t + plane);
         const double zm4[4] = {zq[0], zq[1], zq[2], zq[3]};
         if (k + 1 < k1) { zq[0] = zq[1]; zq[1] = S.rdzc[k + 1]; zq[2] = zq[3]; zq[3] = k + 2 < S.nz ? S.rdzm[k + 2] : 0.0; }
-        cp_async_wait<1>();                          // everything but the newest group (plane k+2): planes <= k+1 have landed
+        cp_async_wait<FSEI_EXPL_AHEAD - 1>();        // everything but the newest AHEAD-1 groups: planes <= k+1 have landed
         __syncthreads();                             // ... for every thread; and every thread is done with slot (k-2) mod R
-        issue();                                     // plane k+3 -> slot (k+3) mod R = (k-2) mod R
+        issue();                                     // plane k+AHEAD+1 -> slot (k+AHEAD+1) mod R = (k-2) mod R
         const int sm_ = sc == 0 ? R - 1 : sc - 1, sp_ = sc + 1 == R ? 0 : sc + 1;
         if (in) {
             const double* s0 = ring + sc * SLOT;

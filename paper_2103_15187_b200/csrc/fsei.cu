@@ -667,8 +667,12 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
         for (int b = a + 1; b < 6; b++) if (out[a] == out[b]) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: outputs must not alias each other");
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta};
-    const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (P->T.nz + FSEI_EXPL_KZ - 1) / FSEI_EXPL_KZ);
+    // planes per CTA: long marches amortise the ring's prologue (two halo planes per chunk); short ones keep small grids busy
+    const long tiles = (long)((P->T.nx + 31) / 32) * ((P->T.ny + 7) / 8);
+    int kz = 64;
+    while (kz > 8 && tiles * ((P->T.nz + kz - 1) / kz) < 1184) kz >>= 1;
+    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz};
+    const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (P->T.nz + kz - 1) / kz);
     { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), FSEI_EXPL_SMEM, st>>>(A); }
     CU(cudaGetLastError());
     P->last_launches = 1;
