@@ -571,7 +571,7 @@ def run_slab(args) -> dict:
         else:
             dist.init_process_group("gloo", init_method="tcp://127.0.0.1:29533", rank=0, world_size=1)
     case = inputs.make_case(args.config, fields=False)
-    sp = slab.SlabProjection(case.grid, rank, world, device=dev)
+    sp = (slab.SlabFluid if args.slab_substep else slab.SlabProjection)(case.grid, rank, world, device=dev)
     g = torch.Generator(device=dev).manual_seed(100 + rank)
     for t in (sp.u, sp.v, sp.w):
         t.copy_(torch.randn(t.shape, dtype=torch.float64, device=dev, generator=g))
@@ -590,8 +590,15 @@ def run_slab(args) -> dict:
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.slab_substep:                                # the whole fluid substep on slabs (explicit terms, viscous step, projection)
+        for t in (sp.u, sp.v, sp.w):
+            t.mul_(0.05)
+        beta = case.alpha_dt / (2 * 3000.0)
+        step = lambda: sp.substep(comm, 1.5 * case.alpha_dt, -0.5 * case.alpha_dt, case.alpha_dt, beta)
+    else:
+        step = lambda: sp.project(comm, case.alpha_dt, 0.0)
     for _ in range(max(args.warmup, 3)):
-        sp.project(comm, case.alpha_dt, 0.0)
+        step()
     barrier()
     sampler = ClockSampler(local)
     time.sleep(0.3)
@@ -601,7 +608,7 @@ def run_slab(args) -> dict:
     t0 = time.time()
     e0.record()
     for _ in range(args.steps):
-        sp.project(comm, case.alpha_dt, 0.0)
+        step()
     e1.record()
     barrier()
     t1 = time.time()
@@ -612,7 +619,8 @@ def run_slab(args) -> dict:
            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
            "config": {"workload": _workload_name(case), "cells": case.cells, "parallelism": f"z-slabs x{world} / x-slot pencils x{world}" + (", peer-store exchange" if args.slab_peers else ", grouped send/recv"),
-                      "exchange_bytes_per_rank_per_step": 2 * 16 * x.nzl * x.ny * (x.N - x.nsl) + 0,
+                      "step": "fluid substep (explicit terms, viscous step, projection)" if args.slab_substep else "projection",
+                      "exchange_bytes_per_rank_per_step": (8 if args.slab_substep else 2) * 16 * x.nzl * x.ny * (x.N - x.nsl),
                       "note": "unfused fast-family kernels per rank + 2 all-to-all exchanges (NCCL grouped send/recv); inputs N(0,1) "
                               "generated on the device; fields larger than L2"},
            "clocks": clocks, "gpu_launches": sp.launches,
@@ -639,6 +647,7 @@ def main():
     ap.add_argument("--no-all-configs", action="store_true", help="skip the compact table of the other configs")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
                     help="--parallel slab: process-group backend (gloo stages through the host and lets several ranks share one GPU)")
+    ap.add_argument("--slab-substep", action="store_true", help="--parallel slab: time the whole fluid substep instead of the projection")
     ap.add_argument("--slab-peers", action="store_true", help="--parallel slab: exchanges by peer stores from the kernels' epilogues")
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default; the headline path is single-GPU) or ONE projection decomposed into "

@@ -151,6 +151,8 @@ int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double*
  *   hu, hv, hw     : in: H of the previous substep (zeros on the first); out: H of this substep.
  *   ru, rv, rw     : out.  No output may alias an input or another output           else FSEI_ERR_ARG
  *   Wall-face rows (w at k = 0; u at i = 0 / v at j = 0 on a wall-bounded box) get H = rhs = 0.
+ *   On a slab plan (fsei_slab_plan_create) all fields are the rank's planes [k0, k1); u, v, w, p must be preceded in memory
+ *   by plane k0-1 unless k0 == 0 and followed by plane k1 unless k1 == nz (one halo layer).
  */
 int fsei_explicit_terms(fsei_plan* plan, const double* u, const double* v, const double* w, const double* p,
                         const double* fu, const double* fv, const double* fw, double* hu, double* hv, double* hw,
@@ -254,6 +256,19 @@ int fsei_slab_backward(fsei_plan* plan, double* spec, double* phi, void* cuda_st
 /* a7 on the slab (halo planes of phi as described above). */
 int fsei_slab_project(fsei_plan* plan, double* u, double* v, double* w, double* p, const double* phi,
                       double alpha_dt, double beta, void* cuda_stream);
+
+/*
+ * The implicit viscous step on slabs (the all-to-all also serves "the equation for the provisional velocity").
+ * fsei_slab_viscous_xy : the x and y sweeps of (I - beta dxx)(I - beta dyy) dq = r on the rank's planes, in place in ru, rv, rw.
+ * fsei_pencil_viscous_z: the z sweep (I - beta dzz) of component comp (0 u, 1 v, 2 w) on full z columns, in place.  The real
+ *                        slab field [nzl][ny][nx] is read as [nzl][ny][nx/2] pairs, so the pencil [nz][ny][2 nsl] doubles holds
+ *                        columns x in [2 s0, 2 s1) and the spectrum's exchange lists serve unchanged.
+ * fsei_slab_field_add  : q += r on the rank's planes (the provisional velocity q^ = q + dq).
+ * The three together give the same result as fsei_viscous_step on the whole grid (same sweeps, same order).
+ */
+int fsei_slab_viscous_xy(fsei_plan* plan, double* ru, double* rv, double* rw, double beta, void* cuda_stream);
+int fsei_pencil_viscous_z(fsei_plan* plan, double* pencil, int comp, double beta, void* cuda_stream);
+int fsei_slab_field_add(fsei_plan* plan, double* q, const double* r, void* cuda_stream);
 
 /*
  * Kernel-level timing aid for bench.py: number of kernels enqueued by the last

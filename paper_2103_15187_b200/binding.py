@@ -22,7 +22,8 @@ EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family",
            "fsei_plan_profile", "fsei_plan_profile_read",
            "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep",
            "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing",
-           "fsei_slab_plan_create", "fsei_slab_set_peers", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project")
+           "fsei_slab_plan_create", "fsei_slab_set_peers", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project",
+           "fsei_slab_viscous_xy", "fsei_pencil_viscous_z", "fsei_slab_field_add")
 
 _lib = None
 _vp, _d, _i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
@@ -102,6 +103,12 @@ def lib() -> ctypes.CDLL:
     L.fsei_slab_backward.argtypes = [_vp, _vp, _vp, _vp]
     L.fsei_slab_project.restype = _i
     L.fsei_slab_project.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _d, _d, _vp]
+    L.fsei_slab_viscous_xy.restype = _i
+    L.fsei_slab_viscous_xy.argtypes = [_vp, _vp, _vp, _vp, _d, _vp]
+    L.fsei_pencil_viscous_z.restype = _i
+    L.fsei_pencil_viscous_z.argtypes = [_vp, _vp, _i, _d, _vp]
+    L.fsei_slab_field_add.restype = _i
+    L.fsei_slab_field_add.argtypes = [_vp, _vp, _vp, _vp]
     _lib = L
     return L
 
@@ -282,3 +289,12 @@ class SlabPlan(Plan):
     def slab_project(self, u, v, w, p, phi, alpha_dt, beta=0.0, stream=None):
         _chk(lib().fsei_slab_project(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), _ptr(phi), float(alpha_dt), float(beta),
                                      _stream(stream)))
+
+    def slab_viscous_xy(self, ru, rv, rw, beta, stream=None):
+        _chk(lib().fsei_slab_viscous_xy(self._h, _ptr(ru), _ptr(rv), _ptr(rw), float(beta), _stream(stream)))
+
+    def pencil_viscous_z(self, pencil, comp, beta, stream=None):
+        _chk(lib().fsei_pencil_viscous_z(self._h, _ptr(pencil), int(comp), float(beta), _stream(stream)))
+
+    def slab_field_add(self, q, r, stream=None):
+        _chk(lib().fsei_slab_field_add(self._h, _ptr(q), _ptr(r), _stream(stream)))

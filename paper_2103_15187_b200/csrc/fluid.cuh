@@ -384,11 +384,13 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         return (size_t)gj * S.nx + gi;
     };
     const int kfirst = k0 - 1;                       // first plane the loader is asked for
-    size_t o0 = srcidx(tid) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
-    size_t o1 = srcidx(has1 ? e1 : tid) + (size_t)(kfirst < 0 ? 0 : kfirst) * plane;
-    int kk = kfirst, slot = (kfirst + R) % R;
+    // planes the fields hold: [klo, khi) = [0, nz), widened by the halo planes of a z-slab (S.halo_lo / S.halo_hi)
+    const int klo = S.halo_lo ? -1 : 0, khi = S.nz + (S.halo_hi ? 1 : 0);
+    long long o0 = (long long)srcidx(tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
+    long long o1 = (long long)srcidx(has1 ? e1 : tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
+    int kk = kfirst, slot = (kfirst + 2 * R) % R;
     auto issue = [&]() {                             // next plane kk -> its ring slot (nothing for a plane outside the grid)
-        if (kk >= 0 && kk < S.nz) {
+        if (kk >= klo && kk < khi) {
             double* sl = ring + slot * SLOT;
             cp_async8(sl + tid, A.u + o0); cp_async8(sl + TILE + tid, A.v + o0);
             cp_async8(sl + 2 * TILE + tid, A.w + o0); cp_async8(sl + 3 * TILE + tid, A.p + o0);
@@ -396,7 +398,7 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
                 cp_async8(sl + e1, A.u + o1); cp_async8(sl + TILE + e1, A.v + o1);
                 cp_async8(sl + 2 * TILE + e1, A.w + o1); cp_async8(sl + 3 * TILE + e1, A.p + o1);
             }
-            o0 += plane; o1 += plane;
+            o0 += (long long)plane; o1 += (long long)plane;
         }
         cp_async_commit();
         kk++; slot = slot + 1 == R ? 0 : slot + 1;
@@ -417,13 +419,15 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     if (in) fetch_hf(t);
     // z metrics of plane k: rdzc[k-1], rdzc[k], rdzm[k], rdzm[k+1], rolled along the march; the two new ones of the next plane
     // are loaded one iteration ahead of their use
-    double zq[4] = {k0 > 0 ? S.rdzc[k0 - 1] : 0.0, S.rdzc[k0], S.rdzm[k0], k0 + 1 < S.nz ? S.rdzm[k0 + 1] : 0.0};
+    const double* __restrict__ rdzc = S.rdzc + S.kofs;              // slab view: the metric tables are global
+    const double* __restrict__ rdzm = S.rdzm + S.kofs;
+    double zq[4] = {k0 > klo ? rdzc[k0 - 1] : 0.0, rdzc[k0], rdzm[k0], k0 + 1 < khi ? rdzm[k0 + 1] : 0.0};
 
     for (int k = k0; k < k1; k++, t += plane) {
         const double hprev[3] = {hnext[0], hnext[1], hnext[2]}, fb3[3] = {fnext[0], fnext[1], fnext[2]};
         if (in && k + 1 < k1) fetch_hf(t + plane);
         const double zm4[4] = {zq[0], zq[1], zq[2], zq[3]};
-        if (k + 1 < k1) { zq[0] = zq[1]; zq[1] = S.rdzc[k + 1]; zq[2] = zq[3]; zq[3] = k + 2 < S.nz ? S.rdzm[k + 2] : 0.0; }
+        if (k + 1 < k1) { zq[0] = zq[1]; zq[1] = rdzc[k + 1]; zq[2] = zq[3]; zq[3] = k + 2 < khi ? rdzm[k + 2] : 0.0; }
         cp_async_wait<FSEI_EXPL_AHEAD - 1>();        // everything but the newest AHEAD-1 groups: planes <= k+1 have landed
         __syncthreads();                             // ... for every thread; and every thread is done with slot (k-2) mod R
         issue();                                     // plane k+AHEAD+1 -> slot (k+AHEAD+1) mod R = (k-2) mod R
@@ -432,7 +436,7 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
             const double* s0 = ring + sc * SLOT;
             const double* sm = ring + sm_ * SLOT;
             const double* sp = ring + sp_ * SLOT;
-            const bool zlo = k == 0, zhi = k == S.nz - 1;
+            const bool zlo = k == 0 && !S.halo_lo, zhi = k == S.nz - 1 && !S.halo_hi;     // a wall, not a slab boundary
             if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, hprev, fb3, zm4, t, xlo, xhi, ylo, yhi, zlo, zhi);
             else explicit_cell<false>(A, s0, sm, sp, c, hprev, fb3, zm4, t, false, false, false, false, false, false);
         }

@@ -62,6 +62,7 @@ struct fsei_plan {
     size_t smem_x = 0, smem_y = 0;
     int last_launches = 0;
     const double* zc_dev = nullptr;      // z-face coordinates (IB-MLS node positions)
+    SParams Sg;                        // slab plans: the stencil parameters of the GLOBAL grid (z tables of the viscous step)
     bool slab = false; int k0 = 0, k1 = 0, s0 = 0, s1 = 0;   // z-slab / x-slot-pencil share of a multi-GPU decomposition (fsei_slab_plan_create)
     // implicit viscous step: factorisation tables of the last FSEI_VSLOTS values of beta (a three-stage Runge-Kutta scheme
     // cycles through three), device tables in vtab[slot], host-built line tables of the fast family beside them
@@ -657,7 +658,6 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
                                    double* ru, double* rv, double* rw, double gamma_dt, double rho_dt, double alpha_dt,
                                    double beta, void* cuda_stream)
 {
-    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: this is a slab plan (use the fsei_slab_* calls)");
     if (!P || !u || !v || !w || !p || !hu || !hv || !hw || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: NULL argument");
     if (gamma_dt != gamma_dt || rho_dt != rho_dt || alpha_dt != alpha_dt || !(beta >= 0.0)) return fail(FSEI_ERR_ARG, "fsei_explicit_terms: NaN parameter or beta < 0");
     const double* in[4] = {u, v, w, p};
@@ -670,9 +670,10 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     // planes per CTA: long marches amortise the ring's prologue (two halo planes per chunk); short ones keep small grids busy
     const long tiles = (long)((P->T.nx + 31) / 32) * ((P->T.ny + 7) / 8);
     int kz = 64;
-    while (kz > 8 && tiles * ((P->T.nz + kz - 1) / kz) < 1184) kz >>= 1;
+    const int nzl = P->S.nz;                           // planes held by the fields (a slab plan: its own planes)
+    while (kz > 8 && tiles * ((nzl + kz - 1) / kz) < 1184) kz >>= 1;
     ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz};
-    const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (P->T.nz + kz - 1) / kz);
+    const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (nzl + kz - 1) / kz);
     { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), FSEI_EXPL_SMEM, st>>>(A); }
     CU(cudaGetLastError());
     P->last_launches = 1;
@@ -693,22 +694,13 @@ static VTab visc_tab(const fsei_plan* P, int slot, int comp, int dir)
     return V;
 }
 
-extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, double* ru, double* rv, double* rw,
-                                 double beta, void* cuda_stream)
+// factorisation tables of the implicit viscous step for this beta: kept per value in FSEI_VSLOTS slots (round-robin
+// replacement).  Under stream capture the device tables are rebuilt inside the graph even on a hit, so a replay never depends
+// on a slot that an eager call with other betas has overwritten in the meantime (the host-built tables travel as kernel
+// parameters).  Returns the slot; *launches counts the factor kernel if it ran.
+static int visc_tables(fsei_plan* P, double beta, cudaStream_t st, int* slot_out, int* launches)
 {
-    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_viscous_step: this is a slab plan (use the fsei_slab_* calls)");
-    if (!P || !u || !v || !w || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_viscous_step: NULL argument");
-    if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_viscous_step: beta must be finite and >= 0");
-    double* q[3] = {u, v, w};
-    double* r[3] = {ru, rv, rw};
-    for (int a = 0; a < 3; a++)
-        for (int b = 0; b < 3; b++) if (r[a] == q[b] || (a != b && (r[a] == r[b] || q[a] == q[b]))) return fail(FSEI_ERR_ARG, "fsei_viscous_step: fields must not alias");
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const HostTables& T = P->T;
-    int launches = 0;
-    // factorisation tables for this beta: kept per value in FSEI_VSLOTS slots (round-robin replacement).  Under stream
-    // capture the device tables are rebuilt inside the graph even on a hit, so a replay never depends on a slot that an
-    // eager call with other betas has overwritten in the meantime (the host-built tables travel as kernel parameters).
     int slot = -1;
     for (int i = 0; i < FSEI_VSLOTS; i++) if (P->visc_beta[i] == beta) slot = i;
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -723,11 +715,30 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
         P->visc_beta[slot] = beta;
     }
     if (miss || cap != cudaStreamCaptureStatusNone) {
-        VFactorArgs A{P->S, beta, P->vtab + (size_t)slot * 9 * vtab_set_doubles(P->vnmax), P->vnmax};
+        VFactorArgs A{P->slab ? P->Sg : P->S, beta, P->vtab + (size_t)slot * 9 * vtab_set_doubles(P->vnmax), P->vnmax};
         { LaunchTimer t(P, K_VFACT, st); k_visc_factor<<<9, 32, 0, st>>>(A); }
         CU(cudaGetLastError());
-        launches++;
+        (*launches)++;
     }
+    *slot_out = slot;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, double* ru, double* rv, double* rw,
+                                 double beta, void* cuda_stream)
+{
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_viscous_step: this is a slab plan (use the fsei_slab_* calls)");
+    if (!P || !u || !v || !w || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_viscous_step: NULL argument");
+    if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_viscous_step: beta must be finite and >= 0");
+    double* q[3] = {u, v, w};
+    double* r[3] = {ru, rv, rw};
+    for (int a = 0; a < 3; a++)
+        for (int b = 0; b < 3; b++) if (r[a] == q[b] || (a != b && (r[a] == r[b] || q[a] == q[b]))) return fail(FSEI_ERR_ARG, "fsei_viscous_step: fields must not alias");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const HostTables& T = P->T;
+    int launches = 0;
+    int slot = 0;
+    { int rc0 = visc_tables(P, beta, st, &slot, &launches); if (rc0) return rc0; }
     if (P->visc_fast) {
         VFastArgs A;
         for (int c = 0; c < 3; c++) {
@@ -883,6 +894,14 @@ static int slab_plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, doub
     if ((rc = upload(P, T.rdzc, &S.rdzc))) return rc;
     if ((rc = upload(P, T.rdzm, &S.rdzm))) return rc;
     S.kofs = k0; S.halo_lo = k0 > 0; S.halo_hi = k1 < nz;
+    P->Sg = S; P->Sg.nz = nz; P->Sg.kofs = 0; P->Sg.halo_lo = 0; P->Sg.halo_hi = 0;
+    {
+        P->vnmax = nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz);
+        void* qv = nullptr;
+        if ((rc = dalloc(P, sizeof(double) * FSEI_VSLOTS * 9 * vtab_set_doubles(P->vnmax), &qv))) return rc;
+        P->vtab = static_cast<double*>(qv);
+        CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM));
+    }
     XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
     XF.nx = nx; XF.ny = ny; XF.nz = nzl; XF.N = nx / 2; XF.tw = X.tw; XF.tw_r2c = X.tw_r2c; XF.tw_dct = X.tw_dct; XF.scale = T.scale;
     {
@@ -1018,6 +1037,69 @@ extern "C" int fsei_slab_project(fsei_plan* P, double* u, double* v, double* w, 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t n = (size_t)P->T.nx * P->T.ny * (P->k1 - P->k0);
     { LaunchTimer t(P, K_PROJ, st); k_project_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, p, phi, alpha_dt, beta); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
+}
+
+// ---- slab decomposition of the implicit viscous step: x and y sweeps are local to a z-slab, the z sweep runs on pencils
+// that hold full z columns (here: every row and plane of a range of x, the real field viewed as nx/2 complex slots so that
+// the spectrum's exchange buffers and lists serve unchanged); q += dq afterwards, on the slab.
+__global__ void __launch_bounds__(256) k_field_add(double* __restrict__ q, const double* __restrict__ r, size_t n2)
+{
+    const size_t t = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (t >= n2) return;
+    cplx a = *reinterpret_cast<cplx*>(q + 2 * t);
+    const cplx b = *reinterpret_cast<const cplx*>(r + 2 * t);
+    a.re += b.re; a.im += b.im;
+    *reinterpret_cast<cplx*>(q + 2 * t) = a;
+}
+
+extern "C" int fsei_slab_viscous_xy(fsei_plan* P, double* ru, double* rv, double* rw, double beta, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_slab_viscous_xy");
+    if (!ru || !rv || !rw || ru == rv || ru == rw || rv == rw) return fail(FSEI_ERR_ARG, "fsei_slab_viscous_xy: NULL or aliased fields");
+    if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_slab_viscous_xy: beta must be finite and >= 0");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const HostTables& T = P->T;
+    int launches = 0, slot = 0, rc;
+    if ((rc = visc_tables(P, beta, st, &slot, &launches))) return rc;
+    const int nzl = P->k1 - P->k0;
+    const long nlx = (long)T.ny * nzl, nly = (long)T.nx * nzl;
+    const size_t plane = (size_t)T.nx * T.ny;
+    double* r[3] = {ru, rv, rw};
+    for (int c = 0; c < 3; c++) {
+        { VTab V = visc_tab(P, slot, c, DIR_X); LaunchTimer t(P, K_VX, st); k_visc_sweep_x<true, false><<<(unsigned)((nlx + 127) / 128), 128, 0, st>>>(V, r[c], nullptr, nlx); }
+        CU(cudaGetLastError());
+        { VTab V = visc_tab(P, slot, c, DIR_Y); LaunchTimer t(P, K_VY, st); k_visc_sweep_strided<true, false><<<(unsigned)((nly + 127) / 128), 128, 0, st>>>(V, r[c], nullptr, T.nx, (size_t)T.nx, plane, nly); }
+        CU(cudaGetLastError());
+        launches += 2;
+    }
+    P->last_launches = launches;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_pencil_viscous_z(fsei_plan* P, double* pencil, int comp, double beta, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_pencil_viscous_z");
+    if (!pencil || comp < 0 || comp > 2) return fail(FSEI_ERR_ARG, "fsei_pencil_viscous_z: NULL pencil or component not in 0..2");
+    if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_pencil_viscous_z: beta must be finite and >= 0");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0, slot = 0, rc;
+    if ((rc = visc_tables(P, beta, st, &slot, &launches))) return rc;
+    const long ncol = (long)P->T.ny * 2 * (P->s1 - P->s0);            // real columns of the pencil [nz][ny][2 nsl]
+    { VTab V = visc_tab(P, slot, comp, DIR_Z); LaunchTimer t(P, K_VZ, st); k_visc_sweep_strided<false, false><<<(unsigned)((ncol + 127) / 128), 128, 0, st>>>(V, pencil, nullptr, (int)ncol, (size_t)ncol, 0, ncol); }
+    CU(cudaGetLastError());
+    P->last_launches = launches + 1;
+    return FSEI_OK;
+}
+
+extern "C" int fsei_slab_field_add(fsei_plan* P, double* q, const double* r, void* cuda_stream)
+{
+    SLAB_ONLY("fsei_slab_field_add");
+    if (!q || !r || q == r || misaligned(q) || misaligned(r)) return fail(FSEI_ERR_ARG, "fsei_slab_field_add: NULL, aliased or misaligned fields");
+    const size_t n2 = (size_t)P->T.nx * P->T.ny * (P->k1 - P->k0) / 2;
+    k_field_add<<<(unsigned)((n2 + 255) / 256), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(q, r, n2);
     CU(cudaGetLastError());
     P->last_launches = 1;
     return FSEI_OK;

@@ -57,10 +57,12 @@ class SlabExchange:
         return sends, recvs
 
     # ---- slab spectrum -> pencils (between a3 and a4) ----------------------------------------------------------
-    def to_pencils(self):
+    def to_pencils(self, src=None):
+        """src: a slab array [nzl][ny][N][2] other than the spectrum (a real field read as pairs: the viscous z sweep)."""
+        src = self.spec if src is None else src
         sends, recvs = [], []
         for d, (s0, s1) in enumerate(self.sr):
-            self.send[d].copy_(self.spec[:, :, s0:s1, :])
+            self.send[d].copy_(src[:, :, s0:s1, :])
             sends.append((self.send[d], d))
         for s, (k0, k1) in enumerate(self.kr):
             recvs.append((self.pencil[k0:k1], s))                     # contiguous: lands in place
@@ -72,9 +74,10 @@ class SlabExchange:
         recvs = [(self.recv[s], s) for s in range(self.world)]
         return sends, recvs
 
-    def unpack_slabs(self):
+    def unpack_slabs(self, dst=None):
+        dst = self.spec if dst is None else dst
         for s, (s0, s1) in enumerate(self.sr):
-            self.spec[:, :, s0:s1, :].copy_(self.recv[s])
+            dst[:, :, s0:s1, :].copy_(self.recv[s])
 
     # ---- halo of phi (before a7): my last plane goes up; with beta != 0 my first plane also goes down ---------
     def phi_halo(self, both: bool):
@@ -256,6 +259,85 @@ class SlabProjection:
 
     def destroy(self):
         self.plan.destroy()
+
+
+class SlabFluid(SlabProjection):
+    """One rank of the decomposed fluid substep: explicit terms (one halo layer of u, v, w, p), implicit viscous step (x and
+    y sweeps on the slab, z sweep on pencils: P:L248) and the projection.  Plumbing only, as above."""
+
+    def __init__(self, grid, rank: int, world: int, device="cuda"):
+        import torch
+        super().__init__(grid, rank, world, device)
+        nx, ny, nzl = self.x.nx, self.x.ny, self.x.nzl
+        mk = lambda: torch.zeros((nzl + 2, ny, nx), dtype=torch.float64, device=device)
+        self.ext = [mk() for _ in range(4)]                            # u, v, w, p with the planes below and above
+        self.u, self.v, self.w, self.p = (e[1:nzl + 1] for e in self.ext)
+        self.h = [torch.zeros((nzl, ny, nx), dtype=torch.float64, device=device) for _ in range(3)]
+        self.r = [torch.zeros_like(self.h[0]) for _ in range(3)]
+        self.f = (None, None, None)
+
+    def stage_w_halo(self):
+        x = self.x
+        sends = [(self.w[0], x.rank - 1)] if x.rank > 0 else []
+        recvs = [(self.ext[2][x.nzl + 1], x.rank + 1)] if x.rank + 1 < x.world else []
+        return sends, recvs
+
+    def stage_halos(self):
+        """One halo layer of u, v, w, p on each side."""
+        x, sends, recvs = self.x, [], []
+        for e in self.ext:
+            if x.rank > 0:
+                sends.append((e[1], x.rank - 1)); recvs.append((e[0], x.rank - 1))
+            if x.rank + 1 < x.world:
+                sends.append((e[x.nzl], x.rank + 1)); recvs.append((e[x.nzl + 1], x.rank + 1))
+        return sends, recvs
+
+    def stage_explicit(self, gamma_dt, rho_dt, alpha_dt, beta, stream=None):
+        self.plan.explicit_terms(self.u, self.v, self.w, self.p, *self.h, *self.r, gamma_dt, rho_dt, alpha_dt, beta,
+                                 f=self.f, stream=stream)
+        self.launches += self.plan.last_launch_count
+        self.plan.slab_viscous_xy(*self.r, beta, stream)
+        self.launches += self.plan.last_launch_count
+
+    def _pairs(self, c):
+        return self.r[c].view(self.x.nzl, self.x.ny, self.x.N, 2)
+
+    def stage_visc_to_pencils(self, c):
+        return self.x.to_pencils(self._pairs(c))
+
+    def stage_visc_z(self, c, beta, stream=None):
+        self.plan.pencil_viscous_z(self.x.pencil, c, beta, stream)
+        self.launches += self.plan.last_launch_count
+        return self.x.to_slabs()
+
+    def stage_visc_add(self, c, stream=None):
+        self.x.unpack_slabs(self._pairs(c))
+        self.plan.slab_field_add((self.u, self.v, self.w)[c], self.r[c], stream)
+        self.launches += self.plan.last_launch_count
+
+    def substep(self, comm: DistComm, gamma_dt, rho_dt, alpha_dt, beta, stream=None):
+        """One substep of this rank, exchanges over `comm` (all ranks call it together).  The viscous z sweeps exchange by
+        explicit send/recv lists also when the projection uses peer stores."""
+        comm.exchange(*self.stage_halos())
+        self.stage_explicit(gamma_dt, rho_dt, alpha_dt, beta, stream)
+        for c in range(3):
+            comm.exchange(*self.stage_visc_to_pencils(c))
+            comm.exchange(*self.stage_visc_z(c, beta, stream))
+            self.stage_visc_add(c, stream)
+        self.project(comm, alpha_dt, beta, stream)
+
+
+def substep_local(ranks: Sequence["SlabFluid"], gamma_dt, rho_dt, alpha_dt, beta):
+    """All ranks in one process, stage by stage (LocalComm)."""
+    LocalComm.exchange_all([r.stage_halos() for r in ranks])
+    for r in ranks:
+        r.stage_explicit(gamma_dt, rho_dt, alpha_dt, beta)
+    for c in range(3):
+        LocalComm.exchange_all([r.stage_visc_to_pencils(c) for r in ranks])
+        LocalComm.exchange_all([r.stage_visc_z(c, beta) for r in ranks])
+        for r in ranks:
+            r.stage_visc_add(c)
+    project_local(ranks, alpha_dt, beta)
 
 
 def local_peers(ranks: Sequence[SlabProjection]):

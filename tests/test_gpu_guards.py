@@ -129,3 +129,27 @@ def test_slab_stages_inside_guards(world):
         for t in (r.u, r.v, r.w, r.p, r.phi):
             assert bool(torch.isfinite(t).all())
         r.destroy()
+
+
+def test_slab_viscous_calls_reject_bad_arguments():
+    import torch
+    from paper_2103_15187_b200 import inputs
+    from paper_2103_15187_b200.binding import FseiError, ERR_ARG, SlabPlan
+    from tests.util import make_plan
+    g = inputs.make_grid(2, shape=(32, 32, 16))
+    sp = SlabPlan(g, 0, 8, 0, 8)
+    a, b, c = (torch.zeros((8, 32, 32), dtype=torch.float64, device="cuda") for _ in range(3))
+    pencil = torch.zeros((16, 32, 16), dtype=torch.float64, device="cuda")
+    for call in (lambda: sp.slab_viscous_xy(a, a, c, 1e-3), lambda: sp.slab_viscous_xy(a, b, c, -1.0),
+                 lambda: sp.pencil_viscous_z(pencil, 3, 1e-3), lambda: sp.pencil_viscous_z(pencil, 0, float("inf")),
+                 lambda: sp.slab_field_add(a, a)):
+        with pytest.raises(FseiError) as e:
+            call()
+        assert e.value.code == ERR_ARG
+    sp.destroy()
+    plan = make_plan(g)                                          # a whole-grid plan has no slab stages
+    with pytest.raises(FseiError) as e:
+        plan_call = SlabPlan.slab_viscous_xy
+        plan_call(plan, a, b, c, 1e-3)
+    assert e.value.code == ERR_ARG
+    plan.destroy()

@@ -282,3 +282,136 @@ def test_peer_store_exchange_across_processes(tmp_path, oracle_ld, world, shape,
     assert rel_l2(got["phi"], ref[4]) <= 1e-11
     for f, r in zip(("u", "v", "w", "p"), ref[:4]):
         assert np.abs(got[f] - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
+
+
+# ---------------------------------------------------------------------------------------------
+# the whole fluid substep on slabs: explicit terms with one halo layer, viscous z sweep on pencils, projection
+# ---------------------------------------------------------------------------------------------
+RK3 = ((8 / 15, 5 / 12, 3 / 4), (0.0, -17 / 60, -5 / 12))
+
+
+def _fluid_case(shape, seed=71):
+    nx, ny, nz = shape
+    g = inputs.make_grid(2, shape=shape)
+    u, v, w = [0.1 * inputs.normal_field(seed, i, (nz, ny, nx)) for i in range(3)]
+    w[0] = 0
+    f = [0.05 * inputs.normal_field(seed, 3 + i, (nz, ny, nx)) for i in range(3)]
+    return g, u, v, w, f
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [1, 2, 3, 4])
+@pytest.mark.parametrize("shape,force", [((64, 32, 24), False), ((128, 64, 37), True), ((96, 48, 16), True)])
+def test_decomposed_fluid_substeps_vs_oracle_and_single_plan(oracle_ld, world, shape, force):
+    """Three RK3 substeps on `world` slabs stepped stage by stage in one process against the oracle's chain and the
+    single-plan fsei_fluid_substep.  Explicit terms are bit-exact stencils on either path (the halo planes hold the
+    neighbour's values), so the first rhs is bit-identical to the oracle's."""
+    from tests.util import make_plan
+    g, u, v, w, f = _fluid_case(shape)
+    dt, Re = 2e-3, 200.0
+    ranks = [slab.SlabFluid(g, r, world) for r in range(world)]
+    for r in ranks:
+        r.load(u, v, w)
+        if force:
+            r.f = tuple(torch.as_tensor(t[r.x.k0:r.x.k1].copy()).cuda() for t in f)
+    uo, vo, wo, po = u.copy(), v.copy(), w.copy(), np.zeros_like(u)
+    ho = [np.zeros_like(u) for _ in range(3)]
+    fo = f if force else (None, None, None)
+    plan = make_plan(g)
+    d = [torch.as_tensor(t.copy()).cuda() for t in (u, v, w, po, *ho)]
+    df = tuple(torch.as_tensor(t).cuda() for t in f) if force else (None, None, None)
+    scratch = [torch.empty_like(d[0]) for _ in range(4)]
+    for l in range(3):
+        al = RK3[0][l] + RK3[1][l]
+        beta = al * dt / (2 * Re)
+        slab.substep_local(ranks, RK3[0][l] * dt, RK3[1][l] * dt, al * dt, beta)
+        plan.fluid_substep(*d[:4], *d[4:], *scratch, RK3[0][l] * dt, RK3[1][l] * dt, al * dt, beta, f=df)
+        rr = oracle_ld.explicit_terms(g, uo, vo, wo, po, *ho, RK3[0][l] * dt, RK3[1][l] * dt, al * dt, beta, f=fo)
+        if l == 0:
+            hh = [np.concatenate([r.h[c].cpu().numpy() for r in ranks], axis=0) for c in range(3)]
+            for c in range(3):
+                assert np.array_equal(hh[c], ho[c]), c                      # H of the first substep: bit-exact across slab boundaries
+        oracle_ld.viscous_step(g, uo, vo, wo, *rr, beta)
+        oracle_ld.pressure_projection(g, uo, vo, wo, po, al * dt, beta)
+    torch.cuda.synchronize()
+    got = [np.concatenate([getattr(r, n).cpu().numpy() for r in ranks], axis=0) for n in ("u", "v", "w", "p")]
+    for c, ref in enumerate((uo, vo, wo, po)):
+        assert np.abs(got[c] - ref).max() <= 1e-11 * max(1.0, np.abs(ref).max()), (c, np.abs(got[c] - ref).max())
+        one = d[c].cpu().numpy()
+        assert np.abs(got[c] - one).max() <= 1e-12 * max(1.0, np.abs(one).max()), (c, np.abs(got[c] - one).max())
+    div = np.abs(oracle_ld.divergence(g, got[0], got[1], got[2], 1.0)).max()
+    assert div <= 1e-10, div
+    plan.destroy()
+    for r in ranks:
+        r.destroy()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_viscous_stages_vs_oracle(oracle_ld, world):
+    """The viscous stages alone (x, y sweeps on slabs; z sweep on pencils; q += dq) against the oracle's viscous step at a
+    stiff beta, where the z coupling across slab boundaries is strong."""
+    shape = (64, 32, 30)
+    g, u, v, w, f = _fluid_case(shape, seed=72)
+    beta = 5e-3
+    uo, vo, wo = u.copy(), v.copy(), w.copy()
+    oracle_ld.viscous_step(g, uo, vo, wo, *[t.copy() for t in f], beta)
+    ranks = [slab.SlabFluid(g, r, world) for r in range(world)]
+    for r in ranks:
+        r.load(u, v, w)
+        for c in range(3):
+            r.r[c].copy_(torch.as_tensor(f[c][r.x.k0:r.x.k1].copy()))
+        r.plan.slab_viscous_xy(*r.r, beta)
+    for c in range(3):
+        slab.LocalComm.exchange_all([r.stage_visc_to_pencils(c) for r in ranks])
+        slab.LocalComm.exchange_all([r.stage_visc_z(c, beta) for r in ranks])
+        for r in ranks:
+            r.stage_visc_add(c)
+    torch.cuda.synchronize()
+    for c, (q0, qo) in enumerate(((u, uo), (v, vo), (w, wo))):
+        got = np.concatenate([(r.u, r.v, r.w)[c].cpu().numpy() for r in ranks], axis=0)
+        assert np.abs(got - qo).max() <= 1e-12 * np.abs(qo - q0).max() + 4e-16 * np.abs(qo).max(), c
+    for r in ranks:
+        r.destroy()
+
+
+def _gpu_fluid_worker(rank, world, port, shape, out):
+    sys.path.insert(0, ROOT)
+    import numpy as _np
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    g, u, v, w, f = _fluid_case(shape)
+    r = slab.SlabFluid(g, rank, world, device="cuda:0")
+    r.load(u, v, w)
+    comm = slab.DistComm()
+    dt, Re = 2e-3, 200.0
+    for l in range(3):
+        al = RK3[0][l] + RK3[1][l]
+        r.substep(comm, RK3[0][l] * dt, RK3[1][l] * dt, al * dt, al * dt / (2 * Re))
+    torch.cuda.synchronize()
+    _np.savez(os.path.join(out, f"r{rank}.npz"), **{n: getattr(r, n).cpu().numpy() for n in ("u", "v", "w", "p")})
+    r.destroy()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world,shape", [(2, (64, 32, 24)), (3, (96, 48, 16))])
+def test_fluid_substeps_real_process_group(tmp_path, oracle_ld, world, shape):
+    """One process per rank, all exchanges (halos, viscous transposes, projection transposes) through torch.distributed."""
+    port = _free_port()
+    mp.spawn(_gpu_fluid_worker, args=(world, port, shape, str(tmp_path)), nprocs=world, join=True)
+    parts = [np.load(os.path.join(tmp_path, f"r{r}.npz")) for r in range(world)]
+    got = {n: np.concatenate([p[n] for p in parts], axis=0) for n in ("u", "v", "w", "p")}
+    g, u, v, w, f = _fluid_case(shape)
+    uo, vo, wo, po = u.copy(), v.copy(), w.copy(), np.zeros_like(u)
+    ho = [np.zeros_like(u) for _ in range(3)]
+    dt, Re = 2e-3, 200.0
+    for l in range(3):
+        al = RK3[0][l] + RK3[1][l]
+        beta = al * dt / (2 * Re)
+        rr = oracle_ld.explicit_terms(g, uo, vo, wo, po, *ho, RK3[0][l] * dt, RK3[1][l] * dt, al * dt, beta)
+        oracle_ld.viscous_step(g, uo, vo, wo, *rr, beta)
+        oracle_ld.pressure_projection(g, uo, vo, wo, po, al * dt, beta)
+    for n, ref in zip(("u", "v", "w", "p"), (uo, vo, wo, po)):
+        assert np.abs(got[n] - ref).max() <= 1e-11 * max(1.0, np.abs(ref).max()), n
