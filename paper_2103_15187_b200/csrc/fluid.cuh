@@ -218,9 +218,9 @@ FSEI_GLOBAL(128, 1) k_visc_sweep_x(VTab T, double* __restrict__ f, double* __res
 
 // ---------------------------------------------------------------------------------------------------------------
 // explicit terms.  CTA = 32 x 8 threads on a tile of 32 x-cells by 8 y-rows, marching KZ planes along z (2.5-D
-// blocking): the (34 x 10) halo tiles of u, v, w, p and the tile of the three H_prev fields of plane k+3 are on their way
-// to a five-slot shared-memory ring (cp.async, 8-byte copies, one commit group per plane) while plane k is evaluated
-// from slots k-1, k, k+1 -- so the bytes in flight per SM do not depend on how many registers a thread can spare, every
+// blocking): the (34 x 10) halo tiles of u, v, w, p of plane k+3 are on their way to a four-slot shared-memory ring
+// (cp.async, 8-byte copies, one commit group per plane) while plane k is evaluated from slots k, k+1 and from registers
+// carried along the march (everything it needs of plane k-1, and what it already read of plane k one iteration ago) -- so the bytes in flight per SM do not depend on how many registers a thread can spare, every
 // input plane is read from L2/DRAM once per CTA (+ halo), and the only global accesses of the compute phase are the six
 // coalesced stores.  Every floating-point operation is individually rounded in the order of the definition
 // (V10 states it), so the results are bit-identical.
@@ -251,12 +251,13 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
 #ifndef FSEI_EXPL_MINB
 #define FSEI_EXPL_MINB 2
 #endif
+#define FSEI_EXPL_KZMAX 64             // most planes a CTA marches (ExplicitArgs::kz)
 #define FSEI_EXPL_TX 32
 #define FSEI_EXPL_TY 8
 #ifndef FSEI_EXPL_AHEAD
 #define FSEI_EXPL_AHEAD 2              // planes in flight beyond k+1
 #endif
-#define FSEI_EXPL_RING (3 + FSEI_EXPL_AHEAD)
+#define FSEI_EXPL_RING (2 + FSEI_EXPL_AHEAD)    // planes k, k+1 being read + AHEAD in flight (plane k-1 lives in registers)
 #define FSEI_EXPL_PW (FSEI_EXPL_TX + 2)
 #define FSEI_EXPL_TILE (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
 // doubles per ring slot: four halo tiles (u, v, w, p); H_prev of the next plane waits in three registers
@@ -264,18 +265,25 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
 #define FSEI_EXPL_SMEM (FSEI_EXPL_RING * FSEI_EXPL_SLOT * 8)
 
 #if defined(__CUDACC__)
-__device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc)
+__device__ __forceinline__ void cp_async8(uint32_t sdst, const double* gsrc)
 {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sdst)), "l"(gsrc) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sdst), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// one cell of the three components from the ring slots of planes k-1 (sm), k (s0), k+1 (sp).  EDGE = false: a cell with
-// no wall or z boundary among its neighbours (every cell of a periodic box except on its bottom and top planes): the
+// what a thread carries along the z march instead of reading it again from shared memory: the values of plane k+1 it
+// used at plane k are plane k's at the next iteration (cur), and plane k's become the plane below (bel)
+struct ExplicitCarry {
+    double u00, v00, w00, wM0, w0M;                  // plane k     : u, v, w at the cell, w at i-1 and at j-1
+    double u_km, v_km, w_km, p_km, uP_km, v0P_km;    // plane k - 1 : u, v, w, p at the cell, u at i+1, v at j+1 (0 beyond a wall)
+};
+
+// one cell of the three components from the ring slots of planes k (s0), k+1 (sp) and the carried registers.  EDGE = false: a
+// cell with no wall or z boundary among its neighbours (every cell of a periodic box except on its bottom and top planes): the
 // wall selects compile away.  The arithmetic of the two variants is the same, operation for operation.
 template <bool EDGE>
-__device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const double* __restrict__ s0, const double* __restrict__ sm,
+__device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const double* __restrict__ s0, ExplicitCarry& C,
                                               const double* __restrict__ sp, int c, const double (&hprev)[3], const double (&fb3)[3], const double (&zm4)[4], size_t t,
                                               bool xlo, bool xhi, bool ylo, bool yhi, bool zlo, bool zhi)
 {
@@ -283,19 +291,20 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
     const SParams& S = A.S;
     const double rdx = S.rdx, rdy = S.rdy;
     const double *U0 = s0, *V0 = s0 + TILE, *W0 = s0 + 2 * TILE, *P0 = s0 + 3 * TILE;
-    const double *Um = sm, *Vm = sm + TILE, *Wm = sm + 2 * TILE, *Pm = sm + 3 * TILE;
     const double *Up = sp, *Vp = sp + TILE, *Wp = sp + 2 * TILE;
-    const double u00 = U0[c], v00 = V0[c], w00 = W0[c], p00 = P0[c];
+    const double u00 = C.u00, v00 = C.v00, w00 = C.w00, p00 = P0[c];
     const double uP0 = (EDGE && xhi) ? 0.0 : U0[c + 1], uM0 = U0[c - 1], uPM = U0[c - PW + 1];
     double u0P = U0[c + PW], u0M = U0[c - PW];
     double vP0 = V0[c + 1], vM0 = V0[c - 1];
     const double v0P = (EDGE && yhi) ? 0.0 : V0[c + PW], v0M = V0[c - PW], vMP = V0[c + PW - 1];
-    double wP0 = W0[c + 1], w0P = W0[c + PW], wM0 = W0[c - 1], w0M = W0[c - PW];
+    double wP0 = W0[c + 1], w0P = W0[c + PW], wM0 = C.wM0, w0M = C.w0M;
     const double pM0 = P0[c - 1], p0M = P0[c - PW];
     // plane above (fluxes through the upper face; never used on the top plane) and below (never used on the bottom one)
     const double u_kp = Up[c], v_kp = Vp[c], w_kp = (EDGE && zhi) ? 0.0 : Wp[c], wM_kp = Wp[c - 1], w0M_kp = Wp[c - PW];
-    const double u_km = Um[c], v_km = Vm[c], w_km = Wm[c], p_km = Pm[c];
-    const double uP_km = (EDGE && xhi) ? 0.0 : Um[c + 1], v0P_km = (EDGE && yhi) ? 0.0 : Vm[c + PW];
+    const double u_km = C.u_km, v_km = C.v_km, w_km = C.w_km, p_km = C.p_km, uP_km = C.uP_km, v0P_km = C.v0P_km;
+    // the next plane's carry (the ghosts below overwrite only local copies)
+    C.u_km = u00; C.v_km = v00; C.w_km = w00; C.p_km = p00; C.uP_km = uP0; C.v0P_km = v0P;
+    C.u00 = u_kp; C.v00 = v_kp; C.w00 = w_kp; C.wM0 = wM_kp; C.w0M = w0M_kp;
     if (EDGE) {                                      // ghosts of the tangential components beyond a wall
         if (ylo) u0M = -u00; if (yhi) u0P = -u00;
         if (xlo) vM0 = -v00; if (xhi) vP0 = -v00;
@@ -362,7 +371,8 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     const SParams& S = A.S;
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, i = i0 + tx, j = j0 + ty;
-    const bool in = i < S.nx && j < S.ny;
+    int in = i < S.nx && j < S.ny;
+    asm volatile("" : "+r"(in));                     // kept in a register: recomputing it costs four S2R / LDC round trips per plane
     const bool xper = S.bcx == BC_PERIODIC, yper = S.bcy == BC_PERIODIC;
     const bool xlo = !xper && i == 0, xhi = !xper && i == S.nx - 1;      // x-face i / i+1 is a wall
     const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
@@ -389,14 +399,16 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     long long o0 = (long long)srcidx(tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
     long long o1 = (long long)srcidx(has1 ? e1 : tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
     int kk = kfirst, slot = (kfirst + 2 * R) % R;
+    uint32_t ring_tid = smem_u32(ring + tid);        // shared-window address of this thread's first element of slot 0
+    asm volatile("" : "+r"(ring_tid));
     auto issue = [&]() {                             // next plane kk -> its ring slot (nothing for a plane outside the grid)
         if (kk >= klo && kk < khi) {
-            double* sl = ring + slot * SLOT;
-            cp_async8(sl + tid, A.u + o0); cp_async8(sl + TILE + tid, A.v + o0);
-            cp_async8(sl + 2 * TILE + tid, A.w + o0); cp_async8(sl + 3 * TILE + tid, A.p + o0);
+            const uint32_t sl = ring_tid + (uint32_t)(slot * SLOT * 8);
+            cp_async8(sl, A.u + o0); cp_async8(sl + TILE * 8, A.v + o0);
+            cp_async8(sl + 2 * TILE * 8, A.w + o0); cp_async8(sl + 3 * TILE * 8, A.p + o0);
             if (has1) {
-                cp_async8(sl + e1, A.u + o1); cp_async8(sl + TILE + e1, A.v + o1);
-                cp_async8(sl + 2 * TILE + e1, A.w + o1); cp_async8(sl + 3 * TILE + e1, A.p + o1);
+                cp_async8(sl + 256 * 8, A.u + o1); cp_async8(sl + (TILE + 256) * 8, A.v + o1);
+                cp_async8(sl + (2 * TILE + 256) * 8, A.w + o1); cp_async8(sl + (3 * TILE + 256) * 8, A.p + o1);
             }
             o0 += (long long)plane; o1 += (long long)plane;
         }
@@ -417,28 +429,45 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         if (A.fw) fnext[2] = A.fw[tt];
     };
     if (in) fetch_hf(t);
-    // z metrics of plane k: rdzc[k-1], rdzc[k], rdzm[k], rdzm[k+1], rolled along the march; the two new ones of the next plane
-    // are loaded one iteration ahead of their use
-    const double* __restrict__ rdzc = S.rdzc + S.kofs;              // slab view: the metric tables are global
-    const double* __restrict__ rdzm = S.rdzm + S.kofs;
-    double zq[4] = {k0 > klo ? rdzc[k0 - 1] : 0.0, rdzc[k0], rdzm[k0], k0 + 1 < khi ? rdzm[k0 + 1] : 0.0};
+    // z metrics of planes k0-1 .. k1+1 staged in shared memory (they are warp-uniform: read from global memory in the loop
+    // they end up in uniform registers, and the conversion waits out the full load latency every plane)
+    __shared__ double zc_s[FSEI_EXPL_KZMAX + 3], zm_s[FSEI_EXPL_KZMAX + 3];
+    for (int q = tid; q < k1 - k0 + 3; q += 256) {
+        const int kq = k0 - 1 + q;                                  // slab view: the metric tables are global, hence + kofs
+        const bool there = kq >= klo && kq < khi;
+        zc_s[q] = there ? S.rdzc[kq + S.kofs] : 0.0;
+        zm_s[q] = there ? S.rdzm[kq + S.kofs] : 0.0;
+    }
+
+    // the carried registers of the first plane: plane k0 and the plane below it (not there below the bottom: never used)
+    ExplicitCarry C;
+    cp_async_wait<FSEI_EXPL_AHEAD>();                // planes <= k0 have landed
+    __syncthreads();
+    {
+        const double* s0 = ring + sc * SLOT;
+        const double* sm = ring + (sc == 0 ? R - 1 : sc - 1) * SLOT;
+        C.u00 = s0[c]; C.v00 = s0[TILE + c]; C.w00 = s0[2 * TILE + c]; C.wM0 = s0[2 * TILE + c - 1]; C.w0M = s0[2 * TILE + c - PW];
+        const bool below = kfirst >= klo;
+        C.u_km = below ? sm[c] : 0.0; C.v_km = below ? sm[TILE + c] : 0.0; C.w_km = below ? sm[2 * TILE + c] : 0.0;
+        C.p_km = below ? sm[3 * TILE + c] : 0.0;
+        C.uP_km = (below && !xhi) ? sm[c + 1] : 0.0; C.v0P_km = (below && !yhi) ? sm[TILE + c + PW] : 0.0;
+    }
 
     for (int k = k0; k < k1; k++, t += plane) {
         const double hprev[3] = {hnext[0], hnext[1], hnext[2]}, fb3[3] = {fnext[0], fnext[1], fnext[2]};
         if (in && k + 1 < k1) fetch_hf(t + plane);
-        const double zm4[4] = {zq[0], zq[1], zq[2], zq[3]};
-        if (k + 1 < k1) { zq[0] = zq[1]; zq[1] = rdzc[k + 1]; zq[2] = zq[3]; zq[3] = k + 2 < khi ? rdzm[k + 2] : 0.0; }
+        const int kq = k - k0;                       // rdzc[k-1], rdzc[k], rdzm[k], rdzm[k+1]
+        const double zm4[4] = {zc_s[kq], zc_s[kq + 1], zm_s[kq + 1], zm_s[kq + 2]};
         cp_async_wait<FSEI_EXPL_AHEAD - 1>();        // everything but the newest AHEAD-1 groups: planes <= k+1 have landed
-        __syncthreads();                             // ... for every thread; and every thread is done with slot (k-2) mod R
-        issue();                                     // plane k+AHEAD+1 -> slot (k+AHEAD+1) mod R = (k-2) mod R
-        const int sm_ = sc == 0 ? R - 1 : sc - 1, sp_ = sc + 1 == R ? 0 : sc + 1;
+        __syncthreads();                             // ... for every thread; and every thread is done with slot (k-1) mod R
+        issue();                                     // plane k+AHEAD+1 -> slot (k+AHEAD+1) mod R = (k-1) mod R
+        const int sp_ = sc + 1 == R ? 0 : sc + 1;
         if (in) {
             const double* s0 = ring + sc * SLOT;
-            const double* sm = ring + sm_ * SLOT;
             const double* sp = ring + sp_ * SLOT;
             const bool zlo = k == 0 && !S.halo_lo, zhi = k == S.nz - 1 && !S.halo_hi;     // a wall, not a slab boundary
-            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, sm, sp, c, hprev, fb3, zm4, t, xlo, xhi, ylo, yhi, zlo, zhi);
-            else explicit_cell<false>(A, s0, sm, sp, c, hprev, fb3, zm4, t, false, false, false, false, false, false);
+            if (xyedge || zlo || zhi) explicit_cell<true>(A, s0, C, sp, c, hprev, fb3, zm4, t, xlo, xhi, ylo, yhi, zlo, zhi);
+            else explicit_cell<false>(A, s0, C, sp, c, hprev, fb3, zm4, t, false, false, false, false, false, false);
         }
         sc = sp_;
     }

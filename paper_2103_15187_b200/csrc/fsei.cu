@@ -669,7 +669,7 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // planes per CTA: long marches amortise the ring's prologue (two halo planes per chunk); short ones keep small grids busy
     const long tiles = (long)((P->T.nx + 31) / 32) * ((P->T.ny + 7) / 8);
-    int kz = 64;
+    int kz = FSEI_EXPL_KZMAX;
     const int nzl = P->S.nz;                           // planes held by the fields (a slab plan: its own planes)
     while (kz > 8 && tiles * ((nzl + kz - 1) / kz) < 1184) kz >>= 1;
     ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz};
