@@ -241,6 +241,8 @@ struct ExplicitArgs {
     double *ru, *rv, *rw;                           // out: right-hand sides of the implicit step
     double gdt, rdt, adt, tb;                       // gamma dt, rho dt, alpha dt, 2 beta
     int kz;                                         // planes per CTA (host: 64 on large grids, fewer when the grid would not fill the GPU)
+    int tma;                                        // the four maps below are valid (nx even, encode succeeded)
+    TmaMap3D mu, mv, mw, mp;                        // (nx, ny, planes incl. slab halos) fp64, box (PW, TY + 2, 1)
 };
 
 FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const ExplicitArgs& A)
@@ -258,8 +260,9 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
 #define FSEI_EXPL_AHEAD 2              // planes in flight beyond k+1
 #endif
 #define FSEI_EXPL_RING (2 + FSEI_EXPL_AHEAD)    // planes k, k+1 being read + AHEAD in flight (plane k-1 lives in registers)
-#define FSEI_EXPL_PW (FSEI_EXPL_TX + 2)
-#define FSEI_EXPL_TILE (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
+#define FSEI_EXPL_PW (FSEI_EXPL_TX + 4)                             // columns i0-2 .. i0+33: the box starts on a 16-byte boundary
+#define FSEI_EXPL_TILE_ELEMS (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
+#define FSEI_EXPL_TILE ((FSEI_EXPL_TILE_ELEMS + 15) / 16 * 16)      // tile pitch: every tile starts 128-byte aligned (TMA destination)
 // doubles per ring slot: four halo tiles (u, v, w, p); H_prev of the next plane waits in three registers
 #define FSEI_EXPL_SLOT (4 * FSEI_EXPL_TILE)
 #define FSEI_EXPL_SMEM (FSEI_EXPL_RING * FSEI_EXPL_SLOT * 8)
@@ -377,16 +380,22 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     const bool xlo = !xper && i == 0, xhi = !xper && i == S.nx - 1;      // x-face i / i+1 is a wall
     const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
     const bool xyedge = xlo || xhi || ylo || yhi;
+    // tiles whose halo lies inside the grid take their planes as ONE TMA box per field (issued by one thread); tiles on the rim
+    // (periodic wrap or a wall in the halo; ragged edges) keep the per-thread copies, whose source index wraps / clamps
+    const bool tile_tma = A.tma && i0 >= 2 && i0 + TX + 2 <= S.nx && j0 >= 1 && j0 + TY + 1 <= S.ny;
+    __shared__ __align__(8) uint64_t bars[FSEI_EXPL_RING];
+    if (tile_tma && tid == 0)
+        for (int q = 0; q < R; q++) abar_init(&bars[q]);
     const size_t plane = (size_t)S.nx * S.ny;
     const int k0 = blockIdx.z * A.kz, k1 = (k0 + A.kz < S.nz) ? k0 + A.kz : S.nz;
 
     // loader: tile elements e = tid and tid + 256 of the halo tiles (source index wrapped in a periodic direction, clamped at
     // a wall or a ragged edge) and this thread's own cell of the H_prev tiles; source pointers advance one plane per issue
     const int e1 = tid + 256;
-    const bool has1 = e1 < TILE;
+    const bool has1 = e1 < FSEI_EXPL_TILE_ELEMS;
     auto srcidx = [&](int e) {
         const int jj = e / PW, ii = e - jj * PW;
-        int gi = i0 + ii - 1, gj = j0 + jj - 1;
+        int gi = i0 + ii - 2, gj = j0 + jj - 1;
         if (xper) { gi = gi < 0 ? gi + S.nx : (gi >= S.nx ? gi - S.nx : gi); }
         gi = gi < 0 ? 0 : (gi >= S.nx ? S.nx - 1 : gi);
         if (yper) { gj = gj < 0 ? gj + S.ny : (gj >= S.ny ? gj - S.ny : gj); }
@@ -401,8 +410,18 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     int kk = kfirst, slot = (kfirst + 2 * R) % R;
     uint32_t ring_tid = smem_u32(ring + tid);        // shared-window address of this thread's first element of slot 0
     asm volatile("" : "+r"(ring_tid));
-    auto issue = [&]() {                             // next plane kk -> its ring slot (nothing for a plane outside the grid)
-        if (kk >= klo && kk < khi) {
+    auto issue = [&]() {                             // next plane kk -> its ring slot (nothing for a plane outside the grid or beyond k1)
+        if (tile_tma) {
+            if (tid == 0 && kk >= klo && kk < khi && kk <= k1) {
+                double* sl = ring + slot * SLOT;
+                const int zc = kk + (S.halo_lo ? 1 : 0);
+                abar_expect(&bars[slot], 4u * FSEI_EXPL_TILE_ELEMS * 8u);
+                tma_load_3d(sl, &A.mu, i0 - 2, j0 - 1, zc, &bars[slot]);
+                tma_load_3d(sl + TILE, &A.mv, i0 - 2, j0 - 1, zc, &bars[slot]);
+                tma_load_3d(sl + 2 * TILE, &A.mw, i0 - 2, j0 - 1, zc, &bars[slot]);
+                tma_load_3d(sl + 3 * TILE, &A.mp, i0 - 2, j0 - 1, zc, &bars[slot]);
+            }
+        } else if (kk >= klo && kk < khi && kk <= k1) {
             const uint32_t sl = ring_tid + (uint32_t)(slot * SLOT * 8);
             cp_async8(sl, A.u + o0); cp_async8(sl + TILE * 8, A.v + o0);
             cp_async8(sl + 2 * TILE * 8, A.w + o0); cp_async8(sl + 3 * TILE * 8, A.p + o0);
@@ -412,12 +431,20 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
             }
             o0 += (long long)plane; o1 += (long long)plane;
         }
-        cp_async_commit();
+        if (!tile_tma) cp_async_commit();
         kk++; slot = slot + 1 == R ? 0 : slot + 1;
     };
+    unsigned phases = 0;                             // TMA tiles: parity of the next phase of every slot's mbarrier
+    auto landed = [&](int kq, int sq) {              // plane kq (in slot sq) is waited for exactly once, in plane order
+        if (kq >= klo && kq < khi) {
+            abar_wait(&bars[sq], (phases >> sq) & 1u);
+            phases ^= 1u << sq;
+        }
+    };
+    __syncthreads();                                 // the mbarriers are initialised
 #pragma unroll
     for (int q = 0; q < FSEI_EXPL_AHEAD + 2; q++) issue();       // planes k0-1 .. k0+AHEAD
-    const int c = (ty + 1) * PW + tx + 1;
+    const int c = (ty + 1) * PW + tx + 2;
     int sc = k0 % R;                                 // slot of plane k
     size_t t = (size_t)k0 * plane + (size_t)j * S.nx + i;
     // H_prev and the body force of the NEXT plane wait in registers (loaded one iteration ahead of their use)
@@ -441,7 +468,8 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
 
     // the carried registers of the first plane: plane k0 and the plane below it (not there below the bottom: never used)
     ExplicitCarry C;
-    cp_async_wait<FSEI_EXPL_AHEAD>();                // planes <= k0 have landed
+    if (tile_tma) { landed(kfirst, sc == 0 ? R - 1 : sc - 1); landed(k0, sc); }
+    else cp_async_wait<FSEI_EXPL_AHEAD>();           // planes <= k0 have landed
     __syncthreads();
     {
         const double* s0 = ring + sc * SLOT;
@@ -458,7 +486,8 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         if (in && k + 1 < k1) fetch_hf(t + plane);
         const int kq = k - k0;                       // rdzc[k-1], rdzc[k], rdzm[k], rdzm[k+1]
         const double zm4[4] = {zc_s[kq], zc_s[kq + 1], zm_s[kq + 1], zm_s[kq + 2]};
-        cp_async_wait<FSEI_EXPL_AHEAD - 1>();        // everything but the newest AHEAD-1 groups: planes <= k+1 have landed
+        if (tile_tma) landed(k + 1, sc + 1 == R ? 0 : sc + 1);
+        else cp_async_wait<FSEI_EXPL_AHEAD - 1>();   // everything but the newest AHEAD-1 groups: planes <= k+1 have landed
         __syncthreads();                             // ... for every thread; and every thread is done with slot (k-1) mod R
         issue();                                     // plane k+AHEAD+1 -> slot (k+AHEAD+1) mod R = (k-1) mod R
         const int sp_ = sc + 1 == R ? 0 : sc + 1;

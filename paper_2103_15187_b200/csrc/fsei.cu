@@ -24,6 +24,7 @@
 #include "fluid.cuh"
 #include "ibm.cuh"
 #include "visc_fast.cuh"
+#include "tma_host.hpp"
 #include <cmath>
 #include <cstdlib>
 
@@ -672,7 +673,25 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     int kz = FSEI_EXPL_KZMAX;
     const int nzl = P->S.nz;                           // planes held by the fields (a slab plan: its own planes)
     while (kz > 8 && tiles * ((nzl + kz - 1) / kz) < 1184) kz >>= 1;
-    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz};
+    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz, 0, {}, {}, {}, {}};
+    // TMA boxes for the tiles whose halo lies inside the grid: (nx, ny, planes) views of u, v, w, p that start at the halo plane
+    // below a slab.  Rows must be 16-byte multiples (nx even) and the fields 16-byte aligned; otherwise every tile copies per thread.
+    if (P->T.nx % 2 == 0 && P->T.nx >= 2 * FSEI_EXPL_TX + 4 && P->T.ny >= 3 * FSEI_EXPL_TY && !misaligned(u) && !misaligned(v) &&
+        !misaligned(w) && !misaligned(p)) {
+        EncodeTiledFn fn = tma_encode_fn();
+        const size_t plane = (size_t)P->T.nx * P->T.ny;
+        const int below = P->S.halo_lo ? 1 : 0, planes = nzl + below + (P->S.halo_hi ? 1 : 0);
+        cuuint64_t dims[3] = {(cuuint64_t)P->T.nx, (cuuint64_t)P->T.ny, (cuuint64_t)planes};
+        cuuint64_t strides[2] = {(cuuint64_t)P->T.nx * sizeof(double), (cuuint64_t)plane * sizeof(double)};
+        cuuint32_t box[3] = {FSEI_EXPL_PW, FSEI_EXPL_TY + 2, 1u}, estr[3] = {1, 1, 1};
+        TmaMap3D* maps[4] = {&A.mu, &A.mv, &A.mw, &A.mp};
+        bool ok = fn != nullptr;
+        for (int q = 0; q < 4 && ok; q++)
+            ok = fn(&maps[q]->m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(in[q] - (size_t)below * plane), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        A.tma = ok ? 1 : 0;
+    }
     const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (nzl + kz - 1) / kz);
     { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), FSEI_EXPL_SMEM, st>>>(A); }
     CU(cudaGetLastError());
