@@ -241,8 +241,10 @@ struct ExplicitArgs {
     double *ru, *rv, *rw;                           // out: right-hand sides of the implicit step
     double gdt, rdt, adt, tb;                       // gamma dt, rho dt, alpha dt, 2 beta
     int kz;                                         // planes per CTA (host: 64 on large grids, fewer when the grid would not fill the GPU)
+    int ring, slot;                                 // ring slots (>= FSEI_EXPL_RING) and doubles per slot, sized by the host to two CTAs per SM
     int tma;                                        // the four maps below are valid (nx even, encode succeeded)
     TmaMap3D mu, mv, mw, mp;                        // (nx, ny, planes incl. slab halos) fp64, box (PW, TY + 2, 1)
+    TmaMap3D mh[3], mf[3];                          // (nx, ny, planes) views of H_prev and of the body force, box (TX, TY, 1)
 };
 
 FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const ExplicitArgs& A)
@@ -264,8 +266,12 @@ FSEI_DEV double rhs_assemble(double H, double Hp, double gp, double lap, const E
 #define FSEI_EXPL_TILE_ELEMS (FSEI_EXPL_PW * (FSEI_EXPL_TY + 2))
 #define FSEI_EXPL_TILE ((FSEI_EXPL_TILE_ELEMS + 15) / 16 * 16)      // tile pitch: every tile starts 128-byte aligned (TMA destination)
 // doubles per ring slot: four halo tiles (u, v, w, p); H_prev of the next plane waits in three registers
-#define FSEI_EXPL_SLOT (4 * FSEI_EXPL_TILE)
-#define FSEI_EXPL_SMEM (FSEI_EXPL_RING * FSEI_EXPL_SLOT * 8)
+#define FSEI_EXPL_CELLS (FSEI_EXPL_TX * FSEI_EXPL_TY)
+// doubles per ring slot: four halo tiles (u, v, w, p) + the CTA's cells of H_prev and of the body force (TMA tiles; rim tiles
+// prefetch those into registers)
+#define FSEI_EXPL_SLOT(nforce) (4 * FSEI_EXPL_TILE + (3 + (nforce)) * FSEI_EXPL_CELLS)
+#define FSEI_EXPL_MAXRING 6
+#define FSEI_EXPL_SMEM_MAX (110 * 1024)            // two CTAs per SM
 
 #if defined(__CUDACC__)
 __device__ __forceinline__ void cp_async8(uint32_t sdst, const double* gsrc)
@@ -366,11 +372,18 @@ __device__ __forceinline__ void explicit_cell(const ExplicitArgs& A, const doubl
 }
 
 // grid (ceil(nx/32), ceil(ny/8), ceil(nz/kz)), block (32, 8), dynamic shared memory FSEI_EXPL_SMEM
-FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
+// TMA_TILE: a tile whose halo lies inside the grid takes its planes as ONE TMA box per field (issued by one thread); tiles on the
+// rim (periodic wrap or a wall in the halo; ragged edges) keep the per-thread copies, whose source index wraps / clamps.  The
+// two variants are separate instantiations so that neither carries the other's loader state in registers.
+template <bool TMA_TILE>
+__device__ __forceinline__ void explicit_march(const ExplicitArgs& A, double* ring, uint64_t* bars, double* zc_s, double* zm_s)
 {
-    constexpr int TX = FSEI_EXPL_TX, TY = FSEI_EXPL_TY, PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE, R = FSEI_EXPL_RING, SLOT = FSEI_EXPL_SLOT;
-    FSEI_DYN_SMEM(smraw);
-    double* ring = reinterpret_cast<double*>(smraw);
+    constexpr int TX = FSEI_EXPL_TX, TY = FSEI_EXPL_TY, PW = FSEI_EXPL_PW, TILE = FSEI_EXPL_TILE;
+    constexpr bool tile_tma = TMA_TILE;
+    // ring depth: TMA tiles use every slot the host could fit (planes k, k+1 being read, the rest in flight); rim tiles wait by
+    // cp.async group counts, which are immediates: AHEAD planes in flight whatever the ring holds
+    const int R = A.ring, SLOT = A.slot, ahead = tile_tma ? R - 2 : FSEI_EXPL_AHEAD;
+    const int f_u = 3, f_v = f_u + (A.fu ? 1 : 0), f_w = f_v + (A.fv ? 1 : 0);      // the force tiles follow H_prev's, those given only
     const SParams& S = A.S;
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, i = i0 + tx, j = j0 + ty;
@@ -380,10 +393,6 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     const bool xlo = !xper && i == 0, xhi = !xper && i == S.nx - 1;      // x-face i / i+1 is a wall
     const bool ylo = !yper && j == 0, yhi = !yper && j == S.ny - 1;
     const bool xyedge = xlo || xhi || ylo || yhi;
-    // tiles whose halo lies inside the grid take their planes as ONE TMA box per field (issued by one thread); tiles on the rim
-    // (periodic wrap or a wall in the halo; ragged edges) keep the per-thread copies, whose source index wraps / clamps
-    const bool tile_tma = A.tma && i0 >= 2 && i0 + TX + 2 <= S.nx && j0 >= 1 && j0 + TY + 1 <= S.ny;
-    __shared__ __align__(8) uint64_t bars[FSEI_EXPL_RING];
     if (tile_tma && tid == 0)
         for (int q = 0; q < R; q++) abar_init(&bars[q]);
     const size_t plane = (size_t)S.nx * S.ny;
@@ -405,8 +414,11 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     const int kfirst = k0 - 1;                       // first plane the loader is asked for
     // planes the fields hold: [klo, khi) = [0, nz), widened by the halo planes of a z-slab (S.halo_lo / S.halo_hi)
     const int klo = S.halo_lo ? -1 : 0, khi = S.nz + (S.halo_hi ? 1 : 0);
-    long long o0 = (long long)srcidx(tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
-    long long o1 = (long long)srcidx(has1 ? e1 : tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
+    long long o0 = 0, o1 = 0;
+    if (!tile_tma) {
+        o0 = (long long)srcidx(tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
+        o1 = (long long)srcidx(has1 ? e1 : tid) + (long long)(kfirst < klo ? klo : kfirst) * (long long)plane;
+    }
     int kk = kfirst, slot = (kfirst + 2 * R) % R;
     uint32_t ring_tid = smem_u32(ring + tid);        // shared-window address of this thread's first element of slot 0
     asm volatile("" : "+r"(ring_tid));
@@ -415,7 +427,17 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
             if (tid == 0 && kk >= klo && kk < khi && kk <= k1) {
                 double* sl = ring + slot * SLOT;
                 const int zc = kk + (S.halo_lo ? 1 : 0);
-                abar_expect(&bars[slot], 4u * FSEI_EXPL_TILE_ELEMS * 8u);
+                const bool own = kk >= k0 && kk < k1;                  // a plane this CTA evaluates: its H_prev and force come along
+                const unsigned nf = (A.fu ? 1u : 0u) + (A.fv ? 1u : 0u) + (A.fw ? 1u : 0u);
+                abar_expect(&bars[slot], 4u * FSEI_EXPL_TILE_ELEMS * 8u + (own ? (3u + nf) * FSEI_EXPL_CELLS * 8u : 0u));
+                if (own) {
+                    double* hs = sl + 4 * TILE;
+#pragma unroll
+                    for (int q = 0; q < 3; q++) tma_load_3d(hs + q * FSEI_EXPL_CELLS, &A.mh[q], i0, j0, kk, &bars[slot]);
+                    if (A.fu) tma_load_3d(hs + f_u * FSEI_EXPL_CELLS, &A.mf[0], i0, j0, kk, &bars[slot]);
+                    if (A.fv) tma_load_3d(hs + f_v * FSEI_EXPL_CELLS, &A.mf[1], i0, j0, kk, &bars[slot]);
+                    if (A.fw) tma_load_3d(hs + f_w * FSEI_EXPL_CELLS, &A.mf[2], i0, j0, kk, &bars[slot]);
+                }
                 tma_load_3d(sl, &A.mu, i0 - 2, j0 - 1, zc, &bars[slot]);
                 tma_load_3d(sl + TILE, &A.mv, i0 - 2, j0 - 1, zc, &bars[slot]);
                 tma_load_3d(sl + 2 * TILE, &A.mw, i0 - 2, j0 - 1, zc, &bars[slot]);
@@ -442,8 +464,7 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         }
     };
     __syncthreads();                                 // the mbarriers are initialised
-#pragma unroll
-    for (int q = 0; q < FSEI_EXPL_AHEAD + 2; q++) issue();       // planes k0-1 .. k0+AHEAD
+    for (int q = 0; q < ahead + 2; q++) issue();     // planes k0-1 .. k0+ahead
     const int c = (ty + 1) * PW + tx + 2;
     int sc = k0 % R;                                 // slot of plane k
     size_t t = (size_t)k0 * plane + (size_t)j * S.nx + i;
@@ -455,10 +476,9 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         if (A.fv) fnext[1] = A.fv[tt];
         if (A.fw) fnext[2] = A.fw[tt];
     };
-    if (in) fetch_hf(t);
+    if (!tile_tma && in) fetch_hf(t);
     // z metrics of planes k0-1 .. k1+1 staged in shared memory (they are warp-uniform: read from global memory in the loop
     // they end up in uniform registers, and the conversion waits out the full load latency every plane)
-    __shared__ double zc_s[FSEI_EXPL_KZMAX + 3], zm_s[FSEI_EXPL_KZMAX + 3];
     for (int q = tid; q < k1 - k0 + 3; q += 256) {
         const int kq = k0 - 1 + q;                                  // slab view: the metric tables are global, hence + kofs
         const bool there = kq >= klo && kq < khi;
@@ -482,14 +502,20 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
     }
 
     for (int k = k0; k < k1; k++, t += plane) {
-        const double hprev[3] = {hnext[0], hnext[1], hnext[2]}, fb3[3] = {fnext[0], fnext[1], fnext[2]};
-        if (in && k + 1 < k1) fetch_hf(t + plane);
+        double hprev[3] = {hnext[0], hnext[1], hnext[2]}, fb3[3] = {fnext[0], fnext[1], fnext[2]};
+        if (tile_tma) {                              // plane k's slot landed one iteration ago
+            const double* hs = ring + sc * SLOT + 4 * TILE + tid;
+            hprev[0] = hs[0]; hprev[1] = hs[FSEI_EXPL_CELLS]; hprev[2] = hs[2 * FSEI_EXPL_CELLS];
+            if (A.fu) fb3[0] = hs[f_u * FSEI_EXPL_CELLS];
+            if (A.fv) fb3[1] = hs[f_v * FSEI_EXPL_CELLS];
+            if (A.fw) fb3[2] = hs[f_w * FSEI_EXPL_CELLS];
+        } else if (in && k + 1 < k1) fetch_hf(t + plane);
         const int kq = k - k0;                       // rdzc[k-1], rdzc[k], rdzm[k], rdzm[k+1]
         const double zm4[4] = {zc_s[kq], zc_s[kq + 1], zm_s[kq + 1], zm_s[kq + 2]};
         if (tile_tma) landed(k + 1, sc + 1 == R ? 0 : sc + 1);
         else cp_async_wait<FSEI_EXPL_AHEAD - 1>();   // everything but the newest AHEAD-1 groups: planes <= k+1 have landed
         __syncthreads();                             // ... for every thread; and every thread is done with slot (k-1) mod R
-        issue();                                     // plane k+AHEAD+1 -> slot (k+AHEAD+1) mod R = (k-1) mod R
+        issue();                                     // plane k+ahead+1 -> the slot plane k-1 was in (TMA tiles: slot (k-1) mod R)
         const int sp_ = sc + 1 == R ? 0 : sc + 1;
         if (in) {
             const double* s0 = ring + sc * SLOT;
@@ -500,7 +526,20 @@ FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT Expli
         }
         sc = sp_;
     }
-    cp_async_wait<0>();
+    if (!tile_tma) cp_async_wait<0>();
+}
+
+FSEI_GLOBAL(256, FSEI_EXPL_MINB) k_explicit_terms(const FSEI_GRID_CONSTANT ExplicitArgs A)
+{
+    FSEI_DYN_SMEM(smraw);
+    __shared__ __align__(8) uint64_t bars[FSEI_EXPL_MAXRING];
+    __shared__ double zc_s[FSEI_EXPL_KZMAX + 3], zm_s[FSEI_EXPL_KZMAX + 3];
+    double* ring = reinterpret_cast<double*>(smraw);
+    const int i0 = blockIdx.x * FSEI_EXPL_TX, j0 = blockIdx.y * FSEI_EXPL_TY;
+    if (A.tma && i0 >= 2 && i0 + FSEI_EXPL_TX + 2 <= A.S.nx && j0 >= 1 && j0 + FSEI_EXPL_TY + 1 <= A.S.ny)
+        explicit_march<true>(A, ring, bars, zc_s, zm_s);
+    else
+        explicit_march<false>(A, ring, bars, zc_s, zm_s);
 }
 #endif  // __CUDACC__
 

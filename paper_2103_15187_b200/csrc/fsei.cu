@@ -283,7 +283,7 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
         void* q = nullptr;
         if ((rc = dalloc(P, sizeof(double) * FSEI_VSLOTS * 9 * vtab_set_doubles(P->vnmax), &q))) return rc;
         P->vtab = static_cast<double*>(q);
-        CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM));
+        CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM_MAX));
         P->visc_fast = !(flags & FSEI_PLAN_VISC_GENERIC) && bcx == BC_PERIODIC && bcy == BC_PERIODIC && visc_fast_supported(nx, ny);
         if (P->visc_fast) CU(visc_fast_init());
     }
@@ -673,7 +673,7 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
     int kz = FSEI_EXPL_KZMAX;
     const int nzl = P->S.nz;                           // planes held by the fields (a slab plan: its own planes)
     while (kz > 8 && tiles * ((nzl + kz - 1) / kz) < 1184) kz >>= 1;
-    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz, 0, {}, {}, {}, {}};
+    ExplicitArgs A{P->S, u, v, w, p, fu, fv, fw, hu, hv, hw, ru, rv, rw, gamma_dt, rho_dt, alpha_dt, 2.0 * beta, kz, 0, 0, 0, {}, {}, {}, {}, {}, {}};
     // TMA boxes for the tiles whose halo lies inside the grid: (nx, ny, planes) views of u, v, w, p that start at the halo plane
     // below a slab.  Rows must be 16-byte multiples (nx even) and the fields 16-byte aligned; otherwise every tile copies per thread.
     if (P->T.nx % 2 == 0 && P->T.nx >= 2 * FSEI_EXPL_TX + 4 && P->T.ny >= 3 * FSEI_EXPL_TY && !misaligned(u) && !misaligned(v) &&
@@ -690,10 +690,27 @@ extern "C" int fsei_explicit_terms(fsei_plan* P, const double* u, const double* 
             ok = fn(&maps[q]->m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(in[q] - (size_t)below * plane), dims, strides, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        // H_prev and the body force of the CTA's own cells: (nx, ny, nzl) views, box (32, 8, 1)
+        cuuint64_t hdims[3] = {(cuuint64_t)P->T.nx, (cuuint64_t)P->T.ny, (cuuint64_t)nzl};
+        cuuint32_t hbox[3] = {FSEI_EXPL_TX, FSEI_EXPL_TY, 1u};
+        const double* hf[6] = {hu, hv, hw, fu, fv, fw};
+        for (int q = 0; q < 6 && ok; q++) {
+            if (!hf[q]) continue;
+            ok = !misaligned(hf[q]) &&
+                 fn(&(q < 3 ? A.mh[q] : A.mf[q - 3]).m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(hf[q]), hdims, strides, hbox, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        }
         A.tma = ok ? 1 : 0;
     }
+    // ring: as many slots as two CTAs per SM leave room for (the force tiles take their share of a slot only when given)
+    A.slot = FSEI_EXPL_SLOT((fu ? 1 : 0) + (fv ? 1 : 0) + (fw ? 1 : 0));
+    A.ring = FSEI_EXPL_SMEM_MAX / (A.slot * (int)sizeof(double));
+    if (A.ring > FSEI_EXPL_MAXRING) A.ring = FSEI_EXPL_MAXRING;
+    if (A.ring > kz + 2) A.ring = kz + 2 < FSEI_EXPL_RING ? FSEI_EXPL_RING : kz + 2;
+    const size_t smem = (size_t)A.ring * A.slot * sizeof(double);
     const dim3 grid((P->T.nx + 31) / 32, (P->T.ny + 7) / 8, (nzl + kz - 1) / kz);
-    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), FSEI_EXPL_SMEM, st>>>(A); }
+    { LaunchTimer t(P, K_EXPL, st); k_explicit_terms<<<grid, dim3(32, 8), smem, st>>>(A); }
     CU(cudaGetLastError());
     P->last_launches = 1;
     return FSEI_OK;
@@ -919,7 +936,7 @@ static int slab_plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, doub
         void* qv = nullptr;
         if ((rc = dalloc(P, sizeof(double) * FSEI_VSLOTS * 9 * vtab_set_doubles(P->vnmax), &qv))) return rc;
         P->vtab = static_cast<double*>(qv);
-        CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM));
+        CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM_MAX));
     }
     XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
     XF.nx = nx; XF.ny = ny; XF.nz = nzl; XF.N = nx / 2; XF.tw = X.tw; XF.tw_r2c = X.tw_r2c; XF.tw_dct = X.tw_dct; XF.scale = T.scale;
