@@ -57,7 +57,7 @@ enum { FSEI_OK = 0, FSEI_ERR_ARG = 1, FSEI_ERR_SIZE = 2, FSEI_ERR_GRID = 3, FSEI
  * Plan for an nx x ny x nz grid (cells), uniform in x,y with extents Lx, Ly, wall-normal
  * z with face coordinates zc[0..nz] (strictly increasing; zc[0], zc[nz] are the walls;
  * cell centres are the midpoints).  DESIGN.md R2, R3, R5, R6.
- *   nx, ny : of the form 2^a 3^b in [4, 8192], nx a multiple of 4, ny even;
+ *   nx, ny : of the form 2^a 3^b 5^c in [4, 8192], nx a multiple of 4, ny even;
  *            2 <= nz <= 8192                                                    else FSEI_ERR_SIZE
  *   Lx, Ly > 0, zc finite and strictly increasing                              else FSEI_ERR_GRID
  *   bc_x, bc_y in {PERIODIC, NEUMANN}, zc != NULL                              else FSEI_ERR_ARG

@@ -1,5 +1,5 @@
 // fft_core.cuh -- register-level pieces of the transforms: complex type, small DFTs
-// (radix 2, 3, 4, 8, 16) and one in-place decimation-in-frequency / decimation-in-time pass
+// (radix 2, 3, 4, 5, 8, 16) and one in-place decimation-in-frequency / decimation-in-time pass
 // over a shared-memory tile.  Everything is __host__ __device__ so that the per-thread phases
 // of the kernels can also be stepped through on the host by tests/emu (thread by thread,
 // phase by phase) -- that harness is a test of this code, not a fallback: libfsei.so holds
@@ -60,6 +60,24 @@ template <bool INV> struct SmallDft<3, INV> {
         cplx m = cmake(v[0].re - 0.5 * s.re, v[0].im - 0.5 * s.im);
         cplx n = cscale(crot<INV>(d), FSEI_SQRT3_2);          // (-+ i sqrt3/2) d
         v[0] = cadd(v[0], s); v[1] = cadd(m, n); v[2] = csub(m, n);
+    }
+};
+// 5: X_k = x0 + sum_{r=1..4} w5^{rk} x_r with the pairs (x1, x4), (x2, x3) folded (Winograd-style, 2 real tables)
+#define FSEI_COS_2PI_5 0.30901699437494742410229341718281905886
+#define FSEI_COS_4PI_5 -0.80901699437494742410229341718281905886
+#define FSEI_SIN_2PI_5 0.95105651629515357211643933337938214340
+#define FSEI_SIN_4PI_5 0.58778525229247312916870595463907276860
+template <bool INV> struct SmallDft<5, INV> {
+    static FSEI_HD void run(cplx* v) {
+        const cplx a1 = cadd(v[1], v[4]), a2 = cadd(v[2], v[3]), b1 = csub(v[1], v[4]), b2 = csub(v[2], v[3]);
+        const cplx m1 = cmake(v[0].re + FSEI_COS_2PI_5 * a1.re + FSEI_COS_4PI_5 * a2.re, v[0].im + FSEI_COS_2PI_5 * a1.im + FSEI_COS_4PI_5 * a2.im);
+        const cplx m2 = cmake(v[0].re + FSEI_COS_4PI_5 * a1.re + FSEI_COS_2PI_5 * a2.re, v[0].im + FSEI_COS_4PI_5 * a1.im + FSEI_COS_2PI_5 * a2.im);
+        // (-+ i) (s1 b1 + s2 b2) and (-+ i) (s2 b1 - s1 b2)
+        const cplx n1 = crot<INV>(cmake(FSEI_SIN_2PI_5 * b1.re + FSEI_SIN_4PI_5 * b2.re, FSEI_SIN_2PI_5 * b1.im + FSEI_SIN_4PI_5 * b2.im));
+        const cplx n2 = crot<INV>(cmake(FSEI_SIN_4PI_5 * b1.re - FSEI_SIN_2PI_5 * b2.re, FSEI_SIN_4PI_5 * b1.im - FSEI_SIN_2PI_5 * b2.im));
+        v[0] = cadd(v[0], cadd(a1, a2));
+        v[1] = cadd(m1, n1); v[4] = csub(m1, n1);
+        v[2] = cadd(m2, n2); v[3] = csub(m2, n2);
     }
 };
 template <bool INV> struct SmallDft<4, INV> {

@@ -28,8 +28,9 @@ struct HostTables {
 static const long double FSEI_PI_L = 3.14159265358979323846264338327950288L;
 
 inline bool is_2a3b(int n) { if (n < 1) return false; while (n % 2 == 0) n /= 2; while (n % 3 == 0) n /= 3; return n == 1; }
+inline bool is_2a3b5c(int n) { if (n < 1) return false; while (n % 5 == 0) n /= 5; return is_2a3b(n); }
 
-// radices: all factors 3 first (large strides), then the power of two split into ceil(a/4)
+// radices: all factors 3 and 5 first (large strides), then the power of two split into ceil(a/4)
 // passes of radix 16/8/4/2, largest first.
 inline FftPlan1D make_fft_plan(int N)
 {
@@ -37,6 +38,7 @@ inline FftPlan1D make_fft_plan(int N)
     for (int i = 0; i < 8; i++) f.radix[i] = 1;
     int n = N, a = 0;
     while (n % 3 == 0) { f.radix[f.npass++] = 3; n /= 3; }
+    while (n % 5 == 0) { f.radix[f.npass++] = 5; n /= 5; }
     while (n % 2 == 0) { a++; n /= 2; }
     if (a > 0) {
         int np = (a + 3) / 4, base = a / np, extra = a % np;
@@ -68,8 +70,8 @@ inline std::string build_tables(HostTables& T, int nx, int ny, int nz, double Lx
     code = 0;
     if (zc == nullptr) { code = 1; return "zc is NULL"; }
     if ((bcx != BC_PERIODIC && bcx != BC_NEUMANN) || (bcy != BC_PERIODIC && bcy != BC_NEUMANN)) { code = 1; return "unknown boundary condition"; }
-    if (nx < 4 || ny < 4 || nx > 8192 || ny > 8192 || nx % 4 != 0 || ny % 2 != 0 || !is_2a3b(nx) || !is_2a3b(ny)) {
-        code = 2; return "nx must be a multiple of 4, ny even, both of the form 2^a 3^b in [4, 8192]";
+    if (nx < 4 || ny < 4 || nx > 8192 || ny > 8192 || nx % 4 != 0 || ny % 2 != 0 || !is_2a3b5c(nx) || !is_2a3b5c(ny)) {
+        code = 2; return "nx must be a multiple of 4, ny even, both of the form 2^a 3^b 5^c in [4, 8192]";
     }
     if (nz < 2 || nz > 8192) { code = 2; return "nz must be in [2, 8192]"; }
     if (!(Lx > 0) || !(Ly > 0) || !std::isfinite(Lx) || !std::isfinite(Ly)) { code = 3; return "Lx, Ly must be positive and finite"; }

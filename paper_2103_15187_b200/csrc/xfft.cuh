@@ -52,6 +52,7 @@ FSEI_HD void x_pass_dispatch(const XParams& P, cplx* sm, int lines, int R, int N
     switch (R) {
         case 16: x_pass<16, INV>(P, sm, lines, Ns, tid, nt); break;
         case 8:  x_pass<8, INV>(P, sm, lines, Ns, tid, nt); break;
+        case 5:  x_pass<5, INV>(P, sm, lines, Ns, tid, nt); break;
         case 4:  x_pass<4, INV>(P, sm, lines, Ns, tid, nt); break;
         case 3:  x_pass<3, INV>(P, sm, lines, Ns, tid, nt); break;
         default: x_pass<2, INV>(P, sm, lines, Ns, tid, nt); break;

@@ -29,6 +29,7 @@ FSEI_HD void y_pass_dispatch(const YParams& P, cplx* sm, int C, int R, int Ns, i
     switch (R) {
         case 16: y_pass<16, INV, NEUMANN>(P, sm, C, Ns, tid, nt); break;
         case 8:  y_pass<8, INV, NEUMANN>(P, sm, C, Ns, tid, nt); break;
+        case 5:  y_pass<5, INV, NEUMANN>(P, sm, C, Ns, tid, nt); break;
         case 4:  y_pass<4, INV, NEUMANN>(P, sm, C, Ns, tid, nt); break;
         case 3:  y_pass<3, INV, NEUMANN>(P, sm, C, Ns, tid, nt); break;
         default: y_pass<2, INV, NEUMANN>(P, sm, C, Ns, tid, nt); break;

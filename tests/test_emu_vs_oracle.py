@@ -14,7 +14,7 @@ P, N = 0, 1
 
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
-@pytest.mark.parametrize("shape", [(8, 8, 8), (16, 12, 10), (48, 24, 20), (12, 36, 7), (64, 16, 5)])
+@pytest.mark.parametrize("shape", [(8, 8, 8), (16, 12, 10), (48, 24, 20), (12, 36, 7), (64, 16, 5), (20, 10, 6), (40, 50, 5), (60, 30, 4)])
 def test_stepped_phases_match_oracle(oracle_ld, bc, shape):
     for cfg, beta in ((1, 0.0), (2, 1e-4)):
         case = inputs.make_case(cfg, shape=shape, bc=bc)
@@ -33,7 +33,8 @@ def test_stepped_phases_config1_full(oracle_ld):
 
 
 @pytest.mark.parametrize("n,expect", [(16, [16]), (32, [8, 4]), (128, [16, 8]), (256, [16, 16]), (512, [8, 8, 8]),
-                                      (1024, [16, 8, 8]), (384, [3, 16, 8]), (768, [3, 16, 16]), (6, [3, 2]), (2, [2])])
+                                      (1024, [16, 8, 8]), (384, [3, 16, 8]), (768, [3, 16, 16]), (6, [3, 2]), (2, [2]),
+                                      (10, [5, 2]), (320, [5, 8, 8]), (60, [3, 5, 4]), (1250, [5, 5, 5, 5, 2])])
 def test_radix_plan(n, expect):
     L = emu_lib()
     r = (ctypes.c_int * 8)()
@@ -47,7 +48,10 @@ def test_plan_argument_checks():
     zc = np.linspace(0, 1, 9)
     chk = lambda nx, ny, nz, Lx, Ly, z, bx, by: L.emu_plan_check(nx, ny, nz, Lx, Ly, z.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), bx, by)
     assert chk(8, 8, 8, 1.0, 1.0, zc, 0, 0) == 0
-    assert chk(10, 8, 8, 1.0, 1.0, zc, 0, 0) == 2          # 10 = 2*5
+    assert chk(28, 8, 8, 1.0, 1.0, zc, 0, 0) == 2          # 28 = 4*7
+    assert chk(8, 14, 8, 1.0, 1.0, zc, 0, 0) == 2          # 14 = 2*7
+    assert chk(20, 10, 8, 1.0, 1.0, zc, 0, 0) == 0         # radix 5
+    assert chk(10, 8, 8, 1.0, 1.0, zc, 0, 0) == 2          # nx not a multiple of 4
     assert chk(6, 8, 8, 1.0, 1.0, zc, 0, 0) == 2           # nx not a multiple of 4
     assert chk(8, 8, 8, 0.0, 1.0, zc, 0, 0) == 3
     assert chk(8, 8, 8, 1.0, 1.0, zc[::-1].copy(), 0, 0) == 3

@@ -19,7 +19,7 @@ pytestmark = pytest.mark.gpu
 P, W = 0, 1
 EPS = 2.0 ** -52
 ALL_BC = [(P, P), (W, W), (P, W), (W, P)]
-SHAPES = [(32, 32, 32), (48, 24, 20), (36, 16, 33), (64, 12, 7)]
+SHAPES = [(32, 32, 32), (48, 24, 20), (36, 16, 33), (64, 12, 7), (40, 20, 12)]
 # + grids with tiles whose halo lies inside the grid (they take TMA boxes; the rim keeps per-thread copies), ragged tiles on
 # both axes and several z chunks per column of tiles
 EXPL_SHAPES = SHAPES + [(96, 36, 9), (192, 54, 70), (144, 24, 5)]

@@ -70,7 +70,8 @@ def test_project_bit_exact(oracle_ld, bc, shape, beta):
 # ---------------------------------------------------------------------------------------------
 # Poisson solve and whole projection: small and ragged shapes, every bc combination
 # ---------------------------------------------------------------------------------------------
-SHAPES = [(8, 8, 8), (16, 12, 10), (32, 32, 32), (48, 24, 20), (12, 36, 7), (64, 16, 5), (96, 72, 40), (128, 64, 64)]
+SHAPES = [(8, 8, 8), (16, 12, 10), (32, 32, 32), (48, 24, 20), (12, 36, 7), (64, 16, 5), (96, 72, 40), (128, 64, 64),
+          (20, 10, 6), (320, 160, 9), (640, 50, 5), (60, 250, 7)]           # the last four: lengths with a factor 5 (generic family)
 
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
