@@ -254,7 +254,7 @@ def fused_path(monkeypatch):
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
 @pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 6), (512, 768, 5), (2048, 1024, 3), (32, 32, 33), (64, 16, 9),
-                                   (96, 48, 40)])
+                                   (96, 48, 40), (320, 160, 9), (640, 640, 5), (1280, 1280, 3)])
 def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
     from paper_2103_15187_b200.binding import Plan
     for cfg, beta in ((1, 0.0), (2, 1e-4)):
@@ -276,7 +276,8 @@ def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
 
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
-@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 64), (512, 1024, 4), (32, 32, 33), (96, 16, 5), (64, 48, 4)])
+@pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 64), (512, 1024, 4), (32, 32, 33), (96, 16, 5), (64, 48, 4), (640, 640, 6),
+                                   (320, 1280, 5)])
 def test_fused_twisted_factorisation(oracle_ld, fused_path, monkeypatch, bc, shape):
     """two CTAs per tile sweep towards each other (the plan's choice when there are fewer tiles than SMs; forced
     here), against the oracle and against the plain Thomas order of the same kernels"""
@@ -319,6 +320,24 @@ def test_fused_is_the_default_on_large_grids():
     assert plan.last_launch_count == 6
     plan.destroy()
     assert np.isfinite(got[4]).all()
+
+
+@pytest.mark.parametrize("bc", [(P, P), (N, N)])
+@pytest.mark.parametrize("shape,family", [((320, 160, 9), 1), ((640, 320, 5), 1), ((1280, 640, 3), 2), ((160, 1280, 4), 1), ((320, 80, 6), 1),
+                                          ((640, 640, 7), 2)])
+def test_factor5_lengths_take_the_register_resident_families(oracle_ld, shape, family, bc):
+    """nx/2 in {80, 160, 320, 640}, ny in {80, ..., 1280}: Stockham passes with a radix-5 last pass; 1 = fast, 2 = fused (blocked
+    layout, from 128 x-slot tiles on, where both lengths have a fused instantiation)."""
+    case = inputs.make_case(2, shape=shape, bc=bc)
+    plan = make_plan(case.grid)
+    assert plan.kernel_family & 3 == family and plan.last_launch_count == 0
+    got = gpu_projection(case, plan=plan)
+    assert plan.last_launch_count == (7 if family == 1 else 6)
+    plan.destroy()
+    ref = oracle_projection(oracle_ld, case)
+    assert rel_l2(got[4], ref[4]) <= 1e-11
+    for g, r in zip(got[:4], ref[:4]):
+        assert np.abs(g - r).max() <= 1e-10 * max(1.0, np.abs(r).max())
 
 
 # ---------------------------------------------------------------------------------------------
