@@ -44,7 +44,7 @@ ALGO_BYTES_PER_CELL = {
     # forward + backward pass each (the z sweep also reads and writes the velocity component)
     "explicit_terms": 104.0, "visc_x": 32.0, "visc_y": 32.0, "visc_z": 40.0, "visc_factor": 0.0,
     # fast viscous family, three components per launch: rhs -> d' in place (3 x 16); d' + q in, q out (3 x 24)
-    "visc_xz": 48.0, "visc_zy": 72.0, "ib_mls": 0.0,
+    "visc_xz": 48.0, "visc_zy": 72.0, "ib_mls": 0.0, "ib_apply": 0.0,
 }
 A_REF = 184.0          # unfused reference accounting of one projection, B/cell
 SLAB_NY = 64           # single-thread CPU leg: the workload's grid with ny cut to this many rows
@@ -327,18 +327,21 @@ def _fluid_leg(plan, case, fields, stream, barrier, dev, peak, world, steps=3):
                                                 vel=(0.0, 0.0, 0.0))
     mk = [torch.from_numpy(a).to(u.device) for a in (xm, ym, zm, area, *V)]
     Fb = [torch.empty(nmark, dtype=torch.float64, device=u.device) for _ in range(3)]
-    fib = [torch.zeros_like(u) for _ in range(3)] if free > 9.6 * case.cells * 8 else None
+    fib = [torch.zeros_like(u) for _ in range(3)] if free > 9.6 * case.cells * 8 else None     # zero-filled ONCE
 
     def substep():
+        if fib is None:
+            plan.fluid_substep(u, v, w, p, *h, *r, phi, gdt, rdt, adt, beta, stream=stream)
+            return plan.last_launch_count
         n = 0
-        if fib is not None:
-            for t in fib:
-                t.zero_()
-            plan.ibm_forcing(nmark, *mk[:4], *mk[4:], u, v, w, 1.0 / dt, *Fb, *fib, stream=stream)
+        for call, a in ((plan.ibm_forcing, (nmark, *mk[:4], *mk[4:], u, v, w, 1.0 / dt, *Fb, *fib)),
+                        (plan.explicit_terms, (u, v, w, p, *h, *r, gdt, rdt, adt, beta)),
+                        (plan.ibm_apply_forcing, (nmark, *mk[:3], *fib, *r, adt)),       # rhs += alpha dt f on the supports; clears f
+                        (plan.viscous_step, (u, v, w, *r, beta)),
+                        (plan.pressure_projection, (u, v, w, p, phi, adt, beta))):
+            call(*a, stream=stream)
             n += plan.last_launch_count
-        plan.fluid_substep(u, v, w, p, *h, *r, phi, gdt, rdt, adt, beta, f=fib if fib is not None else (None, None, None),
-                           stream=stream)
-        return n + plan.last_launch_count
+        return n
 
     nl = 0
     for _ in range(2):
@@ -365,12 +368,14 @@ def _fluid_leg(plan, case, fields, stream, barrier, dev, peak, world, steps=3):
     vms = sum(prof[k][0] for k in visc) / steps
     vbytes = sum(ALGO_BYTES_PER_CELL[k] * prof[k][1] for k in visc) / steps * case.cells
     finite = bool(torch.isfinite(u).all().item())
+    has_ib = fib is not None
     del h, r, fib
     torch.cuda.empty_cache()
     out = {"ms_per_substep": round(ms, 4), "ib_markers": nmark, "Mcell_per_s": round(replica_throughput(case.cells, world, ms), 1), "steps": steps,
            "params": {"gamma_dt": gdt, "rho_dt": rdt, "alpha_dt": adt, "beta": beta, "Re": Re},
-           "chain": "3 zero-fills of the forcing fields (torch) -> fsei_ibm_forcing -> fsei_fluid_substep (explicit terms, viscous "
-                    "step, projection)",
+           "chain": "fsei_ibm_forcing -> fsei_explicit_terms -> fsei_ibm_apply_forcing (the forcing enters the rhs on the markers' "
+                    "supports only) -> fsei_viscous_step -> fsei_pressure_projection" if has_ib else "fsei_fluid_substep",
+           "ib_forcing_fields": has_ib,
            "moved_bytes_per_cell": round(moved, 1), "achieved_GBps": round(moved * case.cells / (ms * 1e-3) / 1e9, 1),
            "viscous_step": {"ms": round(vms, 4), "bytes_per_cell": round(vbytes / case.cells, 1), "bound": "hbm",
                             "achieved": round(vbytes / (vms * 1e-3) / 1e9, 1), "peak": peak, "unit": "GB/s",

@@ -203,6 +203,11 @@ int fsei_fluid_substep(fsei_plan* plan, double* u, double* v, double* w, double*
  *                          fv, fw alike.  fp64 atomic adds: the sum over markers has no fixed order.
  *   fsei_ibm_forcing     : Fu[l] = (Vu[l] - ub[l]) * inv_dt (out), then the spreading of Fu into fu (+=); v, w alike:
  *                          the IB forcing f of Eq. 3 that fsei_explicit_terms takes as fu, fv, fw.  One kernel.
+ *   fsei_ibm_apply_forcing: the forcing fields are zero except on the supports of the markers, so a substep need not stream
+ *                          them: call fsei_explicit_terms WITHOUT a body force, then this -- it visits the support nodes of the
+ *                          same markers and forms rhs += alpha_dt * f there (the two operations of the dense path, in its
+ *                          order: same result), each node once, and leaves fu, fv, fw all-zero for the next substep.
+ *                          Requires fu, fv, fw to be zero outside those supports (zero-fill them once, at allocation).
  * The forcing fields must not alias the velocity fields                                              else FSEI_ERR_ARG
  */
 int fsei_mls_interpolate(fsei_plan* plan, long n, const double* xm, const double* ym, const double* zm,
@@ -215,6 +220,8 @@ int fsei_ibm_forcing(fsei_plan* plan, long n, const double* xm, const double* ym
                      const double* Vu, const double* Vv, const double* Vw, const double* u, const double* v, const double* w,
                      double inv_dt, double* Fu, double* Fv, double* Fw, double* fu, double* fv, double* fw,
                      void* cuda_stream);
+int fsei_ibm_apply_forcing(fsei_plan* plan, long n, const double* xm, const double* ym, const double* zm, double* fu, double* fv,
+                           double* fw, double* ru, double* rv, double* rw, double alpha_dt, void* cuda_stream);
 
 /*
  * ---- Multi-GPU slab decomposition of the projection: per-rank stages -------------------------

@@ -21,7 +21,7 @@ EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family",
            "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
            "fsei_plan_profile", "fsei_plan_profile_read",
            "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep",
-           "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing",
+           "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing", "fsei_ibm_apply_forcing",
            "fsei_slab_plan_create", "fsei_slab_set_peers", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project",
            "fsei_slab_viscous_xy", "fsei_pencil_viscous_z", "fsei_slab_field_add")
 
@@ -91,6 +91,8 @@ def lib() -> ctypes.CDLL:
     L.fsei_mls_spread.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_vp]
     L.fsei_ibm_forcing.restype = _i
     L.fsei_ibm_forcing.argtypes = [_vp, ctypes.c_long] + [_vp] * 10 + [_d] + [_vp] * 6 + [_vp]
+    L.fsei_ibm_apply_forcing.restype = _i
+    L.fsei_ibm_apply_forcing.argtypes = [_vp, ctypes.c_long] + [_vp] * 9 + [_d, _vp]
     L.fsei_slab_plan_create.restype = _vp
     L.fsei_slab_plan_create.argtypes = [_i, _i, _i, _d, _d, _vp, _i, _i, _i, _i, _i, _i]
     L.fsei_slab_set_peers.restype = _i
@@ -238,6 +240,10 @@ class Plan:
     def mls_interpolate(self, n, xm, ym, zm, u, v, w, ub, vb, wb, stream=None):
         _chk(lib().fsei_mls_interpolate(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(u), _ptr(v), _ptr(w), _ptr(ub),
                                         _ptr(vb), _ptr(wb), _stream(stream)))
+
+    def ibm_apply_forcing(self, n, xm, ym, zm, fu, fv, fw, ru, rv, rw, alpha_dt, stream=None):
+        _chk(lib().fsei_ibm_apply_forcing(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(fu), _ptr(fv), _ptr(fw), _ptr(ru), _ptr(rv),
+                                          _ptr(rw), float(alpha_dt), _stream(stream)))
 
     def mls_spread(self, n, xm, ym, zm, area, Fu, Fv, Fw, fu, fv, fw, stream=None):
         _chk(lib().fsei_mls_spread(self._h, int(n), _ptr(xm), _ptr(ym), _ptr(zm), _ptr(area), _ptr(Fu), _ptr(Fv), _ptr(Fw),

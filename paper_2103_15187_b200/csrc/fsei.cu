@@ -47,7 +47,7 @@ static bool misaligned(const void* p) { return (reinterpret_cast<size_t>(p) & 15
 // plan
 // ------------------------------------------------------------------------------------------
 #define FSEI_VSLOTS 4
-enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, K_MLS, K_VXZ, K_VZY, FSEI_NKERNELS };
+enum { K_DIV = 0, K_XF, K_YF, K_GAUGE, K_ZD, K_ZP, K_YI, K_XI, K_PROJ, K_DIVXF, K_YZF, K_YZB, K_EXPL, K_VFACT, K_VX, K_VY, K_VZ, K_MLS, K_VXZ, K_VZY, K_MLSAPPLY, FSEI_NKERNELS };
 
 struct fsei_plan {
     HostTables T;
@@ -81,7 +81,7 @@ struct fsei_plan {
 
 static const char* const k_names[FSEI_NKERNELS] = {"divergence", "x_forward", "y_forward", "z_gauge", "z_direct", "z_paired",
                                                    "y_inverse", "x_inverse", "project", "div_x_forward", "yz_forward", "yz_backward",
-                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z", "ib_mls", "visc_xz", "visc_zy"};
+                                                   "explicit_terms", "visc_factor", "visc_x", "visc_y", "visc_z", "ib_mls", "visc_xz", "visc_zy", "ib_apply"};
 
 // record an event pair around one launch when profiling is on
 struct LaunchTimer {
@@ -890,6 +890,26 @@ extern "C" int fsei_ibm_forcing(fsei_plan* P, long n, const double* xm, const do
     if (P->T.nz < 3) return fail(FSEI_ERR_SIZE, "fsei_ibm_forcing: the 27-node support needs nz >= 3");
     MlsArgs A{mls_grid(P), n, xm, ym, zm, area, {u, v, w}, {Vu, Vv, Vw}, {Fu, Fv, Fw}, {fu, fv, fw}, inv_dt};
     return mls_launch<1>(P, A, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int fsei_ibm_apply_forcing(fsei_plan* P, long n, const double* xm, const double* ym, const double* zm, double* fu, double* fv,
+                                      double* fw, double* ru, double* rv, double* rw, double alpha_dt, void* cuda_stream)
+{
+    if (!P || n < 0 || (n > 0 && (!xm || !ym || !zm || !fu || !fv || !fw || !ru || !rv || !rw))) return fail(FSEI_ERR_ARG, "fsei_ibm_apply_forcing: NULL argument or n < 0");
+    if (P->slab) return fail(FSEI_ERR_ARG, "fsei_ibm_apply_forcing: not available on a slab plan");
+    if (alpha_dt != alpha_dt) return fail(FSEI_ERR_ARG, "fsei_ibm_apply_forcing: NaN alpha_dt");
+    double* fs[3] = {fu, fv, fw};
+    double* rs[3] = {ru, rv, rw};
+    for (int a = 0; a < 3; a++)
+        for (int b = 0; b < 3; b++) if (fs[a] == rs[b] || (a != b && (fs[a] == fs[b] || rs[a] == rs[b]))) return fail(FSEI_ERR_ARG, "fsei_ibm_apply_forcing: aliased fields");
+    if (P->T.nz < 3) return fail(FSEI_ERR_SIZE, "fsei_ibm_apply_forcing: the 27-node support needs nz >= 3");
+    if (n == 0) { P->last_launches = 0; return FSEI_OK; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    MlsApplyArgs A{mls_grid(P), n, xm, ym, zm, {fu, fv, fw}, {ru, rv, rw}, alpha_dt};
+    { LaunchTimer t(P, K_MLSAPPLY, st); k_mls_apply<<<(unsigned)((3 * n + 127) / 128), 128, 0, st>>>(A); }
+    CU(cudaGetLastError());
+    P->last_launches = 1;
+    return FSEI_OK;
 }
 
 // ------------------------------------------------------------------------------------------

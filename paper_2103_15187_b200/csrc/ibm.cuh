@@ -47,18 +47,25 @@ FSEI_DEV int mls_nearest(double x, double h, double off, int n, bool periodic, d
     return c;
 }
 
+// centre node (ic, jc, kc) of the 3 x 3 x 3 support of one (marker, component); xr, yr: coordinates reduced to the period
+FSEI_DEV void mls_centre(const MlsGrid& G, int comp, double xb, double yb, double zb, int& ic, int& jc, int& kc, double& xr, double& yr)
+{
+    ic = mls_nearest(xb, G.dx, comp == 0 ? 0.0 : 0.5, G.nx, G.bcx == BC_PERIODIC, G.Lx, xr);
+    jc = mls_nearest(yb, G.dy, comp == 1 ? 0.0 : 0.5, G.ny, G.bcy == BC_PERIODIC, G.Ly, yr);
+    // nearest z node: bisection for the last node <= zb, then the closer of it and the next (ties: the lower one)
+    int lo = 0, hi = G.nz - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (mls_znode(G, comp, mid) <= zb) lo = mid; else hi = mid - 1; }
+    kc = lo;
+    if (kc + 1 < G.nz && fabs(mls_znode(G, comp, kc + 1) - zb) < fabs(mls_znode(G, comp, kc) - zb)) kc++;
+    kc = kc < 1 ? 1 : (kc > G.nz - 2 ? G.nz - 2 : kc);
+}
+
 // the 27 shape functions of one (marker, component)
 FSEI_DEV void mls_stencil(const MlsGrid& G, int comp, double xb, double yb, double zb, MlsStencil& M)
 {
     double xr, yr;
-    const int ic = mls_nearest(xb, G.dx, comp == 0 ? 0.0 : 0.5, G.nx, G.bcx == BC_PERIODIC, G.Lx, xr);
-    const int jc = mls_nearest(yb, G.dy, comp == 1 ? 0.0 : 0.5, G.ny, G.bcy == BC_PERIODIC, G.Ly, yr);
-    // nearest z node: bisection for the last node <= zb, then the closer of it and the next (ties: the lower one)
-    int lo = 0, hi = G.nz - 1;
-    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (mls_znode(G, comp, mid) <= zb) lo = mid; else hi = mid - 1; }
-    int kc = lo;
-    if (kc + 1 < G.nz && fabs(mls_znode(G, comp, kc + 1) - zb) < fabs(mls_znode(G, comp, kc) - zb)) kc++;
-    kc = kc < 1 ? 1 : (kc > G.nz - 2 ? G.nz - 2 : kc);
+    int ic, jc, kc;
+    mls_centre(G, comp, xb, yb, zb, ic, jc, kc, xr, yr);
     const double zk[3] = {mls_znode(G, comp, kc - 1), mls_znode(G, comp, kc), mls_znode(G, comp, kc + 1)};
     const double rhz = 2.0 / (zk[2] - zk[0]);
     // per-direction scaled offsets of the three nodes and their node indices
@@ -150,6 +157,48 @@ FSEI_GLOBAL(128, 1) k_mls(const FSEI_GRID_CONSTANT MlsArgs A)
     double* __restrict__ f = A.f[c];
 #pragma unroll
     for (int k = 0; k < 27; k++) atomicAdd(f + M.base[k], cl * M.phi[k]);
+}
+
+// The forcing fields are zero except on the supports of the markers, so the substep need not stream them: after the explicit
+// terms (evaluated without a body force) this kernel visits the support nodes again and forms rhs += alpha_dt f there -- the
+// same two operations, in the same order, as the dense path of k_explicit_terms.  A node shared by several supports is taken
+// by whichever thread swaps its accumulated sum out of f first (the others read back 0 and leave); f is all-zero again
+// afterwards.  Wall-face rows (u at i = 0 / v at j = 0 on a wall-bounded box, w at k = 0) keep rhs = 0 (V7).
+struct MlsApplyArgs {
+    MlsGrid G;
+    long n;
+    const double *xm, *ym, *zm;
+    double* f[3];
+    double* r[3];
+    double adt;
+};
+
+FSEI_GLOBAL(128, 1) k_mls_apply(const FSEI_GRID_CONSTANT MlsApplyArgs A)
+{
+    const long t = (long)blockIdx.x * 128 + threadIdx.x;
+    if (t >= 3 * A.n) return;
+    const long l = t / 3; const int c = (int)(t - 3 * l);
+    const MlsGrid& G = A.G;
+    double xr, yr;
+    int ic, jc, kc;
+    mls_centre(G, c, A.xm[l], A.ym[l], A.zm[l], ic, jc, kc, xr, yr);
+    double* __restrict__ f = A.f[c];
+    double* __restrict__ r = A.r[c];
+#pragma unroll
+    for (int dk = -1; dk <= 1; dk++)
+#pragma unroll
+        for (int dj = -1; dj <= 1; dj++)
+#pragma unroll
+            for (int di = -1; di <= 1; di++) {
+                int i = ic + di, j = jc + dj;
+                const int k = kc + dk;
+                if (G.bcx == BC_PERIODIC) i = i < 0 ? i + G.nx : (i >= G.nx ? i - G.nx : i);
+                if (G.bcy == BC_PERIODIC) j = j < 0 ? j + G.ny : (j >= G.ny ? j - G.ny : j);
+                const size_t b = ((size_t)k * G.ny + j) * G.nx + i;
+                const double val = __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long*>(f + b), 0ull));
+                const bool wall_row = (c == 0 && i == 0 && G.bcx != BC_PERIODIC) || (c == 1 && j == 0 && G.bcy != BC_PERIODIC) || (c == 2 && k == 0);
+                if (val != 0.0 && !wall_row) r[b] = __dadd_rn(r[b], __dmul_rn(A.adt, val));
+            }
 }
 
 }  // namespace fsei

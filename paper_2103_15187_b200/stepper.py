@@ -4,8 +4,10 @@ One time step of the paper's scheme (Eq. 3; V1) is one subst
 rho = -1/2) or three (the low-storage third-order Runge-Kutta scheme of the paper's refs [12],[13]:
 gamma = (8/15, 5/12, 3/4), rho = (0, -17/60, -5/12), alpha_l = gamma_l + rho_l); a substep is
 
-    [IB forcing of the markers, if any: fsei_ibm_forcing]  ->  fsei_fluid_substep
-    (explicit terms -> implicit viscous step -> pressure projection)
+    without markers:  fsei_fluid_substep  (explicit terms -> implicit viscous step -> pressure projection)
+    with markers:     fsei_ibm_forcing -> fsei_explicit_terms (no body force) -> fsei_ibm_apply_forcing (rhs += alpha dt f on the
+                      markers' supports, which also clears f) -> fsei_viscous_step -> fsei_pressure_projection
+                      -- the forcing fields are zero-filled once and never streamed as a whole again
 
 with beta_l = alpha_l dt / (2 Re).  The first Adams-Bashforth step has no H^{n-1} and runs as forward Euler
 (gamma = 1, rho = 0).  All fields live on the device; nothing synchronises, so a step can be captured in a CUDA graph.
@@ -42,18 +44,25 @@ class FluidStepper:
     def substep(self, gamma: float, rho: float, stream=None):
         dt, alpha = self.dt, gamma + rho
         beta = alpha * dt / (2.0 * self.Re)
-        f = (None, None, None)
-        if self.markers is not None:
-            m = self.markers
-            for t in self.f:
-                t.zero_()
-            self.plan.ibm_forcing(m["xm"].shape[0], m["xm"], m["ym"], m["zm"], m["area"], m["Vu"], m["Vv"], m["Vw"],
-                                  self.u, self.v, self.w, 1.0 / (alpha * dt), *self.F, *self.f, stream=stream)
-            self.launches += self.plan.last_launch_count
-            f = tuple(self.f)
-        self.plan.fluid_substep(self.u, self.v, self.w, self.p, *self.h, *self.r, self.phi, gamma * dt, rho * dt, alpha * dt, beta,
-                                f=f, stream=stream)
-        self.launches += self.plan.last_launch_count
+        P = self.plan
+        if self.markers is None:
+            P.fluid_substep(self.u, self.v, self.w, self.p, *self.h, *self.r, self.phi, gamma * dt, rho * dt, alpha * dt, beta,
+                            stream=stream)
+            self.launches += P.last_launch_count
+            return
+        m = self.markers
+        n = m["xm"].shape[0]
+        P.ibm_forcing(n, m["xm"], m["ym"], m["zm"], m["area"], m["Vu"], m["Vv"], m["Vw"], self.u, self.v, self.w,
+                      1.0 / (alpha * dt), *self.F, *self.f, stream=stream)
+        self.launches += P.last_launch_count
+        P.explicit_terms(self.u, self.v, self.w, self.p, *self.h, *self.r, gamma * dt, rho * dt, alpha * dt, beta, stream=stream)
+        self.launches += P.last_launch_count
+        P.ibm_apply_forcing(n, m["xm"], m["ym"], m["zm"], *self.f, *self.r, alpha * dt, stream=stream)
+        self.launches += P.last_launch_count
+        P.viscous_step(self.u, self.v, self.w, *self.r, beta, stream=stream)
+        self.launches += P.last_launch_count
+        P.pressure_projection(self.u, self.v, self.w, self.p, self.phi, alpha * dt, beta, stream=stream)
+        self.launches += P.last_launch_count
 
     def step(self, stream=None):
         gam, rho = SCHEMES[self.scheme]

@@ -144,6 +144,52 @@ def test_substep_with_ib_forcing_vs_oracle(oracle_ld):
     plan.destroy()
 
 
+@pytest.mark.parametrize("shape,bc,n,centre,radius", CASES)
+def test_apply_forcing_equals_dense_body_force(oracle_ld, shape, bc, n, centre, radius):
+    """explicit terms without a force + fsei_ibm_apply_forcing on the markers' supports == explicit terms with the dense forcing
+    fields: bit for bit given the same f (the same two operations per node), and against the oracle's chain; f is all-zero
+    afterwards; a second apply is a no-op."""
+    import torch
+    from paper_2103_15187_b200.binding import Plan
+    g, vel, mk, area, V = _setup(shape, bc, n, centre, radius, seed=7)
+    if bc[0] == W: vel[0][:, :, 0] = 0
+    if bc[1] == W: vel[1][:, 0, :] = 0
+    vel[2][0] = 0
+    dt, beta = 2e-3, 1e-5
+    plan = Plan.from_grid(g)
+    u, v, w = _dev(vel)
+    z = lambda: torch.zeros_like(u)
+    p, fu, fv, fw = z(), z(), z(), z()
+    ha, hb, ra, rb = [z() for _ in range(3)], [z() for _ in range(3)], [z() for _ in range(3)], [z() for _ in range(3)]
+    dm, (da,), dV = _dev(mk), _dev([area]), _dev(V)
+    dF = [torch.empty(n, dtype=torch.float64, device="cuda:0") for _ in range(3)]
+    plan.ibm_forcing(n, *dm, da, *dV, u, v, w, 1.0 / dt, *dF, fu, fv, fw)
+    dense_f = [t.clone() for t in (fu, fv, fw)]
+    plan.explicit_terms(u, v, w, p, *ha, *ra, 1.5 * dt, -0.5 * dt, dt, beta, f=(fu, fv, fw))            # dense path
+    plan.explicit_terms(u, v, w, p, *hb, *rb, 1.5 * dt, -0.5 * dt, dt, beta)                            # sparse path
+    plan.ibm_apply_forcing(n, *dm, fu, fv, fw, *rb, dt)
+    assert plan.last_launch_count == 1
+    torch.cuda.synchronize()
+    for c in range(3):
+        assert torch.equal(ra[c], rb[c]), c
+        assert torch.equal(ha[c], hb[c]), c
+        assert not (fu, fv, fw)[c].any(), c                                                              # cleared for the next substep
+    keep = [t.clone() for t in rb]
+    plan.ibm_apply_forcing(n, *dm, fu, fv, fw, *rb, dt)
+    torch.cuda.synchronize()
+    for c in range(3):
+        assert torch.equal(keep[c], rb[c]), c
+    # the oracle's chain (dense by definition); the spread's atomic order is the only difference
+    fo = [np.zeros_like(vel[0]) for _ in range(3)]
+    ho = [np.zeros_like(vel[0]) for _ in range(3)]
+    oracle_ld.ibm_forcing(g, *mk, area, V, *vel, 1.0 / dt, fo)
+    ro = oracle_ld.explicit_terms(g, *vel, np.zeros_like(vel[0]), *ho, 1.5 * dt, -0.5 * dt, dt, beta, f=fo)
+    for c in range(3):
+        assert np.abs(rb[c].cpu().numpy() - ro[c]).max() <= 1e-12 * max(1.0, np.abs(ro[c]).max()), c
+        assert np.abs(dense_f[c].cpu().numpy() - fo[c]).max() <= 1e-12 * max(1.0, np.abs(fo[c]).max()), c
+    plan.destroy()
+
+
 def test_mls_edge_cases():
     import torch
     from paper_2103_15187_b200.binding import Plan, FseiError, ERR_ARG
