@@ -127,9 +127,12 @@ int fsei_pressure_projection(fsei_plan* plan, double* u, double* v, double* w, d
 
 /*
  * Host-buffer convenience used for end-to-end timing: u,v,w,p are HOST pointers (pinned for
- * full speed); copies them to plan-owned device fields, runs fsei_pressure_projection, copies
- * u,v,w,p back and synchronises the stream.  The 5 staging fields are allocated at plan creation
- * when the plan was made with FSEI_PLAN_HOST_FIELDS, else on first use; freed with the plan.
+ * full speed and for the overlap below); copies them to plan-owned device fields, runs the projection,
+ * copies u,v,w,p back and synchronises the stream.  The link is full duplex and p is not needed before the
+ * correction a7, so u,v,w go up first, a1-a6 run, and a7 runs in up to 8 z chunks: chunk c of p goes up on a
+ * plan-owned copy stream while the corrected chunks before it come down on another (same kernels, same results
+ * as fsei_pressure_projection).  The 5 staging fields are allocated at plan creation when the plan was made with
+ * FSEI_PLAN_HOST_FIELDS, else on first use; the two copy streams on first use; all freed with the plan.
  */
 int fsei_pressure_projection_host(fsei_plan* plan, double* u, double* v, double* w, double* p,
                                   double alpha_dt, double beta, void* cuda_stream);

@@ -70,6 +70,8 @@ struct fsei_plan {
     bool visc_fast = false; VFastLine vline_x[FSEI_VSLOTS], vline_y[FSEI_VSLOTS]; int vnsig_x[FSEI_VSLOTS], vnsig_y[FSEI_VSLOTS];
     double* vtab = nullptr; int vnmax = 0; double visc_beta[FSEI_VSLOTS] = {NAN, NAN, NAN, NAN}; int visc_next = 0;
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
+    cudaStream_t host_up = nullptr, host_dn = nullptr;                     // its copy streams (p up / results down, in z chunks)
+    std::vector<cudaEvent_t> host_ev;
     // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;      // 2 events per recorded launch
@@ -458,6 +460,9 @@ extern "C" void fsei_plan_destroy(fsei_plan* P)
     for (void* p : P->owned) cudaFree(p);
     for (double* p : P->hostpath) if (p) cudaFree(p);
     for (cudaEvent_t e : P->ev_pool) cudaEventDestroy(e);
+    for (cudaEvent_t e : P->host_ev) cudaEventDestroy(e);
+    if (P->host_up) cudaStreamDestroy(P->host_up);
+    if (P->host_dn) cudaStreamDestroy(P->host_dn);
     delete P;
 }
 
@@ -606,6 +611,14 @@ extern "C" int fsei_project(fsei_plan* P, double* u, double* v, double* w, doubl
     return FSEI_OK;
 }
 
+// a1 .. a6 of the register-resident families: phi = solution of the Poisson problem for D(u, v, w) / alpha_dt
+static int fast_projection_solve(fsei_plan* P, const double* u, const double* v, const double* w, double* phi, double alpha_dt, cudaStream_t st)
+{
+    cplx* spec = P->fused ? P->work : reinterpret_cast<cplx*>(phi);
+    { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, P->T.bcx == BC_NEUMANN, true, u, v, w, 1.0 / alpha_dt, spec, st, P->fused)); }
+    return P->fused ? fused_spectral_solve(P, phi, st) : fast_spectral_solve(P, spec, st);
+}
+
 extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, double* w, double* p, double* phi,
                                         double alpha_dt, double beta, void* cuda_stream)
 {
@@ -617,9 +630,7 @@ extern "C" int fsei_pressure_projection(fsei_plan* P, double* u, double* v, doub
         if (phi == u || phi == v || phi == w || phi == p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: phi must not alias u, v, w, p");
         if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(p) || misaligned(phi)) return fail(FSEI_ERR_ARG, "fsei_pressure_projection: field pointers must be 16-byte aligned");
         cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-        cplx* spec = P->fused ? P->work : reinterpret_cast<cplx*>(phi);
-        { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, P->T.bcx == BC_NEUMANN, true, u, v, w, 1.0 / alpha_dt, spec, st, P->fused)); }
-        if ((rc = P->fused ? fused_spectral_solve(P, phi, st) : fast_spectral_solve(P, spec, st))) return rc;
+        if ((rc = fast_projection_solve(P, u, v, w, phi, alpha_dt, st))) return rc;
         if ((rc = fsei_project(P, u, v, w, p, phi, alpha_dt, beta, cuda_stream))) return rc;
         P->last_launches = P->fused ? 6 : 7;
         return FSEI_OK;
@@ -638,16 +649,61 @@ extern "C" int fsei_pressure_projection_host(fsei_plan* P, double* u, double* v,
                                              double alpha_dt, double beta, void* cuda_stream)
 {
     if (!P || !u || !v || !w || !p) return fail(FSEI_ERR_ARG, "fsei_pressure_projection_host: NULL argument");
+    if (P->slab) return fail(FSEI_ERR_ARG, "fsei_pressure_projection_host: this is a slab plan");
+    if (alpha_dt == 0.0 || alpha_dt != alpha_dt || beta != beta) return fail(FSEI_ERR_ARG, "fsei_pressure_projection_host: alpha_dt must be non-zero, beta not NaN");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const size_t bytes = sizeof(double) * (size_t)P->T.nx * P->T.ny * P->T.nz;
+    const HostTables& T = P->T;
+    const size_t plane = (size_t)T.nx * T.ny, bytes = sizeof(double) * plane * T.nz;
     { int rc0 = host_fields(P); if (rc0) return rc0; }          // no-op when the plan was created with FSEI_PLAN_HOST_FIELDS
+    // The link is full duplex and p is not needed before the correction: u, v, w go up, the Poisson problem is solved, then the
+    // correction runs in z chunks -- chunk c of p goes up on one copy stream while the corrected chunks c-1, c-2, ... of u, v, w,
+    // p come down on another.
+    constexpr int NCH = 8;
+    const int nch = T.nz < NCH ? T.nz : NCH;
+    if (!P->host_up) {
+        CU(cudaStreamCreateWithFlags(&P->host_up, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&P->host_dn, cudaStreamNonBlocking));
+        P->host_ev.resize(2 * NCH + 2);
+        for (cudaEvent_t& e : P->host_ev) CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
     double* h[4] = {u, v, w, p};
-    for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(P->hostpath[f], h[f], bytes, cudaMemcpyHostToDevice, st));
-    int rc = fsei_pressure_projection(P, P->hostpath[0], P->hostpath[1], P->hostpath[2], P->hostpath[3], P->hostpath[4],
-                                      alpha_dt, beta, cuda_stream);
-    if (rc) return rc;
-    for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(h[f], P->hostpath[f], bytes, cudaMemcpyDeviceToHost, st));
+    double** d = P->hostpath;
+    cudaEvent_t ev_in = P->host_ev[2 * NCH], ev_out = P->host_ev[2 * NCH + 1];
+    for (int f = 0; f < 3; f++) CU(cudaMemcpyAsync(d[f], h[f], bytes, cudaMemcpyHostToDevice, st));
+    CU(cudaEventRecord(ev_in, st));
+    CU(cudaStreamWaitEvent(P->host_up, ev_in, 0));              // p follows u, v, w on the way up (and the previous call's work)
+    CU(cudaStreamWaitEvent(P->host_dn, ev_in, 0));
+    int rc, launches = 0;
+    if (P->fast) {
+        if ((rc = fast_projection_solve(P, d[0], d[1], d[2], d[4], alpha_dt, st))) return rc;
+        launches = P->fused ? 5 : 6;
+    } else {
+        if ((rc = fsei_divergence(P, d[0], d[1], d[2], alpha_dt, d[4], cuda_stream))) return rc;
+        launches = P->last_launches;
+        if ((rc = fsei_poisson_solve(P, d[4], d[4], cuda_stream))) return rc;
+        launches += P->last_launches;
+    }
+    for (int c = 0; c < nch; c++) {
+        const int k0 = (int)((long)T.nz * c / nch), k1 = (int)((long)T.nz * (c + 1) / nch);
+        const size_t off = (size_t)k0 * plane, cb = sizeof(double) * plane * (size_t)(k1 - k0);
+        cudaEvent_t ev_up = P->host_ev[2 * c], ev_pr = P->host_ev[2 * c + 1];
+        CU(cudaMemcpyAsync(d[3] + off, p + off, cb, cudaMemcpyHostToDevice, P->host_up));
+        CU(cudaEventRecord(ev_up, P->host_up));
+        CU(cudaStreamWaitEvent(st, ev_up, 0));
+        SParams S = P->S;                                       // the correction on planes [k0, k1): phi has its neighbours in place
+        S.nz = k1 - k0; S.kofs = k0; S.halo_lo = k0 > 0; S.halo_hi = k1 < T.nz;
+        const size_t n2 = plane * (size_t)(k1 - k0) / 2;
+        { LaunchTimer t(P, K_PROJ, st); k_project_fast<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(S, d[0] + off, d[1] + off, d[2] + off, d[3] + off, d[4] + off, alpha_dt, beta); }
+        CU(cudaGetLastError());
+        launches++;
+        CU(cudaEventRecord(ev_pr, st));
+        CU(cudaStreamWaitEvent(P->host_dn, ev_pr, 0));
+        for (int f = 0; f < 4; f++) CU(cudaMemcpyAsync(h[f] + off, d[f] + off, cb, cudaMemcpyDeviceToHost, P->host_dn));
+    }
+    CU(cudaEventRecord(ev_out, P->host_dn));
+    CU(cudaStreamWaitEvent(st, ev_out, 0));
     CU(cudaStreamSynchronize(st));
+    P->last_launches = launches;
     return FSEI_OK;
 }
 
