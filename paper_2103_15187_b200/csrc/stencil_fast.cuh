@@ -48,7 +48,7 @@ FSEI_GLOBAL(256, 1) k_divergence_fast(SParams S, const double* __restrict__ u, c
 }
 
 // grid ceil(nx ny nz / 2 / 256), block 256
-FSEI_GLOBAL(256, 1) k_project_fast(SParams S, double* __restrict__ u, double* __restrict__ v, double* __restrict__ w,
+FSEI_GLOBAL(256, 4) k_project_fast(SParams S, double* __restrict__ u, double* __restrict__ v, double* __restrict__ w,
                                    double* __restrict__ p, const double* __restrict__ phi, double adt, double beta)
 {
     const int hx = S.nx >> 1;
