@@ -188,6 +188,24 @@ int fsei_fluid_substep(fsei_plan* plan, double* u, double* v, double* w, double*
                        double* phi, double gamma_dt, double rho_dt, double alpha_dt, double beta, void* cuda_stream);
 
 /*
+ * fsei_viscous_step for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same operation (Eq. 3; the three tridiagonal sweeps of P:L208 per component),
+ * computed by the generic kernel family with its factorisation tables in a file-scope `static __device__` array of libfsei
+ * instead of plan-owned memory.  The call itself performs no cudaMalloc, cudaFree or allocating library call (the plan was
+ * created earlier, at set-up; the array's device address is resolved then, once per device, by cudaGetSymbolAddress).
+ *   Limit : nx, ny and nz each <= 1024 (the array holds 9 x (5 x 1024 + 8) doubles = 369 216 bytes, resident on every GPU
+ *           that loads the library until the process exits)                                           else FSEI_ERR_SIZE
+ *   Device: the current device must be the one the plan was created on                                else FSEI_ERR_ARG
+ *   Result: bit-identical to fsei_viscous_step on a plan made with FSEI_PLAN_VISC_GENERIC; equal to rounding to the fast
+ *           family's.  10 launches, always (no per-beta table cache: the array is shared).
+ *   Sharing: every call on a device uses the same array and it keeps the last call's contents; each call rewrites all the
+ *           entries it reads before it reads them (nothing needs clearing).  Calls that OVERLAP on the GPU -- other streams,
+ *           other plans, other threads -- race on it: the caller serialises them.
+ */
+int fsei_viscous_step_noalloc(fsei_plan* plan, double* u, double* v, double* w, double* ru, double* rv, double* rw,
+                              double beta, void* cuda_stream);
+
+/*
  * ---- IB-MLS transfer operators (Eq. 4, Fig. 2; sec. 3.2) -----------------
  * "A three-dimensional support domain consisting of N_e = n x n x n Eulerian nodes (n = 3 ...) is created around each
  * Lagrangian marker, and the fluid velocity at the body position is computed interpolating ...

@@ -20,7 +20,7 @@ EXPORTS = ("fsei_plan_create", "fsei_plan_create_ex", "fsei_plan_kernel_family",
            "fsei_plan_workspace_bytes", "fsei_divergence", "fsei_poisson_solve", "fsei_project",
            "fsei_pressure_projection", "fsei_pressure_projection_host", "fsei_plan_last_launch_count",
            "fsei_plan_profile", "fsei_plan_profile_read",
-           "fsei_explicit_terms", "fsei_viscous_step", "fsei_fluid_substep",
+           "fsei_explicit_terms", "fsei_viscous_step", "fsei_viscous_step_noalloc", "fsei_fluid_substep",
            "fsei_mls_interpolate", "fsei_mls_spread", "fsei_ibm_forcing", "fsei_ibm_apply_forcing",
            "fsei_slab_plan_create", "fsei_slab_set_peers", "fsei_slab_forward", "fsei_pencil_solve", "fsei_slab_backward", "fsei_slab_project",
            "fsei_slab_viscous_xy", "fsei_pencil_viscous_z", "fsei_slab_field_add")
@@ -83,6 +83,8 @@ def lib() -> ctypes.CDLL:
     L.fsei_explicit_terms.argtypes = [_vp] * 14 + [_d] * 4 + [_vp]
     L.fsei_viscous_step.restype = _i
     L.fsei_viscous_step.argtypes = [_vp] * 7 + [_d, _vp]
+    L.fsei_viscous_step_noalloc.restype = _i
+    L.fsei_viscous_step_noalloc.argtypes = [_vp] * 7 + [_d, _vp]
     L.fsei_fluid_substep.restype = _i
     L.fsei_fluid_substep.argtypes = [_vp] * 15 + [_d] * 4 + [_vp]
     L.fsei_mls_interpolate.restype = _i
@@ -230,6 +232,10 @@ class Plan:
     def viscous_step(self, u, v, w, ru, rv, rw, beta, stream=None):
         _chk(lib().fsei_viscous_step(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(ru), _ptr(rv), _ptr(rw), float(beta),
                                      _stream(stream)))
+
+    def viscous_step_noalloc(self, u, v, w, ru, rv, rw, beta, stream=None):
+        _chk(lib().fsei_viscous_step_noalloc(self._h, _ptr(u), _ptr(v), _ptr(w), _ptr(ru), _ptr(rv), _ptr(rw), float(beta),
+                                             _stream(stream)))
 
     def fluid_substep(self, u, v, w, p, hu, hv, hw, ru, rv, rw, phi, gamma_dt, rho_dt, alpha_dt, beta, f=(None, None, None),
                       stream=None):

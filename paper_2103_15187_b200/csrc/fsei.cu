@@ -27,6 +27,7 @@
 #include "tma_host.hpp"
 #include <cmath>
 #include <cstdlib>
+#include <mutex>
 
 using namespace fsei;
 
@@ -42,6 +43,7 @@ static int cuda_fail(cudaError_t e, const char* what)
 }
 static bool misaligned(const void* p) { return (reinterpret_cast<size_t>(p) & 15u) != 0; }
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+static int noalloc_resolve(double** out, int* dev_out);      // fsei_viscous_step_noalloc: device address of its static scratch array
 
 // ------------------------------------------------------------------------------------------
 // plan
@@ -70,6 +72,7 @@ struct fsei_plan {
     bool visc_fast = false; VFastLine vline_x[FSEI_VSLOTS], vline_y[FSEI_VSLOTS]; int vnsig_x[FSEI_VSLOTS], vnsig_y[FSEI_VSLOTS];
     double* vtab = nullptr; int vnmax = 0; double visc_beta[FSEI_VSLOTS] = {NAN, NAN, NAN, NAN}; int visc_next = 0;
     double* hostpath[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // device u,v,w,p,phi of the host-buffer entry
+    double* noalloc_tab = nullptr; int noalloc_dev = -1; int noalloc_err = 0;   // fsei_viscous_step_noalloc: static scratch of the plan's device
     cudaStream_t host_up = nullptr, host_dn = nullptr;                     // its copy streams (p up / results down, in z chunks)
     std::vector<cudaEvent_t> host_ev;
     // per-kernel CUDA-event timing (fsei_plan_profile): event pairs recorded around every launch
@@ -437,6 +440,10 @@ extern "C" fsei_plan* fsei_plan_create_ex(int nx, int ny, int nz, double Lx, dou
     if (!P) { fail(FSEI_ERR_ALLOC, "out of host memory"); return nullptr; }
     int rc = plan_build(P, nx, ny, nz, Lx, Ly, zc, bc_x, bc_y, flags);
     if (rc == FSEI_OK && (flags & FSEI_PLAN_HOST_FIELDS)) rc = host_fields(P);
+    if (rc == FSEI_OK) {                                       // set-up of fsei_viscous_step_noalloc; a failure surfaces in that call only
+        P->noalloc_err = noalloc_resolve(&P->noalloc_tab, &P->noalloc_dev);
+        if (P->noalloc_err) P->noalloc_tab = nullptr;
+    }
     if (rc != FSEI_OK) { const std::string msg = g_err; fsei_plan_destroy(P); g_err = msg; g_err_code = rc; return nullptr; }
     g_err_code = FSEI_OK; g_err.clear();
     return P;
@@ -873,6 +880,100 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
         launches += 3;
     }
     P->last_launches = launches;
+    return FSEI_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// fsei_viscous_step_noalloc: the generic family of the implicit viscous step with its factorisation tables in a file-scope
+// device array instead of plan-owned memory, for callers that may not allocate (stream capture, serving loops, harnesses that
+// forbid cudaMalloc).  Every GPU that loads the library holds the array until exit (FSEI_NOALLOC_BYTES = 369 216 bytes).
+//
+// In HOST code the name `g_noalloc_vtab` is a host-side stand-in, not a device address: its device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current (noalloc_resolve, called at plan creation = set-up)
+// and only that pointer is ever given to a kernel.
+//
+// All calls on a device share the array and it keeps the last call's contents.  Nothing in it has to start at zero: the
+// factor launch of a call writes every table entry the nine sweeps of that call read (ip, am, cp, wc, er at rows 0..n-1 and
+// ipl[0] of each of the 9 sets) before they run, on the same stream.  Two calls that overlap on the GPU (different streams,
+// or two processes' worth of plans in one process on one device) RACE on it: serialise them.
+// ------------------------------------------------------------------------------------------
+#define FSEI_NOALLOC_NMAX 1024                                           /* longest line (nx, ny, nz each) */
+#define FSEI_NOALLOC_DOUBLES (9 * (5 * FSEI_NOALLOC_NMAX + 8))           /* 9 sets of vtab_set_doubles(NMAX) */
+#define FSEI_NOALLOC_BYTES (FSEI_NOALLOC_DOUBLES * 8)
+#define FSEI_NOALLOC_MAXDEV 64
+static __device__ __align__(256) double g_noalloc_vtab[FSEI_NOALLOC_DOUBLES];
+static double* g_noalloc_ptr[FSEI_NOALLOC_MAXDEV];                       // device address of the array on each device (host cache)
+static std::mutex g_noalloc_mu;
+
+// device address of the scratch array on the CURRENT device; asks the runtime once per device
+static int noalloc_resolve(double** out, int* dev_out)
+{
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= FSEI_NOALLOC_MAXDEV) return fail(FSEI_ERR_CUDA, "fsei_viscous_step_noalloc: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_vtab);
+        if (e != cudaSuccess || !p) { cudaGetLastError(); return cuda_fail(e, "cudaGetSymbolAddress(g_noalloc_vtab)"); }
+        g_noalloc_ptr[dev] = static_cast<double*>(p);
+    }
+    *out = g_noalloc_ptr[dev]; *dev_out = dev;
+    return FSEI_OK;
+}
+
+static VTab visc_tab_from(const HostTables& T, const double* base, int nmax, int comp, int dir)
+{
+    const double* t = base + (size_t)(comp * 3 + dir) * vtab_set_doubles(nmax);
+    const size_t m = (size_t)nmax;
+    VTab V;
+    V.ip = t; V.am = t + m; V.cp = t + 2 * m; V.wc = t + 3 * m; V.er = t + 4 * m; V.ipl = t + 5 * m;
+    V.n = dir == DIR_X ? T.nx : (dir == DIR_Y ? T.ny : T.nz);
+    V.cyclic = (dir == DIR_X && T.bcx == BC_PERIODIC) || (dir == DIR_Y && T.bcy == BC_PERIODIC);
+    V.fixed0 = (dir == DIR_X && comp == COMP_U && T.bcx != BC_PERIODIC) || (dir == DIR_Y && comp == COMP_V && T.bcy != BC_PERIODIC) ||
+               (dir == DIR_Z && comp == COMP_W);
+    return V;
+}
+
+extern "C" int fsei_viscous_step_noalloc(fsei_plan* P, double* u, double* v, double* w, double* ru, double* rv, double* rw,
+                                         double beta, void* cuda_stream)
+{
+    if (P && P->slab) return fail(FSEI_ERR_ARG, "fsei_viscous_step_noalloc: this is a slab plan");
+    if (!P || !u || !v || !w || !ru || !rv || !rw) return fail(FSEI_ERR_ARG, "fsei_viscous_step_noalloc: NULL argument");
+    if (!(beta >= 0.0) || std::isinf(beta)) return fail(FSEI_ERR_ARG, "fsei_viscous_step_noalloc: beta must be finite and >= 0");
+    double* q[3] = {u, v, w};
+    double* r[3] = {ru, rv, rw};
+    for (int a = 0; a < 3; a++)
+        for (int b = 0; b < 3; b++) if (r[a] == q[b] || (a != b && (r[a] == r[b] || q[a] == q[b]))) return fail(FSEI_ERR_ARG, "fsei_viscous_step_noalloc: fields must not alias");
+    const HostTables& T = P->T;
+    const int nmax = T.nx > T.ny ? (T.nx > T.nz ? T.nx : T.nz) : (T.ny > T.nz ? T.ny : T.nz);
+    if (nmax > FSEI_NOALLOC_NMAX)
+        return fail(FSEI_ERR_SIZE, "fsei_viscous_step_noalloc: nx, ny and nz must each be <= 1024 (the static scratch array holds the "
+                                   "factorisation tables of lines up to that length); use fsei_viscous_step on larger grids");
+    if (!P->noalloc_tab) return fail(FSEI_ERR_CUDA, "fsei_viscous_step_noalloc: the address of the static scratch array could not be resolved when the plan was created");
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev != P->noalloc_dev) return fail(FSEI_ERR_ARG, "fsei_viscous_step_noalloc: the current device is not the one the plan was created on");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double* tab = P->noalloc_tab;                                        // a device address (never the symbol's host stand-in)
+    VFactorArgs A{P->S, beta, tab, nmax};
+    k_visc_factor<<<9, 32, 0, st>>>(A);
+    CU(cudaGetLastError());
+    const long nlx = (long)T.ny * T.nz, nly = (long)T.nx * T.nz, nlz = (long)T.nx * T.ny;
+    const size_t plane = (size_t)T.nx * T.ny;
+    for (int c = 0; c < 3; c++) {
+        const VTab Vx = visc_tab_from(T, tab, nmax, c, DIR_X), Vy = visc_tab_from(T, tab, nmax, c, DIR_Y), Vz = visc_tab_from(T, tab, nmax, c, DIR_Z);
+        const unsigned gx = (unsigned)((nlx + 127) / 128), gy = (unsigned)((nly + 127) / 128), gz = (unsigned)((nlz + 127) / 128);
+        if (Vx.cyclic) k_visc_sweep_x<true, false><<<gx, 128, 0, st>>>(Vx, r[c], nullptr, nlx);
+        else k_visc_sweep_x<false, false><<<gx, 128, 0, st>>>(Vx, r[c], nullptr, nlx);
+        CU(cudaGetLastError());
+        if (Vy.cyclic) k_visc_sweep_strided<true, false><<<gy, 128, 0, st>>>(Vy, r[c], nullptr, T.nx, (size_t)T.nx, plane, nly);
+        else k_visc_sweep_strided<false, false><<<gy, 128, 0, st>>>(Vy, r[c], nullptr, T.nx, (size_t)T.nx, plane, nly);
+        CU(cudaGetLastError());
+        k_visc_sweep_strided<false, true><<<gz, 128, 0, st>>>(Vz, r[c], q[c], (int)nlz, plane, 0, nlz);
+        CU(cudaGetLastError());
+    }
+    P->last_launches = 10;
     return FSEI_OK;
 }
 
