@@ -254,3 +254,93 @@ def test_viscous_beta_cache_and_graph_capture(oracle_ld):
     for c, ref in enumerate((uo, vo, wo, po)):
         assert np.abs(fld[c].cpu().numpy() - ref).max() <= 1e-11 * max(1.0, np.abs(ref).max()), c
     plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# configs[3] at FULL size (1024 x 1024 x 768), the launch configuration bench.py's fluid leg times: IB forcing of 1.19 M
+# markers, explicit terms from TMA tiles in 64-plane marches, forcing applied on the markers' supports, fast viscous family
+# ---------------------------------------------------------------------------------------------
+def test_config4_full_size_fluid_rows(oracle_ld):
+    """IB forcing: marker forces and the whole forcing fields against the oracle.  Explicit terms (+ apply): bit-exact on
+    sampled groups of planes the oracle computes from sub-grids (a local stencil: the interior planes of a sub-grid of 8
+    planes see the same inputs and metrics as in the whole grid) -- bottom wall, a 64-plane march boundary, the planes through
+    the immersed body, top wall.  Viscous step: every output against the long-double oracle run on the whole grid."""
+    import torch
+    from paper_2103_15187_b200.binding import Plan
+    if torch.cuda.get_device_properties(0).total_memory < 100e9:
+        pytest.skip("needs a GPU with >= 100 GB")
+    avail = 0.0
+    with open("/proc/meminfo") as fh:
+        for line in fh:
+            if line.startswith("MemAvailable"):
+                avail = int(line.split()[1]) / 1e6
+    if avail < 120:
+        pytest.skip(f"full-size oracle needs about 90 GB of host memory, {avail:.0f} GB available")
+    case = inputs.make_case(4)
+    g, nx, ny, nz = case.grid, case.nx, case.ny, case.nz
+    zc = np.asarray(g[5])
+    hu = [case.u, case.v, case.w]
+    for a in hu:
+        a *= 0.05
+    hu[2][0] = 0
+    dt, Re = case.alpha_dt, 3000.0
+    gdt, rdt, adt, beta = 1.5 * dt, -0.5 * dt, dt, dt / (2 * Re)
+    plan = Plan.from_grid(g)
+    u, v, w = (torch.from_numpy(a).cuda() for a in hu)
+    z = lambda: torch.zeros_like(u)
+    p, h, r, f = z(), [z(), z(), z()], [z(), z(), z()], [z(), z(), z()]
+    # ---- IB forcing (the marker cloud of bench.py)
+    n = int(4 * 3.14159 * 0.3 ** 2 * nx * ny / (case.Lx * case.Ly))
+    xm, ym, zm, area, V = inputs.sphere_markers(n, (0.5 * case.Lx, 0.5 * case.Ly, 0.5), 0.3, seed=7)
+    dm = _dev([xm, ym, zm, area, *V])
+    F = [torch.empty(n, dtype=torch.float64, device="cuda:0") for _ in range(3)]
+    plan.ibm_forcing(n, *dm[:4], *dm[4:], u, v, w, 1.0 / dt, *F, *f)
+    torch.cuda.synchronize()
+    fo = [np.zeros((nz, ny, nx)) for _ in range(3)]
+    Fo = oracle_ld.ibm_forcing(g, xm, ym, zm, area, V, *hu, 1.0 / dt, fo)
+    groups = [(0, 8, 0, 6), (60, 68, 2, 6), (380, 388, 2, 6), (nz - 8, nz, 2, 8)]        # sub-grid [a, b), compared sub-planes [lo, hi)
+    fsub = [[None] * 3 for _ in groups]
+    for c in range(3):
+        assert np.abs(F[c].cpu().numpy() - Fo[c]).max() <= 1e-12 * np.abs(Fo[c]).max(), c
+        got = f[c].cpu().numpy()
+        assert np.count_nonzero(got) > n                                                   # the supports are there
+        assert np.abs(got - fo[c]).max() <= 1e-12 * np.abs(fo[c]).max(), c
+        for gi, (a, b, _, _) in enumerate(groups):
+            fsub[gi][c] = got[a:b].copy()
+        fo[c] = None
+        del got
+    del fo
+    # ---- explicit terms without a dense force, then the forcing on the supports
+    plan.explicit_terms(u, v, w, p, *h, *r, gdt, rdt, adt, beta)
+    assert plan.last_launch_count == 1
+    plan.ibm_apply_forcing(n, *dm[:3], *f, *r, adt)
+    torch.cuda.synchronize()
+    for c in range(3):
+        assert not bool(f[c].any()), c                                                     # cleared for the next substep
+    del f
+    for gi, (a, b, lo, hi) in enumerate(groups):
+        gs = (nx, ny, b - a, g[3], g[4], zc[a:b + 1].copy(), g[6], g[7])
+        sub = [np.ascontiguousarray(t[a:b]) for t in hu]
+        hs = [np.zeros_like(sub[0]) for _ in range(3)]
+        rs = oracle_ld.explicit_terms(gs, *sub, np.zeros_like(sub[0]), *hs, gdt, rdt, adt, beta, f=tuple(fsub[gi]))
+        for c in range(3):
+            assert np.array_equal(r[c][a + lo:a + hi].cpu().numpy(), rs[c][lo:hi]), ("rhs", gi, c)
+            assert np.array_equal(h[c][a + lo:a + hi].cpu().numpy(), hs[c][lo:hi]), ("H", gi, c)
+    del h, fsub
+    # ---- implicit viscous step on the whole grid
+    hr = [t.cpu().numpy() for t in r]
+    plan.viscous_step(u, v, w, *r, beta)
+    assert plan.last_launch_count == 3                                                     # tables + the two fused passes
+    torch.cuda.synchronize()
+    q0max = [float(np.abs(a).max()) for a in hu]
+    q0 = [a[nz // 2].copy() for a in hu]
+    oracle_ld.viscous_step(g, *hu, *hr, beta)
+    del hr
+    for c, t in enumerate((u, v, w)):
+        got = t.cpu().numpy()
+        scale = float(np.abs(hu[c][nz // 2] - q0[c]).max())                                # size of the increment (one plane is enough)
+        err = float(np.abs(got - hu[c]).max())
+        print(f"cfg 4 FULL viscous comp {c}: max err {err:.2e}  increment ~{scale:.2e}  max|q| {q0max[c]:.2e}")
+        assert err <= 1e-12 * scale + 2 * EPS * q0max[c], c
+        del got
+    plan.destroy()
