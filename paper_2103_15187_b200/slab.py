@@ -79,6 +79,16 @@ class SlabExchange:
         for s, (s0, s1) in enumerate(self.sr):
             dst[:, :, s0:s1, :].copy_(self.recv[s])
 
+    # ---- one halo layer of whole fields (explicit terms): exts = arrays [nzl + 2][ny][nx], own planes at 1 .. nzl --------
+    def field_halos(self, exts):
+        sends, recvs = [], []
+        for e in exts:
+            if self.rank > 0:
+                sends.append((e[1], self.rank - 1)); recvs.append((e[0], self.rank - 1))
+            if self.rank + 1 < self.world:
+                sends.append((e[self.nzl], self.rank + 1)); recvs.append((e[self.nzl + 1], self.rank + 1))
+        return sends, recvs
+
     # ---- halo of phi (before a7): my last plane goes up; with beta != 0 my first plane also goes down ---------
     def phi_halo(self, both: bool):
         sends, recvs = [], []
@@ -284,13 +294,7 @@ class SlabFluid(SlabProjection):
 
     def stage_halos(self):
         """One halo layer of u, v, w, p on each side."""
-        x, sends, recvs = self.x, [], []
-        for e in self.ext:
-            if x.rank > 0:
-                sends.append((e[1], x.rank - 1)); recvs.append((e[0], x.rank - 1))
-            if x.rank + 1 < x.world:
-                sends.append((e[x.nzl], x.rank + 1)); recvs.append((e[x.nzl + 1], x.rank + 1))
-        return sends, recvs
+        return self.x.field_halos(self.ext)
 
     def stage_explicit(self, gamma_dt, rho_dt, alpha_dt, beta, stream=None):
         self.plan.explicit_terms(self.u, self.v, self.w, self.p, *self.h, *self.r, gamma_dt, rho_dt, alpha_dt, beta,

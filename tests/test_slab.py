@@ -61,6 +61,24 @@ def _worker(rank, world, port, shape, out):
     ok["phi_lo"] = bool(x.k0 == 0 or torch.equal(x.phi_ext[0], PHI[x.k0 - 1]))
     ok["phi_hi"] = bool(x.k1 == nz or torch.equal(x.phi_ext[x.nzl + 1], PHI[x.k1]))
     ok["ranges"] = (x.kr == slab.split(nz, world)) and (x.sr == slab.split(nx // 2, world))
+    # the fluid substep's exchanges: one halo layer of four whole fields; a REAL slab field read as pairs goes to pencils,
+    # comes back and lands in another real field
+    fields = [W, PHI, 2.0 * W, W + PHI]
+    exts = [torch.zeros((x.nzl + 2, ny, nx), dtype=torch.float64) for _ in fields]
+    for e, F in zip(exts, fields):
+        e[1:x.nzl + 1].copy_(F[x.k0:x.k1])
+    comm.exchange(*x.field_halos(exts))
+    ok["halos_lo"] = all(x.k0 == 0 or torch.equal(e[0], F[x.k0 - 1]) for e, F in zip(exts, fields))
+    ok["halos_hi"] = all(x.k1 == nz or torch.equal(e[x.nzl + 1], F[x.k1]) for e, F in zip(exts, fields))
+    ok["halos_edge"] = all((x.k0 > 0 or not e[0].any()) and (x.k1 < nz or not e[x.nzl + 1].any()) for e in exts)
+    real = PHI[x.k0:x.k1].clone()
+    comm.exchange(*x.to_pencils(real.view(x.nzl, ny, nx // 2, 2)))
+    ok["real_pencil"] = torch.equal(x.pencil.reshape(nz, ny, 2 * x.nsl), PHI[:, :, 2 * x.s0:2 * x.s1])
+    x.pencil.mul_(-3.0)
+    back = torch.zeros((x.nzl, ny, nx), dtype=torch.float64)
+    comm.exchange(*x.to_slabs())
+    x.unpack_slabs(back.view(x.nzl, ny, nx // 2, 2))
+    ok["real_slab"] = torch.equal(back, -3.0 * PHI[x.k0:x.k1])
     torch.save(ok, os.path.join(out, f"r{rank}.pt"))
     dist.destroy_process_group()
 
