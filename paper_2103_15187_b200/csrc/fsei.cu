@@ -1195,13 +1195,11 @@ extern "C" int fsei_slab_forward(fsei_plan* P, const double* u, const double* v,
     if (spec == u || spec == v || spec == w) return fail(FSEI_ERR_ARG, "fsei_slab_forward: spec must not alias u, v, w");
     if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(spec)) return fail(FSEI_ERR_ARG, "fsei_slab_forward: field pointers must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const size_t n = (size_t)P->T.nx * P->T.ny * (P->k1 - P->k0);
-    { LaunchTimer t(P, K_DIV, st); k_divergence_fast<<<(unsigned)((n / 2 + 255) / 256), 256, 0, st>>>(P->S, u, v, w, 1.0 / alpha_dt, spec); }
-    CU(cudaGetLastError());
     cplx* sp = reinterpret_cast<cplx*>(spec);
-    { LaunchTimer t(P, K_XF, st); CU(launch_xf_fast(P->XF, P->S, false, false, spec, nullptr, nullptr, 0.0, sp, st)); }
+    // a1 fused into the x transform (the kernel takes the slab's plane offset and the halo plane of w from SParams)
+    { LaunchTimer t(P, K_DIVXF, st); CU(launch_xf_fast(P->XF, P->S, false, true, u, v, w, 1.0 / alpha_dt, sp, st, false)); }
     { LaunchTimer t(P, K_YF, st); CU(launch_y_fast(P->YF, false, false, sp, st)); }
-    P->last_launches = 3;
+    P->last_launches = 2;
     return FSEI_OK;
 }
 

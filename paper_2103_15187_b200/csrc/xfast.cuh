@@ -183,6 +183,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
     const bool act = j < ny;
     const int k0 = blockIdx.y * P.kchunk, k1 = (k0 + P.kchunk < nz) ? k0 + P.kchunk : nz;
     const size_t plane = (size_t)ny * n;
+    const int nzw = nz + (S.halo_hi ? 1 : 0);                     // planes of w there are: a z-slab is followed by its neighbour's first plane
     const bool yper = S.bcy == BC_PERIODIC, xper = S.bcx == BC_PERIODIC;
     const bool wrap = (j0 + nl == ny);                            // row j+1 of the last line wraps (or is a wall)
     const bool has_jp = (j + 1 < ny) || yper;
@@ -198,7 +199,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
             return;
         }
         const int nv = wrap ? nl : nl + 1;
-        const bool first = (k == k0), up = (k + 1 < nz);
+        const bool first = (k == k0), up = (k + 1 < nzw);
         unsigned total = nl * lb + nv * lb + ((wrap && yper) ? lb : 0) + (first ? nl * lb : 0) + (up ? nl * lb : 0);
         abar_expect(bar, total);
         bulk_g2s(LU, u + g0, nl * lb, bar);
@@ -209,7 +210,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
         if (k + 1 < k1) {                                          // the plane after: DRAM -> L2 now
             bulk_prefetch_l2(u + g0 + plane, nl * lb);
             bulk_prefetch_l2(v + g0 + plane, nv * lb);
-            if (k + 2 < nz) bulk_prefetch_l2(w + g0 + 2 * plane, nl * lb);
+            if (k + 2 < nzw) bulk_prefetch_l2(w + g0 + 2 * plane, nl * lb);
         }
     };
 
@@ -226,10 +227,10 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
     const double* lu = LU + li * n;
     const double* lv = LV + li * n;
 
-    double rdz_next = (FUSED && k0 < k1) ? S.rdzc[k0] : 0.0;
+    double rdz_next = (FUSED && k0 < k1) ? S.rdzc[k0 + S.kofs] : 0.0;      // (a z-slab: the metric tables are global)
     for (int k = k0; k < k1; k++) {
         const double rdz_k = rdz_next;                             // metric of this plane, loaded one plane ahead
-        if (FUSED && k + 1 < k1) rdz_next = S.rdzc[k + 1];
+        if (FUSED && k + 1 < k1) rdz_next = S.rdzc[k + 1 + S.kofs];
         abar_wait(bar, parity); parity ^= 1;
         // (rhs[2t], rhs[2t+1]) of line (j,k) from the landing tile
         auto rhs_pair = [&](int t) -> cplx {
@@ -241,7 +242,7 @@ FSEI_GLOBAL(C::T * LPB, 1) k_xf_fast(XFast P, SParams S, const double* u, const 
             cplx vv = ld2(lv + 2 * t);
             cplx vp = has_jp ? ld2(lv + n + 2 * t) : cmake(0.0, 0.0);
             cplx wk = ld2(lwk + 2 * t);
-            cplx wp = (k + 1 < nz) ? ld2(lwp + 2 * t) : cmake(0.0, 0.0);
+            cplx wp = (k + 1 < nzw) ? ld2(lwp + 2 * t) : cmake(0.0, 0.0);
             const double rdz = rdz_k;
             return cmake(div_cell(uu.re, uu.im, vv.re, vp.re, wk.re, wp.re, S.rdx, S.rdy, rdz, inv_adt),
                          div_cell(uu.im, un, vv.im, vp.im, wk.im, wp.im, S.rdx, S.rdy, rdz, inv_adt));

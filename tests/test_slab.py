@@ -123,7 +123,7 @@ def test_decomposed_projection_vs_single_plan_and_oracle(oracle_ld, world, shape
     slab.project_local(ranks, case.alpha_dt, beta)
     torch.cuda.synchronize()
     got = [np.concatenate([getattr(r, f).cpu().numpy() for r in ranks], axis=0) for f in ("u", "v", "w", "p", "phi")]
-    assert ranks[0].launches == 8 and all(r.launches == 7 for r in ranks[1:])      # 3 + 1 + 2 + 1; rank 0 also solves the gauge column
+    assert ranks[0].launches == 7 and all(r.launches == 6 for r in ranks[1:])      # 2 + 1 + 2 + 1; rank 0 also solves the gauge column
     ref = oracle_projection(oracle_ld, case, beta)
     assert rel_l2(got[4], ref[4]) <= 1e-11
     for g, r in zip(got[:4], ref[:4]):
