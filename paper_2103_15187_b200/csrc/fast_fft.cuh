@@ -1,7 +1,7 @@
 // fast_fft.cuh -- register-resident Stockham passes shared by the fast x and y transforms.
 //
 // Fast path (lengths 2^a and 3*2^a, a line of N complex values): N = R0 R1 R2 with radices from
-// {2,4,6,8,16}.  Pass s with Ns = R0..R_{s-1}: butterfly b in [0, N/R) reads elements b + q N/R
+// {2,4,5,6,8,10,12,16}.  Pass s with Ns = R0..R_{s-1}: butterfly b in [0, N/R) reads elements b + q N/R
 // (q < R), multiplies element q by w_{Ns R}^{q (b mod Ns)}, takes the R-point DFT in registers and
 // writes output q to (b / Ns) Ns R + (b mod Ns) + q Ns  (Stockham autosort: natural order in, natural
 // order out, every pass reads with unit stride across threads).  The first pass reads global memory
@@ -25,6 +25,47 @@ template <bool INV> struct SmallDft<6, INV> {
         o[2] = ctw<INV>(o[2], -0.5, -FSEI_SQRT3_2);
 #pragma unroll
         for (int k = 0; k < 3; k++) { v[k] = cadd(e[k], o[k]); v[k + 3] = csub(e[k], o[k]); }
+    }
+};
+
+// 10 = 5 x 2:  n = 2 n1 + n2,  k = k1 + 5 k2
+#define FSEI_COS_PI_5 0.80901699437494742410229341718281905886
+#define FSEI_SIN_PI_5 0.58778525229247312916870595463907276860
+template <bool INV> struct SmallDft<10, INV> {
+    static FSEI_HD void run(cplx* v) {
+        cplx e[5] = {v[0], v[2], v[4], v[6], v[8]}, o[5] = {v[1], v[3], v[5], v[7], v[9]};
+        SmallDft<5, INV>::run(e); SmallDft<5, INV>::run(o);
+        o[1] = ctw<INV>(o[1], FSEI_COS_PI_5, -FSEI_SIN_PI_5);
+        o[2] = ctw<INV>(o[2], FSEI_COS_2PI_5, -FSEI_SIN_2PI_5);
+        o[3] = ctw<INV>(o[3], -FSEI_COS_2PI_5, -FSEI_SIN_2PI_5);
+        o[4] = ctw<INV>(o[4], -FSEI_COS_PI_5, -FSEI_SIN_PI_5);
+#pragma unroll
+        for (int k = 0; k < 5; k++) { v[k] = cadd(e[k], o[k]); v[k + 5] = csub(e[k], o[k]); }
+    }
+};
+
+// 12 = 3 x 4:  n = 4 n1 + n2,  k = k1 + 3 k2
+template <bool INV> struct SmallDft<12, INV> {
+    static FSEI_HD void run(cplx* v) {
+        cplx y[4][3];                                  // y[n2][k1]
+#pragma unroll
+        for (int n2 = 0; n2 < 4; n2++) {
+            cplx t[3] = {v[n2], v[4 + n2], v[8 + n2]};
+            SmallDft<3, INV>::run(t);
+#pragma unroll
+            for (int k1 = 0; k1 < 3; k1++) y[n2][k1] = t[k1];
+        }
+        // twiddles w12^{n2 k1}
+        y[1][1] = ctw<INV>(y[1][1], FSEI_SQRT3_2, -0.5);  y[1][2] = ctw<INV>(y[1][2], 0.5, -FSEI_SQRT3_2);
+        y[2][1] = ctw<INV>(y[2][1], 0.5, -FSEI_SQRT3_2);  y[2][2] = ctw<INV>(y[2][2], -0.5, -FSEI_SQRT3_2);
+        y[3][1] = crot<INV>(y[3][1]);                     y[3][2] = cmake(-y[3][2].re, -y[3][2].im);
+#pragma unroll
+        for (int k1 = 0; k1 < 3; k1++) {
+            cplx t[4] = {y[0][k1], y[1][k1], y[2][k1], y[3][k1]};
+            SmallDft<4, INV>::run(t);
+#pragma unroll
+            for (int k2 = 0; k2 < 4; k2++) v[k1 + 3 * k2] = t[k2];
+        }
     }
 };
 

@@ -31,13 +31,13 @@ def test_fast_kernels_match_oracle(oracle_ld, bc, shape):
 
 
 # every x line length (nx = 2 N) and every y column length with an instantiation, both transforms types
-@pytest.mark.parametrize("nx", [32, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 2048, 160, 320, 640, 1280])
+@pytest.mark.parametrize("nx", [32, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 2048, 160, 320, 640, 1280, 480, 576, 960, 1152])
 def test_every_x_length(oracle_ld, nx):
     for bc in ((P, P), (N, N)):
         _check(oracle_ld, (nx, 16, 2), bc)
 
 
-@pytest.mark.parametrize("ny", [16, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 80, 160, 320, 640, 1280])
+@pytest.mark.parametrize("ny", [16, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 80, 160, 320, 640, 1280, 240, 288, 480, 576, 960, 1152])
 def test_every_y_length(oracle_ld, ny):
     for bc in ((P, P), (N, N), (N, P)):
         _check(oracle_ld, (32, ny, 2), bc)

@@ -254,7 +254,7 @@ def fused_path(monkeypatch):
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N), (P, N), (N, P)])
 @pytest.mark.parametrize("shape", [(512, 384, 9), (768, 512, 6), (512, 768, 5), (2048, 1024, 3), (32, 32, 33), (64, 16, 9),
-                                   (96, 48, 40), (320, 160, 9), (640, 640, 5), (1280, 1280, 3)])
+                                   (96, 48, 40), (320, 160, 9), (640, 640, 5), (1280, 1280, 3), (576, 480, 5), (960, 576, 4)])
 def test_fused_path_small(oracle_ld, fused_path, monkeypatch, bc, shape):
     from paper_2103_15187_b200.binding import Plan
     for cfg, beta in ((1, 0.0), (2, 1e-4)):
@@ -324,9 +324,11 @@ def test_fused_is_the_default_on_large_grids():
 
 @pytest.mark.parametrize("bc", [(P, P), (N, N)])
 @pytest.mark.parametrize("shape,family", [((320, 160, 9), 1), ((640, 320, 5), 1), ((1280, 640, 3), 2), ((160, 1280, 4), 1), ((320, 80, 6), 1),
-                                          ((640, 640, 7), 2)])
+                                          ((640, 640, 7), 2), ((480, 240, 6), 1), ((576, 288, 5), 1), ((960, 480, 4), 2),
+                                          ((1152, 576, 3), 2), ((576, 480, 5), 2), ((960, 960, 3), 2), ((1152, 1152, 3), 2), ((480, 960, 4), 1)])
 def test_factor5_lengths_take_the_register_resident_families(oracle_ld, shape, family, bc):
-    """nx/2 in {80, 160, 320, 640}, ny in {80, ..., 1280}: Stockham passes with a radix-5 last pass; 1 = fast, 2 = fused (blocked
+    """nx/2 in {80, 160, 320, 640}, ny in {80, ..., 1280}: Stockham passes with a radix-5 last pass; nx/2, ny in {240, 288, 480,
+    576}: radices (8 | 16, 6, 5 | 6); ny in {960, 1152}: (16, 6, 10 | 12); 1 = fast, 2 = fused (blocked
     layout, from 128 x-slot tiles on, where both lengths have a fused instantiation)."""
     case = inputs.make_case(2, shape=shape, bc=bc)
     plan = make_plan(case.grid)
