@@ -8,8 +8,8 @@
 namespace fsei {
 
 // chunk lengths with an instantiation: pass A needs M % 4 == 0 (conflict-free 128-bit slots; 2 for small test grids)
-#define FSEI_VA_LIST(X) X(2) X(4) X(8) X(12) X(16) X(24) X(32) X(10) X(20)
-#define FSEI_VB_LIST(X) X(2) X(3) X(4) X(6) X(8) X(12) X(16) X(24) X(32) X(5) X(10) X(20)
+#define FSEI_VA_LIST(X) X(2) X(4) X(8) X(12) X(16) X(24) X(32) X(10) X(20) X(18) X(30)
+#define FSEI_VB_LIST(X) X(2) X(3) X(4) X(6) X(8) X(12) X(16) X(24) X(32) X(5) X(10) X(20) X(18) X(30)
 
 bool visc_fast_supported(int nx, int ny)
 {

@@ -176,7 +176,7 @@ def test_fluid_error_codes():
 # fast family of the viscous step (periodic x, y; partition solves in registers; two fused launches)
 # ---------------------------------------------------------------------------------------------
 FAST_SHAPES = [(64, 64, 9), (128, 96, 12), (256, 192, 7), (384, 256, 5), (512, 384, 5), (768, 512, 4), (1024, 768, 3),
-               (1024, 1024, 2), (64, 1024, 40), (1024, 64, 33), (320, 160, 6), (640, 640, 4), (640, 320, 3)]
+               (1024, 1024, 2), (64, 1024, 40), (1024, 64, 33), (320, 160, 6), (640, 640, 4), (640, 320, 3), (576, 576, 4), (960, 576, 3), (576, 960, 3)]
 
 
 @pytest.mark.parametrize("shape", FAST_SHAPES)
