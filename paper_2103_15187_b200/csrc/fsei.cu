@@ -1084,7 +1084,7 @@ static int slab_plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, doub
     std::string msg = build_tables(P->T, nx, ny, nz, Lx, Ly, zc, bcx, bcy, code, true);
     if (code) return fail(code, msg);
     if (!(xfast_supported(nx / 2) && yfast_supported(ny) && (size_t)nz * 4 * sizeof(cplx) <= 200 * 1024))
-        return fail(FSEI_ERR_SIZE, "fsei_slab_plan_create: nx/2 and ny need a register-resident transform (16..1024, 3*2^a up to 768), nz <= 3200");
+        return fail(FSEI_ERR_SIZE, "fsei_slab_plan_create: nx/2 and ny need a register-resident transform (the lengths of the fast family: DESIGN.md sec. 1), nz <= 3200");
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FSEI_ERR_CUDA, "no CUDA device: libfsei has no CPU fallback"); }
