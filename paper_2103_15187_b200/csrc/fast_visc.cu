@@ -132,7 +132,7 @@ static cudaError_t field_map(const VFastArgs& A, int box_rows, double* f, TmaMap
 
 cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st)
 {
-    const dim3 grid(A.nx / 8);
+    const dim3 grid(A.split ? 3 * (A.nx / 8) : A.nx / 8);
     VFastMaps Mp;
     Mp.box_rows = 256;
     while (A.ny % Mp.box_rows) Mp.box_rows--;                   // largest divisor of ny that fits a TMA box

@@ -42,6 +42,7 @@ struct VFastArgs {
     double* q[3];               // velocity components (pass B)
     int nx, ny, nz;
     int nsig;                   // terms of sinv kept on either side of s = 0 (16 = all)
+    int split;                  // pass B: 1 = one CTA per (tile, component) instead of one per tile (host: grids with few tiles)
 };
 
 #if defined(__CUDACC__)
@@ -178,11 +179,16 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
     double* tile0 = reinterpret_cast<double*>(smraw + 128);     // [2][NY][8]
     double* carry = tile0 + 2 * NY * 8 + threadIdx.x;           // [M][256]
     const int tid = threadIdx.x, i = tid & 7, c = tid >> 3;
-    const int col0 = blockIdx.x * 8, nb = NY / Mp.box_rows, nz = A.nz, nit = 3 * nz;
+    // one CTA per tile of 8 columns walking u, v, w in turn -- all CTAs then sit on the same plane of the same field, which is what
+    // keeps the 64-byte rows of neighbouring tiles in open DRAM pages -- or, where that leaves SMs idle (up to 1.5 marches per SM), one CTA
+    // per (tile, component).  (Dealing the marches out in equal item ranges with carry hand-offs was tried: the CTAs drift apart
+    // in k and large grids lose half their bandwidth.)
+    const int col0 = (A.split ? blockIdx.x / 3 : blockIdx.x) * 8, comp0 = A.split ? blockIdx.x % 3 : 0;
+    const int nb = NY / Mp.box_rows, nz = A.nz, nit = (A.split ? 1 : 3) * nz;
     const VFastLine& L = A.L;
     // items it = comp * nz + (nz - 1 - k): the tile walks down each component in turn; item it uses tile it & 1
     auto issue = [&](int it) {
-        const int cc = it / nz, k = nz - 1 - (it - cc * nz);
+        const int ci = it / nz, k = nz - 1 - (it - ci * nz), cc = comp0 + ci;
         double* t = tile0 + (it & 1) * NY * 8;
         abar_expect(bar + (it & 1), (unsigned)(NY * 64));
         for (int b = 0; b < nb; b++) tma_load_2d(t + b * Mp.box_rows * 8, &Mp.d[cc], col0, k * NY + b * Mp.box_rows, bar + (it & 1));
@@ -191,7 +197,7 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
     __syncthreads();
     if (tid == 0) issue(0);
     for (int it = 0; it < nit; it++) {
-        const int comp = it / nz, k = nz - 1 - (it - comp * nz), pb = it & 1;
+        const int ci = it / nz, k = nz - 1 - (it - ci * nz), comp = comp0 + ci, pb = it & 1;
         double* tl = tile0 + pb * NY * 8 + (c * M) * 8 + i;
         if (tid == 0 && it + 1 < nit) { bulk_wait_read<0>(); issue(it + 1); }   // the other tile: its reduce-store has been read out
         abar_wait(bar + pb, (it >> 1) & 1);
