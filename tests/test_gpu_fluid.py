@@ -344,3 +344,69 @@ def test_config4_full_size_fluid_rows(oracle_ld):
         assert err <= 1e-12 * scale + 2 * EPS * q0max[c], c
         del got
     plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# degenerate and extreme cases of the fluid rows
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,bc", [((8192, 4, 3), (P, P)), ((4, 8192, 3), (P, P)), ((8192, 4, 3), (W, W)), ((4, 4, 2), (P, P)),
+                                      ((4, 4, 2), (W, W)), ((8, 6, 1025), (P, W))])
+def test_fluid_rows_at_extreme_sizes(oracle_ld, shape, bc):
+    """the longest lines the plan accepts (8192), the smallest grid (4 x 4 x 2), a column longer than any other test's: explicit
+    terms bit-exact, viscous step to rounding"""
+    import torch
+    g, f = _case(shape, bc, seed=46, n=7)
+    u, v, w, p, h0, h1, h2 = f
+    gdt, rdt, adt, beta = 1.5e-3, -0.5e-3, 1e-3, 2e-3
+    ho = [h0.copy(), h1.copy(), h2.copy()]
+    ro = oracle_ld.explicit_terms(g, u, v, w, p, *ho, gdt, rdt, adt, beta)
+    plan = _plan(g)
+    d = _dev(f)
+    dr = [torch.empty_like(d[0]) for _ in range(3)]
+    plan.explicit_terms(*d, *dr, gdt, rdt, adt, beta)
+    torch.cuda.synchronize()
+    for c in range(3):
+        assert np.array_equal(dr[c].cpu().numpy(), ro[c]), ("rhs", c)
+        assert np.array_equal(d[4 + c].cpu().numpy(), ho[c]), ("H", c)
+    uo, vo, wo = u.copy(), v.copy(), w.copy()
+    oracle_ld.viscous_step(g, uo, vo, wo, *ro, beta)
+    plan.viscous_step(d[0], d[1], d[2], *dr, beta)
+    torch.cuda.synchronize()
+    for c, (q0, qo) in enumerate(((u, uo), (v, vo), (w, wo))):
+        assert np.abs(d[c].cpu().numpy() - qo).max() <= 1e-12 * np.abs(qo - q0).max() + 2 * EPS * np.abs(qo).max(), c
+    plan.destroy()
+
+
+@pytest.mark.parametrize("shape", [(64, 64, 9), (36, 16, 33)])
+def test_fluid_rows_degenerate_inputs(shape):
+    """beta = 0: the implicit operator is the identity, q += r exactly (both families).  u = v = w = 0, p = const: H = 0 and the rhs
+    is exactly alpha dt f (0 without a force); rho dt Hprev passes through."""
+    import torch
+    from paper_2103_15187_b200 import binding
+    g, f = _case(shape, (P, P), seed=47, n=9)
+    for flags in (0, binding.VISC_GENERIC):
+        plan = binding.Plan.from_grid(g, flags)
+        d = _dev(f[:6])
+        want = [d[c] + d[3 + c] for c in range(3)]
+        want[2][0] = d[2][0]                                                       # the wall face of w is a fixed row (V7)
+        plan.viscous_step(*d, 0.0)
+        torch.cuda.synchronize()
+        for c in range(3):
+            assert torch.equal(d[c], want[c]), (flags, c)
+        plan.destroy()
+    plan = _plan(g)
+    z = [torch.zeros(f[0].shape, dtype=torch.float64, device="cuda:0") for _ in range(3)]
+    p = torch.full_like(z[0], 3.25)
+    hp = _dev(f[3:6])
+    force = _dev(f[6:9])
+    r = [torch.empty_like(z[0]) for _ in range(3)]
+    hprev = [t.clone() for t in hp]
+    plan.explicit_terms(*z, p, *hp, *r, 1.5e-3, -0.5e-3, 1e-3, 1e-4, f=tuple(force))
+    torch.cuda.synchronize()
+    for c in range(3):
+        assert not bool(hp[c].any()), c                                           # H = 0
+        want = (-0.5e-3 * hprev[c]) + 1e-3 * force[c]
+        if c == 2:
+            want[0] = 0                                                           # the wall face of w
+        assert torch.equal(r[c], want), c
+    plan.destroy()
