@@ -126,6 +126,13 @@ static int dalloc(fsei_plan* P, size_t n, void** d)
 // ------------------------------------------------------------------------------------------
 #define NT 256
 
+// generic family: CTAs per SM the FORWARD transform kernels are compiled for (they would take 148 registers = one CTA per SM; the
+// inverse ones fit two as they are and lose when squeezed) -- with the shared-memory carve-out of the forward kernels set to its
+// maximum in plan_build, or the driver's default admits ONE 28-64 KB tile per SM (the inverse kernels get two by default and
+// want their L1: with the maximum carve-out y_inverse goes from 4.9 to 7.5 ms at configs[3])
+#ifndef FSEI_GEN_MINB
+#define FSEI_GEN_MINB 2
+#endif
 template <bool INV> __device__ __forceinline__ void x_all_passes(const XParams& X, cplx* sm, int lines)
 {
     int Ns[8]; int n = X.N;
@@ -138,7 +145,7 @@ template <bool INV> __device__ __forceinline__ void x_all_passes(const XParams& 
     }
 }
 
-__global__ void __launch_bounds__(NT) k_x_forward(XParams X, const double* src, cplx* dst, long nlines, int LX)
+__global__ void __launch_bounds__(NT, FSEI_GEN_MINB) k_x_forward(XParams X, const double* src, cplx* dst, long nlines, int LX)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
     cplx* sm = reinterpret_cast<cplx*>(smraw);
@@ -180,7 +187,7 @@ template <bool INV, bool NEU> __device__ __forceinline__ void y_all_passes(const
 
 // grid (nxc / C, nz): one tile = C adjacent slots of every row of one z-plane
 template <bool INV, bool NEU>
-__global__ void __launch_bounds__(NT) k_y_transform(YParams Y, cplx* spec, int nxc, int C)
+__global__ void __launch_bounds__(NT, (INV ? 0 : FSEI_GEN_MINB)) k_y_transform(YParams Y, cplx* spec, int nxc, int C)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
     cplx* sm = reinterpret_cast<cplx*>(smraw);
@@ -418,10 +425,13 @@ static int plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, double Ly
     P->CY = CY; P->smem_y = (size_t)ny * CY * sizeof(cplx);
     CU(cudaFuncSetAttribute(k_z_gauge, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * sizeof(double) * nz)));
     CU(cudaFuncSetAttribute(k_x_forward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_x));
+    CU(cudaFuncSetAttribute(k_x_forward, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     CU(cudaFuncSetAttribute(k_x_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_x));
     CU(cudaFuncSetAttribute(k_y_transform<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
+    CU(cudaFuncSetAttribute(k_y_transform<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     CU(cudaFuncSetAttribute(k_y_transform<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
     CU(cudaFuncSetAttribute(k_y_transform<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
+    CU(cudaFuncSetAttribute(k_y_transform<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     CU(cudaFuncSetAttribute(k_y_transform<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->smem_y));
     return FSEI_OK;
 }
