@@ -80,7 +80,12 @@ FSEI_DEV void mls_stencil(const MlsGrid& G, int comp, double xb, double yb, doub
         ii[d] = i; jj[d] = j;
     }
     // weights and the moment matrix A = sum W p p^T (symmetric, p = [1, xi, eta, zeta])
+    // the weight exp(-(xi^2 + eta^2 + zeta^2) / (1.5 eps)^2) is a product of three one-dimensional factors: 9 exponentials per
+    // (marker, component) instead of 27 (the product differs from the exponential of the sum by rounding only: ~2 ulp)
     const double inv = 1.0 / (1.5 * 1.5 * 0.3 * 0.3);
+    double wx[3], wy[3], wz[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) { wx[d] = exp(-(xi[d] * xi[d]) * inv); wy[d] = exp(-(et[d] * et[d]) * inv); wz[d] = exp(-(ze[d] * ze[d]) * inv); }
     double a00 = 0, a01 = 0, a02 = 0, a03 = 0, a11 = 0, a12 = 0, a13 = 0, a22 = 0, a23 = 0, a33 = 0;
 #pragma unroll
     for (int dk = 0; dk < 3; dk++)
@@ -89,7 +94,7 @@ FSEI_DEV void mls_stencil(const MlsGrid& G, int comp, double xb, double yb, doub
 #pragma unroll
             for (int di = 0; di < 3; di++) {
                 const int s = (dk * 3 + dj) * 3 + di;
-                const double W = exp(-(xi[di] * xi[di] + et[dj] * et[dj] + ze[dk] * ze[dk]) * inv);
+                const double W = wx[di] * (wy[dj] * wz[dk]);
                 M.phi[s] = W;
                 a00 += W; a01 += W * xi[di]; a02 += W * et[dj]; a03 += W * ze[dk];
                 a11 += W * xi[di] * xi[di]; a12 += W * xi[di] * et[dj]; a13 += W * xi[di] * ze[dk];
