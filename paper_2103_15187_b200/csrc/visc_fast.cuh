@@ -155,6 +155,101 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// pass A through tensor maps (chunk lengths 16 and 32, i.e. nx = 512 and 1024): a line is the 2-D array [32 chunks][M doubles];
+// boxes of (16 doubles = 128 bytes) x 32 chunks land with the 128-byte swizzle, which puts the 16-byte piece i of chunk l at
+// piece i ^ (l & 7) of its row, so that the 32 lanes -- each reading ITS chunk with 128-bit loads -- fall on all banks.  Two
+// TMA instructions per line and direction instead of 32 bulk copies issued lane by lane (a warp-serial loop that took half
+// of k_visc_xz's stall samples).  Same arithmetic as k_visc_xz.  Dynamic shared memory: 1024 + WPB * (S * 256 M + 64) bytes.
+// ---------------------------------------------------------------------------------------------------------------
+struct VFastMapsA { TmaMap2D r[3]; };      // per component: fp64 [32 ny nz rows][M], box 16 x 32, CU_TENSOR_MAP_SWIZZLE_128B
+
+__device__ __forceinline__ void tma_store_2d(const TmaMap2D* map, int x0, int y0, const void* src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(map), "r"(x0), "r"(y0), "r"(smem_u32(src)) : "memory");
+}
+
+template <int M>
+FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_GRID_CONSTANT VFastMapsA Mp)
+{
+    static_assert(M % 16 == 0, "whole 128-byte boxes");
+    constexpr int S = FSEI_VA_STAGES, NBOX = M / 16, STAGE = NBOX * 4096;
+    FSEI_DYN_SMEM(smraw);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, comp = blockIdx.y;
+    const int j = blockIdx.x * FSEI_VA_WPB + wid;
+    if (j >= A.ny) return;
+    unsigned char* base = smraw + ((1024u - (smem_u32(smraw) & 1023u)) & 1023u);       // the swizzle pattern repeats every 1024 bytes
+    unsigned char* buf = base + (size_t)wid * (S * STAGE);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(base + (size_t)FSEI_VA_WPB * S * STAGE) + wid * 8;
+    const double* __restrict__ zam = A.zam[comp];
+    const double* __restrict__ zip = A.zip[comp];
+    const VFastLine& L = A.L;
+    const int nz = A.nz, nsig = A.nsig, ny = A.ny;
+    const TmaMap2D* map = &Mp.r[comp];
+    auto load_line = [&](int s, int k) {             // plane k of line j -> stage s (lane 0)
+        abar_expect(bar + s, 32 * 8 * M);
+#pragma unroll
+        for (int h = 0; h < NBOX; h++) tma_load_2d(buf + s * STAGE + h * 4096, map, 16 * h, (k * ny + j) * 32, bar + s);
+    };
+    if (lane == 0) for (int s = 0; s < S; s++) abar_init(bar + s);
+    __syncwarp();
+    if (lane == 0) for (int s = 0; s < S - 1 && s < nz; s++) load_line(s, s);          // prologue: planes 0 .. S-2 in flight
+    double dprev[M];
+#pragma unroll
+    for (int i = 0; i < M; i++) dprev[i] = 0.0;
+    const bool wfix = comp == COMP_W;                                       // w: plane 0 is the wall (row fixed)
+    int st = 0; unsigned par = 0;
+    const int sw = lane & 7;
+    for (int k = 0; k < nz; k++) {
+        abar_wait(bar + st, par);
+        double x[M];
+        unsigned char* row = buf + st * STAGE + lane * 128;
+#pragma unroll
+        for (int h = 0; h < NBOX; h++)
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+                const double2 t = *reinterpret_cast<const double2*>(row + h * 4096 + ((i ^ sw) << 4));
+                x[16 * h + 2 * i] = t.x; x[16 * h + 2 * i + 1] = t.y;
+            }
+        // ---- periodic x-solve of the line
+        const double sep = x[M - 1];
+        chunk_interior<M>(L, x);
+        const double y0n = __shfl_sync(0xffffffffu, x[0], (lane + 1) & 31);
+        const double g = fma(L.r, x[M - 2] + y0n, sep);
+        double xs = L.sinv[0] * g;
+        for (int s = 1; s <= nsig; s++) {
+            const double gm = __shfl_sync(0xffffffffu, g, (lane - s) & 31), gp = __shfl_sync(0xffffffffu, g, (lane + s) & 31);
+            xs = fma(L.sinv[s], s == 16 ? gm : gm + gp, xs);
+        }
+        const double xl = __shfl_sync(0xffffffffu, xs, (lane - 1) & 31);
+        chunk_correct<M>(L, x, xl, xs);
+        // ---- forward elimination of the z system: d'_k = (x_k - a_k d'_{k-1}) / piv_k
+        const double am = zam[k], ipk = zip[k];
+        const bool zero = wfix && k == 0;
+#pragma unroll
+        for (int i = 0; i < M; i++) dprev[i] = zero ? 0.0 : fma(-am, dprev[i], x[i]) * ipk;
+        // ---- out: through the same slot
+#pragma unroll
+        for (int h = 0; h < NBOX; h++)
+#pragma unroll
+            for (int i = 0; i < 8; i++)
+                *reinterpret_cast<double2*>(row + h * 4096 + ((i ^ sw) << 4)) = make_double2(dprev[16 * h + 2 * i], dprev[16 * h + 2 * i + 1]);
+        fence_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+#pragma unroll
+            for (int h = 0; h < NBOX; h++) tma_store_2d(map, 16 * h, (k * ny + j) * 32, buf + st * STAGE + h * 4096);
+            bulk_commit();
+            // ---- next load into the slot of plane k-1 once its store has been read out
+            if (k + S - 1 < nz) { bulk_wait_read<1>(); load_line(st == 0 ? S - 1 : st - 1, k + S - 1); }
+        }
+        if (++st == S) { st = 0; par ^= 1u; }
+    }
+    if (lane == 0) bulk_wait_all<0>();
+    __syncwarp();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // pass B: grid nx / 8, block 256 (the CTA walks its tile through u, v, w): thread = (column i = tid & 7, chunk c = tid >> 3).
 // The (ny x 8) tile of d' of plane k-1 lands by 2-D TMA boxes in one of two shared-memory tiles while plane k is being
 // solved in the other; the result goes back into its tile and leaves as a TMA REDUCE-ADD onto q (the addition q + dq is
