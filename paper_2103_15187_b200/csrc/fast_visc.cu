@@ -28,7 +28,7 @@ static size_t vb_smem(int M) { return 128 + (size_t)2 * 32 * M * 64 + (size_t)M 
 static size_t va_smem(int M) { return (size_t)FSEI_VA_WPB * (FSEI_VA_STAGES * 32 * (8 * M + 16) + 64); }
 static size_t va_tma_smem(int M) { return 1024 + (size_t)FSEI_VA_WPB * (FSEI_VA_STAGES * 256 * M + 64); }
 #ifndef FSEI_VA_TMA
-#define FSEI_VA_TMA 1               // chunk lengths 16 and 32 take the tensor-map variant of pass A
+#define FSEI_VA_TMA 1               // chunk lengths 8, 16, 24, 32 take the tensor-map variant of pass A
 #endif
 
 cudaError_t visc_fast_init()
@@ -37,7 +37,9 @@ cudaError_t visc_fast_init()
 #define X(M) if (e == cudaSuccess) e = kernel_smem(k_visc_xz<M>, (int)va_smem(M));
     FSEI_VA_LIST(X)
 #undef X
+    if (e == cudaSuccess) e = kernel_smem(k_visc_xz_tma<8>, (int)va_tma_smem(8));
     if (e == cudaSuccess) e = kernel_smem(k_visc_xz_tma<16>, (int)va_tma_smem(16));
+    if (e == cudaSuccess) e = kernel_smem(k_visc_xz_tma<24>, (int)va_tma_smem(24));
     if (e == cudaSuccess) e = kernel_smem(k_visc_xz_tma<32>, (int)va_tma_smem(32));
 #define X(M) if (e == cudaSuccess) e = kernel_smem(k_visc_zy<M>, (int)vb_smem(M));
     FSEI_VB_LIST(X)
@@ -114,20 +116,25 @@ cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st)
 {
     const dim3 grid((A.ny + FSEI_VA_WPB - 1) / FSEI_VA_WPB, 3);
     const int M = A.nx / 32;
-    if (FSEI_VA_TMA && (M == 16 || M == 32) && (size_t)32 * A.ny * A.nz < (1ull << 31)) {
+    if (FSEI_VA_TMA && M % 8 == 0 && M <= 32 && (size_t)32 * A.ny * A.nz < (1ull << 31)) {
         EncodeTiledFn fn = tma_encode_fn();
         if (!fn) return cudaErrorNotSupported;
         VFastMapsA Mp;
         for (int c = 0; c < 3; c++) {                               // the field as [32 ny nz chunks][M doubles]
             cuuint64_t dims[2] = {(cuuint64_t)M, (cuuint64_t)32 * A.ny * A.nz};
             cuuint64_t strides[1] = {(cuuint64_t)M * sizeof(double)};
-            cuuint32_t box[2] = {16u, 32u}, estr[2] = {1, 1};
+            const bool wide = M % 16 == 0;                        // 128-byte boxes and swizzle, else 64-byte
+            cuuint32_t box[2] = {wide ? 16u : 8u, 32u}, estr[2] = {1, 1};
             if (fn(&Mp.r[c].m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, A.r[c], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                   wide ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return cudaErrorInvalidValue;
         }
-        if (M == 16) k_visc_xz_tma<16><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(16), st>>>(A, Mp);
-        else k_visc_xz_tma<32><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(32), st>>>(A, Mp);
+        switch (M) {
+            case 8: k_visc_xz_tma<8><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(8), st>>>(A, Mp); break;
+            case 16: k_visc_xz_tma<16><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(16), st>>>(A, Mp); break;
+            case 24: k_visc_xz_tma<24><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(24), st>>>(A, Mp); break;
+            default: k_visc_xz_tma<32><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(32), st>>>(A, Mp); break;
+        }
         return cudaGetLastError();
     }
     switch (A.nx / 32) {

@@ -155,7 +155,7 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// pass A through tensor maps (chunk lengths 16 and 32, i.e. nx = 512 and 1024): a line is the 2-D array [32 chunks][M doubles];
+// pass A through tensor maps (chunk lengths 8, 16, 24, 32, i.e. nx = 256, 512, 768, 1024): a line is the 2-D array [32 chunks][M doubles];
 // boxes of (16 doubles = 128 bytes) x 32 chunks land with the 128-byte swizzle, which puts the 16-byte piece i of chunk l at
 // piece i ^ (l & 7) of its row, so that the 32 lanes -- each reading ITS chunk with 128-bit loads -- fall on all banks.  Two
 // TMA instructions per line and direction instead of 32 bulk copies issued lane by lane (a warp-serial loop that took half
@@ -172,8 +172,10 @@ __device__ __forceinline__ void tma_store_2d(const TmaMap2D* map, int x0, int y0
 template <int M>
 FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_GRID_CONSTANT VFastMapsA Mp)
 {
-    static_assert(M % 16 == 0, "whole 128-byte boxes");
-    constexpr int S = FSEI_VA_STAGES, NBOX = M / 16, STAGE = NBOX * 4096;
+    static_assert(M % 8 == 0, "whole 64- or 128-byte boxes");
+    // box width: 16 doubles with the 128-byte swizzle where M allows it, else 8 doubles with the 64-byte swizzle (there the 16-byte
+    // piece i of chunk l sits at piece i ^ ((l >> 1) & 3))
+    constexpr int S = FSEI_VA_STAGES, BW = (M % 16 == 0) ? 16 : 8, CH = BW / 2, ROWB = 8 * BW, BOXB = 32 * ROWB, NBOX = M / BW, STAGE = NBOX * BOXB;
     FSEI_DYN_SMEM(smraw);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, comp = blockIdx.y;
     const int j = blockIdx.x * FSEI_VA_WPB + wid;
@@ -189,7 +191,7 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArg
     auto load_line = [&](int s, int k) {             // plane k of line j -> stage s (lane 0)
         abar_expect(bar + s, 32 * 8 * M);
 #pragma unroll
-        for (int h = 0; h < NBOX; h++) tma_load_2d(buf + s * STAGE + h * 4096, map, 16 * h, (k * ny + j) * 32, bar + s);
+        for (int h = 0; h < NBOX; h++) tma_load_2d(buf + s * STAGE + h * BOXB, map, BW * h, (k * ny + j) * 32, bar + s);
     };
     if (lane == 0) for (int s = 0; s < S; s++) abar_init(bar + s);
     __syncwarp();
@@ -199,17 +201,17 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArg
     for (int i = 0; i < M; i++) dprev[i] = 0.0;
     const bool wfix = comp == COMP_W;                                       // w: plane 0 is the wall (row fixed)
     int st = 0; unsigned par = 0;
-    const int sw = lane & 7;
+    const int sw = BW == 16 ? (lane & 7) : ((lane >> 1) & 3);
     for (int k = 0; k < nz; k++) {
         abar_wait(bar + st, par);
         double x[M];
-        unsigned char* row = buf + st * STAGE + lane * 128;
+        unsigned char* row = buf + st * STAGE + lane * ROWB;
 #pragma unroll
         for (int h = 0; h < NBOX; h++)
 #pragma unroll
-            for (int i = 0; i < 8; i++) {
-                const double2 t = *reinterpret_cast<const double2*>(row + h * 4096 + ((i ^ sw) << 4));
-                x[16 * h + 2 * i] = t.x; x[16 * h + 2 * i + 1] = t.y;
+            for (int i = 0; i < CH; i++) {
+                const double2 t = *reinterpret_cast<const double2*>(row + h * BOXB + ((i ^ sw) << 4));
+                x[BW * h + 2 * i] = t.x; x[BW * h + 2 * i + 1] = t.y;
             }
         // ---- periodic x-solve of the line
         const double sep = x[M - 1];
@@ -232,13 +234,13 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArg
 #pragma unroll
         for (int h = 0; h < NBOX; h++)
 #pragma unroll
-            for (int i = 0; i < 8; i++)
-                *reinterpret_cast<double2*>(row + h * 4096 + ((i ^ sw) << 4)) = make_double2(dprev[16 * h + 2 * i], dprev[16 * h + 2 * i + 1]);
+            for (int i = 0; i < CH; i++)
+                *reinterpret_cast<double2*>(row + h * BOXB + ((i ^ sw) << 4)) = make_double2(dprev[BW * h + 2 * i], dprev[BW * h + 2 * i + 1]);
         fence_async_smem();
         __syncwarp();
         if (lane == 0) {
 #pragma unroll
-            for (int h = 0; h < NBOX; h++) tma_store_2d(map, 16 * h, (k * ny + j) * 32, buf + st * STAGE + h * 4096);
+            for (int h = 0; h < NBOX; h++) tma_store_2d(map, BW * h, (k * ny + j) * 32, buf + st * STAGE + h * BOXB);
             bulk_commit();
             // ---- next load into the slot of plane k-1 once its store has been read out
             if (k + S - 1 < nz) { bulk_wait_read<1>(); load_line(st == 0 ? S - 1 : st - 1, k + S - 1); }
