@@ -26,7 +26,7 @@ bool visc_fast_supported(int nx, int ny)
 
 static size_t vb_smem(int M) { return 128 + (size_t)2 * 32 * M * 64 + (size_t)M * 256 * 8; }
 static size_t va_smem(int M) { return (size_t)FSEI_VA_WPB * (FSEI_VA_STAGES * 32 * (8 * M + 16) + 64); }
-static size_t va_tma_smem(int M) { return 1024 + (size_t)FSEI_VA_WPB * (FSEI_VA_STAGES * 256 * M + 64); }
+static size_t va_tma_smem(int M) { return 1024 + (size_t)FSEI_VA_TMA_WPB * (FSEI_VA_STAGES * 256 * M + 64); }
 #ifndef FSEI_VA_TMA
 #define FSEI_VA_TMA 1               // chunk lengths 8, 16, 24, 32 take the tensor-map variant of pass A
 #endif
@@ -129,11 +129,12 @@ cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st)
                    wide ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return cudaErrorInvalidValue;
         }
+        const dim3 gt((A.ny + FSEI_VA_TMA_WPB - 1) / FSEI_VA_TMA_WPB, 3);
         switch (M) {
-            case 8: k_visc_xz_tma<8><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(8), st>>>(A, Mp); break;
-            case 16: k_visc_xz_tma<16><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(16), st>>>(A, Mp); break;
-            case 24: k_visc_xz_tma<24><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(24), st>>>(A, Mp); break;
-            default: k_visc_xz_tma<32><<<grid, 32 * FSEI_VA_WPB, va_tma_smem(32), st>>>(A, Mp); break;
+            case 8: k_visc_xz_tma<8><<<gt, 32 * FSEI_VA_TMA_WPB, va_tma_smem(8), st>>>(A, Mp); break;
+            case 16: k_visc_xz_tma<16><<<gt, 32 * FSEI_VA_TMA_WPB, va_tma_smem(16), st>>>(A, Mp); break;
+            case 24: k_visc_xz_tma<24><<<gt, 32 * FSEI_VA_TMA_WPB, va_tma_smem(24), st>>>(A, Mp); break;
+            default: k_visc_xz_tma<32><<<gt, 32 * FSEI_VA_TMA_WPB, va_tma_smem(32), st>>>(A, Mp); break;
         }
         return cudaGetLastError();
     }

@@ -161,6 +161,9 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz(const FSEI_GRID_CONSTANT VFastArgs A)
 // TMA instructions per line and direction instead of 32 bulk copies issued lane by lane (a warp-serial loop that took half
 // of k_visc_xz's stall samples).  Same arithmetic as k_visc_xz.  Dynamic shared memory: 1024 + WPB * (S * 256 M + 64) bytes.
 // ---------------------------------------------------------------------------------------------------------------
+#ifndef FSEI_VA_TMA_WPB
+#define FSEI_VA_TMA_WPB 1            // warps per CTA of the tensor-map variant
+#endif
 struct VFastMapsA { TmaMap2D r[3]; };      // per component: fp64 [32 ny nz rows][M], box 16 x 32, CU_TENSOR_MAP_SWIZZLE_128B
 
 __device__ __forceinline__ void tma_store_2d(const TmaMap2D* map, int x0, int y0, const void* src)
@@ -170,7 +173,7 @@ __device__ __forceinline__ void tma_store_2d(const TmaMap2D* map, int x0, int y0
 }
 
 template <int M>
-FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_GRID_CONSTANT VFastMapsA Mp)
+FSEI_GLOBAL(32 * FSEI_VA_TMA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_GRID_CONSTANT VFastMapsA Mp)
 {
     static_assert(M % 8 == 0, "whole 64- or 128-byte boxes");
     // box width: 16 doubles with the 128-byte swizzle where M allows it, else 8 doubles with the 64-byte swizzle (there the 16-byte
@@ -178,11 +181,11 @@ FSEI_GLOBAL(32 * FSEI_VA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFastArg
     constexpr int S = FSEI_VA_STAGES, BW = (M % 16 == 0) ? 16 : 8, CH = BW / 2, ROWB = 8 * BW, BOXB = 32 * ROWB, NBOX = M / BW, STAGE = NBOX * BOXB;
     FSEI_DYN_SMEM(smraw);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, comp = blockIdx.y;
-    const int j = blockIdx.x * FSEI_VA_WPB + wid;
+    const int j = blockIdx.x * FSEI_VA_TMA_WPB + wid;
     if (j >= A.ny) return;
     unsigned char* base = smraw + ((1024u - (smem_u32(smraw) & 1023u)) & 1023u);       // the swizzle pattern repeats every 1024 bytes
     unsigned char* buf = base + (size_t)wid * (S * STAGE);
-    uint64_t* bar = reinterpret_cast<uint64_t*>(base + (size_t)FSEI_VA_WPB * S * STAGE) + wid * 8;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(base + (size_t)FSEI_VA_TMA_WPB * S * STAGE) + wid * 8;
     const double* __restrict__ zam = A.zam[comp];
     const double* __restrict__ zip = A.zip[comp];
     const VFastLine& L = A.L;
