@@ -44,6 +44,7 @@ cudaError_t launch_xi_fast(const XFast& P, bool neu, const cplx* spec, double* p
 // fast family of the implicit viscous step (visc_fast.cuh): periodic x and y, nx/32 and ny/32 instantiated
 struct VFastLine; struct VFastArgs;
 bool visc_fast_supported(int nx, int ny);
+bool visc_fast_slab_supported(int nx, int ny);
 cudaError_t visc_fast_init();
 void visc_fast_line(int n, double h_recip, double beta, VFastLine* out);
 int visc_fast_nsig(const VFastLine& L);

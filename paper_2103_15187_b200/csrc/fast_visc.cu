@@ -7,9 +7,21 @@
 
 namespace fsei {
 
+#ifndef FSEI_VA_TMA
+#define FSEI_VA_TMA 1               // chunk lengths 8, 16, 24, 32 take the tensor-map variant of pass A
+#endif
+#define FSEI_VA_TMA_ON (FSEI_VA_TMA != 0)
+
 // chunk lengths with an instantiation: pass A needs M % 4 == 0 (conflict-free 128-bit slots; 2 for small test grids)
 #define FSEI_VA_LIST(X) X(2) X(4) X(8) X(12) X(16) X(24) X(32) X(10) X(20) X(18) X(30)
 #define FSEI_VB_LIST(X) X(2) X(3) X(4) X(6) X(8) X(12) X(16) X(24) X(32) X(5) X(10) X(20) X(18) X(30)
+
+// z-slabs: pass A only in its tensor-map variant (chunk lengths 8, 16, 24, 32)
+bool visc_fast_slab_supported(int nx, int ny)
+{
+    const int M = nx / 32;
+    return visc_fast_supported(nx, ny) && M % 8 == 0 && M <= 32 && FSEI_VA_TMA_ON;
+}
 
 bool visc_fast_supported(int nx, int ny)
 {
@@ -116,7 +128,8 @@ cudaError_t launch_visc_xz(const VFastArgs& A, cudaStream_t st)
 {
     const dim3 grid((A.ny + FSEI_VA_WPB - 1) / FSEI_VA_WPB, 3);
     const int M = A.nx / 32;
-    if (FSEI_VA_TMA && M % 8 == 0 && M <= 32 && (size_t)32 * A.ny * A.nz < (1ull << 31)) {
+    if (A.slab && !(FSEI_VA_TMA && M % 8 == 0 && M <= 32 && (size_t)32 * A.ny * A.nz < (1ull << 31))) return cudaErrorInvalidValue;
+    if (FSEI_VA_TMA && M % 8 == 0 && M <= 32 && ((size_t)32 * A.ny * A.nz < (1ull << 31) || A.slab)) {
         EncodeTiledFn fn = tma_encode_fn();
         if (!fn) return cudaErrorNotSupported;
         VFastMapsA Mp;
@@ -169,7 +182,7 @@ cudaError_t launch_visc_zy(const VFastArgs& A, cudaStream_t st)
     while (A.ny % Mp.box_rows) Mp.box_rows--;                   // largest divisor of ny that fits a TMA box
     for (int c = 0; c < 3; c++) {
         cudaError_t e = field_map(A, Mp.box_rows, A.r[c], &Mp.d[c]);
-        if (e == cudaSuccess) e = field_map(A, Mp.box_rows, A.q[c], &Mp.q[c]);
+        if (e == cudaSuccess) e = field_map(A, Mp.box_rows, A.slab ? A.r[c] : A.q[c], &Mp.q[c]);
         if (e != cudaSuccess) return e;
     }
     switch (A.ny / 32) {

@@ -859,7 +859,7 @@ extern "C" int fsei_viscous_step(fsei_plan* P, double* u, double* v, double* w, 
             const VTab V = visc_tab(P, slot, c, DIR_Z);
             A.zam[c] = V.am; A.zip[c] = V.ip; A.zcp[c] = V.cp; A.r[c] = r[c]; A.q[c] = q[c];
         }
-        A.nx = T.nx; A.ny = T.ny; A.nz = T.nz;
+        A.nx = T.nx; A.ny = T.ny; A.nz = T.nz; A.slab = 0;
         A.split = 2 * (T.nx / 8) <= P->nsm ? 1 : 0;           // up to 1.5 marches per SM (measured: nx <= 576 gain 1.1-3x, nx >= 640 lose)
         A.L = P->vline_x[slot]; A.nsig = P->vnsig_x[slot];
         { LaunchTimer t(P, K_VXZ, st); CU(launch_visc_xz(A, st)); }
@@ -1130,6 +1130,12 @@ static int slab_plan_build(fsei_plan* P, int nx, int ny, int nz, double Lx, doub
         if ((rc = dalloc(P, sizeof(double) * FSEI_VSLOTS * 9 * vtab_set_doubles(P->vnmax), &qv))) return rc;
         P->vtab = static_cast<double*>(qv);
         CU(kernel_smem(k_explicit_terms, FSEI_EXPL_SMEM_MAX));
+        P->visc_fast = visc_fast_slab_supported(nx, ny);               // x and y sweeps of fsei_slab_viscous_xy by the partition kernels
+        if (P->visc_fast) {
+            CU(visc_fast_init());
+            int dev = 0;
+            CU(cudaGetDevice(&dev)); CU(cudaDeviceGetAttribute(&P->nsm, cudaDevAttrMultiProcessorCount, dev));
+        }
     }
     XFast& XF = P->XF; YFast& YF = P->YF; ZFast& ZF = P->ZF;
     XF.nx = nx; XF.ny = ny; XF.nz = nzl; XF.N = nx / 2; XF.tw = X.tw; XF.tw_r2c = X.tw_r2c; XF.tw_dct = X.tw_dct; XF.scale = T.scale;
@@ -1295,6 +1301,19 @@ extern "C" int fsei_slab_viscous_xy(fsei_plan* P, double* ru, double* rv, double
     const long nlx = (long)T.ny * nzl, nly = (long)T.nx * nzl;
     const size_t plane = (size_t)T.nx * T.ny;
     double* r[3] = {ru, rv, rw};
+    if (P->visc_fast && (size_t)32 * T.ny * nzl < (1ull << 31) && !misaligned(ru) && !misaligned(rv) && !misaligned(rw)) {
+        // the fast family's two passes without their z parts: periodic x solves, then periodic y solves, in place
+        VFastArgs A;
+        for (int c = 0; c < 3; c++) { A.zam[c] = A.zip[c] = A.zcp[c] = nullptr; A.r[c] = r[c]; A.q[c] = r[c]; }
+        A.nx = T.nx; A.ny = T.ny; A.nz = nzl; A.slab = 1;
+        A.split = 2 * (T.nx / 8) <= P->nsm ? 1 : 0;
+        A.L = P->vline_x[slot]; A.nsig = P->vnsig_x[slot];
+        { LaunchTimer t(P, K_VXZ, st); CU(launch_visc_xz(A, st)); }
+        A.L = P->vline_y[slot]; A.nsig = P->vnsig_y[slot];
+        { LaunchTimer t(P, K_VZY, st); CU(launch_visc_zy(A, st)); }
+        P->last_launches = launches + 2;
+        return FSEI_OK;
+    }
     for (int c = 0; c < 3; c++) {
         { VTab V = visc_tab(P, slot, c, DIR_X); LaunchTimer t(P, K_VX, st); k_visc_sweep_x<true, false><<<(unsigned)((nlx + 127) / 128), 128, 0, st>>>(V, r[c], nullptr, nlx); }
         CU(cudaGetLastError());

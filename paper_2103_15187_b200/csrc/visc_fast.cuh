@@ -42,6 +42,7 @@ struct VFastArgs {
     double* q[3];               // velocity components (pass B)
     int nx, ny, nz;
     int nsig;                   // terms of sinv kept on either side of s = 0 (16 = all)
+    int slab;                   // 1 = a z-slab (fsei_slab_viscous_xy): pass A solves x only, pass B solves y only and stores in place of d'
     int split;                  // pass B: 1 = one CTA per (tile, component) instead of one per tile (host: grids with few tiles)
 };
 
@@ -228,11 +229,16 @@ FSEI_GLOBAL(32 * FSEI_VA_TMA_WPB, 1) k_visc_xz_tma(const FSEI_GRID_CONSTANT VFas
         }
         const double xl = __shfl_sync(0xffffffffu, xs, (lane - 1) & 31);
         chunk_correct<M>(L, x, xl, xs);
-        // ---- forward elimination of the z system: d'_k = (x_k - a_k d'_{k-1}) / piv_k
-        const double am = zam[k], ipk = zip[k];
-        const bool zero = wfix && k == 0;
+        if (A.slab) {                                // a z-slab: the z system is solved on pencils, after a transpose
 #pragma unroll
-        for (int i = 0; i < M; i++) dprev[i] = zero ? 0.0 : fma(-am, dprev[i], x[i]) * ipk;
+            for (int i = 0; i < M; i++) dprev[i] = x[i];
+        } else {
+            // ---- forward elimination of the z system: d'_k = (x_k - a_k d'_{k-1}) / piv_k
+            const double am = zam[k], ipk = zip[k];
+            const bool zero = wfix && k == 0;
+#pragma unroll
+            for (int i = 0; i < M; i++) dprev[i] = zero ? 0.0 : fma(-am, dprev[i], x[i]) * ipk;
+        }
         // ---- out: through the same slot
 #pragma unroll
         for (int h = 0; h < NBOX; h++)
@@ -320,8 +326,9 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
             for (int m = 0; m < M; m++) x[m] = tl[m * 8];
         }
         // ---- back substitution of the z system: x_k = d'_k - c'_k x_{k+1}   (top plane: nothing above)
-        const double cpk = A.zcp[comp][k];
-        if (k == nz - 1) {
+        const double cpk = A.slab ? 0.0 : A.zcp[comp][k];
+        if (A.slab) {                                // a z-slab: no z coupling here
+        } else if (k == nz - 1) {
 #pragma unroll
             for (int m = 0; m < M; m++) carry[m * 256] = x[m];
         } else {
@@ -360,7 +367,8 @@ FSEI_GLOBAL(256, 1) k_visc_zy(const FSEI_GRID_CONSTANT VFastArgs A, const FSEI_G
         __syncthreads();
         if (tid == 0) {
             const double* t = tile0 + pb * NY * 8;
-            for (int b = 0; b < nb; b++) tma_reduce_add_2d(&Mp.q[comp], col0, k * NY + b * Mp.box_rows, t + b * Mp.box_rows * 8);
+            if (A.slab) for (int b = 0; b < nb; b++) tma_store_2d(&Mp.d[comp], col0, k * NY + b * Mp.box_rows, t + b * Mp.box_rows * 8);
+            else for (int b = 0; b < nb; b++) tma_reduce_add_2d(&Mp.q[comp], col0, k * NY + b * Mp.box_rows, t + b * Mp.box_rows * 8);
             bulk_commit();
         }
     }

@@ -319,7 +319,8 @@ def _fluid_case(shape, seed=71):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("world", [1, 2, 3, 4])
-@pytest.mark.parametrize("shape,force", [((64, 32, 24), False), ((128, 64, 37), True), ((96, 48, 16), True)])
+@pytest.mark.parametrize("shape,force", [((64, 32, 24), False), ((128, 64, 37), True), ((96, 48, 16), True), ((256, 64, 13), True),
+                                         ((512, 96, 9), False)])       # the last two: x and y sweeps by the partition kernels
 def test_decomposed_fluid_substeps_vs_oracle_and_single_plan(oracle_ld, world, shape, force):
     """Three RK3 substeps on `world` slabs stepped stage by stage in one process against the oracle's chain and the
     single-plan fsei_fluid_substep.  Explicit terms are bit-exact stencils on either path (the halo planes hold the
@@ -366,10 +367,10 @@ def test_decomposed_fluid_substeps_vs_oracle_and_single_plan(oracle_ld, world, s
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("world", [2, 3])
-def test_slab_viscous_stages_vs_oracle(oracle_ld, world):
-    """The viscous stages alone (x, y sweeps on slabs; z sweep on pencils; q += dq) against the oracle's viscous step at a
-    stiff beta, where the z coupling across slab boundaries is strong."""
-    shape = (64, 32, 30)
+@pytest.mark.parametrize("shape", [(64, 32, 30), (256, 128, 10)])
+def test_slab_viscous_stages_vs_oracle(oracle_ld, world, shape):
+    """The viscous stages alone (x, y sweeps on slabs -- generic sweeps, or the partition kernels on the second shape; z sweep on
+    pencils; q += dq) against the oracle's viscous step at a stiff beta, where the z coupling across slab boundaries is strong."""
     g, u, v, w, f = _fluid_case(shape, seed=72)
     beta = 5e-3
     uo, vo, wo = u.copy(), v.copy(), w.copy()
